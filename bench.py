@@ -1,0 +1,325 @@
+#!/usr/bin/env python
+"""bench.py -- the driver's measurement contract for the B200 beam-tracking hot path.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload fodo_channel|...]
+
+Metric (BASELINE.json): particle-element pushes/s (fp64).  One *element push* = one particle through one
+lattice element (all its slices).  Workload at N=1 = BASELINE configs[1] ("Linear FODO channel": 10^6
+particles, the FODO cell x100 = 500 elements / 5300 slice maps, 1 pass), synthetic seeded input from
+workloads/.  A *step* = one pass of the hot path over the bunch = one bt_track(1) call = ONE kernel launch.
+
+N > 1 (torchrun): particles are independent, so the path shards with no data-path collective; every rank
+tracks its own 10^6-particle bunch (seed + rank) -> "scaling": "weak"; value = all ranks' pushes / max-over-ranks time.
+
+Timing: W >= 3 warm-up steps; every timed step is bracketed by CUDA events on the beam's stream (torch's current
+stream); L2 is flushed (256 MiB write) between timed steps, outside the event intervals; the K-step region is
+bracketed by barrier + torch.cuda.synchronize(); ms_per_step = sum of event intervals / K, max over ranks.
+
+The same JSON line carries: roofline (FP64-pipe issue slots), cpu_baseline (the oracle as
+it stands on a bounded sample, host cores), e2e (host pinned buffers -> bt_beam_upload -> bt_track ->
+bt_beam_download inside the timed region), gpu_launches, clocks.
+"""
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+import workloads as W  # noqa: E402
+
+METRIC = "particle-element pushes/s (fp64)"
+UNIT = "pushes/s"
+
+# FP64 issue slots per slice map (DESIGN.md section 7 / SURVEY 8d): minimal DFMA/DMUL sequences.
+SLOTS = {"drift": 3, "quad": 9, "sbend": 10, "dipedge": 2, "shortrf": 4}
+
+
+def slots_per_particle_per_turn(lattice):
+    total = 0
+    for el in lattice:
+        kind, ns = el[0], el[2]
+        if kind == "multipole":
+            m, ks = int(el[3]), el[5]
+            per = 5 if (m == 3 and ks == 0.0) else 8 if (m == 4 and ks == 0.0) else 4 * max(m - 1, 0) + 6
+        elif kind == "quad" and el[3] == 0.0:
+            per = SLOTS["drift"]
+        else:
+            per = SLOTS[kind]
+        total += per * ns
+    return total
+
+
+def load_peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        with open(path) as f:
+            return json.load(f), "measured"
+    return {"hbm_gbs": 6650.0, "sm_max_mhz": 1965.0}, "fallback"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons DURING the timed region (B200_PROFILING.md recipe)."""
+    QUERY = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+             "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+             "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.index, self.proc, self.lines = index, None, []
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.QUERY,
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._read, daemon=True)
+            self.thread.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.lines.append(line.strip())
+
+    def stop(self):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=2)
+        except Exception:
+            self.proc.kill()
+        sm, mx, pw, reasons = [], [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for ln in self.lines:
+            f = [x.strip() for x in ln.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0])), mx.append(float(f[1])), pw.append(float(f[2]))
+            except ValueError:
+                continue
+            for name, val in zip(names, f[3:7]):
+                if val.lower().startswith("active"):
+                    reasons.add(name)
+        return {"sm_mhz": statistics.median(sm) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "power_w_max": max(pw) if pw else None, "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def get_workload(name, rank):
+    idx = {"tiny_fodo": 0, "fodo_channel": 1, "chicane": 2, "nonlinear_ring": 3}[name]
+    cfg = W.config(idx)
+    cfg.seed = cfg.seed + 1000 * rank      # every rank its own bunch (weak scaling)
+    return cfg
+
+
+# ---------------------------------------------------------------------------------------------------
+# reference arm: the oracle as it stands, on the host cores, on a bounded sample of the same workload
+# ---------------------------------------------------------------------------------------------------
+def oracle_rate(cfg, n_sample, reps=1):
+    import oracle as O
+    coords = W.make_bunch(cfg, n=n_sample)
+    g0 = O.ref_from_kinetic(cfg.kin_energy_MeV, cfg.mass_MeV)[0]
+    times = []
+    for _ in range(reps):
+        c = [a.copy() for a in coords]
+        t0 = time.perf_counter()
+        O.track(c, cfg.lattice, cfg.nturns, g0)
+        times.append(time.perf_counter() - t0)
+    pushes = n_sample * cfg.n_elements * cfg.nturns
+    return pushes, times, O.num_threads()
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    cfg = get_workload(args.workload, 0)
+    n_sample = min(cfg.n, args.ref_sample)
+    for _ in range(args.warmup and 1):
+        oracle_rate(cfg, max(1000, n_sample // 20))
+    pushes, times, cores = oracle_rate(cfg, n_sample, reps=max(1, min(args.steps, 5)))
+    t = sum(times) / len(times)
+    value = pushes / t
+    sample = "%d of %d particles (seed %d), full lattice (%d elements, %d slice maps), %d turn(s) per step" % (
+        n_sample, cfg.n, cfg.seed, cfg.n_elements, cfg.slice_maps_per_turn, cfg.nturns)
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": len(times),
+        "warmup": 1, "ms_per_step": t * 1e3, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f64", "data": "synthetic",
+        "config": {"workload": "configs[1] " + cfg.name + " (bounded sample)", "particles": n_sample,
+                   "elements": cfg.n_elements, "slice_maps_per_turn": cfg.slice_maps_per_turn, "turns": cfg.nturns},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+    return 0
+
+
+# ---------------------------------------------------------------------------------------------------
+# our arm
+# ---------------------------------------------------------------------------------------------------
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    import paper_2208_02382_b200 as bt
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the product path has no CPU fallback")
+    torch.cuda.set_device(local)
+    if world > 1:
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    cfg = get_workload(args.workload, rank)
+    coords = W.make_bunch(cfg)
+    n = cfg.n
+    pushes_per_step = n * cfg.n_elements * cfg.nturns
+    slots_pp = slots_per_particle_per_turn(cfg.lattice) * cfg.nturns
+    slots_per_launch = float(n) * slots_pp
+
+    beam = bt.Beam(n)                       # six torch.float64 CUDA tensors lent to the library
+    beam.set_ref(cfg.kin_energy_MeV, cfg.mass_MeV, cfg.charge_qe)
+    beam.lattice_set(cfg.lattice)
+    pinned = [torch.from_numpy(a).pin_memory() for a in coords]
+    pinned_out = [torch.empty(n, dtype=torch.float64).pin_memory() for _ in range(6)]
+    pristine = [t.to("cuda", non_blocking=True) for t in pinned]
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
+
+    def restore():
+        for dst, src in zip(beam.tensors, pristine):
+            dst.copy_(src, non_blocking=True)
+
+    # ---- device-resident timing ----------------------------------------------------------------
+    restore()
+    for _ in range(max(args.warmup, 3)):
+        beam.track(cfg.nturns)
+    torch.cuda.synchronize()
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+    launches0 = bt.launch_count()
+    barrier()
+    t_wall0 = time.perf_counter()
+    for k in range(args.steps):
+        restore()                            # same input every step (outside the event interval)
+        flush.zero_()                        # L2 flush between timed iterations (outside the event interval)
+        ev[k][0].record()
+        beam.track(cfg.nturns)               # ONE fused-walk launch
+        ev[k][1].record()
+    barrier()
+    t_wall = time.perf_counter() - t_wall0
+    launches = bt.launch_count() - launches0
+    step_ms = [a.elapsed_time(b) for a, b in ev]
+    ms_sum = sum(step_ms)
+
+    # ---- end to end through the C-ABI with host buffers -----------------------------------------
+    for _ in range(2):
+        beam.upload(pinned), beam.track(cfg.nturns), beam.download(pinned_out)
+    barrier()
+    t0 = time.perf_counter()
+    for k in range(args.steps):
+        beam.upload(pinned)                  # bt_beam_upload: 6 x H2D from pinned host memory
+        beam.track(cfg.nturns)
+        beam.download(pinned_out)            # bt_beam_download: 6 x D2H, synchronises
+    barrier()
+    t_e2e = time.perf_counter() - t0
+    clocks = sampler.stop() if rank == 0 else None
+
+    # max over ranks
+    tt = torch.tensor([ms_sum, t_e2e, t_wall], dtype=torch.float64, device="cuda")
+    if world > 1:
+        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+    ms_sum, t_e2e, t_wall = [float(v) for v in tt.cpu()]
+    launch_info = beam.last_launch()
+
+    result = None
+    if rank == 0:
+        peaks, peaks_kind = load_peaks()
+        ms_per_step = ms_sum / args.steps
+        value = world * pushes_per_step / (ms_per_step * 1e-3)
+        e2e_value = world * pushes_per_step * args.steps / t_e2e
+        # roofline of the dominant (only) kernel: FP64 pipe issue slots
+        nominal_peak = 148 * 64 * float(peaks.get("sm_max_mhz", 1965.0)) * 1e6       # slots/s at max SM clock
+        measured_fp64 = bt.calib_fp64(300.0)
+        measured_rw6 = bt.calib_rw6(min(64_000_000, max(n, 8_000_000)), 5)
+        achieved = slots_per_launch / (statistics.mean(step_ms) * 1e-3)
+        hbm_time_ms = 96.0 * n / (float(peaks["hbm_gbs"]) * 1e9) * 1e3
+        alu_time_ms = slots_per_launch / nominal_peak * 1e3
+        bound = "alu" if alu_time_ms >= hbm_time_ms else "hbm"
+        if bound == "alu":
+            roof = {"bound": "alu", "achieved": achieved / 1e12, "peak": nominal_peak / 1e12, "unit": "Tslot/s",
+                    "frac": achieved / nominal_peak, "traffic": None,
+                    "peak_kind": "derived: 148 SMs x 64 FP64 lanes x %s sm_max_mhz (DESIGN.md s7)" % peaks_kind,
+                    "peak_measured_dfma_chain": measured_fp64 / 1e12, "frac_of_measured_dfma_chain": achieved / measured_fp64,
+                    "slots_per_particle": slots_pp, "tflops": None}
+        else:
+            gbs = 96.0 * n / (statistics.mean(step_ms) * 1e-3) / 1e9
+            roof = {"bound": "hbm", "achieved": gbs, "peak": float(peaks["hbm_gbs"]), "unit": "GB/s",
+                    "frac": gbs / float(peaks["hbm_gbs"]), "traffic": None, "peak_kind": peaks_kind + " copy bandwidth",
+                    "rw6_stream_ceiling_gbs": measured_rw6}
+        roof["kernel"] = "bt::track_kernel<P=%d> grid=%d block=%d smem=%dB" % (
+            launch_info["particles_per_thread"], launch_info["grid"], launch_info["block"], launch_info["smem_bytes"])
+        roof["roofline_time_ms"] = max(alu_time_ms, hbm_time_ms)
+        roof["rw6_stream_ceiling_gbs"] = measured_rw6
+        # CPU baseline: the oracle as it stands, bounded sample, host cores
+        cb_pushes, cb_times, cores = oracle_rate(get_workload(args.workload, 0), min(n, args.ref_sample))
+        cpu_baseline = {"value": cb_pushes / cb_times[0], "unit": UNIT, "cores": cores, "kind": "oracle",
+                        "sample": "%d of %d particles, full lattice, %d turn(s); %.1f s" % (min(n, args.ref_sample), n, cfg.nturns, cb_times[0])}
+        result = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
+            "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f64", "data": "synthetic",
+            "config": {"workload": "configs[1] " + cfg.name, "particles_per_gpu": n, "elements": cfg.n_elements,
+                       "slice_maps_per_turn": cfg.slice_maps_per_turn, "turns_per_step": cfg.nturns,
+                       "slice_maps_per_s": world * n * cfg.slice_maps_per_turn * cfg.nturns / (ms_per_step * 1e-3),
+                       "l2": "flushed between timed steps (256 MiB write)", "parallelism": "particles sharded, %d rank(s), no collective" % world},
+            "roofline": roof, "cpu_baseline": cpu_baseline,
+            "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": 48 * n, "d2h_bytes_per_step": 48 * n,
+                    "ms_per_step": t_e2e / args.steps * 1e3},
+            "gpu_launches": int(launches), "clocks": clocks,
+            "step_ms_min_median_max": [min(step_ms), statistics.median(step_ms), max(step_ms)],
+            "wall_s_timed_region": t_wall,
+        }
+    beam.close()
+    if world > 1:
+        dist.destroy_process_group()
+    if rank == 0:
+        print(json.dumps(result), flush=True)
+    return 0
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=100)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="fodo_channel", choices=["tiny_fodo", "fodo_channel", "chicane", "nonlinear_ring"])
+    ap.add_argument("--ref-sample", type=int, default=200_000, help="particles of the workload the oracle is timed on")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+    return run_ours(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

@@ -1,0 +1,198 @@
+/*
+ * bt.h -- C-ABI of libbt.so: the data-parallel hot path of the s-based beam-dynamics PIC method of
+ * arxiv 2208.02382 (Huebl et al., "Next generation computational tools for the modeling and design
+ * of particle accelerators at exascale"), built for NVIDIA B200 (sm_100a).
+ *
+ * Citation convention: "P:l.N" = line N of the paper text; "R<n>" = reading n of the
+ * paper stated in DESIGN.md section 3 (the paper prints no formulas; P:l.47 states the method:
+ * "Tracking through lattice elements is performed by pushing particles in s using a symplectic
+ * map ... accurate through linear order").
+ *
+ * General rules
+ *  - Every function returns int: BT_OK (0) or a negative bt_status.  No exception crosses the ABI.
+ *    bt_last_error() returns a thread-local, human-readable description of the last failure.
+ *  - "host" pointers are ordinary CPU memory (pinned memory makes uploads/downloads asynchronous
+ *    to the host until the next synchronising call); "device" pointers are CUDA global memory of
+ *    the device that was current when bt_beam_create was called.
+ *  - All floating point data is IEEE fp64.  Coordinates (R1): x [m], px = Px/p0, y [m], py = Py/p0,
+ *    t = c*(arrival time - reference arrival time) [m], pt = -(E - E0)/(p0 c); array order is always
+ *    x, px, y, py, t, pt; each is a separate contiguous array of n doubles (SoA).
+ *  - Asynchrony: calls enqueue work on the beam's CUDA stream and return.  bt_beam_download,
+ *    bt_grid_download_rho and bt_sync synchronise that stream.  A bt_grid used with a beam is
+ *    accessed on that beam's stream.
+ *  - Arguments are validated before anything is launched; an invalid call changes no state.
+ *  - There is no CPU fallback: without a CUDA device every entry point that touches the device
+ *    fails with BT_ERR_CUDA.
+ *  - Particle order seen through bt_beam_download / bt_beam_ptrs never changes.
+ *  - NaN/Inf coordinates are not checked on the hot path; in deposit/gather they count as
+ *    "outside the grid" (R13).
+ */
+#ifndef BT_H_
+#define BT_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define BT_VERSION 100 /* 0.1.0 */
+
+typedef struct bt_beam bt_beam; /* opaque: 6 device arrays (owned or borrowed), reference particle, lattice tables */
+typedef struct bt_grid bt_grid; /* opaque: rho (nx*ny*nz doubles) and optionally a 3-component node field     */
+
+typedef enum {
+    BT_OK = 0,
+    BT_ERR_INVALID = -1,     /* bad argument (null, n <= 0, nslice < 1, ds < 0, rc == 0, cos(psi) == 0, ...) */
+    BT_ERR_CUDA = -2,        /* a CUDA runtime call failed; text in bt_last_error()                          */
+    BT_ERR_OOM = -3,         /* host or device allocation failed                                             */
+    BT_ERR_STATE = -4,       /* call order: bt_track before bt_lattice_set / bt_beam_set_ref, no field set..  */
+    BT_ERR_UNSUPPORTED = -5  /* valid request this build does not implement                                  */
+} bt_status;
+
+/* Element kinds (P:l.86-91 Drift, Quad; P:l.108, l.124 name the others). */
+typedef enum {
+    BT_DRIFT = 0,     /* R4 */
+    BT_QUAD = 1,      /* R5 thick quadrupole, k > 0 focuses x */
+    BT_SBEND = 2,     /* R6 sector bend, no field index */
+    BT_DIPEDGE = 3,   /* R7 thin pole-face rotation with fringe correction */
+    BT_MULTIPOLE = 4, /* R8 thin multipole kick */
+    BT_SHORTRF = 5    /* R9 short RF cavity, linearised, energy kick only, updates the reference energy */
+} bt_element_type;
+
+/*
+ * One lattice element: 64 bytes of plain data, caller-owned, copied by bt_lattice_set.
+ * Mirrors the user-facing element vocabulary of the paper's Listing 1, e.g.
+ * elements.Quad(ds=1.0, k=1.0, nslice=ns) (P:l.88).
+ *   type    bt_element_type
+ *   nslice  >= 1; the element is applied as nslice maps of length ds/nslice (R3; P:l.47, l.87).
+ *           Thin elements (DIPEDGE, MULTIPOLE, SHORTRF) must have nslice == 1.
+ *   ds      length [m], >= 0; ignored for the map of thin elements but still added to s.
+ *   p[6]    QUAD:      p0 = k [m^-2]
+ *           SBEND:     p0 = rc [m], signed bending radius, != 0
+ *           DIPEDGE:   p0 = psi [rad], p1 = rc [m] (!= 0), p2 = g [m] full gap, p3 = K fringe integral
+ *           MULTIPOLE: p0 = m (integer 1..10; 1 dipole, 2 quad, 3 sext, 4 oct), p1 = Kn, p2 = Ks
+ *                      (integrated strengths [m^-(m-1)], MAD-X sign: Kn > 0 at m = 2 focuses x)
+ *           SHORTRF:   p0 = Vhat = qV/(mc^2), p1 = frequency [Hz], p2 = phase [deg] (cosine convention)
+ *           unused entries are ignored.
+ */
+typedef struct {
+    int32_t type;
+    int32_t nslice;
+    double ds;
+    double p[6];
+} bt_element;
+
+/* ---- beam (particle container, S0) ---------------------------------------------------------- */
+
+/*
+ * Create a beam of n particles (n >= 1) on the current CUDA device.
+ *   dev_ptrs   NULL: the library allocates 6 arrays of n doubles (256-byte aligned, uninitialised).
+ *              else: 6 device pointers, BORROWED -- the caller (e.g. torch.empty(n, dtype=float64,
+ *              device="cuda")) keeps them alive until bt_beam_destroy and frees them; each must be
+ *              8-byte aligned (16-byte alignment enables the vectorised path).
+ *   cuda_stream  a cudaStream_t cast to void* (0 = legacy default stream); all work of this beam is
+ *              enqueued there.
+ * Mirrors ImpactX() + add_particles(..., npart) (P:l.58, l.81).
+ */
+int bt_beam_create(bt_beam **out, int64_t n, double *const dev_ptrs[6], void *cuda_stream);
+void bt_beam_destroy(bt_beam *beam);
+
+/*
+ * Reference particle (R2): kinetic energy [MeV] (> 0), rest mass [MeV] (> 0), charge [e] (informational).
+ * gamma0 = 1 + E_kin/mc^2.  Resets s = 0 and turn = 0 and invalidates the coefficient tables (they are
+ * rebuilt by the next bt_track).  Mirrors ref_particle().set_energy_MeV(energy_MeV, mass_MeV) (P:l.82-83).
+ */
+int bt_beam_set_ref(bt_beam *beam, double kin_energy_MeV, double mass_MeV, double charge_qe);
+int bt_beam_get_ref(const bt_beam *beam, double *gamma, double *s, int64_t *turn); /* any out may be NULL */
+
+/* Copy 6 host arrays of n doubles to / from the device arrays (order x,px,y,py,t,pt). upload is
+ * enqueued (the host arrays must stay valid until the next synchronising call unless they are pageable
+ * memory); download returns after the data has arrived. */
+int bt_beam_upload(bt_beam *beam, const double *const host[6]);
+int bt_beam_download(const bt_beam *beam, double *const host[6]);
+/* Zero-copy view of the 6 device arrays (P:l.102 "zero-copy access"); valid until bt_beam_destroy. */
+int bt_beam_ptrs(bt_beam *beam, double *dev_ptrs_out[6]);
+int64_t bt_beam_size(const bt_beam *beam);
+
+/* ---- lattice (S1) and fused walk (S2, S3) --------------------------------------------------- */
+
+/*
+ * Validate and copy the element list (n_elems >= 1).  Mirrors sim.lattice.extend([...]) (P:l.93).
+ * The per-slice map coefficients are computed on the host from (type, params, beta0, beta0*gamma0)
+ * when bt_track needs them, packed into 64-byte device records and uploaded once per bt_track call
+ * (once per turn-chunk if an RF cavity changes the reference energy).
+ */
+int bt_lattice_set(bt_beam *beam, const bt_element *elems, int32_t n_elems);
+
+/*
+ * Fused lattice walk (R3): for turn in 1..nturns, for each element in list order, for each slice:
+ * apply the element's map of length ds/nslice to every particle.  ONE kernel: each particle is
+ * loaded once, every element map and slice is applied in registers, and it is stored once per launch
+ * (96 bytes of HBM traffic per particle per launch).  Lattices whose RF cavities change the reference
+ * energy are processed in chunks of turns (one launch per chunk, per-turn coefficient tables).
+ * Updates the reference gamma, s and turn.  Bit-reproducible run to run.  nturns >= 0.
+ * Mirrors sim.evolve() (P:l.95) without space charge.
+ */
+int bt_track(bt_beam *beam, int32_t nturns);
+
+/* ---- grid, CIC deposit (S4, S5) and gather + kick (S6, S7) ---------------------------------- */
+
+/*
+ * Node-centred grid (R10): nx,ny,nz >= 2 nodes per axis, node (i,j,k) at lo + (i,j,k)*d, d > 0,
+ * linear index (k*ny + j)*nx + i (x fastest).  Third axis coordinate zeta = zscale * t.
+ * Allocates rho (zeroed).  Mirrors init_grids() (P:l.64).
+ */
+int bt_grid_create(bt_grid **out, int32_t nx, int32_t ny, int32_t nz, const double lo[3], const double d[3]);
+void bt_grid_destroy(bt_grid *grid);
+/* Field at the nodes, 3 arrays of nx*ny*nz doubles, x fastest; on_device != 0: device pointers (copied
+ * device-to-device), else host pointers.  The library keeps its own (internally re-laid-out) copy. */
+int bt_grid_set_field(bt_grid *grid, const double *Ex, const double *Ey, const double *Ez, int on_device);
+int bt_grid_rho(bt_grid *grid, double **dev_rho_out);    /* zero-copy device view of rho */
+int bt_grid_download_rho(bt_grid *grid, double *host_rho); /* synchronises the last beam stream used */
+
+/*
+ * CIC (order-1) charge deposition (R11, R13; P:l.43 "charge deposition", P:l.60 particle shape):
+ *   rho[node] += q_weight * (wx*wy)*wz for the 8 nodes around each particle, with per axis
+ *   u = (q - lo)*(1/d), i = floor(u), w1 = u - i, w0 = 1 - w1, third axis q = zscale*t.
+ * rho is charge per node.  Particles with i outside [0, n-2] on any axis (or NaN) are skipped.
+ * zero_first != 0 clears rho first (on the beam's stream).  The summation order is not deterministic;
+ * results are reproducible to fp64 rounding of the per-node sums only.
+ */
+int bt_deposit_cic(bt_beam *beam, bt_grid *grid, double q_weight, double zscale, int zero_first);
+
+/*
+ * Split-operator space-charge push (R12; P:l.49 "map-based split-operator approach"):
+ *   [drift(half_drift_before)]  ->  E = trilinear(field) at (x, y, zscale*t), outside => 0
+ *   px += coef[0]*Ex; py += coef[1]*Ey; pt += coef[2]*Ez   ->  [drift(half_drift_after)]
+ * in one pass over the particles (96 bytes per particle).  The drifts are R4 with the beam's current
+ * reference energy and advance s; 0, 0 => kick only.  Requires bt_grid_set_field and bt_beam_set_ref.
+ */
+int bt_gather_kick(bt_beam *beam, const bt_grid *grid, const double coef[3], double zscale,
+                   double half_drift_before, double half_drift_after);
+
+/* ---- utilities ------------------------------------------------------------------------------ */
+int bt_sync(bt_beam *beam); /* cudaStreamSynchronize on the beam's stream */
+const char *bt_last_error(void);
+int bt_version(void);
+/* Number of CUDA kernels this library has launched in this process (all beams/grids). */
+int64_t bt_launch_count(void);
+/* Name and launch geometry of the last fused-walk launch (diagnostic; any out may be NULL). */
+int bt_track_last_launch(const bt_beam *beam, int32_t *grid_dim, int32_t *block_dim,
+                         int32_t *particles_per_thread, int32_t *smem_bytes);
+
+/*
+ * Measurement utilities (roofline denominators measured on the box):
+ *  bt_calib_fp64: runs a register-only kernel of independent DFMA chains on all SMs for about
+ *     `min_ms` milliseconds and returns the achieved FP64 pipe instruction slots per second
+ *     (thread-level DFMA count / elapsed; one slot = one DFMA/DMUL/DADD of one thread).
+ *  bt_calib_rw6: streams 6 arrays of n doubles in and 6 out (the access pattern of bt_track)
+ *     and returns GB/s (96*n bytes / elapsed).  Allocates and frees its own buffers.
+ */
+int bt_calib_fp64(void *cuda_stream, double min_ms, double *slots_per_s);
+int bt_calib_rw6(void *cuda_stream, int64_t n, int32_t reps, double *gbytes_per_s);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* BT_H_ */

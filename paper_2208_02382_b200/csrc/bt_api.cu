@@ -1,0 +1,485 @@
+// C-ABI entry points of libbt.so (include/bt.h): handles, validation, host-side coefficient
+// precompute (S1, S3) and the call sequence of the hot path.  All particle work runs in the
+// kernels of track.cu / grid.cu.
+#include <math.h>
+#include <stdlib.h>
+#include <string.h>
+
+#include <new>
+
+#include "bt_internal.h"
+
+namespace bt {
+
+static thread_local std::string t_last_error;
+std::atomic<int64_t> g_launch_count{0};
+
+void set_error(const std::string &msg) { t_last_error = msg; }
+int fail(int code, const std::string &msg) {
+    t_last_error = msg;
+    return code;
+}
+
+static const double kPi = 3.14159265358979323846264338327950288;
+static const double kCLight = 299792458.0;
+
+// ---- validation (SURVEY 8b "Errors") ------------------------------------------------------------
+static int validate_element(const bt_element &e, int idx) {
+    auto bad = [&](const char *why) {
+        return fail(BT_ERR_INVALID, "element " + std::to_string(idx) + ": " + why);
+    };
+    if (e.nslice < 1) return bad("nslice < 1");
+    if (!(e.ds >= 0.0) || !isfinite(e.ds)) return bad("ds < 0 or not finite");
+    switch (e.type) {
+        case BT_DRIFT:
+            break;
+        case BT_QUAD:
+            if (!isfinite(e.p[0])) return bad("k not finite");
+            break;
+        case BT_SBEND:
+            if (e.p[0] == 0.0 || !isfinite(e.p[0])) return bad("rc == 0 or not finite");
+            break;
+        case BT_DIPEDGE:
+            if (e.nslice != 1) return bad("thin element needs nslice == 1");
+            if (e.p[1] == 0.0 || !isfinite(e.p[1])) return bad("rc == 0 or not finite");
+            if (!isfinite(e.p[0]) || cos(e.p[0]) == 0.0) return bad("cos(psi) == 0");
+            if (!isfinite(e.p[2]) || !isfinite(e.p[3])) return bad("g or K not finite");
+            break;
+        case BT_MULTIPOLE:
+            if (e.nslice != 1) return bad("thin element needs nslice == 1");
+            if (!(e.p[0] >= 1.0 && e.p[0] <= 10.0) || e.p[0] != floor(e.p[0])) return bad("m not an integer in [1,10]");
+            if (!isfinite(e.p[1]) || !isfinite(e.p[2])) return bad("Kn or Ks not finite");
+            break;
+        case BT_SHORTRF:
+            if (e.nslice != 1) return bad("thin element needs nslice == 1");
+            if (!isfinite(e.p[0]) || !isfinite(e.p[1]) || !isfinite(e.p[2])) return bad("RF parameter not finite");
+            break;
+        default:
+            return bad("unknown element type");
+    }
+    return BT_OK;
+}
+
+// ---- S1/S3: coefficients of one slice map per element, for one pass at reference gamma ----------
+double build_turn_table(const std::vector<bt_element> &lat, double gamma, DevOp *ops) {
+    for (size_t i = 0; i < lat.size(); ++i) {
+        const bt_element &e = lat[i];
+        DevOp &o = ops[i];
+        memset(&o, 0, sizeof(o));
+        o.nslice = e.nslice;
+        const double bg = sqrt(gamma * gamma - 1.0);
+        const double beta = bg / gamma;
+        const double h = e.ds / (double)e.nslice;  // R3: one rounded division
+        const double tc = h / (bg * bg);
+        switch (e.type) {
+            case BT_DRIFT:
+                o.op = OP_DRIFT;
+                o.c[0] = h;
+                o.c[1] = tc;
+                break;
+            case BT_QUAD: {
+                const double k = e.p[0];
+                if (k == 0.0) {  // R5: k = 0 is a drift
+                    o.op = OP_DRIFT;
+                    o.c[0] = h;
+                    o.c[1] = tc;
+                    break;
+                }
+                const double w = sqrt(fabs(k));
+                const double c = cos(w * h), s = sin(w * h), ch = cosh(w * h), sh = sinh(w * h);
+                const double f[3] = {c, s / w, -w * s};
+                const double d[3] = {ch, sh / w, w * sh};
+                const double *xb = k > 0.0 ? f : d, *yb = k > 0.0 ? d : f;
+                o.op = OP_QUAD;
+                o.c[0] = xb[0];
+                o.c[1] = xb[1];
+                o.c[2] = xb[2];
+                o.c[3] = yb[0];
+                o.c[4] = yb[1];
+                o.c[5] = yb[2];
+                o.c[6] = tc;
+                break;
+            }
+            case BT_SBEND: {
+                const double rho = e.p[0];
+                const double th = h / rho;
+                const double C = cos(th), S = sin(th);
+                o.op = OP_SBEND;
+                o.c[0] = C;
+                o.c[1] = rho * S;
+                o.c[2] = -(S / rho);
+                o.c[3] = -(rho * (1.0 - C)) / beta;
+                o.c[4] = -S / beta;
+                o.c[5] = rho * (S / (beta * beta) - th);
+                o.c[6] = h;
+                break;
+            }
+            case BT_DIPEDGE: {
+                const double psi = e.p[0], rho = e.p[1], g = e.p[2], K = e.p[3];
+                const double sp = sin(psi), cp = cos(psi);
+                const double psi_c = K * (g / rho) * (1.0 + sp * sp) / cp;
+                o.op = OP_EDGE;
+                o.c[0] = tan(psi) / rho;
+                o.c[1] = -tan(psi - psi_c) / rho;
+                break;
+            }
+            case BT_MULTIPOLE: {
+                const int m = (int)e.p[0];
+                const double Kn = e.p[1], Ks = e.p[2];
+                double fact = 1.0;
+                for (int j = 2; j <= m - 1; ++j) fact *= (double)j;
+                if (m == 3 && Ks == 0.0) {
+                    o.op = OP_SEXT;
+                    o.c[0] = Kn / 2.0;
+                    o.c[1] = Kn;
+                } else if (m == 4 && Ks == 0.0) {
+                    o.op = OP_OCT;
+                    o.c[0] = Kn / 6.0;
+                } else {
+                    o.op = OP_MULT;
+                    o.c[0] = (double)m;
+                    o.c[1] = Kn / fact;
+                    o.c[2] = Ks / fact;
+                }
+                break;
+            }
+            case BT_SHORTRF: {
+                const double Vhat = e.p[0], freq = e.p[1], phi = e.p[2] * (kPi / 180.0);
+                const double gamma_f = gamma + Vhat * cos(phi);
+                const double bg_f = sqrt(gamma_f * gamma_f - 1.0);
+                const double krf = 2.0 * kPi * freq / kCLight;
+                o.op = OP_RF;
+                o.c[0] = bg / bg_f;
+                o.c[1] = Vhat * krf * sin(phi) / bg_f;
+                gamma = gamma_f;  // S3: later elements see the new reference energy
+                break;
+            }
+        }
+    }
+    return gamma;
+}
+
+static int ensure_table(Beam *b, size_t n_ops) {
+    if (b->d_table_cap >= n_ops) return BT_OK;
+    if (b->d_table) {
+        BT_CUDA_TRY(cudaStreamSynchronize(b->stream));
+        BT_CUDA_TRY(cudaFree(b->d_table));
+        b->d_table = nullptr;
+        b->d_table_cap = 0;
+    }
+    BT_CUDA_TRY(cudaMalloc(&b->d_table, n_ops * sizeof(DevOp)));
+    b->d_table_cap = n_ops;
+    return BT_OK;
+}
+
+}  // namespace bt
+
+using namespace bt;
+
+extern "C" {
+
+const char *bt_last_error(void) { return t_last_error.c_str(); }
+int bt_version(void) { return BT_VERSION; }
+int64_t bt_launch_count(void) { return g_launch_count.load(); }
+
+int bt_beam_create(bt_beam **out, int64_t n, double *const dev_ptrs[6], void *cuda_stream) {
+    if (!out) return fail(BT_ERR_INVALID, "bt_beam_create: out is NULL");
+    *out = nullptr;
+    if (n <= 0) return fail(BT_ERR_INVALID, "bt_beam_create: n <= 0");
+    if (n > ((int64_t)1 << 40)) return fail(BT_ERR_INVALID, "bt_beam_create: n too large");
+    if (dev_ptrs)
+        for (int i = 0; i < 6; ++i) {
+            if (!dev_ptrs[i]) return fail(BT_ERR_INVALID, "bt_beam_create: dev_ptrs has a NULL entry");
+            if (((uintptr_t)dev_ptrs[i]) & 7u) return fail(BT_ERR_INVALID, "bt_beam_create: device pointer not 8-byte aligned");
+        }
+    int dev = 0;
+    BT_CUDA_TRY(cudaGetDevice(&dev));
+    cudaDeviceProp prop;
+    BT_CUDA_TRY(cudaGetDeviceProperties(&prop, dev));
+    bt_beam *h = new (std::nothrow) bt_beam();
+    if (!h) return fail(BT_ERR_OOM, "bt_beam_create: host allocation failed");
+    Beam &b = h->b;
+    b.n = n;
+    b.device = dev;
+    b.num_sms = prop.multiProcessorCount;
+    b.max_smem_optin = (int)prop.sharedMemPerBlockOptin;
+    b.stream = (cudaStream_t)cuda_stream;
+    if (dev_ptrs) {
+        for (int i = 0; i < 6; ++i) b.q[i] = dev_ptrs[i];
+        b.owns = false;
+    } else {
+        // one allocation, 6 slices, each 256-byte aligned (S0)
+        const size_t stride = (((size_t)n * sizeof(double)) + 255u) & ~(size_t)255u;
+        double *base = nullptr;
+        cudaError_t e = cudaMalloc(&base, stride * 6);
+        if (e != cudaSuccess) {
+            delete h;
+            return fail(e == cudaErrorMemoryAllocation ? BT_ERR_OOM : BT_ERR_CUDA,
+                        std::string("bt_beam_create: cudaMalloc: ") + cudaGetErrorString(e));
+        }
+        for (int i = 0; i < 6; ++i) b.q[i] = (double *)((char *)base + stride * i);
+        b.owns = true;
+    }
+    b.aligned16 = true;
+    for (int i = 0; i < 6; ++i)
+        if (((uintptr_t)b.q[i]) & 15u) b.aligned16 = false;
+    *out = h;
+    return BT_OK;
+}
+
+void bt_beam_destroy(bt_beam *beam) {
+    if (!beam) return;
+    Beam &b = beam->b;
+    cudaStreamSynchronize(b.stream);
+    if (b.owns && b.q[0]) cudaFree(b.q[0]);
+    if (b.d_table) cudaFree(b.d_table);
+    delete beam;
+}
+
+int bt_beam_set_ref(bt_beam *beam, double kin_energy_MeV, double mass_MeV, double charge_qe) {
+    if (!beam) return fail(BT_ERR_INVALID, "bt_beam_set_ref: beam is NULL");
+    if (!(kin_energy_MeV > 0.0) || !isfinite(kin_energy_MeV)) return fail(BT_ERR_INVALID, "bt_beam_set_ref: energy <= 0");
+    if (!(mass_MeV > 0.0) || !isfinite(mass_MeV)) return fail(BT_ERR_INVALID, "bt_beam_set_ref: mass <= 0");
+    Beam &b = beam->b;
+    b.gamma = 1.0 + kin_energy_MeV / mass_MeV;  // R2: kinetic energy
+    if (!(b.gamma > 1.0)) return fail(BT_ERR_INVALID, "bt_beam_set_ref: gamma == 1 in fp64");
+    b.mass_MeV = mass_MeV;
+    b.charge_qe = charge_qe;
+    b.s = 0.0;
+    b.turn = 0;
+    b.has_ref = true;
+    b.table_valid = false;
+    return BT_OK;
+}
+
+int bt_beam_get_ref(const bt_beam *beam, double *gamma, double *s, int64_t *turn) {
+    if (!beam) return fail(BT_ERR_INVALID, "bt_beam_get_ref: beam is NULL");
+    if (!beam->b.has_ref) return fail(BT_ERR_STATE, "bt_beam_get_ref: bt_beam_set_ref not called");
+    if (gamma) *gamma = beam->b.gamma;
+    if (s) *s = beam->b.s;
+    if (turn) *turn = beam->b.turn;
+    return BT_OK;
+}
+
+int64_t bt_beam_size(const bt_beam *beam) { return beam ? beam->b.n : 0; }
+
+int bt_beam_upload(bt_beam *beam, const double *const host[6]) {
+    if (!beam || !host) return fail(BT_ERR_INVALID, "bt_beam_upload: NULL argument");
+    for (int i = 0; i < 6; ++i)
+        if (!host[i]) return fail(BT_ERR_INVALID, "bt_beam_upload: host has a NULL entry");
+    Beam &b = beam->b;
+    for (int i = 0; i < 6; ++i)
+        BT_CUDA_TRY(cudaMemcpyAsync(b.q[i], host[i], (size_t)b.n * sizeof(double), cudaMemcpyHostToDevice, b.stream));
+    return BT_OK;
+}
+
+int bt_beam_download(const bt_beam *beam, double *const host[6]) {
+    if (!beam || !host) return fail(BT_ERR_INVALID, "bt_beam_download: NULL argument");
+    for (int i = 0; i < 6; ++i)
+        if (!host[i]) return fail(BT_ERR_INVALID, "bt_beam_download: host has a NULL entry");
+    const Beam &b = beam->b;
+    for (int i = 0; i < 6; ++i)
+        BT_CUDA_TRY(cudaMemcpyAsync(host[i], b.q[i], (size_t)b.n * sizeof(double), cudaMemcpyDeviceToHost, b.stream));
+    BT_CUDA_TRY(cudaStreamSynchronize(b.stream));
+    return BT_OK;
+}
+
+int bt_beam_ptrs(bt_beam *beam, double *dev_ptrs_out[6]) {
+    if (!beam || !dev_ptrs_out) return fail(BT_ERR_INVALID, "bt_beam_ptrs: NULL argument");
+    for (int i = 0; i < 6; ++i) dev_ptrs_out[i] = beam->b.q[i];
+    return BT_OK;
+}
+
+int bt_sync(bt_beam *beam) {
+    if (!beam) return fail(BT_ERR_INVALID, "bt_sync: beam is NULL");
+    BT_CUDA_TRY(cudaStreamSynchronize(beam->b.stream));
+    return BT_OK;
+}
+
+int bt_lattice_set(bt_beam *beam, const bt_element *elems, int32_t n_elems) {
+    if (!beam || !elems) return fail(BT_ERR_INVALID, "bt_lattice_set: NULL argument");
+    if (n_elems < 1) return fail(BT_ERR_INVALID, "bt_lattice_set: n_elems < 1");
+    bool energy_changes = false;
+    double length = 0.0;
+    for (int32_t i = 0; i < n_elems; ++i) {
+        int rc = validate_element(elems[i], i);
+        if (rc != BT_OK) return rc;
+        if (elems[i].type == BT_SHORTRF && elems[i].p[0] * cos(elems[i].p[2] * (kPi / 180.0)) != 0.0) energy_changes = true;
+        length += elems[i].ds;
+    }
+    Beam &b = beam->b;
+    b.lattice.assign(elems, elems + n_elems);
+    b.energy_changes = energy_changes;
+    b.lattice_length = length;
+    b.table_valid = false;
+    return BT_OK;
+}
+
+int bt_track(bt_beam *beam, int32_t nturns) {
+    if (!beam) return fail(BT_ERR_INVALID, "bt_track: beam is NULL");
+    if (nturns < 0) return fail(BT_ERR_INVALID, "bt_track: nturns < 0");
+    Beam &b = beam->b;
+    if (b.lattice.empty()) return fail(BT_ERR_STATE, "bt_track: bt_lattice_set not called");
+    if (!b.has_ref) return fail(BT_ERR_STATE, "bt_track: bt_beam_set_ref not called");
+    if (nturns == 0) return BT_OK;
+    const size_t n_ops = b.lattice.size();
+
+    if (!b.energy_changes) {
+        // one table serves every turn
+        int rc = BT_OK;
+        if (!b.table_valid) {  // "uploaded once": reused until the lattice or the reference changes
+            std::vector<DevOp> ops(n_ops);
+            build_turn_table(b.lattice, b.gamma, ops.data());
+            rc = ensure_table(&b, n_ops);
+            if (rc != BT_OK) return rc;
+            // pageable source: the call returns after the source has been staged
+            BT_CUDA_TRY(cudaMemcpyAsync(b.d_table, ops.data(), n_ops * sizeof(DevOp), cudaMemcpyHostToDevice, b.stream));
+            b.table_valid = true;
+        }
+        rc = launch_track(&b, b.d_table, (int32_t)n_ops, nturns, 0);
+        if (rc != BT_OK) return rc;
+    } else {
+        // S3: per-turn tables; chunks of turns bounded by a table budget (16 MiB)
+        const size_t max_ops = ((size_t)16 << 20) / sizeof(DevOp);
+        int32_t chunk = (int32_t)(max_ops / n_ops);
+        if (chunk < 1) chunk = 1;
+        if (chunk > nturns) chunk = nturns;
+        b.table_valid = false;
+        int rc = ensure_table(&b, n_ops * (size_t)chunk);
+        if (rc != BT_OK) return rc;
+        std::vector<DevOp> ops(n_ops * (size_t)chunk);
+        double gamma = b.gamma;
+        for (int32_t done = 0; done < nturns; done += chunk) {
+            const int32_t nt = (nturns - done < chunk) ? (nturns - done) : chunk;
+            for (int32_t t = 0; t < nt; ++t) gamma = build_turn_table(b.lattice, gamma, ops.data() + (size_t)t * n_ops);
+            if (done > 0) BT_CUDA_TRY(cudaStreamSynchronize(b.stream));  // previous chunk still reads the table
+            BT_CUDA_TRY(cudaMemcpyAsync(b.d_table, ops.data(), n_ops * (size_t)nt * sizeof(DevOp), cudaMemcpyHostToDevice, b.stream));
+            rc = launch_track(&b, b.d_table, (int32_t)n_ops, nt, (int32_t)n_ops);
+            if (rc != BT_OK) return rc;
+        }
+        b.gamma = gamma;
+    }
+    b.s += b.lattice_length * (double)nturns;
+    b.turn += nturns;
+    return BT_OK;
+}
+
+int bt_track_last_launch(const bt_beam *beam, int32_t *grid_dim, int32_t *block_dim, int32_t *ppt, int32_t *smem) {
+    if (!beam) return fail(BT_ERR_INVALID, "bt_track_last_launch: beam is NULL");
+    const TrackLaunchInfo &li = beam->b.last_launch;
+    if (grid_dim) *grid_dim = li.grid;
+    if (block_dim) *block_dim = li.block;
+    if (ppt) *ppt = li.ppt;
+    if (smem) *smem = li.smem;
+    return BT_OK;
+}
+
+// ---- grid ---------------------------------------------------------------------------------------
+
+int bt_grid_create(bt_grid **out, int32_t nx, int32_t ny, int32_t nz, const double lo[3], const double d[3]) {
+    if (!out) return fail(BT_ERR_INVALID, "bt_grid_create: out is NULL");
+    *out = nullptr;
+    if (!lo || !d) return fail(BT_ERR_INVALID, "bt_grid_create: NULL argument");
+    if (nx < 2 || ny < 2 || nz < 2) return fail(BT_ERR_INVALID, "bt_grid_create: need >= 2 nodes per axis");
+    const int64_t nn = (int64_t)nx * ny * nz;
+    if (nn > ((int64_t)1 << 31) - 1) return fail(BT_ERR_INVALID, "bt_grid_create: nx*ny*nz overflows int32");
+    for (int a = 0; a < 3; ++a)
+        if (!(d[a] > 0.0) || !isfinite(d[a]) || !isfinite(lo[a])) return fail(BT_ERR_INVALID, "bt_grid_create: d <= 0 or not finite");
+    bt_grid *h = new (std::nothrow) bt_grid();
+    if (!h) return fail(BT_ERR_OOM, "bt_grid_create: host allocation failed");
+    Grid &g = h->g;
+    g.nx = nx;
+    g.ny = ny;
+    g.nz = nz;
+    g.nn = nn;
+    for (int a = 0; a < 3; ++a) {
+        g.lo[a] = lo[a];
+        g.d[a] = d[a];
+        g.inv_d[a] = 1.0 / d[a];  // R11: computed once on the host
+    }
+    cudaError_t e = cudaMalloc(&g.rho, (size_t)nn * sizeof(double));
+    if (e == cudaSuccess) e = cudaMemset(g.rho, 0, (size_t)nn * sizeof(double));
+    if (e != cudaSuccess) {
+        if (g.rho) cudaFree(g.rho);
+        delete h;
+        return fail(e == cudaErrorMemoryAllocation ? BT_ERR_OOM : BT_ERR_CUDA, std::string("bt_grid_create: ") + cudaGetErrorString(e));
+    }
+    *out = h;
+    return BT_OK;
+}
+
+void bt_grid_destroy(bt_grid *grid) {
+    if (!grid) return;
+    cudaDeviceSynchronize();
+    if (grid->g.rho) cudaFree(grid->g.rho);
+    if (grid->g.field) cudaFree(grid->g.field);
+    delete grid;
+}
+
+int bt_grid_set_field(bt_grid *grid, const double *Ex, const double *Ey, const double *Ez, int on_device) {
+    if (!grid || !Ex || !Ey || !Ez) return fail(BT_ERR_INVALID, "bt_grid_set_field: NULL argument");
+    Grid &g = grid->g;
+    const size_t bytes = (size_t)g.nn * sizeof(double);
+    if (!g.field) BT_CUDA_TRY(cudaMalloc(&g.field, bytes * 4));
+    cudaStream_t s = g.last_stream;
+    if (on_device) return launch_field_pack(&g, Ex, Ey, Ez, s);
+    double *tmp = nullptr;
+    BT_CUDA_TRY(cudaMalloc(&tmp, bytes * 3));
+    cudaError_t e = cudaMemcpyAsync(tmp, Ex, bytes, cudaMemcpyHostToDevice, s);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(tmp + g.nn, Ey, bytes, cudaMemcpyHostToDevice, s);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(tmp + 2 * g.nn, Ez, bytes, cudaMemcpyHostToDevice, s);
+    int rc = BT_OK;
+    if (e != cudaSuccess)
+        rc = fail(BT_ERR_CUDA, std::string("bt_grid_set_field: ") + cudaGetErrorString(e));
+    else
+        rc = launch_field_pack(&g, tmp, tmp + g.nn, tmp + 2 * g.nn, s);
+    cudaStreamSynchronize(s);
+    cudaFree(tmp);
+    return rc;
+}
+
+int bt_grid_rho(bt_grid *grid, double **dev_rho_out) {
+    if (!grid || !dev_rho_out) return fail(BT_ERR_INVALID, "bt_grid_rho: NULL argument");
+    *dev_rho_out = grid->g.rho;
+    return BT_OK;
+}
+
+int bt_grid_download_rho(bt_grid *grid, double *host_rho) {
+    if (!grid || !host_rho) return fail(BT_ERR_INVALID, "bt_grid_download_rho: NULL argument");
+    Grid &g = grid->g;
+    BT_CUDA_TRY(cudaMemcpyAsync(host_rho, g.rho, (size_t)g.nn * sizeof(double), cudaMemcpyDeviceToHost, g.last_stream));
+    BT_CUDA_TRY(cudaStreamSynchronize(g.last_stream));
+    return BT_OK;
+}
+
+int bt_deposit_cic(bt_beam *beam, bt_grid *grid, double q_weight, double zscale, int zero_first) {
+    if (!beam || !grid) return fail(BT_ERR_INVALID, "bt_deposit_cic: NULL argument");
+    if (!isfinite(q_weight) || !isfinite(zscale)) return fail(BT_ERR_INVALID, "bt_deposit_cic: q_weight or zscale not finite");
+    Beam &b = beam->b;
+    Grid &g = grid->g;
+    g.last_stream = b.stream;
+    if (zero_first) BT_CUDA_TRY(cudaMemsetAsync(g.rho, 0, (size_t)g.nn * sizeof(double), b.stream));
+    return launch_deposit(&b, &g, q_weight, zscale);
+}
+
+int bt_gather_kick(bt_beam *beam, const bt_grid *grid, const double coef[3], double zscale, double half_drift_before,
+                   double half_drift_after) {
+    if (!beam || !grid || !coef) return fail(BT_ERR_INVALID, "bt_gather_kick: NULL argument");
+    if (!isfinite(zscale) || !isfinite(coef[0]) || !isfinite(coef[1]) || !isfinite(coef[2]))
+        return fail(BT_ERR_INVALID, "bt_gather_kick: coef or zscale not finite");
+    if (!(half_drift_before >= 0.0) || !(half_drift_after >= 0.0) || !isfinite(half_drift_before) || !isfinite(half_drift_after))
+        return fail(BT_ERR_INVALID, "bt_gather_kick: negative or non-finite drift length");
+    Beam &b = beam->b;
+    const Grid &g = grid->g;
+    if (!g.field) return fail(BT_ERR_STATE, "bt_gather_kick: bt_grid_set_field not called");
+    if (!b.has_ref) return fail(BT_ERR_STATE, "bt_gather_kick: bt_beam_set_ref not called");
+    const double bg2 = b.gamma * b.gamma - 1.0;
+    const double bg = sqrt(bg2);
+    const double tcb = half_drift_before / (bg * bg), tca = half_drift_after / (bg * bg);  // R4
+    int rc = launch_gather_kick(&b, &g, coef, zscale, half_drift_before, tcb, half_drift_after, tca);
+    if (rc != BT_OK) return rc;
+    b.s += half_drift_before + half_drift_after;
+    return BT_OK;
+}
+
+}  // extern "C"

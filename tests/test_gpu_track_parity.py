@@ -1,0 +1,201 @@
+"""Parity of the fused lattice walk (bt_track, through the C-ABI) against the CPU oracle.
+
+Bar (BASELINE.json north_star, made well-posed by reading R14): for every coordinate c and particle i
+    |gpu - oracle| <= 1e-11 * max(|oracle_ci|, rms_c(oracle))        after the full run.
+"""
+import os
+
+import numpy as np
+import pytest
+
+import workloads as W
+from _gpu import gpu_track, oracle_track
+from _util import r14_error
+
+pytestmark = pytest.mark.gpu
+TOL = 1e-11
+
+
+def check(got, ref, tol=TOL):
+    errs = r14_error(got, ref)
+    assert max(errs) <= tol, dict(zip(W.COORD_NAMES, errs))
+    for g in got:
+        assert np.all(np.isfinite(g))
+    return errs
+
+
+def test_config0_tiny_fodo_full():
+    cfg = W.config(0)
+    c = W.make_bunch(cfg)
+    got, (g, s, turn), launch = gpu_track(cfg, c)
+    ref, (g_ref, s_ref) = oracle_track(cfg, c)
+    check(got, ref)
+    assert g == g_ref and abs(s - s_ref) < 1e-9 and turn == 10
+    assert np.array_equal(got[5], c[5])            # pt untouched by drifts and quads: bit exact
+
+
+# sizes: several 512-particle tiles (P=4 x 128 threads) plus a ragged tail, and sub-warp sizes
+@pytest.mark.parametrize("n", [1, 31, 33, 513, 4 * 128 * 5 + 77, 50_001])
+def test_config1_fodo_channel_reduced(n):
+    cfg = W.config(1, n=n)
+    c = W.make_bunch(cfg)
+    got, _, launch = gpu_track(cfg, c)
+    ref, _ = oracle_track(cfg, c)
+    check(got, ref)
+
+
+@pytest.mark.parametrize("ppt,src,block", [(1, 0, 32), (1, 1, 128), (2, 0, 64), (2, 1, 128), (4, 0, 128), (4, 1, 96)])
+def test_all_kernel_variants_agree(ppt, src, block, monkeypatch):
+    """Every (particles-per-thread, table source, block size) instantiation against the oracle, config-3 ring
+    (all op kinds except sbend/edge) and the chicane."""
+    monkeypatch.setenv("BT_TRACK_PPT", str(ppt))
+    monkeypatch.setenv("BT_TRACK_SRC", str(src))
+    monkeypatch.setenv("BT_TRACK_BLOCK", str(block))
+    n = 4 * 128 * 3 + 201
+    cfg = W.config(3, n=n)
+    c = W.make_bunch(cfg)
+    got, ref_state, launch = gpu_track(cfg, c, nturns=7)
+    assert launch["particles_per_thread"] == ppt and launch["block"] == block and (launch["smem_bytes"] > 0) == bool(src)
+    ref, (g_ref, _) = oracle_track(cfg, c, nturns=7)
+    check(got, ref)
+    assert abs(ref_state[0] - g_ref) <= 1e-15 * g_ref
+    cfg = W.config(2, n=n)
+    c = W.make_bunch(cfg)
+    got, _, _ = gpu_track(cfg, c)
+    ref, _ = oracle_track(cfg, c)
+    check(got, ref)
+
+
+def test_config2_chicane_reduced():
+    cfg = W.config(2, n=300_007)
+    c = W.make_bunch(cfg)
+    got, _, _ = gpu_track(cfg, c)
+    ref, _ = oracle_track(cfg, c)
+    check(got, ref)
+    assert abs(got[4].std() / c[4].std() - 0.4658) < 2e-3     # compression by |1 - 20 R56|
+
+
+def test_config3_ring_reduced_100_turns():
+    cfg = W.config(3, n=20_003)
+    c = W.make_bunch(cfg)
+    got, (g, s, turn), _ = gpu_track(cfg, c)
+    ref, (g_ref, s_ref) = oracle_track(cfg, c)
+    errs = check(got, ref)
+    assert abs(g - g_ref) <= 1e-15 * g_ref and abs(s - 7500.0) < 1e-6 and turn == 100
+    assert abs(g - 2.1580889531834284) < 1e-12       # gamma after 100 turns
+
+
+def test_general_multipoles_sbend_slices_and_skew():
+    """Ops that no BASELINE config exercises: general-order / skew multipoles (OP_MULT), sliced sbend, sliced drift,
+    k = 0 quad, dipole kick."""
+    lat = [("drift", 0.3, 3), ("quad", 0.4, 2, 0.0), ("sbend", 0.9, 4, 3.0), ("dipedge", 0.0, 1, 0.1, 3.0, 0.01, 0.45),
+           ("multipole", 0.0, 1, 1, 1e-4, -2e-4), ("multipole", 0.0, 1, 2, 0.3, 0.1), ("multipole", 0.0, 1, 3, 4.0, 2.0),
+           ("multipole", 0.0, 1, 4, 30.0, -10.0), ("multipole", 0.0, 1, 5, 1e3, 5e2), ("multipole", 0.0, 1, 10, 1e9, 1e9),
+           ("sbend", 0.9, 1, -3.0), ("quad", 0.5, 7, -2.0), ("shortrf", 0.0, 1, 1e-3, 1e8, -90.0), ("drift", 1.0, 1)]
+    cfg = W.config(0, n=3000)
+    c = W.make_bunch(cfg)
+    got, _, _ = gpu_track(cfg, c, nturns=3, lattice=lat)
+    ref, _ = oracle_track(cfg, c, nturns=3, lattice=lat)
+    check(got, ref)
+
+
+def test_repeated_calls_continue_and_zero_turns():
+    import paper_2208_02382_b200 as bt
+    cfg = W.config(3, n=1000)
+    c = W.make_bunch(cfg)
+    beam = bt.Beam(cfg.n)
+    beam.set_ref(cfg.kin_energy_MeV, cfg.mass_MeV, 1.0)
+    beam.lattice_set(cfg.lattice)
+    beam.upload(c)
+    beam.track(0)
+    assert all(np.array_equal(a, b) for a, b in zip(beam.download(), c))
+    beam.track(2)
+    beam.track(3)
+    got = beam.download()
+    ref, (g_ref, _) = oracle_track(cfg, c, nturns=5)
+    check(got, ref)
+    assert beam.get_ref()[2] == 5 and abs(beam.get_ref()[0] - g_ref) < 1e-15 * g_ref
+    # bit-reproducible run to run
+    beam.upload(c)
+    beam.set_ref(cfg.kin_energy_MeV, cfg.mass_MeV, 1.0)
+    beam.track(5)
+    again = beam.download()
+    assert all(np.array_equal(a, b) for a, b in zip(got, again))
+    beam.close()
+
+
+def test_borrowed_unaligned_and_library_storage():
+    import torch
+    cfg = W.config(1, n=5000)
+    cfg.lattice = W.fodo_cell(25) * 2
+    c = W.make_bunch(cfg)
+    ref, _ = oracle_track(cfg, c)
+    # borrowed tensors whose data pointers are only 8-byte aligned -> scalar path
+    backing = [torch.empty(cfg.n + 1, dtype=torch.float64, device="cuda") for _ in range(6)]
+    views = [b[1:] for b in backing]
+    got, _, launch = gpu_track(cfg, c, storage=views)
+    assert launch["particles_per_thread"] == 1
+    check(got, ref)
+    assert all(np.array_equal(v.cpu().numpy(), g) for v, g in zip(views, got))      # zero-copy view sees the result
+    got, _, _ = gpu_track(cfg, c, storage="library")
+    check(got, ref)
+
+
+def test_error_paths_on_device():
+    import paper_2208_02382_b200 as bt
+    beam = bt.Beam(100)
+    with pytest.raises(bt.BtError) as ei:
+        beam.track(1)
+    assert ei.value.code == bt.BT_ERR_STATE
+    beam.lattice_set(W.fodo_cell(2))
+    with pytest.raises(bt.BtError) as ei:
+        beam.track(1)
+    assert ei.value.code == bt.BT_ERR_STATE          # no reference particle yet
+    for bad in ([("quad", 1.0, 0, 1.0)], [("sbend", 1.0, 1, 0.0)], [("multipole", 0.0, 1, 11, 1.0, 0.0)],
+                [("dipedge", 0.0, 2, 0.1, 1.0, 0.0, 0.0)], [("drift", -1.0, 1)], [(9, 1.0, 1)]):
+        with pytest.raises(bt.BtError) as ei:
+            beam.lattice_set(bad)
+        assert ei.value.code == bt.BT_ERR_INVALID
+    with pytest.raises(bt.BtError):
+        beam.set_ref(-1.0, 1.0)
+    beam.close()
+
+
+# ---- BASELINE full sizes, in the launch configuration bench.py times ------------------------------------
+def test_config1_full_size_every_particle():
+    cfg = W.config(1)
+    c = W.make_bunch(cfg)
+    got, _, launch = gpu_track(cfg, c)
+    ref, _ = oracle_track(cfg, c)
+    check(got, ref)
+    assert launch["particles_per_thread"] == 4
+
+
+def test_config2_full_size_every_particle():
+    cfg = W.config(2)
+    c = W.make_bunch(cfg)
+    got, _, _ = gpu_track(cfg, c)
+    ref, _ = oracle_track(cfg, c)
+    check(got, ref)
+
+
+@pytest.mark.skipif(os.environ.get("BT_SKIP_HUGE") == "1", reason="BT_SKIP_HUGE=1")
+def test_config3_full_size_sampled():
+    """64M particles x 100 turns on the GPU; the oracle tracks the strided subset i % 64 == 0 (particles are
+    independent, so the subset's result is the full run's result for those particles) + global invariants."""
+    cfg = W.config(3)
+    c = W.make_bunch(cfg)
+    got, (g, s, turn), _ = gpu_track(cfg, c)
+    sub = [a[::64].copy() for a in c]
+    del c
+    ref, (g_ref, _) = oracle_track(cfg, sub)
+    check([a[::64] for a in got], ref)
+    assert abs(g - g_ref) <= 1e-15 * g_ref and turn == 100
+    for a in got:
+        assert np.all(np.isfinite(a))
+    # normalised transverse emittances stay within a few % (nonlinear ring, no losses)
+    from _util import rms_emittance
+    bg = np.sqrt(g * g - 1)
+    bg0 = 1.807618289845165
+    ex = rms_emittance(got[0], got[1]) * bg / bg0
+    assert 0.9e-6 < ex < 1.5e-6
