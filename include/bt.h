@@ -23,7 +23,9 @@
  *  - Arguments are validated before anything is launched; an invalid call changes no state.
  *  - There is no CPU fallback: without a CUDA device every entry point that touches the device
  *    fails with BT_ERR_CUDA.
- *  - Particle order seen through bt_beam_download / bt_beam_ptrs never changes.
+ *  - Particle order seen through bt_beam_upload / bt_beam_download never changes.  bt_beam_ptrs exposes the
+ *    STORAGE order, which equals the caller's order unless the caller has asked for bt_beam_sort_by_cell
+ *    (then bt_beam_ids maps storage slots to original indices).
  *  - NaN/Inf coordinates are not checked on the hot path; in deposit/gather they count as
  *    "outside the grid" (R13).
  */
@@ -114,6 +116,21 @@ int bt_beam_download(const bt_beam *beam, double *const host[6]);
 /* Zero-copy view of the 6 device arrays (P:l.102 "zero-copy access"); valid until bt_beam_destroy. */
 int bt_beam_ptrs(bt_beam *beam, double *dev_ptrs_out[6]);
 int64_t bt_beam_size(const bt_beam *beam);
+
+/*
+ * Cell binning (S4; B:north_star "bins particles by cell").  Physically reorders the beam's six arrays by
+ * the linear index (k*ny + j)*nx + i of each particle's lower-corner node on `grid` (R11 canonical index,
+ * third axis zscale*t; particles outside the grid go last), by a counting sort on the beam's stream.
+ * Opt-in and purely a performance hint: bt_deposit_cic then accumulates runs of same-cell particles in
+ * registers before touching rho, and bt_gather_kick finds its nodes in L1; both remain correct for any order,
+ * so the sort may be repeated at any cadence (particles move a small fraction of a cell per step).
+ * bt_beam_download still returns the original order; bt_beam_upload resets storage to the caller's order.
+ * The order of particles within one cell is not deterministic.  Needs n < 2^31; allocates 24 bytes per
+ * particle of scratch on first use.
+ */
+int bt_beam_sort_by_cell(bt_beam *beam, const bt_grid *grid, double zscale);
+/* Device array of n int32: ids[j] = original index of storage slot j; NULL while storage order == original order. */
+int bt_beam_ids(bt_beam *beam, int32_t **dev_ids_out);
 
 /* ---- lattice (S1) and fused walk (S2, S3) --------------------------------------------------- */
 

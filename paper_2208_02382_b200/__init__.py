@@ -43,6 +43,8 @@ EXPORTS = {
     "bt_beam_download": (C.c_int, [_vp, C.POINTER(_vp)]),
     "bt_beam_ptrs": (C.c_int, [_vp, C.POINTER(_vp)]),
     "bt_beam_size": (C.c_int64, [_vp]),
+    "bt_beam_sort_by_cell": (C.c_int, [_vp, _vp, C.c_double]),
+    "bt_beam_ids": (C.c_int, [_vp, C.POINTER(_vp)]),
     "bt_lattice_set": (C.c_int, [_vp, _vp, C.c_int32]),
     "bt_track": (C.c_int, [_vp, C.c_int32]),
     "bt_grid_create": (C.c_int, [C.POINTER(_vp), C.c_int32, C.c_int32, C.c_int32, _dp, _dp]),
@@ -209,6 +211,14 @@ class Beam:
     def gather_kick(self, grid, coef, zscale=1.0, half_drift_before=0.0, half_drift_after=0.0):
         c = (C.c_double * 3)(*coef)
         _check(lib.bt_gather_kick(self._h, grid._h, c, zscale, half_drift_before, half_drift_after), "bt_gather_kick")
+
+    def sort_by_cell(self, grid, zscale=1.0):
+        _check(lib.bt_beam_sort_by_cell(self._h, grid._h, zscale), "bt_beam_sort_by_cell")
+
+    def ids_ptr(self):
+        p = _vp()
+        _check(lib.bt_beam_ids(self._h, C.byref(p)), "bt_beam_ids")
+        return int(p.value) if p.value else 0
 
     def sync(self):
         _check(lib.bt_sync(self._h), "bt_sync")

@@ -233,6 +233,10 @@ void bt_beam_destroy(bt_beam *beam) {
     cudaStreamSynchronize(b.stream);
     if (b.owns && b.q[0]) cudaFree(b.q[0]);
     if (b.d_table) cudaFree(b.d_table);
+    int *ibufs[] = {b.ids, b.ids_tmp, b.sort_key, b.sort_dest, b.sort_count, b.sort_block_sum};
+    for (int *p : ibufs)
+        if (p) cudaFree(p);
+    if (b.scratch) cudaFree(b.scratch);
     delete beam;
 }
 
@@ -270,6 +274,7 @@ int bt_beam_upload(bt_beam *beam, const double *const host[6]) {
     Beam &b = beam->b;
     for (int i = 0; i < 6; ++i)
         BT_CUDA_TRY(cudaMemcpyAsync(b.q[i], host[i], (size_t)b.n * sizeof(double), cudaMemcpyHostToDevice, b.stream));
+    b.permuted = false;  // storage order = the caller's order again
     return BT_OK;
 }
 
@@ -277,9 +282,16 @@ int bt_beam_download(const bt_beam *beam, double *const host[6]) {
     if (!beam || !host) return fail(BT_ERR_INVALID, "bt_beam_download: NULL argument");
     for (int i = 0; i < 6; ++i)
         if (!host[i]) return fail(BT_ERR_INVALID, "bt_beam_download: host has a NULL entry");
-    const Beam &b = beam->b;
-    for (int i = 0; i < 6; ++i)
-        BT_CUDA_TRY(cudaMemcpyAsync(host[i], b.q[i], (size_t)b.n * sizeof(double), cudaMemcpyDeviceToHost, b.stream));
+    Beam &b = const_cast<Beam &>(beam->b);
+    for (int i = 0; i < 6; ++i) {
+        const double *src = b.q[i];
+        if (b.permuted) {  // storage is cell-sorted: restore the original order through the scratch array
+            int rc = unpermute_to(&b, i, b.scratch);
+            if (rc != BT_OK) return rc;
+            src = b.scratch;
+        }
+        BT_CUDA_TRY(cudaMemcpyAsync(host[i], src, (size_t)b.n * sizeof(double), cudaMemcpyDeviceToHost, b.stream));
+    }
     BT_CUDA_TRY(cudaStreamSynchronize(b.stream));
     return BT_OK;
 }
@@ -287,6 +299,18 @@ int bt_beam_download(const bt_beam *beam, double *const host[6]) {
 int bt_beam_ptrs(bt_beam *beam, double *dev_ptrs_out[6]) {
     if (!beam || !dev_ptrs_out) return fail(BT_ERR_INVALID, "bt_beam_ptrs: NULL argument");
     for (int i = 0; i < 6; ++i) dev_ptrs_out[i] = beam->b.q[i];
+    return BT_OK;
+}
+
+int bt_beam_sort_by_cell(bt_beam *beam, const bt_grid *grid, double zscale) {
+    if (!beam || !grid) return fail(BT_ERR_INVALID, "bt_beam_sort_by_cell: NULL argument");
+    if (!isfinite(zscale)) return fail(BT_ERR_INVALID, "bt_beam_sort_by_cell: zscale not finite");
+    return sort_by_cell(&beam->b, &grid->g, zscale);
+}
+
+int bt_beam_ids(bt_beam *beam, int32_t **dev_ids_out) {
+    if (!beam || !dev_ids_out) return fail(BT_ERR_INVALID, "bt_beam_ids: NULL argument");
+    *dev_ids_out = beam->b.permuted ? beam->b.ids : nullptr;
     return BT_OK;
 }
 

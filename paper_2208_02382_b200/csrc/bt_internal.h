@@ -71,6 +71,12 @@ struct Beam {
     size_t d_table_cap = 0;    // in DevOps
     bool table_valid = false;  // d_table holds the single-turn table for the current lattice and gamma
     TrackLaunchInfo last_launch;
+    // S4 cell binning: storage order != original order once sorted; ids[j] = original index of slot j
+    bool permuted = false;
+    int *ids = nullptr, *ids_tmp = nullptr;
+    int *sort_key = nullptr, *sort_dest = nullptr, *sort_count = nullptr, *sort_block_sum = nullptr;
+    long long sort_count_cap = 0;
+    double *scratch = nullptr;  // one array of n doubles
 };
 
 struct Grid {
@@ -91,6 +97,8 @@ int launch_track(Beam *b, const DevOp *d_table, int32_t n_ops, int32_t nturns, i
 int launch_deposit(Beam *b, Grid *g, double q_weight, double zscale);
 int launch_gather_kick(Beam *b, const Grid *g, const double coef[3], double zscale, double h_before,
                        double tc_before, double h_after, double tc_after);
+int sort_by_cell(Beam *b, const Grid *g, double zscale);
+int unpermute_to(Beam *b, int c, double *out);  // out[ids[j]] = q[c][j] on the beam's stream
 int launch_field_pack(Grid *g, const double *ex, const double *ey, const double *ez, cudaStream_t s);
 
 }  // namespace bt

@@ -7,53 +7,12 @@
 //   i = floor(u), w1 = u - i (exact), w0 = 1 - w1 ; node weight (wx*wy)*wz.
 // Inside iff 0 <= i <= n-2 on all axes, tested as (u >= 0 && u < n-1) so NaN is outside (R13).
 #include "bt_internal.h"
+#include "grid_dev.cuh"
 
+#include <math_constants.h>
 #include <stdlib.h>
 
 namespace bt {
-
-struct GridDev {
-    double lo[3], inv_d[3];
-    double umax[3];  // (double)(n-1)
-    int nx, ny, nz;
-};
-
-static GridDev make_grid_dev(const Grid &g) {
-    GridDev d;
-    for (int a = 0; a < 3; ++a) {
-        d.lo[a] = g.lo[a];
-        d.inv_d[a] = g.inv_d[a];
-    }
-    d.umax[0] = (double)(g.nx - 1);
-    d.umax[1] = (double)(g.ny - 1);
-    d.umax[2] = (double)(g.nz - 1);
-    d.nx = g.nx;
-    d.ny = g.ny;
-    d.nz = g.nz;
-    return d;
-}
-
-struct Cic {
-    int i, j, k;
-    double wx1, wy1, wz1;
-};
-
-__device__ __forceinline__ bool cic_axis(double q, double lo, double inv_d, double umax, int &i, double &w1) {
-    const double u = __dmul_rn(__dsub_rn(q, lo), inv_d);
-    const bool in = (u >= 0.0) && (u < umax);
-    const double fl = floor(u);
-    i = in ? __double2int_rd(u) : 0;
-    w1 = __dsub_rn(u, fl);
-    return in;
-}
-
-__device__ __forceinline__ bool cic_locate(const GridDev &g, double x, double y, double t, double zscale, Cic &c) {
-    const double zeta = __dmul_rn(zscale, t);
-    const bool ix = cic_axis(x, g.lo[0], g.inv_d[0], g.umax[0], c.i, c.wx1);
-    const bool iy = cic_axis(y, g.lo[1], g.inv_d[1], g.umax[1], c.j, c.wy1);
-    const bool iz = cic_axis(zeta, g.lo[2], g.inv_d[2], g.umax[2], c.k, c.wz1);
-    return ix && iy && iz;
-}
 
 // ---- S5 deposit, mode 0: one particle per thread, 8 global fp64 reductions (RED.E.ADD.F64) --------
 __global__ void __launch_bounds__(256) deposit_atomic_kernel(const double *__restrict__ x, const double *__restrict__ y,
@@ -79,13 +38,131 @@ __global__ void __launch_bounds__(256) deposit_atomic_kernel(const double *__res
     }
 }
 
+// ---- S5 deposit, mode 1 (default): run accumulation in registers + warp-segmented merge ------------
+// A warp owns chunks of 32*kRun consecutive particles (storage order); lane L walks particles
+// [L*kRun, (L+1)*kRun) of the chunk and keeps the 8 node sums of the CURRENT cell in registers, flushing
+// them with 8 RED.E.ADD.F64 only when the cell changes.  At the end of the chunk the lanes' open runs are
+// merged by a segmented shuffle reduction over equal cell keys (contiguous after bt_beam_sort_by_cell), so a
+// chunk that sits in one cell costs 8 global reductions for 256 particles.  Correct for ANY particle order:
+// unsorted input just degenerates to one flush per particle.  Weights are the canonical R11 expression, so
+// only the summation order differs from the definition.
+constexpr int kRun = 8;
+
+__device__ __forceinline__ void flush_cell(double *__restrict__ rho, int key, const double (&acc)[8], int nx, long long nxy) {
+    if (key < 0) return;
+    double *base = rho + key;  // key = linear index of the lower-corner node
+    atomicAdd(base, acc[0]);
+    atomicAdd(base + 1, acc[1]);
+    atomicAdd(base + nx, acc[2]);
+    atomicAdd(base + nx + 1, acc[3]);
+    atomicAdd(base + nxy, acc[4]);
+    atomicAdd(base + nxy + 1, acc[5]);
+    atomicAdd(base + nxy + nx, acc[6]);
+    atomicAdd(base + nxy + nx + 1, acc[7]);
+}
+
+template <bool VEC>
+__global__ void __launch_bounds__(256) deposit_runs_kernel(const double *__restrict__ x, const double *__restrict__ y,
+                                                           const double *__restrict__ t, long long n, GridDev g, double qw,
+                                                           double zscale, double *__restrict__ rho) {
+    const int lane = threadIdx.x & 31;
+    const long long warp = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+    const long long nwarps = ((long long)gridDim.x * blockDim.x) >> 5;
+    const long long chunk = 32LL * kRun;
+    const long long nxy = (long long)g.nx * g.ny;
+    for (long long c0 = warp * chunk; c0 < n; c0 += nwarps * chunk) {
+        const long long p0 = c0 + (long long)lane * kRun;
+        double px_[kRun], py_[kRun], pt_[kRun];
+        if (VEC && p0 + kRun <= n) {
+#pragma unroll
+            for (int r = 0; r < kRun; r += 2) {
+                const double2 a = __ldcs(reinterpret_cast<const double2 *>(x + p0 + r));
+                const double2 b = __ldcs(reinterpret_cast<const double2 *>(y + p0 + r));
+                const double2 c = __ldcs(reinterpret_cast<const double2 *>(t + p0 + r));
+                px_[r] = a.x, px_[r + 1] = a.y, py_[r] = b.x, py_[r + 1] = b.y, pt_[r] = c.x, pt_[r + 1] = c.y;
+            }
+        } else {
+#pragma unroll
+            for (int r = 0; r < kRun; ++r) {
+                const bool live = p0 + r < n;
+                px_[r] = live ? x[p0 + r] : CUDART_NAN;  // NaN => outside => contributes nothing
+                py_[r] = live ? y[p0 + r] : 0.0;
+                pt_[r] = live ? t[p0 + r] : 0.0;
+            }
+        }
+        int cur = -1;
+        double acc[8];
+#pragma unroll
+        for (int d = 0; d < 8; ++d) acc[d] = 0.0;
+#pragma unroll
+        for (int r = 0; r < kRun; ++r) {
+            Cic c;
+            const bool in = cic_locate(g, px_[r], py_[r], pt_[r], zscale, c);
+            const int key = in ? (c.k * g.ny + c.j) * g.nx + c.i : -1;
+            const double wx0 = __dsub_rn(1.0, c.wx1), wy0 = __dsub_rn(1.0, c.wy1), wz0 = __dsub_rn(1.0, c.wz1);
+            double w[8];
+            w[0] = __dmul_rn(qw, __dmul_rn(__dmul_rn(wx0, wy0), wz0));
+            w[1] = __dmul_rn(qw, __dmul_rn(__dmul_rn(c.wx1, wy0), wz0));
+            w[2] = __dmul_rn(qw, __dmul_rn(__dmul_rn(wx0, c.wy1), wz0));
+            w[3] = __dmul_rn(qw, __dmul_rn(__dmul_rn(c.wx1, c.wy1), wz0));
+            w[4] = __dmul_rn(qw, __dmul_rn(__dmul_rn(wx0, wy0), c.wz1));
+            w[5] = __dmul_rn(qw, __dmul_rn(__dmul_rn(c.wx1, wy0), c.wz1));
+            w[6] = __dmul_rn(qw, __dmul_rn(__dmul_rn(wx0, c.wy1), c.wz1));
+            w[7] = __dmul_rn(qw, __dmul_rn(__dmul_rn(c.wx1, c.wy1), c.wz1));
+            if (key != cur) {
+                flush_cell(rho, cur, acc, g.nx, nxy);
+                cur = key;
+#pragma unroll
+                for (int d = 0; d < 8; ++d) acc[d] = w[d];
+            } else if (in) {
+#pragma unroll
+                for (int d = 0; d < 8; ++d) acc[d] += w[d];
+            }
+        }
+        // merge the lanes' open runs: segmented suffix reduction over CONTIGUOUS equal keys (after a cell
+        // sort equal keys are contiguous; for arbitrary order non-adjacent equal keys stay separate runs)
+        const int prev = __shfl_up_sync(0xffffffffu, cur, 1);
+        const bool head = (lane == 0) || (prev != cur);
+        const unsigned heads = __ballot_sync(0xffffffffu, head);
+        const unsigned above = (lane == 31) ? 0u : (heads >> (lane + 1));
+        const int end = above ? lane + __ffs(above) - 1 : 31;  // last lane of this lane's run
+#pragma unroll
+        for (int d = 1; d < 32; d <<= 1) {
+            const bool take = lane + d <= end;
+#pragma unroll
+            for (int k = 0; k < 8; ++k) {
+                const double o = __shfl_down_sync(0xffffffffu, acc[k], d);
+                if (take) acc[k] += o;
+            }
+        }
+        if (head) flush_cell(rho, cur, acc, g.nx, nxy);
+    }
+}
+
+static int env_int_grid(const char *name, int dflt) {
+    const char *v = getenv(name);
+    return (v && *v) ? atoi(v) : dflt;
+}
+
 int launch_deposit(Beam *b, Grid *g, double q_weight, double zscale) {
     const GridDev gd = make_grid_dev(*g);
+    const int mode = env_int_grid("BT_DEPOSIT_MODE", 1);
     const int block = 256;
-    long long blocks = (b->n + block - 1) / block;
-    const long long cap = (long long)b->num_sms * 16;
-    if (blocks > cap) blocks = cap;
-    deposit_atomic_kernel<<<(int)blocks, block, 0, b->stream>>>(b->q[0], b->q[2], b->q[4], b->n, gd, q_weight, zscale, g->rho);
+    if (mode == 0) {
+        long long blocks = (b->n + block - 1) / block;
+        const long long cap = (long long)b->num_sms * 16;
+        if (blocks > cap) blocks = cap;
+        deposit_atomic_kernel<<<(int)blocks, block, 0, b->stream>>>(b->q[0], b->q[2], b->q[4], b->n, gd, q_weight, zscale, g->rho);
+    } else {
+        const long long per_block = (long long)block * kRun;
+        long long blocks = (b->n + per_block - 1) / per_block;
+        const long long cap = (long long)b->num_sms * 8;
+        if (blocks > cap) blocks = cap;
+        if (b->aligned16)
+            deposit_runs_kernel<true><<<(int)blocks, block, 0, b->stream>>>(b->q[0], b->q[2], b->q[4], b->n, gd, q_weight, zscale, g->rho);
+        else
+            deposit_runs_kernel<false><<<(int)blocks, block, 0, b->stream>>>(b->q[0], b->q[2], b->q[4], b->n, gd, q_weight, zscale, g->rho);
+    }
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return fail(BT_ERR_CUDA, std::string("bt_deposit_cic launch: ") + cudaGetErrorString(e));
     g_launch_count.fetch_add(1);
@@ -122,9 +199,7 @@ struct GatherArgs {
 };
 
 __device__ __forceinline__ void ld_node(const double *f, double &ex, double &ey, double &ez) {
-    double pad;
-    asm volatile("ld.global.nc.v4.f64 {%0,%1,%2,%3}, [%4];" : "=d"(ex), "=d"(ey), "=d"(ez), "=d"(pad) : "l"(f));
-    (void)pad;
+    asm volatile("{ .reg .f64 pad; ld.global.nc.v4.f64 {%0,%1,%2,pad}, [%3]; }" : "=d"(ex), "=d"(ey), "=d"(ez) : "l"(f));
 }
 
 __global__ void __launch_bounds__(256) gather_kick_kernel(const __grid_constant__ GatherArgs a) {

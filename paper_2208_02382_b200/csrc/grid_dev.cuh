@@ -1,0 +1,55 @@
+// Device-side grid description and the canonical CIC index/weights (R11, R13), shared by grid.cu and sort.cu.
+//   u = (q - lo) * inv_d   (one rounded subtract, one rounded multiply; explicit _rn intrinsics so that nvcc
+//                           can never contract zscale*t - lo into an FMA)
+//   i = floor(u), w1 = u - i (exact), w0 = 1 - w1 ; node weight (wx*wy)*wz.
+// Inside iff 0 <= i <= n-2 on all axes, tested as (u >= 0 && u < n-1) so NaN is outside.
+#pragma once
+#include "bt_internal.h"
+
+namespace bt {
+
+struct GridDev {
+    double lo[3], inv_d[3];
+    double umax[3];  // (double)(n-1)
+    int nx, ny, nz;
+};
+
+static inline GridDev make_grid_dev(const Grid &g) {
+    GridDev d;
+    for (int a = 0; a < 3; ++a) {
+        d.lo[a] = g.lo[a];
+        d.inv_d[a] = g.inv_d[a];
+    }
+    d.umax[0] = (double)(g.nx - 1);
+    d.umax[1] = (double)(g.ny - 1);
+    d.umax[2] = (double)(g.nz - 1);
+    d.nx = g.nx;
+    d.ny = g.ny;
+    d.nz = g.nz;
+    return d;
+}
+
+struct Cic {
+    int i, j, k;
+    double wx1, wy1, wz1;
+};
+
+__device__ __forceinline__ bool cic_axis(double q, double lo, double inv_d, double umax, int &i, double &w1) {
+    const double u = __dmul_rn(__dsub_rn(q, lo), inv_d);
+    const bool in = (u >= 0.0) && (u < umax);
+    const double fl = floor(u);
+    i = in ? __double2int_rd(u) : 0;
+    w1 = __dsub_rn(u, fl);
+    return in;
+}
+
+__device__ __forceinline__ bool cic_locate(const GridDev &g, double x, double y, double t, double zscale, Cic &c) {
+    const double zeta = __dmul_rn(zscale, t);
+    const bool ix = cic_axis(x, g.lo[0], g.inv_d[0], g.umax[0], c.i, c.wx1);
+    const bool iy = cic_axis(y, g.lo[1], g.inv_d[1], g.umax[1], c.j, c.wy1);
+    const bool iz = cic_axis(zeta, g.lo[2], g.inv_d[2], g.umax[2], c.k, c.wz1);
+    return ix && iy && iz;
+}
+
+
+}  // namespace bt

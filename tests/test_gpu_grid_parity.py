@@ -208,3 +208,107 @@ def test_config4_full_size(variant):
     assert max(r14_error(got, ref)) <= 1e-11
     beam.close()
     grid.close()
+
+
+# ---- S4 cell binning ---------------------------------------------------------------------------------
+def _cell_keys(c, sc, zscale=1.0):
+    """Host restatement of the canonical index, for checking sortedness only."""
+    u = [(c[0] - sc.lo[0]) * (1.0 / sc.d[0]), (c[2] - sc.lo[1]) * (1.0 / sc.d[1]), (zscale * c[4] - sc.lo[2]) * (1.0 / sc.d[2])]
+    nx, ny, nz = sc.shape
+    inside = np.ones(len(c[0]), dtype=bool)
+    for a, n in zip(u, (nx, ny, nz)):
+        inside &= (a >= 0) & (a < n - 1)
+    ijk = [np.where(inside, np.floor(np.where(inside, a, 0.0)), 0).astype(np.int64) for a in u]
+    return np.where(inside, (ijk[2] * ny + ijk[1]) * nx + ijk[0], nx * ny * nz)
+
+
+@pytest.mark.parametrize("variant,n,shape", [("A", 1, (8, 8, 8)), ("A", 1023, (8, 8, 8)), ("A", 300_001, (32, 32, 32)),
+                                               ("B", 300_001, (32, 32, 32)), ("A", 500_000, (128, 128, 128))])
+def test_sort_by_cell_orders_storage_and_keeps_api_order(variant, n, shape):
+    import torch
+    sc = W.spacecharge_config(variant, n=n, shape=shape)
+    c = W.make_spacecharge_bunch(sc)
+    if n > 100:
+        c[0][:7] = [1.0, np.nan, -1.0, np.inf, 0.0, 5.9e-3, -5.9e-3]      # some outside particles
+    E = W.gaussian_bunch_field(sc)
+    beam = bt.Beam(n)
+    grid = bt.Grid(sc.shape, sc.lo, sc.d)
+    beam.set_ref(sc.kin_energy_MeV, sc.mass_MeV, 1.0)
+    grid.set_field(*E)
+    beam.upload(c)
+    assert beam.ids_ptr() == 0
+    beam.sort_by_cell(grid, sc.zscale)
+    # API order unchanged, bit for bit
+    back = beam.download()
+    for a, b in zip(back, c):
+        assert np.array_equal(a, b, equal_nan=True)
+    # storage order sorted by cell key; ids is a permutation consistent with the data
+    stored = [t.cpu().numpy() for t in beam.tensors]
+    keys = _cell_keys(stored, sc, sc.zscale)
+    assert np.all(np.diff(keys) >= 0)
+    assert beam.ids_ptr() != 0
+    ids = np.empty(n, dtype=np.int32)
+    import ctypes
+    torch.cuda.synchronize()
+    ids_t = torch.empty(n, dtype=torch.int32, device="cuda")
+    ctypes.cdll.LoadLibrary("libcudart.so").cudaMemcpy(ctypes.c_void_p(ids_t.data_ptr()), ctypes.c_void_p(beam.ids_ptr()), ctypes.c_size_t(4 * n), 3)
+    ids = ids_t.cpu().numpy()
+    assert np.array_equal(np.sort(ids), np.arange(n))
+    assert np.array_equal(stored[1], c[1][ids])
+    # deposit + gather on sorted storage == oracle on the original order
+    beam.deposit_cic(grid, sc.q_weight, sc.zscale, True)
+    rho = grid.download_rho()
+    ref_rho, n_in = O.deposit_cic(c[0], c[2], c[4], sc.shape, sc.lo, sc.d, sc.q_weight, sc.zscale)
+    assert r15_isolated(rho, ref_rho) <= 1e-12
+    beam.gather_kick(grid, sc.kick_coef, sc.zscale, 0.0, sc.ds)
+    beam.sort_by_cell(grid, sc.zscale)            # sorting twice composes the permutations
+    got = beam.download()
+    ref = [a.copy() for a in c]
+    O.gather_kick(ref, sc.shape, sc.lo, sc.d, E, sc.kick_coef, sc.zscale)
+    O.track(ref, [("drift", sc.ds, 1)], 1, O.ref_from_kinetic(sc.kin_energy_MeV, sc.mass_MeV)[0])
+    ok = np.isfinite(ref[0])
+    assert max(r14_error([a[ok] for a in got], [a[ok] for a in ref])) <= 1e-11
+    # upload resets the storage order
+    beam.upload(c)
+    assert beam.ids_ptr() == 0
+    beam.close()
+    grid.close()
+
+
+def test_sorted_tracking_still_matches():
+    """bt_track on cell-sorted storage: download must still be the original order."""
+    cfg = W.config(0, n=5000)
+    c = W.make_bunch(cfg)
+    sc = W.spacecharge_config("A", n=5000, shape=(16, 16, 16))
+    beam = bt.Beam(cfg.n)
+    grid = bt.Grid(sc.shape, sc.lo, sc.d)
+    beam.set_ref(cfg.kin_energy_MeV, cfg.mass_MeV, 1.0)
+    beam.lattice_set(cfg.lattice)
+    beam.upload(c)
+    beam.sort_by_cell(grid, 1.0)
+    beam.track(3)
+    got = beam.download()
+    from _gpu import oracle_track
+    ref, _ = oracle_track(cfg, c, nturns=3)
+    assert max(r14_error(got, ref)) <= 1e-11
+    beam.close()
+    grid.close()
+
+
+@pytest.mark.parametrize("mode", [0, 1])
+@pytest.mark.parametrize("variant", ["A", "B"])
+def test_deposit_modes_unaligned(mode, variant, monkeypatch):
+    import torch
+    monkeypatch.setenv("BT_DEPOSIT_MODE", str(mode))
+    sc = W.spacecharge_config(variant, n=70_001, shape=(32, 32, 32))
+    c = W.make_spacecharge_bunch(sc)
+    backing = [torch.empty(sc.n + 1, dtype=torch.float64, device="cuda") for _ in range(6)]
+    beam = bt.Beam(sc.n, storage=[b[1:] for b in backing])
+    grid = bt.Grid(sc.shape, sc.lo, sc.d)
+    beam.upload(c)
+    beam.deposit_cic(grid, sc.q_weight, sc.zscale, True)
+    rho = grid.download_rho()
+    ref_rho, _ = O.deposit_cic(c[0], c[2], c[4], sc.shape, sc.lo, sc.d, sc.q_weight, sc.zscale)
+    assert r15_isolated(rho, ref_rho) <= 1e-12
+    beam.close()
+    grid.close()
