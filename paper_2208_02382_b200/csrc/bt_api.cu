@@ -61,28 +61,43 @@ static int validate_element(const bt_element &e, int idx) {
 }
 
 // ---- S1/S3: coefficients of one slice map per element, for one pass at reference gamma ----------
-double build_turn_table(const std::vector<bt_element> &lat, double gamma, DevOp *ops) {
+double build_turn_table(const std::vector<bt_element> &lat, double gamma, std::vector<DevOp> &out, double *slots) {
+    double nslots = 0.0;
+    const char *fuse_env = getenv("BT_TRACK_FUSE");  // 0: one record per element (debugging / A-B measurements)
+    const bool fuse = !(fuse_env && fuse_env[0] == '0');
     for (size_t i = 0; i < lat.size(); ++i) {
         const bt_element &e = lat[i];
-        DevOp &o = ops[i];
+        DevOp o;
         memset(&o, 0, sizeof(o));
-        o.nslice = e.nslice;
+        o.count = e.nslice;
         const double bg = sqrt(gamma * gamma - 1.0);
         const double beta = bg / gamma;
         const double h = e.ds / (double)e.nslice;  // R3: one rounded division
         const double tc = h / (bg * bg);
         switch (e.type) {
             case BT_DRIFT:
-                o.op = OP_DRIFT;
+                nslots += 3.0 * e.nslice;
+                // peephole: a single-slice drift right behind a normal sextupole/octupole kick shares its dispatch
+                if (fuse && e.nslice == 1 && i > 0 && !out.empty() && lat[i - 1].type == BT_MULTIPOLE &&
+                    (out.back().op == OP_SEXT || out.back().op == OP_OCT || out.back().op == OP_SEXTOCT)) {
+                    out.back().op |= OP_TAILDRIFT;
+                    out.back().c[3] = h;
+                    out.back().c[4] = tc;
+                    break;
+                }
+                o.op = e.nslice == 1 ? OP_DRIFT1 : OP_DRIFT;
                 o.c[0] = h;
                 o.c[1] = tc;
+                out.push_back(o);
                 break;
             case BT_QUAD: {
                 const double k = e.p[0];
                 if (k == 0.0) {  // R5: k = 0 is a drift
-                    o.op = OP_DRIFT;
+                    o.op = e.nslice == 1 ? OP_DRIFT1 : OP_DRIFT;
                     o.c[0] = h;
                     o.c[1] = tc;
+                    nslots += 3.0 * e.nslice;
+                    out.push_back(o);
                     break;
                 }
                 const double w = sqrt(fabs(k));
@@ -90,7 +105,6 @@ double build_turn_table(const std::vector<bt_element> &lat, double gamma, DevOp 
                 const double f[3] = {c, s / w, -w * s};
                 const double d[3] = {ch, sh / w, w * sh};
                 const double *xb = k > 0.0 ? f : d, *yb = k > 0.0 ? d : f;
-                o.op = OP_QUAD;
                 o.c[0] = xb[0];
                 o.c[1] = xb[1];
                 o.c[2] = xb[2];
@@ -98,6 +112,18 @@ double build_turn_table(const std::vector<bt_element> &lat, double gamma, DevOp 
                 o.c[4] = yb[1];
                 o.c[5] = yb[2];
                 o.c[6] = tc;
+                nslots += 9.0 * e.nslice;
+                // nslice = 5a + b: a groups of five slices, then b single slices (same slice map, same order)
+                if (e.nslice / 5 > 0) {
+                    o.op = OP_QUAD5;
+                    o.count = e.nslice / 5;
+                    out.push_back(o);
+                }
+                if (e.nslice % 5 > 0) {
+                    o.op = e.nslice % 5 == 1 ? OP_QUAD1 : OP_QUAD;
+                    o.count = e.nslice % 5;
+                    out.push_back(o);
+                }
                 break;
             }
             case BT_SBEND: {
@@ -112,6 +138,8 @@ double build_turn_table(const std::vector<bt_element> &lat, double gamma, DevOp 
                 o.c[4] = -S / beta;
                 o.c[5] = rho * (S / (beta * beta) - th);
                 o.c[6] = h;
+                nslots += 10.0 * e.nslice;
+                out.push_back(o);
                 break;
             }
             case BT_DIPEDGE: {
@@ -121,6 +149,8 @@ double build_turn_table(const std::vector<bt_element> &lat, double gamma, DevOp 
                 o.op = OP_EDGE;
                 o.c[0] = tan(psi) / rho;
                 o.c[1] = -tan(psi - psi_c) / rho;
+                nslots += 2.0;
+                out.push_back(o);
                 break;
             }
             case BT_MULTIPOLE: {
@@ -132,15 +162,25 @@ double build_turn_table(const std::vector<bt_element> &lat, double gamma, DevOp 
                     o.op = OP_SEXT;
                     o.c[0] = Kn / 2.0;
                     o.c[1] = Kn;
+                    nslots += 5.0;
                 } else if (m == 4 && Ks == 0.0) {
+                    nslots += 8.0;
+                    // peephole: a normal octupole right behind a normal sextupole shares its dispatch
+                    if (fuse && i > 0 && !out.empty() && out.back().op == OP_SEXT && lat[i - 1].type == BT_MULTIPOLE) {
+                        out.back().op = OP_SEXTOCT;
+                        out.back().c[2] = Kn / 6.0;
+                        break;
+                    }
                     o.op = OP_OCT;
-                    o.c[0] = Kn / 6.0;
+                    o.c[2] = Kn / 6.0;
                 } else {
                     o.op = OP_MULT;
-                    o.c[0] = (double)m;
-                    o.c[1] = Kn / fact;
-                    o.c[2] = Ks / fact;
+                    o.count = m;
+                    o.c[0] = Kn / fact;
+                    o.c[1] = Ks / fact;
+                    nslots += 4.0 * (m - 1) + 6.0;
                 }
+                out.push_back(o);
                 break;
             }
             case BT_SHORTRF: {
@@ -152,24 +192,14 @@ double build_turn_table(const std::vector<bt_element> &lat, double gamma, DevOp 
                 o.c[0] = bg / bg_f;
                 o.c[1] = Vhat * krf * sin(phi) / bg_f;
                 gamma = gamma_f;  // S3: later elements see the new reference energy
+                nslots += 4.0;
+                out.push_back(o);
                 break;
             }
         }
     }
+    if (slots) *slots = nslots;
     return gamma;
-}
-
-static int ensure_table(Beam *b, size_t n_ops) {
-    if (b->d_table_cap >= n_ops) return BT_OK;
-    if (b->d_table) {
-        BT_CUDA_TRY(cudaStreamSynchronize(b->stream));
-        BT_CUDA_TRY(cudaFree(b->d_table));
-        b->d_table = nullptr;
-        b->d_table_cap = 0;
-    }
-    BT_CUDA_TRY(cudaMalloc(&b->d_table, n_ops * sizeof(DevOp)));
-    b->d_table_cap = n_ops;
-    return BT_OK;
 }
 
 }  // namespace bt
@@ -232,7 +262,7 @@ void bt_beam_destroy(bt_beam *beam) {
     Beam &b = beam->b;
     cudaStreamSynchronize(b.stream);
     if (b.owns && b.q[0]) cudaFree(b.q[0]);
-    if (b.d_table) cudaFree(b.d_table);
+    forget_table_owner(&b);
     int *ibufs[] = {b.ids, b.ids_tmp, b.sort_key, b.sort_dest, b.sort_count, b.sort_block_sum};
     for (int *p : ibufs)
         if (p) cudaFree(p);
@@ -346,39 +376,67 @@ int bt_track(bt_beam *beam, int32_t nturns) {
     if (b.lattice.empty()) return fail(BT_ERR_STATE, "bt_track: bt_lattice_set not called");
     if (!b.has_ref) return fail(BT_ERR_STATE, "bt_track: bt_beam_set_ref not called");
     if (nturns == 0) return BT_OK;
-    const size_t n_ops = b.lattice.size();
+    const size_t K = (size_t)kConstTableRecords;
+    // records [lo, hi) of one turn's table, in launches of at most K records
+    auto launch_segments = [&](const std::vector<DevOp> &ops, double spr) -> int {
+        for (size_t lo = 0; lo < ops.size(); lo += K) {
+            const size_t len = ops.size() - lo < K ? ops.size() - lo : K;
+            int rc = launch_track(&b, ops.data() + lo, (int32_t)len, 1, next_table_version(), spr);
+            if (rc != BT_OK) return rc;
+        }
+        return BT_OK;
+    };
 
     if (!b.energy_changes) {
-        // one table serves every turn
-        int rc = BT_OK;
-        if (!b.table_valid) {  // "uploaded once": reused until the lattice or the reference changes
-            std::vector<DevOp> ops(n_ops);
-            build_turn_table(b.lattice, b.gamma, ops.data());
-            rc = ensure_table(&b, n_ops);
-            if (rc != BT_OK) return rc;
-            // pageable source: the call returns after the source has been staged
-            BT_CUDA_TRY(cudaMemcpyAsync(b.d_table, ops.data(), n_ops * sizeof(DevOp), cudaMemcpyHostToDevice, b.stream));
+        // one table serves every turn: "uploaded once", resident until the lattice, the reference or another
+        // beam's table replaces it
+        if (!b.table_valid) {
+            b.h_table.clear();
+            build_turn_table(b.lattice, b.gamma, b.h_table, &b.table_slots);
+            b.table_version = next_table_version();
             b.table_valid = true;
         }
-        rc = launch_track(&b, b.d_table, (int32_t)n_ops, nturns, 0);
-        if (rc != BT_OK) return rc;
+        const double spr = b.table_slots / (double)b.h_table.size();
+        if (b.h_table.size() <= K) {
+            int rc = launch_track(&b, b.h_table.data(), (int32_t)b.h_table.size(), nturns, b.table_version, spr);
+            if (rc != BT_OK) return rc;
+        } else {  // lattice longer than the constant bank: several launches per turn
+            for (int32_t t = 0; t < nturns; ++t) {
+                int rc = launch_segments(b.h_table, spr);
+                if (rc != BT_OK) return rc;
+            }
+        }
     } else {
-        // S3: per-turn tables; chunks of turns bounded by a table budget (16 MiB)
-        const size_t max_ops = ((size_t)16 << 20) / sizeof(DevOp);
-        int32_t chunk = (int32_t)(max_ops / n_ops);
-        if (chunk < 1) chunk = 1;
-        if (chunk > nturns) chunk = nturns;
+        // S3: the reference energy changes at RF passages -> every turn has its own coefficients; as many whole
+        // turns as fit the constant bank go into one launch
         b.table_valid = false;
-        int rc = ensure_table(&b, n_ops * (size_t)chunk);
-        if (rc != BT_OK) return rc;
-        std::vector<DevOp> ops(n_ops * (size_t)chunk);
-        double gamma = b.gamma;
-        for (int32_t done = 0; done < nturns; done += chunk) {
-            const int32_t nt = (nturns - done < chunk) ? (nturns - done) : chunk;
-            for (int32_t t = 0; t < nt; ++t) gamma = build_turn_table(b.lattice, gamma, ops.data() + (size_t)t * n_ops);
-            if (done > 0) BT_CUDA_TRY(cudaStreamSynchronize(b.stream));  // previous chunk still reads the table
-            BT_CUDA_TRY(cudaMemcpyAsync(b.d_table, ops.data(), n_ops * (size_t)nt * sizeof(DevOp), cudaMemcpyHostToDevice, b.stream));
-            rc = launch_track(&b, b.d_table, (int32_t)n_ops, nt, (int32_t)n_ops);
+        std::vector<DevOp> buf, turn_ops;
+        double gamma = b.gamma, buf_spr = 0.0;
+        for (int32_t t = 0; t < nturns; ++t) {
+            turn_ops.clear();
+            double slots = 0.0;
+            gamma = build_turn_table(b.lattice, gamma, turn_ops, &slots);
+            const double spr = slots / (double)turn_ops.size();
+            if (turn_ops.size() > K) {  // a single turn exceeds the bank: flush what is pending, then its segments
+                if (!buf.empty()) {
+                    int rc = launch_track(&b, buf.data(), (int32_t)buf.size(), 1, next_table_version(), buf_spr);
+                    if (rc != BT_OK) return rc;
+                    buf.clear();
+                }
+                int rc = launch_segments(turn_ops, spr);
+                if (rc != BT_OK) return rc;
+                continue;
+            }
+            if (buf.size() + turn_ops.size() > K) {
+                int rc = launch_track(&b, buf.data(), (int32_t)buf.size(), 1, next_table_version(), buf_spr);
+                if (rc != BT_OK) return rc;
+                buf.clear();
+            }
+            buf.insert(buf.end(), turn_ops.begin(), turn_ops.end());
+            buf_spr = spr;
+        }
+        if (!buf.empty()) {
+            int rc = launch_track(&b, buf.data(), (int32_t)buf.size(), 1, next_table_version(), buf_spr);
             if (rc != BT_OK) return rc;
         }
         b.gamma = gamma;

@@ -25,29 +25,40 @@ extern std::atomic<int64_t> g_launch_count;
                               std::string(#expr) + ": " + cudaGetErrorString(_e));               \
     } while (0)
 
-// ---- device op records (S1): one 64-byte record per lattice element ----------------------------
-// The host turns each bt_element into the coefficients of ONE slice map of length h = ds/nslice.
+// ---- device op records (S1): 64-byte records in the constant bank ------------------------------------
+// The host turns each bt_element into the coefficients of ONE slice map of length h = ds/nslice.  Opcodes are
+// one-hot so the kernel can dispatch with a short tree of uniform bit tests (track.cu).
 enum Op : int32_t {
-    OP_DRIFT = 0,  // c0 = h, c1 = h/(b0 g0)^2
-    OP_QUAD = 1,   // x' = c0 x + c1 px, px' = c2 x + c0 px ; y' = c3 y + c4 py, py' = c5 y + c3 py ; t += c6 pt
-    OP_SBEND = 2,  // c0 = C, c1 = rho S, c2 = -S/rho, c3 = r16, c4 = r26, c5 = r56, c6 = h   (r51 = -r26, r52 = -r16)
-    OP_EDGE = 3,   // px += c0 x ; py += c1 y
-    OP_SEXT = 4,   // normal sextupole: px -= c0 (x^2 - y^2) ; py += c1 x y      (c0 = Kn/2, c1 = Kn)
-    OP_OCT = 5,    // normal octupole:  px -= c0 x (x^2 - 3y^2) ; py += c0 y (3x^2 - y^2)   (c0 = Kn/6)
-    OP_MULT = 6,   // general thin multipole: c0 = m, c1 = Kn/(m-1)!, c2 = Ks/(m-1)!
-    OP_RF = 7,     // px *= c0 ; py *= c0 ; pt = c0 pt + c1 t
-    OP_COUNT
+    OP_DRIFT1 = 1 << 0,   // one slice;  c0 = h, c1 = h/(b0 g0)^2
+    OP_DRIFT = 1 << 1,    // count slices, same coefficients
+    OP_QUAD1 = 1 << 2,    // one slice;  x' = c0 x + c1 px, px' = c2 x + c0 px ; y' = c3 y + c4 py, py' = c5 y + c3 py ; t += c6 pt
+    OP_QUAD = 1 << 3,     // count slices, same coefficients
+    OP_QUAD5 = 1 << 4,    // count groups of FIVE slices: a thick quad of nslice = 5a + b slices becomes {QUAD5, a} then
+                          // {QUAD, b} / {QUAD1}, so the unrolled loop needs no remainder logic
+    OP_SBEND = 1 << 5,    // count slices; c0 = C, c1 = rho S, c2 = -S/rho, c3 = r16, c4 = r26, c5 = r56, c6 = h (r51 = -r26, r52 = -r16)
+    OP_EDGE = 1 << 6,     // px += c0 x ; py += c1 y
+    OP_SEXT = 1 << 7,     // normal sextupole: px -= c0 (x^2 - y^2) ; py += c1 x y      (c0 = Kn/2, c1 = Kn)
+    OP_OCT = 1 << 8,      // normal octupole:  px -= c2 x (x^2 - 3y^2) ; py += c2 y (3x^2 - y^2)   (c2 = Kn/6)
+    OP_SEXTOCT = 1 << 9,  // OP_SEXT then OP_OCT (adjacent elements) in one dispatch; same arithmetic, same order
+    OP_MULT = 1 << 10,    // general thin multipole: count = m, c0 = Kn/(m-1)!, c1 = Ks/(m-1)!
+    OP_RF = 1 << 11,      // px *= c0 ; py *= c0 ; pt = c0 pt + c1 t
+    OP_TAILDRIFT = 1 << 12  // modifier of SEXT/OCT/SEXTOCT: the single-slice drift that follows the kick rides in the
+                            // same record (c3 = h, c4 = h/(b0 g0)^2); same arithmetic, same order, one dispatch less
 };
 
 struct alignas(16) DevOp {
     int32_t op;
-    int32_t nslice;
+    int32_t count;  // slices (DRIFT, QUAD, SBEND), groups of five slices (QUAD5), order m (MULT), else 1
     double c[7];
 };
 static_assert(sizeof(DevOp) == 64, "DevOp must be 64 bytes");
 
+constexpr int kConstTableRecords = 1024;  // 64 KiB constant bank / 64 B
+constexpr int kMaxDevices = 64;
+
 struct TrackLaunchInfo {
     int32_t grid = 0, block = 0, ppt = 0, smem = 0;
+    int64_t launches = 0;  // fused-walk kernels launched by this beam so far
 };
 
 struct Beam {
@@ -67,9 +78,10 @@ struct Beam {
     std::vector<bt_element> lattice;
     bool energy_changes = false;  // some SHORTRF with Vhat*cos(phi) != 0
     double lattice_length = 0.0;
-    DevOp *d_table = nullptr;  // device table(s)
-    size_t d_table_cap = 0;    // in DevOps
-    bool table_valid = false;  // d_table holds the single-turn table for the current lattice and gamma
+    std::vector<DevOp> h_table;  // single-turn record table for the current lattice and gamma (static lattices)
+    bool table_valid = false;    // h_table is up to date
+    uint64_t table_version = 0;  // identifies h_table's contents in the device's constant bank (track.cu)
+    double table_slots = 0.0;    // FP64 slots per particle per turn of that table
     TrackLaunchInfo last_launch;
     // S4 cell binning: storage order != original order once sorted; ids[j] = original index of slot j
     bool permuted = false;
@@ -88,12 +100,19 @@ struct Grid {
     cudaStream_t last_stream = nullptr;
 };
 
-// ---- host precompute (S1/S3), bt_lattice.cpp part of bt_api.cu ---------------------------------
-// Fills ops[0..n) for one pass over the lattice starting at reference gamma; returns gamma after.
-double build_turn_table(const std::vector<bt_element> &lat, double gamma, DevOp *ops);
+// ---- host precompute (S1/S3), in bt_api.cu ------------------------------------------------------
+// Appends the records of one pass over the lattice starting at reference gamma; returns gamma after.
+// The number of records appended depends on the lattice only (not on gamma).  *slots (may be NULL) receives the
+// FP64 instruction slots one particle spends in this pass (minimal DFMA/DMUL sequences).
+double build_turn_table(const std::vector<bt_element> &lat, double gamma, std::vector<DevOp> &out, double *slots);
 
 // ---- launchers --------------------------------------------------------------------------------
-int launch_track(Beam *b, const DevOp *d_table, int32_t n_ops, int32_t nturns, int32_t turn_stride);
+// One fused-walk launch: n_ops (<= kConstTableRecords) host records are placed in the constant bank (skipped when
+// `version` of this beam is already resident) and walked nturns times.  slots_per_record (FP64 slots per particle per
+// record, averaged) steers the particles-per-thread choice.
+int launch_track(Beam *b, const DevOp *h_table, int32_t n_ops, int32_t nturns, uint64_t version, double slots_per_record);
+uint64_t next_table_version();
+void forget_table_owner(const Beam *b);
 int launch_deposit(Beam *b, Grid *g, double q_weight, double zscale);
 int launch_gather_kick(Beam *b, const Grid *g, const double coef[3], double zscale, double h_before,
                        double tc_before, double h_after, double tc_after);

@@ -1,70 +1,48 @@
 // S2: the fused lattice walk.  One launch: every particle is loaded once (coalesced, 16-byte
-// vector loads when aligned), all turns x elements x slices are applied in registers, and it is
-// stored once -> 96 B of HBM traffic per particle per launch.  Arithmetic is pure FP64
-// DFMA/DMUL: every transcendental is an element parameter and was folded into the per-slice
-// coefficients on the host (bt_api.cu: build_turn_table).
+// vector loads when aligned), every record of the launch's table is applied in registers (all
+// turns x elements x slices that fit one table), and it is stored once -> 96 B of HBM traffic per
+// particle per launch.  Arithmetic is pure FP64 DFMA/DMUL: every transcendental is an element
+// parameter and was folded into the per-slice coefficients on the host (bt_api.cu: build_turn_table).
 //
-// Thread mapping: each thread owns P particles (P = 1, 2 or 4).  The op table is warp-uniform, so
-// the interpreter overhead (header load, dispatch, coefficient loads, loop control) is paid once
-// per warp-instruction stream and amortised over P particles; with the FP64 pipe accepting one
-// warp-instruction every second issue cycle of an SM sub-partition, P = 4 leaves that overhead
-// hidden behind the DFMA stream.  The P independent particles also give the ILP that covers the
-// DFMA latency at low occupancy.
+// Thread mapping: each thread owns P particles (P = 1, 2, 4 or 8); one warp = one task of 32*P particles
+// that walks the whole record table.
 //
-// Op table source: shared memory (staged per CTA, re-staged per turn when an RF cavity changes the
-// reference energy) when it fits, else global memory through the read-only path.
+// Record table: the CONSTANT bank (64 KiB = 1024 records of 64 B).  The walk is warp-uniform, so every
+// record word is fetched with a uniform-datapath constant load (LDCU) straight into a uniform register and
+// used as the UR operand of the DFMAs -- no vector-register traffic, no R2UR moves, and the dispatch is
+// uniform compares + uniform branches.  Measured on B200 against the alternatives (shared-memory table,
+// global table through L1, either with software-prefetched records in vector registers): vector-register
+// coefficients cost FP64 issue rate (three 64-bit vector operands per DFMA), and R2UR of loaded words sits
+// on the dependency chain of every element; the constant-bank walk keeps the FP64 pipe busiest.
+// Lattices x turns longer than one table are walked in several launches (bt_api.cu plans them).
+//
+// Opcodes are one-hot bits, tested with a short uniform compare tree ordered by how often the kinds occur;
+// the host specialises single-slice elements (no loop control) and groups of five quad slices (unrolled).
 #include "bt_internal.h"
 
 #include <stdlib.h>
 
+#include <mutex>
+
 namespace bt {
 
-constexpr int kMaxBlock = 128;
+constexpr int kMaxBlock = 128;  // launch bound; the default block is 64 threads (fine-grained balance over SMs)
+
+__constant__ DevOp c_table[kConstTableRecords];
+
+// Register budget per instantiation (128-thread blocks per SM the compiler must allow): the per-record latency
+// (constant loads, compare tree, branch) is covered by other warps, so P <= 4 is held to 80 registers
+// (6 warps per sub-partition); P = 8 needs 96 registers for the particles alone.
+template <int P>
+constexpr int kMinBlocks = P <= 2 ? 8 : P == 4 ? 6 : 3;
 
 struct TrackArgs {
     double *q[6];
-    const DevOp *table;
     long long n;
     long long tail_start;  // first particle handled by the guarded P=1 blocks
     int n_full_blocks;     // blocks [0, n_full_blocks) run the unguarded P-particle path
-    int n_ops;
-    int nturns;
-    int turn_stride;  // DevOps between consecutive turns' tables (0: same table every turn)
-};
-
-// ---- table access -------------------------------------------------------------------------------
-template <bool SMEM>
-struct Tab;
-
-template <>
-struct Tab<true> {
-    uint32_t base;  // shared-space address
-    __device__ __forceinline__ void hdr(int e, int &op, int &ns, double &c0) const {
-        uint32_t a, b, lo, hi;
-        asm volatile("ld.shared.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(a), "=r"(b), "=r"(lo), "=r"(hi) : "r"(base + e * 64));
-        op = (int)a;
-        ns = (int)b;
-        c0 = __hiloint2double((int)hi, (int)lo);
-    }
-    // k = 1,2,3 -> (c[2k-1], c[2k])
-    __device__ __forceinline__ void pair(int e, int k, double &u, double &v) const {
-        asm volatile("ld.shared.v2.f64 {%0,%1}, [%2];" : "=d"(u), "=d"(v) : "r"(base + e * 64 + k * 16));
-    }
-};
-
-template <>
-struct Tab<false> {
-    const char *base;
-    __device__ __forceinline__ void hdr(int e, int &op, int &ns, double &c0) const {
-        uint32_t a, b, lo, hi;
-        asm volatile("ld.global.nc.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(a), "=r"(b), "=r"(lo), "=r"(hi) : "l"(base + (size_t)e * 64));
-        op = (int)a;
-        ns = (int)b;
-        c0 = __hiloint2double((int)hi, (int)lo);
-    }
-    __device__ __forceinline__ void pair(int e, int k, double &u, double &v) const {
-        asm volatile("ld.global.nc.v2.f64 {%0,%1}, [%2];" : "=d"(u), "=d"(v) : "l"(base + (size_t)e * 64 + k * 16));
-    }
+    int n_ops;             // records in c_table for this launch
+    int nturns;            // passes over those records
 };
 
 template <int P>
@@ -72,139 +50,146 @@ struct Ptc {
     double x[P], px[P], y[P], py[P], t[P], pt[P];
 };
 
-// ---- one pass over the op table (one turn) -------------------------------------------------------
-template <int P, bool SMEM>
-__device__ __forceinline__ void walk_turn(Ptc<P> &p, const Tab<SMEM> tab, const int n_ops) {
+#define BT_FORP _Pragma("unroll") for (int j = 0; j < P; ++j)
+
+// R5: one slice of a thick quad, 9 slots (4 DMUL + 5 DFMA)
+template <int P>
+__device__ __forceinline__ void quad_slice(Ptc<P> &p, double c0, double c1, double c2, double c3, double c4, double c5, double c6) {
+    BT_FORP {
+        const double x = p.x[j], px = p.px[j], y = p.y[j], py = p.py[j];
+        p.x[j] = fma(c1, px, c0 * x);
+        p.px[j] = fma(c0, px, c2 * x);
+        p.y[j] = fma(c4, py, c3 * y);
+        p.py[j] = fma(c3, py, c5 * y);
+        p.t[j] = fma(c6, p.pt[j], p.t[j]);
+    }
+}
+// R4: 3 slots
+template <int P>
+__device__ __forceinline__ void drift_slice(Ptc<P> &p, double c0, double c1) {
+    BT_FORP {
+        p.x[j] = fma(c0, p.px[j], p.x[j]);
+        p.y[j] = fma(c0, p.py[j], p.y[j]);
+        p.t[j] = fma(c1, p.pt[j], p.t[j]);
+    }
+}
+// R8, m = 3, Ks = 0: 5 slots.  ca = Kn/2, cb = Kn
+template <int P>
+__device__ __forceinline__ void sext_kick(Ptc<P> &p, double ca, double cb) {
+    BT_FORP {
+        const double x = p.x[j], y = p.y[j];
+        const double re = fma(-y, y, x * x);  // Re (x+iy)^2
+        const double xy = x * y;              // Im (x+iy)^2 / 2
+        p.px[j] = fma(-ca, re, p.px[j]);
+        p.py[j] = fma(cb, xy, p.py[j]);
+    }
+}
+// R8, m = 4, Ks = 0: 8 slots.  c = Kn/6
+template <int P>
+__device__ __forceinline__ void oct_kick(Ptc<P> &p, double c) {
+    BT_FORP {
+        const double x = p.x[j], y = p.y[j];
+        const double x2 = x * x, y2 = y * y;
+        const double a = fma(-3.0, y2, x2);  // Re (x+iy)^3 = x (x^2 - 3y^2)
+        const double b = fma(3.0, x2, -y2);  // Im (x+iy)^3 = y (3x^2 - y^2)
+        p.px[j] = fma(-c, x * a, p.px[j]);
+        p.py[j] = fma(c, y * b, p.py[j]);
+    }
+}
+
+// ---- one record applied to the P particles of this thread -----------------------------------------
+template <int P>
+__device__ __forceinline__ void apply(Ptc<P> &p, const DevOp &r) {
+    const int op = r.op;
+    if (op & (OP_QUAD5 | OP_QUAD1 | OP_QUAD)) {
+        const double c0 = r.c[0], c1 = r.c[1], c2 = r.c[2], c3 = r.c[3], c4 = r.c[4], c5 = r.c[5], c6 = r.c[6];
+        if (op & OP_QUAD5) {  // count groups of five slices
+            const int cnt = r.count;
 #pragma unroll 1
-    for (int e = 0; e < n_ops; ++e) {
-        int op, ns;
-        double c0;
-        tab.hdr(e, op, ns, c0);
-        switch (op) {
-            case OP_DRIFT: {  // R4: 3 slots
-                double c1, c2;
-                tab.pair(e, 1, c1, c2);
+            for (int s = 0; s < cnt; ++s) {
+#pragma unroll
+                for (int u = 0; u < 5; ++u) quad_slice<P>(p, c0, c1, c2, c3, c4, c5, c6);
+            }
+        } else if (op & OP_QUAD1) {
+            quad_slice<P>(p, c0, c1, c2, c3, c4, c5, c6);
+        } else {
+            const int cnt = r.count;
 #pragma unroll 1
-                for (int s = 0; s < ns; ++s) {
-#pragma unroll
-                    for (int j = 0; j < P; ++j) {
-                        p.x[j] = fma(c0, p.px[j], p.x[j]);
-                        p.y[j] = fma(c0, p.py[j], p.y[j]);
-                        p.t[j] = fma(c1, p.pt[j], p.t[j]);
-                    }
-                }
-                break;
+            for (int s = 0; s < cnt; ++s) quad_slice<P>(p, c0, c1, c2, c3, c4, c5, c6);
+        }
+    } else if (op & (OP_DRIFT1 | OP_DRIFT)) {
+        const double c0 = r.c[0], c1 = r.c[1];
+        if (op & OP_DRIFT1) {
+            drift_slice<P>(p, c0, c1);
+        } else {
+            const int cnt = r.count;
+#pragma unroll 1
+            for (int s = 0; s < cnt; ++s) drift_slice<P>(p, c0, c1);
+        }
+    } else if (op & (OP_SEXTOCT | OP_SEXT | OP_OCT)) {
+        // OP_SEXTOCT = a sextupole kick followed by an octupole kick at the same place, in one dispatch;
+        // the arithmetic is exactly the two separate kicks in order.
+        if (op & (OP_SEXTOCT | OP_SEXT)) sext_kick<P>(p, r.c[0], r.c[1]);
+        if (op & (OP_SEXTOCT | OP_OCT)) oct_kick<P>(p, r.c[2]);
+        if (op & OP_TAILDRIFT) drift_slice<P>(p, r.c[3], r.c[4]);  // the single-slice drift that follows, same dispatch
+    } else if (op & (OP_SBEND | OP_EDGE)) {
+        if (op & OP_EDGE) {  // R7: 2 slots
+            const double c0 = r.c[0], c1 = r.c[1];
+            BT_FORP {
+                p.px[j] = fma(c0, p.x[j], p.px[j]);
+                p.py[j] = fma(c1, p.y[j], p.py[j]);
             }
-            case OP_QUAD: {  // R5: 9 slots (4 DMUL + 5 DFMA)
-                double c1, c2, c3, c4, c5, c6;
-                tab.pair(e, 1, c1, c2);
-                tab.pair(e, 2, c3, c4);
-                tab.pair(e, 3, c5, c6);
-#pragma unroll 5
-                for (int s = 0; s < ns; ++s) {
-#pragma unroll
-                    for (int j = 0; j < P; ++j) {
-                        const double x = p.x[j], px = p.px[j], y = p.y[j], py = p.py[j];
-                        p.x[j] = fma(c1, px, c0 * x);
-                        p.px[j] = fma(c0, px, c2 * x);
-                        p.y[j] = fma(c4, py, c3 * y);
-                        p.py[j] = fma(c3, py, c5 * y);
-                        p.t[j] = fma(c6, p.pt[j], p.t[j]);
-                    }
+        } else {  // R6: 10 slots per slice (2 DMUL + 8 DFMA)
+            const double c0 = r.c[0], c1 = r.c[1], c2 = r.c[2], c3 = r.c[3], c4 = r.c[4], c5 = r.c[5], c6 = r.c[6];
+            const int cnt = r.count;
+#pragma unroll 1
+            for (int s = 0; s < cnt; ++s) {
+                BT_FORP {
+                    const double x = p.x[j], px = p.px[j], pt = p.pt[j];
+                    p.x[j] = fma(c3, pt, fma(c1, px, c0 * x));
+                    p.px[j] = fma(c4, pt, fma(c0, px, c2 * x));
+                    p.y[j] = fma(c6, p.py[j], p.y[j]);
+                    // t += r51 x + r52 px + r56 pt with r51 = -r26 = -c4, r52 = -r16 = -c3
+                    p.t[j] = fma(c5, pt, fma(-c3, px, fma(-c4, x, p.t[j])));
                 }
-                break;
             }
-            case OP_SBEND: {  // R6: 10 slots (2 DMUL + 8 DFMA)
-                double c1, c2, c3, c4, c5, c6;
-                tab.pair(e, 1, c1, c2);
-                tab.pair(e, 2, c3, c4);
-                tab.pair(e, 3, c5, c6);
-#pragma unroll 2
-                for (int s = 0; s < ns; ++s) {
-#pragma unroll
-                    for (int j = 0; j < P; ++j) {
-                        const double x = p.x[j], px = p.px[j], pt = p.pt[j];
-                        p.x[j] = fma(c3, pt, fma(c1, px, c0 * x));
-                        p.px[j] = fma(c4, pt, fma(c0, px, c2 * x));
-                        p.y[j] = fma(c6, p.py[j], p.y[j]);
-                        // t += r51 x + r52 px + r56 pt with r51 = -r26 = -c4, r52 = -r16 = -c3
-                        p.t[j] = fma(c5, pt, fma(-c3, px, fma(-c4, x, p.t[j])));
-                    }
-                }
-                break;
+        }
+    } else if (op & OP_RF) {  // R9: 4 slots
+        const double c0 = r.c[0], c1 = r.c[1];
+        BT_FORP {
+            p.px[j] *= c0;
+            p.py[j] *= c0;
+            p.pt[j] = fma(c0, p.pt[j], c1 * p.t[j]);
+        }
+    } else if (op & OP_MULT) {  // R8 general order: repeated complex multiplication; count = m
+        const double c0 = r.c[0], c1 = r.c[1];
+        const int m = r.count;
+        BT_FORP {
+            const double x = p.x[j], y = p.y[j];
+            double zr = 1.0, zi = 0.0;
+#pragma unroll 1
+            for (int k = 1; k < m; ++k) {
+                const double nr = fma(-zi, y, zr * x);
+                const double ni = fma(zi, x, zr * y);
+                zr = nr;
+                zi = ni;
             }
-            case OP_EDGE: {  // R7: 2 slots
-                double c1, c2;
-                tab.pair(e, 1, c1, c2);
-#pragma unroll
-                for (int j = 0; j < P; ++j) {
-                    p.px[j] = fma(c0, p.x[j], p.px[j]);
-                    p.py[j] = fma(c1, p.y[j], p.py[j]);
-                }
-                break;
-            }
-            case OP_SEXT: {  // R8, m = 3, Ks = 0: 5 slots
-                double c1, c2;
-                tab.pair(e, 1, c1, c2);
-#pragma unroll
-                for (int j = 0; j < P; ++j) {
-                    const double x = p.x[j], y = p.y[j];
-                    const double re = fma(-y, y, x * x);  // Re (x+iy)^2
-                    const double xy = x * y;              // Im (x+iy)^2 / 2
-                    p.px[j] = fma(-c0, re, p.px[j]);
-                    p.py[j] = fma(c1, xy, p.py[j]);
-                }
-                break;
-            }
-            case OP_OCT: {  // R8, m = 4, Ks = 0: 8 slots
-#pragma unroll
-                for (int j = 0; j < P; ++j) {
-                    const double x = p.x[j], y = p.y[j];
-                    const double x2 = x * x, y2 = y * y;
-                    const double a = fma(-3.0, y2, x2);  // Re (x+iy)^3 = x (x^2 - 3y^2)
-                    const double b = fma(3.0, x2, -y2);  // Im (x+iy)^3 = y (3x^2 - y^2)
-                    p.px[j] = fma(-c0, x * a, p.px[j]);
-                    p.py[j] = fma(c0, y * b, p.py[j]);
-                }
-                break;
-            }
-            case OP_MULT: {  // R8 general order: repeated complex multiplication
-                double c1, c2;
-                tab.pair(e, 1, c1, c2);
-                const int m = (int)c0;
-#pragma unroll
-                for (int j = 0; j < P; ++j) {
-                    const double x = p.x[j], y = p.y[j];
-                    double zr = 1.0, zi = 0.0;
-                    for (int k = 1; k < m; ++k) {
-                        const double nr = fma(-zi, y, zr * x);
-                        const double ni = fma(zi, x, zr * y);
-                        zr = nr;
-                        zi = ni;
-                    }
-                    p.px[j] -= fma(-c2, zi, c1 * zr);
-                    p.py[j] += fma(c2, zr, c1 * zi);
-                }
-                break;
-            }
-            case OP_RF: {  // R9: 4 slots
-                double c1, c2;
-                tab.pair(e, 1, c1, c2);
-#pragma unroll
-                for (int j = 0; j < P; ++j) {
-                    p.px[j] *= c0;
-                    p.py[j] *= c0;
-                    p.pt[j] = fma(c0, p.pt[j], c1 * p.t[j]);
-                }
-                break;
-            }
-            default:
-                break;
+            p.px[j] -= fma(-c1, zi, c0 * zr);
+            p.py[j] += fma(c1, zr, c0 * zi);
         }
     }
 }
 
-// ---- streaming particle access: read once, written once -> keep them out of the way of the table --
+template <int P>
+__device__ __forceinline__ void walk(Ptc<P> &p, const int n_ops, const int nturns) {
+#pragma unroll 1
+    for (int turn = 0; turn < nturns; ++turn) {
+#pragma unroll 1
+        for (int e = 0; e < n_ops; ++e) apply<P>(p, c_table[e]);
+    }
+}
+
+// ---- streaming particle access: read once, written once ------------------------------------------
 __device__ __forceinline__ double2 ld_stream2(const double *p) {
     double2 v;
     asm volatile("ld.global.cs.v2.f64 {%0,%1}, [%2];" : "=d"(v.x), "=d"(v.y) : "l"(p));
@@ -220,32 +205,9 @@ __device__ __forceinline__ double ld_stream1(const double *p) {
 }
 __device__ __forceinline__ void st_stream1(double *p, double v) { asm volatile("st.global.cs.f64 [%0], %1;" ::"l"(p), "d"(v) : "memory"); }
 
-template <int P, bool SMEM>
-__device__ __forceinline__ void run_turns(Ptc<P> &p, const TrackArgs &a, uint32_t smem_addr, uint4 *smem_ptr) {
-#pragma unroll 1
-    for (int turn = 0; turn < a.nturns; ++turn) {
-        const DevOp *gt = a.table + (size_t)turn * a.turn_stride;
-        if constexpr (SMEM) {
-            if (turn == 0 || a.turn_stride != 0) {
-                if (turn != 0) __syncthreads();  // everyone is done with the previous turn's table
-                const uint4 *src = reinterpret_cast<const uint4 *>(gt);
-                for (int i = threadIdx.x; i < a.n_ops * 4; i += blockDim.x) smem_ptr[i] = __ldg(src + i);
-                __syncthreads();
-            }
-            Tab<true> tab{smem_addr};
-            walk_turn<P, true>(p, tab, a.n_ops);
-        } else {
-            Tab<false> tab{reinterpret_cast<const char *>(gt)};
-            walk_turn<P, false>(p, tab, a.n_ops);
-        }
-    }
-}
-
 // P particles per thread (P even: 16-byte vector access; requires 16-byte aligned arrays).
-template <int P, bool SMEM>
-__global__ void __launch_bounds__(kMaxBlock) track_kernel(const __grid_constant__ TrackArgs a) {
-    extern __shared__ uint4 smem_tab[];
-    const uint32_t smem_addr = (uint32_t)__cvta_generic_to_shared(smem_tab);
+template <int P>
+__global__ void __launch_bounds__(kMaxBlock, kMinBlocks<P>) track_kernel(const __grid_constant__ TrackArgs a) {
     const int tid = threadIdx.x;
     const int B = blockDim.x;
 
@@ -268,7 +230,7 @@ __global__ void __launch_bounds__(kMaxBlock) track_kernel(const __grid_constant_
                 v = ld_stream2(q[4] + off), p.t[2 * j] = v.x, p.t[2 * j + 1] = v.y;
                 v = ld_stream2(q[5] + off), p.pt[2 * j] = v.x, p.pt[2 * j + 1] = v.y;
             }
-            run_turns<P, SMEM>(p, a, smem_addr, smem_tab);
+            walk<P>(p, a.n_ops, a.nturns);
 #pragma unroll
             for (int j = 0; j < P / 2; ++j) {
                 const int off = j * 2 * B;
@@ -287,7 +249,7 @@ __global__ void __launch_bounds__(kMaxBlock) track_kernel(const __grid_constant_
             p.py[0] = ld_stream1(a.q[3] + i);
             p.t[0] = ld_stream1(a.q[4] + i);
             p.pt[0] = ld_stream1(a.q[5] + i);
-            run_turns<P, SMEM>(p, a, smem_addr, smem_tab);
+            walk<P>(p, a.n_ops, a.nturns);
             st_stream1(a.q[0] + i, p.x[0]);
             st_stream1(a.q[1] + i, p.px[0]);
             st_stream1(a.q[2] + i, p.y[0]);
@@ -299,22 +261,20 @@ __global__ void __launch_bounds__(kMaxBlock) track_kernel(const __grid_constant_
         // ---- guarded tail: one particle per thread ----
         Ptc<1> p;
         const long long i = a.tail_start + (long long)((int)blockIdx.x - a.n_full_blocks) * B + tid;
-        const bool live = i < a.n;
-        p.x[0] = live ? ld_stream1(a.q[0] + i) : 0.0;
-        p.px[0] = live ? ld_stream1(a.q[1] + i) : 0.0;
-        p.y[0] = live ? ld_stream1(a.q[2] + i) : 0.0;
-        p.py[0] = live ? ld_stream1(a.q[3] + i) : 0.0;
-        p.t[0] = live ? ld_stream1(a.q[4] + i) : 0.0;
-        p.pt[0] = live ? ld_stream1(a.q[5] + i) : 0.0;
-        run_turns<1, SMEM>(p, a, smem_addr, smem_tab);  // every thread walks: the table staging has barriers
-        if (live) {
-            st_stream1(a.q[0] + i, p.x[0]);
-            st_stream1(a.q[1] + i, p.px[0]);
-            st_stream1(a.q[2] + i, p.y[0]);
-            st_stream1(a.q[3] + i, p.py[0]);
-            st_stream1(a.q[4] + i, p.t[0]);
-            st_stream1(a.q[5] + i, p.pt[0]);
-        }
+        if (i >= a.n) return;
+        p.x[0] = ld_stream1(a.q[0] + i);
+        p.px[0] = ld_stream1(a.q[1] + i);
+        p.y[0] = ld_stream1(a.q[2] + i);
+        p.py[0] = ld_stream1(a.q[3] + i);
+        p.t[0] = ld_stream1(a.q[4] + i);
+        p.pt[0] = ld_stream1(a.q[5] + i);
+        walk<1>(p, a.n_ops, a.nturns);
+        st_stream1(a.q[0] + i, p.x[0]);
+        st_stream1(a.q[1] + i, p.px[0]);
+        st_stream1(a.q[2] + i, p.y[0]);
+        st_stream1(a.q[3] + i, p.py[0]);
+        st_stream1(a.q[4] + i, p.t[0]);
+        st_stream1(a.q[5] + i, p.pt[0]);
     }
 }
 
@@ -323,48 +283,54 @@ static int env_int(const char *name, int dflt) {
     return (v && *v) ? atoi(v) : dflt;
 }
 
-template <int P, bool SMEM>
-static cudaError_t do_launch(const TrackArgs &a, int grid, int block, size_t smem, cudaStream_t s) {
-    if (smem > 48 * 1024) {
-        cudaError_t e = cudaFuncSetAttribute(track_kernel<P, SMEM>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e != cudaSuccess) return e;
-    }
-    track_kernel<P, SMEM><<<grid, block, smem, s>>>(a);
-    return cudaGetLastError();
-}
+// ---- the constant table is one per device: serialise its users -----------------------------------
+// An upload (stream-ordered copy into the constant bank) must not overtake the kernels of another beam
+// (another stream) that still read the previous contents.  Every launch records `busy` after its kernel; an
+// upload first makes its stream wait for `busy`.  `owner`/`version` let a beam skip the upload while its
+// table is still the resident one.
+struct ConstTableState {
+    std::mutex mu;
+    cudaEvent_t busy = nullptr;
+    const void *owner = nullptr;
+    uint64_t version = 0;
+};
+static ConstTableState g_ct[kMaxDevices];
+static std::atomic<uint64_t> g_table_version{1};
 
-int launch_track(Beam *b, const DevOp *d_table, int32_t n_ops, int32_t nturns, int32_t turn_stride) {
+uint64_t next_table_version() { return g_table_version.fetch_add(1); }
+
+int launch_track(Beam *b, const DevOp *h_table, int32_t n_ops, int32_t nturns, uint64_t version, double slots_per_record) {
+    if (n_ops < 1 || n_ops > kConstTableRecords) return fail(BT_ERR_INVALID, "launch_track: table size");
+    if (b->device < 0 || b->device >= kMaxDevices) return fail(BT_ERR_UNSUPPORTED, "bt_track: device index too large");
     // ---- launch geometry -------------------------------------------------------------------------
-    // Enough threads to give every SM sub-partition >= 2 warps decides P; small bunches shrink the block
-    // so that the grid still covers all SMs (config 0: 10^4 particles is latency-bound whatever we do).
+    // One warp = one task of 32*P particles walking the whole table.  P amortises the interpreter's per-record
+    // work (what matters when records are short: slots_per_record small) but coarsens the tasks: the last tasks
+    // of a launch run with few warps per SM sub-partition and cannot fill the FP64 pipe, so with long records
+    // (per-record work negligible) P is lowered until every sub-partition gets >= 24 tasks.  Measured on B200:
+    // config 1 (10^6 particles, 92 slots/record) 0.913 of the FP64 roofline at P = 4, 0.945 at P = 2; config 3
+    // (12 slots/record) 0.83 at P = 4, 0.76 at P = 2.  Small blocks keep the tasks balanced over SMs.
     const long long n = b->n;
     const int sms = b->num_sms > 0 ? b->num_sms : 148;
+    const long long sched = (long long)sms * 4;
+    auto tasks = [&](int p) { return n / (32LL * p) / sched; };  // tasks per sub-partition
     int P = 1;
-    const long long per = n / ((long long)sms * 8 * 32);
-    if (per >= 4) P = 4;
-    else if (per >= 2) P = 2;
-    if (!b->aligned16) P = 1;
-    int block = kMaxBlock;
+    if (b->aligned16) {
+        if (slots_per_record < 40.0) P = tasks(4) >= 4 ? 4 : tasks(2) >= 4 ? 2 : 1;
+        else P = tasks(4) >= 24 ? 4 : tasks(2) >= 12 ? 2 : 1;
+    }
+    int block = 64;
     while (block > 32 && n / ((long long)P * block) < 2LL * sms) block >>= 1;
     P = env_int("BT_TRACK_PPT", P);
     block = env_int("BT_TRACK_BLOCK", block);
-    if (!(P == 1 || ((P == 2 || P == 4) && b->aligned16))) return fail(BT_ERR_INVALID, "BT_TRACK_PPT must be 1, 2 or 4 (2, 4 need 16-byte aligned arrays)");
+    if (!(P == 1 || ((P == 2 || P == 4 || P == 8) && b->aligned16)))
+        return fail(BT_ERR_INVALID, "BT_TRACK_PPT must be 1, 2, 4 or 8 (2, 4, 8 need 16-byte aligned arrays)");
     if (block < 32 || block > kMaxBlock || (block & 31)) return fail(BT_ERR_INVALID, "BT_TRACK_BLOCK must be a multiple of 32 in [32,128]");
-
-    const size_t table_bytes = (size_t)n_ops * sizeof(DevOp);
-    const size_t smem_budget = b->max_smem_optin > 0 ? (size_t)b->max_smem_optin : (size_t)48 * 1024;
-    bool use_smem = table_bytes <= smem_budget / 2;  // keep >= 2 CTAs per SM resident
-    const int src = env_int("BT_TRACK_SRC", -1);  // 0: global, 1: shared
-    if (src == 0) use_smem = false;
-    if (src == 1 && table_bytes <= smem_budget) use_smem = true;
 
     TrackArgs a;
     for (int c = 0; c < 6; ++c) a.q[c] = b->q[c];
-    a.table = d_table;
     a.n = n;
     a.n_ops = n_ops;
     a.nturns = nturns;
-    a.turn_stride = turn_stride;
     const long long per_block = (long long)P * block;
     const long long full = n / per_block;
     a.n_full_blocks = (int)full;
@@ -373,25 +339,41 @@ int launch_track(Beam *b, const DevOp *d_table, int32_t n_ops, int32_t nturns, i
     const long long grid_ll = full + (rem + block - 1) / block;
     if (grid_ll > 0x7fffffffLL) return fail(BT_ERR_UNSUPPORTED, "bt_track: grid too large");
     const int grid = (int)grid_ll;
-    const size_t smem = use_smem ? table_bytes : 0;
 
-    cudaError_t e;
-    if (use_smem) {
-        e = P == 4 ? do_launch<4, true>(a, grid, block, smem, b->stream)
-          : P == 2 ? do_launch<2, true>(a, grid, block, smem, b->stream)
-                   : do_launch<1, true>(a, grid, block, smem, b->stream);
-    } else {
-        e = P == 4 ? do_launch<4, false>(a, grid, block, smem, b->stream)
-          : P == 2 ? do_launch<2, false>(a, grid, block, smem, b->stream)
-                   : do_launch<1, false>(a, grid, block, smem, b->stream);
+    ConstTableState &ct = g_ct[b->device];
+    std::lock_guard<std::mutex> lock(ct.mu);
+    if (!ct.busy) BT_CUDA_TRY(cudaEventCreateWithFlags(&ct.busy, cudaEventDisableTiming));
+    if (ct.owner != (const void *)b || ct.version != version) {
+        BT_CUDA_TRY(cudaStreamWaitEvent(b->stream, ct.busy, 0));  // previous readers of the table (any stream)
+        // pageable source: the call returns after the source has been staged
+        BT_CUDA_TRY(cudaMemcpyToSymbolAsync(c_table, h_table, (size_t)n_ops * sizeof(DevOp), 0, cudaMemcpyHostToDevice, b->stream));
+        ct.owner = (const void *)b;
+        ct.version = version;
     }
+    switch (P) {
+        case 8: track_kernel<8><<<grid, block, 0, b->stream>>>(a); break;
+        case 4: track_kernel<4><<<grid, block, 0, b->stream>>>(a); break;
+        case 2: track_kernel<2><<<grid, block, 0, b->stream>>>(a); break;
+        default: track_kernel<1><<<grid, block, 0, b->stream>>>(a); break;
+    }
+    cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return fail(BT_ERR_CUDA, std::string("bt_track launch: ") + cudaGetErrorString(e));
+    BT_CUDA_TRY(cudaEventRecord(ct.busy, b->stream));
     g_launch_count.fetch_add(1);
     b->last_launch.grid = grid;
     b->last_launch.block = block;
     b->last_launch.ppt = P;
-    b->last_launch.smem = (int32_t)smem;
+    b->last_launch.smem = 0;
+    b->last_launch.launches += 1;
     return BT_OK;
+}
+
+// A destroyed beam must not be mistaken for a later one allocated at the same address.
+void forget_table_owner(const Beam *b) {
+    if (b->device < 0 || b->device >= kMaxDevices) return;
+    ConstTableState &ct = g_ct[b->device];
+    std::lock_guard<std::mutex> lock(ct.mu);
+    if (ct.owner == (const void *)b) ct.owner = nullptr;
 }
 
 }  // namespace bt

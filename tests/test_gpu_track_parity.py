@@ -44,18 +44,17 @@ def test_config1_fodo_channel_reduced(n):
     check(got, ref)
 
 
-@pytest.mark.parametrize("ppt,src,block", [(1, 0, 32), (1, 1, 128), (2, 0, 64), (2, 1, 128), (4, 0, 128), (4, 1, 96)])
-def test_all_kernel_variants_agree(ppt, src, block, monkeypatch):
-    """Every (particles-per-thread, table source, block size) instantiation against the oracle, config-3 ring
-    (all op kinds except sbend/edge) and the chicane."""
+@pytest.mark.parametrize("ppt,block", [(1, 32), (1, 128), (2, 64), (2, 128), (4, 128), (4, 96), (4, 32), (8, 64), (8, 32)])
+def test_all_kernel_variants_agree(ppt, block, monkeypatch):
+    """Every (particles-per-thread, block size) instantiation against the oracle, config-3 ring (all op kinds except
+    sbend/edge; 7 turns of per-turn tables = 2 launches) and the chicane."""
     monkeypatch.setenv("BT_TRACK_PPT", str(ppt))
-    monkeypatch.setenv("BT_TRACK_SRC", str(src))
     monkeypatch.setenv("BT_TRACK_BLOCK", str(block))
     n = 4 * 128 * 3 + 201
     cfg = W.config(3, n=n)
     c = W.make_bunch(cfg)
     got, ref_state, launch = gpu_track(cfg, c, nturns=7)
-    assert launch["particles_per_thread"] == ppt and launch["block"] == block and (launch["smem_bytes"] > 0) == bool(src)
+    assert launch["particles_per_thread"] == ppt and launch["block"] == block
     ref, (g_ref, _) = oracle_track(cfg, c, nturns=7)
     check(got, ref)
     assert abs(ref_state[0] - g_ref) <= 1e-15 * g_ref
@@ -64,6 +63,58 @@ def test_all_kernel_variants_agree(ppt, src, block, monkeypatch):
     got, _, _ = gpu_track(cfg, c)
     ref, _ = oracle_track(cfg, c)
     check(got, ref)
+
+
+def test_record_fusion_is_bit_identical(monkeypatch):
+    """Peephole fusion of adjacent thin kicks / trailing drift into one record changes the dispatch count, not the
+    arithmetic: BT_TRACK_FUSE=0 (one record per element) must give the same bits."""
+    cfg = W.config(3, n=5000)
+    c = W.make_bunch(cfg)
+    fused, _, _ = gpu_track(cfg, c, nturns=3)
+    monkeypatch.setenv("BT_TRACK_FUSE", "0")
+    plain, _, _ = gpu_track(cfg, c, nturns=3)
+    assert all(np.array_equal(a, b) for a, b in zip(fused, plain))
+
+
+def test_lattice_longer_than_the_constant_bank():
+    """> 1024 records per turn: the walk is split into several launches per turn (static and per-turn tables)."""
+    cell = [("quad", 0.2, 1, 1.3), ("multipole", 0.0, 1, 3, 0.2, 0.0), ("drift", 0.1, 1), ("quad", 0.2, 7, -1.3),
+            ("multipole", 0.0, 1, 4, 2.0, 0.0), ("multipole", 0.0, 1, 3, -0.2, 0.0), ("multipole", 0.0, 1, 4, 0.9, 0.0), ("drift", 0.1, 2)]
+    lat = cell * 300                                   # 2400 elements -> 2400 records (one fused pair, one split quad per cell)
+    cfg = W.config(0, n=2500)
+    c = W.make_bunch(cfg)
+    got, _, _ = gpu_track(cfg, c, nturns=2, lattice=lat)
+    ref, _ = oracle_track(cfg, c, nturns=2, lattice=lat)
+    check(got, ref)
+    lat_rf = lat + [("shortrf", 0.0, 1, 1e-3, 1e7, -20.0)]
+    got, (g, _, _), _ = gpu_track(cfg, c, nturns=3, lattice=lat_rf)
+    ref, (g_ref, _) = oracle_track(cfg, c, nturns=3, lattice=lat_rf)
+    check(got, ref)
+    assert abs(g - g_ref) <= 1e-15 * g_ref
+
+
+def test_two_beams_share_the_constant_bank():
+    """The record table lives in the device's single constant bank: beams with different lattices on different
+    streams, interleaved, must each see their own table."""
+    import torch
+    import paper_2208_02382_b200 as bt
+    cfg_a, cfg_b = W.config(1, n=40_000), W.config(3, n=30_000)
+    ca, cb = W.make_bunch(cfg_a), W.make_bunch(cfg_b)
+    sa, sb = torch.cuda.Stream(), torch.cuda.Stream()
+    a = bt.Beam(cfg_a.n, stream=sa.cuda_stream)
+    b = bt.Beam(cfg_b.n, stream=sb.cuda_stream)
+    for beam, cfg, c in ((a, cfg_a, ca), (b, cfg_b, cb)):
+        beam.set_ref(cfg.kin_energy_MeV, cfg.mass_MeV, 1.0)
+        beam.lattice_set(cfg.lattice)
+        beam.upload(c)
+    for _ in range(3):
+        a.track(1)
+        b.track(2)
+    got_a, got_b = a.download(), b.download()
+    check(got_a, oracle_track(cfg_a, ca, nturns=3)[0])
+    check(got_b, oracle_track(cfg_b, cb, nturns=6)[0])
+    a.close()
+    b.close()
 
 
 def test_config2_chicane_reduced():
@@ -168,7 +219,7 @@ def test_config1_full_size_every_particle():
     got, _, launch = gpu_track(cfg, c)
     ref, _ = oracle_track(cfg, c)
     check(got, ref)
-    assert launch["particles_per_thread"] == 4
+    assert launch["particles_per_thread"] == 2      # long records: smaller tasks fill the tail better (track.cu)
 
 
 def test_config2_full_size_every_particle():
