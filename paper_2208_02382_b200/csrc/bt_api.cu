@@ -250,9 +250,11 @@ int bt_beam_create(bt_beam **out, int64_t n, double *const dev_ptrs[6], void *cu
         for (int i = 0; i < 6; ++i) b.q[i] = (double *)((char *)base + stride * i);
         b.owns = true;
     }
-    b.aligned16 = true;
-    for (int i = 0; i < 6; ++i)
+    b.aligned16 = b.aligned32 = true;
+    for (int i = 0; i < 6; ++i) {
         if (((uintptr_t)b.q[i]) & 15u) b.aligned16 = false;
+        if (((uintptr_t)b.q[i]) & 31u) b.aligned32 = false;
+    }
     *out = h;
     return BT_OK;
 }

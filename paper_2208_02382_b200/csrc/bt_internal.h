@@ -66,6 +66,7 @@ struct Beam {
     double *q[6] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
     bool owns = false;
     bool aligned16 = false;
+    bool aligned32 = false;  // all six arrays 32-byte aligned: 256-bit lane-run access in the grid kernels
     int device = 0;
     int num_sms = 0;
     int max_smem_optin = 0;

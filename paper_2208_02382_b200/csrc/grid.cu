@@ -38,16 +38,46 @@ __global__ void __launch_bounds__(256) deposit_atomic_kernel(const double *__res
     }
 }
 
-// ---- S5 deposit, mode 1 (default): run accumulation in registers + warp-segmented merge ------------
-// A warp owns chunks of 32*kRun consecutive particles (storage order); lane L walks particles
-// [L*kRun, (L+1)*kRun) of the chunk and keeps the 8 node sums of the CURRENT cell in registers, flushing
-// them with 8 RED.E.ADD.F64 only when the cell changes.  At the end of the chunk the lanes' open runs are
-// merged by a segmented shuffle reduction over equal cell keys (contiguous after bt_beam_sort_by_cell), so a
-// chunk that sits in one cell costs 8 global reductions for 256 particles.  Correct for ANY particle order:
-// unsorted input just degenerates to one flush per particle.  Weights are the canonical R11 expression, so
-// only the summation order differs from the definition.
-constexpr int kRun = 8;
+// ---- per-lane runs of R consecutive particles: 256-bit streaming access --------------------------------
+// A lane owns R consecutive particles of the storage order (R = 4 or 8), i.e. 32*R/4 bytes per array = whole
+// 32-byte sectors: every LDG.256 / STG.256 of a warp touches 32 distinct, fully used sectors.
+__device__ __forceinline__ void ld256(const double *p, double &a, double &b, double &c, double &d) {
+    asm volatile("ld.global.cs.v4.f64 {%0,%1,%2,%3}, [%4];" : "=d"(a), "=d"(b), "=d"(c), "=d"(d) : "l"(p));
+}
+__device__ __forceinline__ void st256(double *p, double a, double b, double c, double d) {
+    asm volatile("st.global.cs.v4.f64 [%0], {%1,%2,%3,%4};" ::"l"(p), "d"(a), "d"(b), "d"(c), "d"(d) : "memory");
+}
+// VEC: p0 + R <= n and 32-byte aligned arrays guaranteed by the caller; else guarded scalar loads with `fill`.
+template <int R, bool VEC>
+__device__ __forceinline__ void load_run(const double *__restrict__ q, long long p0, long long n, double fill, double (&v)[R]) {
+    if (VEC && p0 + R <= n) {
+#pragma unroll
+        for (int r = 0; r < R; r += 4) ld256(q + p0 + r, v[r], v[r + 1], v[r + 2], v[r + 3]);
+    } else {
+#pragma unroll
+        for (int r = 0; r < R; ++r) v[r] = (p0 + r < n) ? q[p0 + r] : fill;
+    }
+}
+template <int R, bool VEC>
+__device__ __forceinline__ void store_run(double *__restrict__ q, long long p0, long long n, const double (&v)[R]) {
+    if (VEC && p0 + R <= n) {
+#pragma unroll
+        for (int r = 0; r < R; r += 4) st256(q + p0 + r, v[r], v[r + 1], v[r + 2], v[r + 3]);
+    } else {
+#pragma unroll
+        for (int r = 0; r < R; ++r)
+            if (p0 + r < n) q[p0 + r] = v[r];
+    }
+}
 
+// ---- S5 deposit, mode 1 (default): run accumulation in registers + warp-segmented merge ------------
+// A warp owns chunks of 32*R consecutive particles (storage order); lane L walks particles [L*R, (L+1)*R) of
+// the chunk and keeps the 8 node sums of the CURRENT cell in registers, flushing them with 8 RED.E.ADD.F64 only
+// when the cell changes.  At the end of the chunk the lanes' open runs are merged by a segmented shuffle
+// reduction over equal cell keys (contiguous after bt_beam_sort_by_cell), so a chunk that sits in one cell costs
+// 8 global reductions for 32*R particles.  Correct for ANY particle order: unsorted input just degenerates to one
+// flush per particle.  Weights are the canonical R11 expression, so only the summation order differs from the
+// definition.
 __device__ __forceinline__ void flush_cell(double *__restrict__ rho, int key, const double (&acc)[8], int nx, long long nxy) {
     if (key < 0) return;
     double *base = rho + key;  // key = linear index of the lower-corner node
@@ -61,41 +91,27 @@ __device__ __forceinline__ void flush_cell(double *__restrict__ rho, int key, co
     atomicAdd(base + nxy + nx + 1, acc[7]);
 }
 
-template <bool VEC>
+template <int R, bool VEC>
 __global__ void __launch_bounds__(256) deposit_runs_kernel(const double *__restrict__ x, const double *__restrict__ y,
                                                            const double *__restrict__ t, long long n, GridDev g, double qw,
                                                            double zscale, double *__restrict__ rho) {
     const int lane = threadIdx.x & 31;
     const long long warp = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
     const long long nwarps = ((long long)gridDim.x * blockDim.x) >> 5;
-    const long long chunk = 32LL * kRun;
+    const long long chunk = 32LL * R;
     const long long nxy = (long long)g.nx * g.ny;
     for (long long c0 = warp * chunk; c0 < n; c0 += nwarps * chunk) {
-        const long long p0 = c0 + (long long)lane * kRun;
-        double px_[kRun], py_[kRun], pt_[kRun];
-        if (VEC && p0 + kRun <= n) {
-#pragma unroll
-            for (int r = 0; r < kRun; r += 2) {
-                const double2 a = __ldcs(reinterpret_cast<const double2 *>(x + p0 + r));
-                const double2 b = __ldcs(reinterpret_cast<const double2 *>(y + p0 + r));
-                const double2 c = __ldcs(reinterpret_cast<const double2 *>(t + p0 + r));
-                px_[r] = a.x, px_[r + 1] = a.y, py_[r] = b.x, py_[r + 1] = b.y, pt_[r] = c.x, pt_[r + 1] = c.y;
-            }
-        } else {
-#pragma unroll
-            for (int r = 0; r < kRun; ++r) {
-                const bool live = p0 + r < n;
-                px_[r] = live ? x[p0 + r] : CUDART_NAN;  // NaN => outside => contributes nothing
-                py_[r] = live ? y[p0 + r] : 0.0;
-                pt_[r] = live ? t[p0 + r] : 0.0;
-            }
-        }
+        const long long p0 = c0 + (long long)lane * R;
+        double px_[R], py_[R], pt_[R];
+        load_run<R, VEC>(x, p0, n, CUDART_NAN, px_);  // NaN => outside => contributes nothing
+        load_run<R, VEC>(y, p0, n, 0.0, py_);
+        load_run<R, VEC>(t, p0, n, 0.0, pt_);
         int cur = -1;
         double acc[8];
 #pragma unroll
         for (int d = 0; d < 8; ++d) acc[d] = 0.0;
 #pragma unroll
-        for (int r = 0; r < kRun; ++r) {
+        for (int r = 0; r < R; ++r) {
             Cic c;
             const bool in = cic_locate(g, px_[r], py_[r], pt_[r], zscale, c);
             const int key = in ? (c.k * g.ny + c.j) * g.nx + c.i : -1;
@@ -144,24 +160,33 @@ static int env_int_grid(const char *name, int dflt) {
     return (v && *v) ? atoi(v) : dflt;
 }
 
+template <int R>
+static void launch_deposit_runs(Beam *b, Grid *g, const GridDev &gd, double q_weight, double zscale) {
+    const int block = 256;
+    const long long per_block = (long long)block * R;
+    long long blocks = (b->n + per_block - 1) / per_block;
+    const long long cap = (long long)b->num_sms * 8;
+    if (blocks > cap) blocks = cap;
+    if (b->aligned32)
+        deposit_runs_kernel<R, true><<<(int)blocks, block, 0, b->stream>>>(b->q[0], b->q[2], b->q[4], b->n, gd, q_weight, zscale, g->rho);
+    else
+        deposit_runs_kernel<R, false><<<(int)blocks, block, 0, b->stream>>>(b->q[0], b->q[2], b->q[4], b->n, gd, q_weight, zscale, g->rho);
+}
+
 int launch_deposit(Beam *b, Grid *g, double q_weight, double zscale) {
     const GridDev gd = make_grid_dev(*g);
+    // mode 0: one particle per thread, 8 reductions each; 1: lane runs of 4; 2: lane runs of 8
     const int mode = env_int_grid("BT_DEPOSIT_MODE", 1);
-    const int block = 256;
     if (mode == 0) {
+        const int block = 256;
         long long blocks = (b->n + block - 1) / block;
         const long long cap = (long long)b->num_sms * 16;
         if (blocks > cap) blocks = cap;
         deposit_atomic_kernel<<<(int)blocks, block, 0, b->stream>>>(b->q[0], b->q[2], b->q[4], b->n, gd, q_weight, zscale, g->rho);
+    } else if (mode == 2) {
+        launch_deposit_runs<8>(b, g, gd, q_weight, zscale);
     } else {
-        const long long per_block = (long long)block * kRun;
-        long long blocks = (b->n + per_block - 1) / per_block;
-        const long long cap = (long long)b->num_sms * 8;
-        if (blocks > cap) blocks = cap;
-        if (b->aligned16)
-            deposit_runs_kernel<true><<<(int)blocks, block, 0, b->stream>>>(b->q[0], b->q[2], b->q[4], b->n, gd, q_weight, zscale, g->rho);
-        else
-            deposit_runs_kernel<false><<<(int)blocks, block, 0, b->stream>>>(b->q[0], b->q[2], b->q[4], b->n, gd, q_weight, zscale, g->rho);
+        launch_deposit_runs<4>(b, g, gd, q_weight, zscale);
     }
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return fail(BT_ERR_CUDA, std::string("bt_deposit_cic launch: ") + cudaGetErrorString(e));
@@ -248,6 +273,83 @@ __global__ void __launch_bounds__(256) gather_kick_kernel(const __grid_constant_
     }
 }
 
+// ---- S6/S7 for cell-sorted storage: lane runs of 4 consecutive particles, field of the current cell cached ----
+// Same arithmetic as gather_kick_kernel per particle.  A lane keeps the 8 node records (24 doubles) of the cell it
+// is in and reloads them only when the next particle of its run sits in another cell; particle I/O is one 256-bit
+// streaming access per array per lane (6 loads, 6 stores per 4 particles, every sector fully used), all issued
+// before the first field access, so a warp has 6 KiB of particle data in flight.
+template <bool VEC>
+__global__ void __launch_bounds__(128) gather_kick_runs_kernel(const __grid_constant__ GatherArgs a) {
+    constexpr int R = 4;
+    const int lane = threadIdx.x & 31;
+    const long long warp = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+    const long long nwarps = ((long long)gridDim.x * blockDim.x) >> 5;
+    const long long chunk = 32LL * R;
+    for (long long c0 = warp * chunk; c0 < a.n; c0 += nwarps * chunk) {
+        const long long p0 = c0 + (long long)lane * R;
+        double x[R], px[R], y[R], py[R], t[R], pt[R];
+        load_run<R, VEC>(a.q[0], p0, a.n, CUDART_NAN, x);
+        load_run<R, VEC>(a.q[1], p0, a.n, 0.0, px);
+        load_run<R, VEC>(a.q[2], p0, a.n, 0.0, y);
+        load_run<R, VEC>(a.q[3], p0, a.n, 0.0, py);
+        load_run<R, VEC>(a.q[4], p0, a.n, 0.0, t);
+        load_run<R, VEC>(a.q[5], p0, a.n, 0.0, pt);
+        int cur = -1;
+        double fx[8], fy[8], fz[8];
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            // R4 drift before the kick
+            x[r] = fma(a.hb, px[r], x[r]);
+            y[r] = fma(a.hb, py[r], y[r]);
+            t[r] = fma(a.tcb, pt[r], t[r]);
+            Cic c;
+            if (cic_locate(a.g, x[r], y[r], t[r], a.zscale, c)) {
+                const int key = (c.k * a.g.ny + c.j) * a.g.nx + c.i;
+                if (key != cur) {
+                    cur = key;
+                    const double *base = a.field + 4 * (long long)key;
+#pragma unroll
+                    for (int dz = 0; dz < 2; ++dz)
+#pragma unroll
+                        for (int dy = 0; dy < 2; ++dy)
+#pragma unroll
+                            for (int dx = 0; dx < 2; ++dx)
+                                ld_node(base + 4 * (((long long)dz * a.g.ny + dy) * a.g.nx + dx), fx[dz * 4 + dy * 2 + dx],
+                                        fy[dz * 4 + dy * 2 + dx], fz[dz * 4 + dy * 2 + dx]);
+                }
+                const double wx[2] = {__dsub_rn(1.0, c.wx1), c.wx1};
+                const double wy[2] = {__dsub_rn(1.0, c.wy1), c.wy1};
+                const double wz[2] = {__dsub_rn(1.0, c.wz1), c.wz1};
+                double ex = 0.0, ey = 0.0, ez = 0.0;
+#pragma unroll
+                for (int dz = 0; dz < 2; ++dz)
+#pragma unroll
+                    for (int dy = 0; dy < 2; ++dy)
+#pragma unroll
+                        for (int dx = 0; dx < 2; ++dx) {
+                            const double w = __dmul_rn(__dmul_rn(wx[dx], wy[dy]), wz[dz]);
+                            ex = fma(w, fx[dz * 4 + dy * 2 + dx], ex);
+                            ey = fma(w, fy[dz * 4 + dy * 2 + dx], ey);
+                            ez = fma(w, fz[dz * 4 + dy * 2 + dx], ez);
+                        }
+                px[r] = fma(a.coef[0], ex, px[r]);
+                py[r] = fma(a.coef[1], ey, py[r]);
+                pt[r] = fma(a.coef[2], ez, pt[r]);
+            }
+            // R4 drift after the kick
+            x[r] = fma(a.ha, px[r], x[r]);
+            y[r] = fma(a.ha, py[r], y[r]);
+            t[r] = fma(a.tca, pt[r], t[r]);
+        }
+        store_run<R, VEC>(a.q[0], p0, a.n, x);
+        store_run<R, VEC>(a.q[1], p0, a.n, px);
+        store_run<R, VEC>(a.q[2], p0, a.n, y);
+        store_run<R, VEC>(a.q[3], p0, a.n, py);
+        store_run<R, VEC>(a.q[4], p0, a.n, t);
+        store_run<R, VEC>(a.q[5], p0, a.n, pt);
+    }
+}
+
 int launch_gather_kick(Beam *b, const Grid *g, const double coef[3], double zscale, double h_before, double tc_before,
                        double h_after, double tc_after) {
     GatherArgs a;
@@ -261,11 +363,25 @@ int launch_gather_kick(Beam *b, const Grid *g, const double coef[3], double zsca
     a.tcb = tc_before;
     a.ha = h_after;
     a.tca = tc_after;
-    const int block = 256;
-    long long blocks = (b->n + block - 1) / block;
-    const long long cap = (long long)b->num_sms * 16;
-    if (blocks > cap) blocks = cap;
-    gather_kick_kernel<<<(int)blocks, block, 0, b->stream>>>(a);
+    // cell-sorted storage (bt_beam_sort_by_cell since the last upload): lane runs with the cell's field cached;
+    // any other order: one particle per thread.  BT_GATHER_MODE=0/1 forces one of them (both are correct for any order).
+    const int mode = env_int_grid("BT_GATHER_MODE", b->permuted ? 1 : 0);
+    if (mode == 1) {
+        const int block = 128;
+        long long blocks = (b->n + block * 4LL - 1) / (block * 4LL);
+        const long long cap = (long long)b->num_sms * 16;
+        if (blocks > cap) blocks = cap;
+        if (b->aligned32)
+            gather_kick_runs_kernel<true><<<(int)blocks, block, 0, b->stream>>>(a);
+        else
+            gather_kick_runs_kernel<false><<<(int)blocks, block, 0, b->stream>>>(a);
+    } else {
+        const int block = 256;
+        long long blocks = (b->n + block - 1) / block;
+        const long long cap = (long long)b->num_sms * 16;
+        if (blocks > cap) blocks = cap;
+        gather_kick_kernel<<<(int)blocks, block, 0, b->stream>>>(a);
+    }
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return fail(BT_ERR_CUDA, std::string("bt_gather_kick launch: ") + cudaGetErrorString(e));
     g_launch_count.fetch_add(1);
