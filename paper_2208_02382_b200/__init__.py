@@ -256,6 +256,16 @@ class Grid:
         _check(lib.bt_grid_rho(self._h, C.byref(p)), "bt_grid_rho")
         return int(p.value)
 
+    def rho_tensor(self):
+        """Zero-copy torch view [nz, ny, nx] of the library-owned rho (valid until close())."""
+        import torch
+        nx, ny, nz = self.shape
+
+        class _View:  # CUDA Array Interface v3 over the raw device pointer
+            __cuda_array_interface__ = {"shape": (nz, ny, nx), "typestr": "<f8", "data": (self.rho_ptr(), False),
+                                        "version": 3, "strides": None}
+        return torch.as_tensor(_View(), device="cuda")
+
     def download_rho(self):
         nx, ny, nz = self.shape
         out = np.empty((nz, ny, nx), dtype=np.float64)
