@@ -117,7 +117,8 @@ class ClockSampler:
 def get_workload(name, rank):
     idx = {"tiny_fodo": 0, "fodo_channel": 1, "chicane": 2, "nonlinear_ring": 3}[name]
     cfg = W.config(idx)
-    cfg.seed = cfg.seed + 1000 * rank      # every rank its own bunch (weak scaling)
+    from paper_2208_02382_b200.shard import rank_seed
+    cfg.seed = rank_seed(cfg.seed, rank)   # every rank its own bunch (weak scaling)
     return cfg
 
 
@@ -143,17 +144,24 @@ def run_reference(args):
     if rank != 0:
         return 0
     cfg = get_workload(args.workload, 0)
-    n_sample = min(cfg.n, args.ref_sample)
-    for _ in range(args.warmup and 1):
-        oracle_rate(cfg, max(1000, n_sample // 20))
-    pushes, times, cores = oracle_rate(cfg, n_sample, reps=max(1, min(args.steps, 5)))
+    # W warm-up steps on a small sample also calibrate the rate; the per-step sample is then sized so that the
+    # K timed steps take about REF_BUDGET_S seconds in total (bounded sample of the same workload).
+    REF_BUDGET_S = 60.0
+    n_cal = min(cfg.n, 20_000)
+    rate = None
+    for _ in range(max(1, args.warmup)):
+        p, tms, _c = oracle_rate(cfg, n_cal)
+        rate = n_cal / tms[0]                                   # particles (through the full lattice) per second
+    n_sample = args.ref_sample if args.ref_sample > 0 else int(rate * REF_BUDGET_S / max(1, args.steps))
+    n_sample = max(1000, min(cfg.n, n_sample))
+    pushes, times, cores = oracle_rate(cfg, n_sample, reps=max(1, args.steps))
     t = sum(times) / len(times)
     value = pushes / t
     sample = "%d of %d particles (seed %d), full lattice (%d elements, %d slice maps), %d turn(s) per step" % (
         n_sample, cfg.n, cfg.seed, cfg.n_elements, cfg.slice_maps_per_turn, cfg.nturns)
     line = {
         "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": len(times),
-        "warmup": 1, "ms_per_step": t * 1e3, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "warmup": max(1, args.warmup), "ms_per_step": t * 1e3, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f64", "data": "synthetic",
         "config": {"workload": "configs[1] " + cfg.name + " (bounded sample)", "particles": n_sample,
                    "elements": cfg.n_elements, "slice_maps_per_turn": cfg.slice_maps_per_turn, "turns": cfg.nturns},
@@ -163,6 +171,124 @@ def run_reference(args):
     }
     print(json.dumps(line), flush=True)
     return 0
+
+
+# ---------------------------------------------------------------------------------------------------
+# the rest of the hot path (N = 1): the other tracking configs and the space-charge kernels of configs[4]
+# ---------------------------------------------------------------------------------------------------
+def _event_ms(torch, fn, reps, flush, pre=None):
+    """CUDA-event time of fn() on the current stream; L2 flushed (and `pre` run) before each repetition, outside."""
+    ts = []
+    for _ in range(reps):
+        if pre:
+            pre()
+        flush.zero_()
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record()
+        fn()
+        b.record()
+        torch.cuda.synchronize()
+        ts.append(a.elapsed_time(b))
+    return ts
+
+
+def bench_other_configs(bt, torch, flush, peaks, nominal_peak):
+    """bt_track on configs[0], [2], [3] at full size (one call = the config's nturns).  configs[3]'s 64e6-particle
+    bunch is a seeded 10^6-particle draw tiled 64 times on the device (timing does not depend on the values)."""
+    out = []
+    hbm = float(peaks["hbm_gbs"]) * 1e9
+    for idx, reps in ((0, 5), (2, 5), (3, 2)):
+        cfg = W.config(idx)
+        n = cfg.n
+        base = W.make_bunch(cfg, n=min(n, 1_000_000))
+        tile = -(-n // len(base[0]))
+        pristine = [torch.from_numpy(a).cuda().repeat(tile)[:n].contiguous() for a in base]
+        beam = bt.Beam(n)
+        beam.lattice_set(cfg.lattice)
+
+        def restore():
+            for d, s in zip(beam.tensors, pristine):
+                d.copy_(s)
+            beam.set_ref(cfg.kin_energy_MeV, cfg.mass_MeV, cfg.charge_qe)   # RF lattices: same energy every repetition
+
+        restore()
+        beam.track(cfg.nturns)
+        launches0 = bt.launch_count()
+        ts = _event_ms(torch, lambda: beam.track(cfg.nturns), reps, flush, restore)
+        launches = (bt.launch_count() - launches0) // reps
+        t = statistics.mean(ts) * 1e-3
+        slots = float(n) * slots_per_particle_per_turn(cfg.lattice) * cfg.nturns
+        t_alu, t_hbm = slots / nominal_peak, 96.0 * n * launches / hbm
+        li = beam.last_launch()
+        entry = {"workload": "configs[%d] %s" % (idx, cfg.name), "particles": n, "elements": cfg.n_elements, "turns": cfg.nturns,
+                 "ms_per_call": t * 1e3, "pushes_per_s": n * cfg.n_elements * cfg.nturns / t, "launches_per_call": launches,
+                 "kernel": "bt::track_kernel<P=%d> grid=%d block=%d" % (li["particles_per_thread"], li["grid"], li["block"])}
+        if idx == 0:
+            entry["roofline"] = {"bound": "latency", "note": "10^4 particles = 313 warps on 148 SMs: neither pipe nor HBM can be filled "
+                                 "(SURVEY 8d); roofline time %.2f us shown for information" % (max(t_alu, t_hbm) * 1e6)}
+        elif t_alu >= t_hbm:
+            entry["roofline"] = {"bound": "alu", "achieved": slots / t / 1e12, "peak": nominal_peak / 1e12, "unit": "Tslot/s",
+                                 "frac": t_alu / t}
+        else:
+            entry["roofline"] = {"bound": "hbm", "achieved": 96.0 * n * launches / t / 1e9, "peak": hbm / 1e9, "unit": "GB/s",
+                                 "frac": t_hbm / t}
+        out.append(entry)
+        beam.close()
+        del pristine, beam
+        torch.cuda.empty_cache()
+    return out
+
+
+def bench_spacecharge(bt, torch, flush, peaks):
+    """configs[4] A and B at full size (8e6 particles, 128^3 nodes): bt_beam_sort_by_cell once, then 10 steps of
+    bt_deposit_cic + bt_gather_kick(0, ds) (SURVEY 8d call sequence), every call timed with CUDA events, L2 flushed
+    before each.  GB/s = ALGORITHMIC bytes / time: deposit 24 B/particle + 2 x 8 B/node (zeroing + result);
+    gather+kick+drift 96 B/particle + 24 B/node."""
+    hbm = float(peaks["hbm_gbs"])
+    out = {}
+    for variant in ("A", "B"):
+        sc = W.spacecharge_config(variant)
+        c = W.make_spacecharge_bunch(sc)
+        E = W.gaussian_bunch_field(sc)
+        n, nn = sc.n, sc.shape[0] * sc.shape[1] * sc.shape[2]
+        dep_bytes, gat_bytes = 24.0 * n + 16.0 * nn, 96.0 * n + 24.0 * nn
+        beam, grid = bt.Beam(n), bt.Grid(sc.shape, sc.lo, sc.d)
+        beam.set_ref(sc.kin_energy_MeV, sc.mass_MeV, sc.charge_qe)
+        grid.set_field(*E)
+        beam.lattice_set([("drift", sc.ds / 2, 1)])
+        beam.upload(c)
+        beam.track(1)                                              # leading half drift
+        # unsorted (caller's order), one call each, for information
+        beam.deposit_cic(grid, sc.q_weight, sc.zscale, True)       # warm-up
+        t_dep_u = min(_event_ms(torch, lambda: beam.deposit_cic(grid, sc.q_weight, sc.zscale, True), 2, flush))
+        pos = [t.clone() for t in beam.tensors]
+        t_gat_u = min(_event_ms(torch, lambda: beam.gather_kick(grid, sc.kick_coef, sc.zscale, 0.0, 0.0), 2, flush))
+        for d, s in zip(beam.tensors, pos):
+            d.copy_(s)
+        del pos
+        t_sort = _event_ms(torch, lambda: beam.sort_by_cell(grid, sc.zscale), 1, flush)[0]
+        t_dep, t_gat = [], []
+        for step in range(sc.nsteps):
+            t_dep += _event_ms(torch, lambda: beam.deposit_cic(grid, sc.q_weight, sc.zscale, True), 1, flush)
+            after = sc.ds if step < sc.nsteps - 1 else sc.ds / 2
+            t_gat += _event_ms(torch, lambda: beam.gather_kick(grid, sc.kick_coef, sc.zscale, 0.0, after), 1, flush)
+        md, mg = statistics.mean(t_dep) * 1e-3, statistics.mean(t_gat) * 1e-3
+        out[variant] = {
+            "workload": "configs[4] %s, %d particles, %dx%dx%d nodes, %d steps" % ((sc.name, n) + tuple(sc.shape) + (sc.nsteps,)),
+            "sort_by_cell_ms_once": t_sort,
+            "deposit": {"ms": md * 1e3, "ms_first_last": [t_dep[0], t_dep[-1]], "unsorted_ms": t_dep_u,
+                        "roofline": {"bound": "hbm", "achieved": dep_bytes / md / 1e9, "peak": hbm, "unit": "GB/s",
+                                     "frac": dep_bytes / md / 1e9 / hbm, "traffic": None}},
+            "gather_kick_drift": {"ms": mg * 1e3, "ms_first_last": [t_gat[0], t_gat[-1]], "unsorted_kick_only_ms": t_gat_u,
+                                  "roofline": {"bound": "hbm", "achieved": gat_bytes / mg / 1e9, "peak": hbm, "unit": "GB/s",
+                                               "frac": gat_bytes / mg / 1e9 / hbm, "traffic": None}},
+            "ms_per_step_incl_sort_amortised": (md + mg) * 1e3 + t_sort / sc.nsteps,
+        }
+        beam.close()
+        grid.close()
+        del beam, grid
+        torch.cuda.empty_cache()
+    return out
 
 
 # ---------------------------------------------------------------------------------------------------
@@ -245,10 +371,8 @@ def run_ours(args):
     clocks = sampler.stop() if rank == 0 else None
 
     # max over ranks
-    tt = torch.tensor([ms_sum, t_e2e, t_wall], dtype=torch.float64, device="cuda")
-    if world > 1:
-        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-    ms_sum, t_e2e, t_wall = [float(v) for v in tt.cpu()]
+    from paper_2208_02382_b200.shard import max_over_ranks
+    ms_sum, t_e2e, t_wall = max_over_ranks([ms_sum, t_e2e, t_wall], device="cuda")
     launch_info = beam.last_launch()
 
     result = None
@@ -281,9 +405,20 @@ def run_ours(args):
         roof["roofline_time_ms"] = max(alu_time_ms, hbm_time_ms)
         roof["rw6_stream_ceiling_gbs"] = measured_rw6
         # CPU baseline: the oracle as it stands, bounded sample, host cores
-        cb_pushes, cb_times, cores = oracle_rate(get_workload(args.workload, 0), min(n, args.ref_sample))
-        cpu_baseline = {"value": cb_pushes / cb_times[0], "unit": UNIT, "cores": cores, "kind": "oracle",
-                        "sample": "%d of %d particles, full lattice, %d turn(s); %.1f s" % (min(n, args.ref_sample), n, cfg.nturns, cb_times[0])}
+        cb_cfg = get_workload(args.workload, 0)
+        n_cb = min(n, 1_000_000)
+        cb_times, cores, cb_pushes = [], 0, 0
+        while sum(cb_times) < 10.0 and len(cb_times) < 12:       # about 10-30 s of CPU work
+            cb_pushes, tms, cores = oracle_rate(cb_cfg, n_cb)
+            cb_times += tms
+        cb_t = sum(cb_times) / len(cb_times)
+        cpu_baseline = {"value": cb_pushes / cb_t, "unit": UNIT, "cores": cores, "kind": "oracle",
+                        "sample": "%d of %d particles, full lattice (%d slice maps), %d turn(s); %d repetitions, %.1f s of CPU work in total"
+                                  % (n_cb, n, cfg.slice_maps_per_turn, cfg.nturns, len(cb_times), sum(cb_times))}
+        extras = {}
+        if world == 1 and not args.no_extras:
+            extras["other_configs"] = bench_other_configs(bt, torch, flush, peaks, nominal_peak)
+            extras["spacecharge"] = bench_spacecharge(bt, torch, flush, peaks)
         result = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
             "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
@@ -299,6 +434,7 @@ def run_ours(args):
             "step_ms_min_median_max": [min(step_ms), statistics.median(step_ms), max(step_ms)],
             "wall_s_timed_region": t_wall,
         }
+        result.update(extras)
     beam.close()
     if world > 1:
         dist.destroy_process_group()
@@ -314,7 +450,10 @@ def main():
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="fodo_channel", choices=["tiny_fodo", "fodo_channel", "chicane", "nonlinear_ring"])
-    ap.add_argument("--ref-sample", type=int, default=200_000, help="particles of the workload the oracle is timed on")
+    ap.add_argument("--ref-sample", type=int, default=0,
+                    help="particles per step the oracle is timed on in --impl reference (0 = sized for ~60 s in total)")
+    ap.add_argument("--no-extras", action="store_true",
+                    help="skip the other configs and the space-charge kernels (N=1 only; the headline is unchanged)")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
