@@ -34,12 +34,17 @@ struct Cic {
     double wx1, wy1, wz1;
 };
 
+// floor(u) without the conversion pipe: for 0 <= u < 2^31, u + 1.5*2^52 rounded toward -inf is exactly
+// 1.5*2^52 + floor(u) (the ulp there is 1), whose low mantissa word is floor(u) as an integer; subtracting the magic
+// constant back is exact.  Two DADDs on the FP64 pipe instead of FRND.F64 + F2I.F64 (quarter-rate conversions).
+// Outside the grid (u < 0, u >= n-1, NaN) the index is forced to 0 and the weight is never used.
 __device__ __forceinline__ bool cic_axis(double q, double lo, double inv_d, double umax, int &i, double &w1) {
+    const double kMagic = 6755399441055744.0;  // 1.5 * 2^52 = 0x4338000000000000
     const double u = __dmul_rn(__dsub_rn(q, lo), inv_d);
     const bool in = (u >= 0.0) && (u < umax);
-    const double fl = floor(u);
-    i = in ? __double2int_rd(u) : 0;
-    w1 = __dsub_rn(u, fl);
+    const double tt = __dadd_rd(u, kMagic);
+    i = in ? __double2loint(tt) : 0;
+    w1 = __dsub_rn(u, __dsub_rn(tt, kMagic));
     return in;
 }
 
