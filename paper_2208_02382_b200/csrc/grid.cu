@@ -8,6 +8,7 @@
 // Inside iff 0 <= i <= n-2 on all axes, tested as (u >= 0 && u < n-1) so NaN is outside (R13).
 #include "bt_internal.h"
 #include "grid_dev.cuh"
+#include "bulk_copy.cuh"
 
 #include <math_constants.h>
 #include <stdlib.h>
@@ -44,9 +45,6 @@ __global__ void __launch_bounds__(256) deposit_atomic_kernel(const double *__res
 __device__ __forceinline__ void ld256(const double *p, double &a, double &b, double &c, double &d) {
     asm volatile("ld.global.cs.v4.f64 {%0,%1,%2,%3}, [%4];" : "=d"(a), "=d"(b), "=d"(c), "=d"(d) : "l"(p));
 }
-__device__ __forceinline__ void st256(double *p, double a, double b, double c, double d) {
-    asm volatile("st.global.cs.v4.f64 [%0], {%1,%2,%3,%4};" ::"l"(p), "d"(a), "d"(b), "d"(c), "d"(d) : "memory");
-}
 // VEC: p0 + R <= n and 32-byte aligned arrays guaranteed by the caller; else guarded scalar loads with `fill`.
 template <int R, bool VEC>
 __device__ __forceinline__ void load_run(const double *__restrict__ q, long long p0, long long n, double fill, double (&v)[R]) {
@@ -58,26 +56,7 @@ __device__ __forceinline__ void load_run(const double *__restrict__ q, long long
         for (int r = 0; r < R; ++r) v[r] = (p0 + r < n) ? q[p0 + r] : fill;
     }
 }
-template <int R, bool VEC>
-__device__ __forceinline__ void store_run(double *__restrict__ q, long long p0, long long n, const double (&v)[R]) {
-    if (VEC && p0 + R <= n) {
-#pragma unroll
-        for (int r = 0; r < R; r += 4) st256(q + p0 + r, v[r], v[r + 1], v[r + 2], v[r + 3]);
-    } else {
-#pragma unroll
-        for (int r = 0; r < R; ++r)
-            if (p0 + r < n) q[p0 + r] = v[r];
-    }
-}
-
-// ---- S5 deposit, mode 1 (default): run accumulation in registers + warp-segmented merge ------------
-// A warp owns chunks of 32*R consecutive particles (storage order); lane L walks particles [L*R, (L+1)*R) of
-// the chunk and keeps the 8 node sums of the CURRENT cell in registers, flushing them with 8 RED.E.ADD.F64 only
-// when the cell changes.  At the end of the chunk the lanes' open runs are merged by a segmented shuffle
-// reduction over equal cell keys (contiguous after bt_beam_sort_by_cell), so a chunk that sits in one cell costs
-// 8 global reductions for 32*R particles.  Correct for ANY particle order: unsorted input just degenerates to one
-// flush per particle.  Weights are the canonical R11 expression, so only the summation order differs from the
-// definition.
+// ---- run flush: the 8 node sums of one cell -> 8 RED.E.ADD.F64 ------------------------------------------------
 __device__ __forceinline__ void flush_cell(double *__restrict__ rho, int key, const double (&acc)[8], int nx, long long nxy) {
     if (key < 0) return;
     double *base = rho + key;  // key = linear index of the lower-corner node
@@ -91,71 +70,7 @@ __device__ __forceinline__ void flush_cell(double *__restrict__ rho, int key, co
     atomicAdd(base + nxy + nx + 1, acc[7]);
 }
 
-template <int R, bool VEC>
-__global__ void __launch_bounds__(256) deposit_runs_kernel(const double *__restrict__ x, const double *__restrict__ y,
-                                                           const double *__restrict__ t, long long n, GridDev g, double qw,
-                                                           double zscale, double *__restrict__ rho) {
-    const int lane = threadIdx.x & 31;
-    const long long warp = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
-    const long long nwarps = ((long long)gridDim.x * blockDim.x) >> 5;
-    const long long chunk = 32LL * R;
-    const long long nxy = (long long)g.nx * g.ny;
-    for (long long c0 = warp * chunk; c0 < n; c0 += nwarps * chunk) {
-        const long long p0 = c0 + (long long)lane * R;
-        double px_[R], py_[R], pt_[R];
-        load_run<R, VEC>(x, p0, n, CUDART_NAN, px_);  // NaN => outside => contributes nothing
-        load_run<R, VEC>(y, p0, n, 0.0, py_);
-        load_run<R, VEC>(t, p0, n, 0.0, pt_);
-        int cur = -1;
-        double acc[8];
-#pragma unroll
-        for (int d = 0; d < 8; ++d) acc[d] = 0.0;
-#pragma unroll
-        for (int r = 0; r < R; ++r) {
-            Cic c;
-            const bool in = cic_locate(g, px_[r], py_[r], pt_[r], zscale, c);
-            const int key = in ? (c.k * g.ny + c.j) * g.nx + c.i : -1;
-            const double wx0 = __dsub_rn(1.0, c.wx1), wy0 = __dsub_rn(1.0, c.wy1), wz0 = __dsub_rn(1.0, c.wz1);
-            double w[8];
-            w[0] = __dmul_rn(qw, __dmul_rn(__dmul_rn(wx0, wy0), wz0));
-            w[1] = __dmul_rn(qw, __dmul_rn(__dmul_rn(c.wx1, wy0), wz0));
-            w[2] = __dmul_rn(qw, __dmul_rn(__dmul_rn(wx0, c.wy1), wz0));
-            w[3] = __dmul_rn(qw, __dmul_rn(__dmul_rn(c.wx1, c.wy1), wz0));
-            w[4] = __dmul_rn(qw, __dmul_rn(__dmul_rn(wx0, wy0), c.wz1));
-            w[5] = __dmul_rn(qw, __dmul_rn(__dmul_rn(c.wx1, wy0), c.wz1));
-            w[6] = __dmul_rn(qw, __dmul_rn(__dmul_rn(wx0, c.wy1), c.wz1));
-            w[7] = __dmul_rn(qw, __dmul_rn(__dmul_rn(c.wx1, c.wy1), c.wz1));
-            if (key != cur) {
-                flush_cell(rho, cur, acc, g.nx, nxy);
-                cur = key;
-#pragma unroll
-                for (int d = 0; d < 8; ++d) acc[d] = w[d];
-            } else if (in) {
-#pragma unroll
-                for (int d = 0; d < 8; ++d) acc[d] += w[d];
-            }
-        }
-        // merge the lanes' open runs: segmented suffix reduction over CONTIGUOUS equal keys (after a cell
-        // sort equal keys are contiguous; for arbitrary order non-adjacent equal keys stay separate runs)
-        const int prev = __shfl_up_sync(0xffffffffu, cur, 1);
-        const bool head = (lane == 0) || (prev != cur);
-        const unsigned heads = __ballot_sync(0xffffffffu, head);
-        const unsigned above = (lane == 31) ? 0u : (heads >> (lane + 1));
-        const int end = above ? lane + __ffs(above) - 1 : 31;  // last lane of this lane's run
-#pragma unroll
-        for (int d = 1; d < 32; d <<= 1) {
-            const bool take = lane + d <= end;
-#pragma unroll
-            for (int k = 0; k < 8; ++k) {
-                const double o = __shfl_down_sync(0xffffffffu, acc[k], d);
-                if (take) acc[k] += o;
-            }
-        }
-        if (head) flush_cell(rho, cur, acc, g.nx, nxy);
-    }
-}
-
-// ---- S4+S5 deposit, mode 3 (default): block-local cell binning in shared memory + run accumulation ------------
+// ---- S4+S5 deposit, mode 1 (default): block-local cell binning in shared memory + run accumulation ------------
 // A block owns chunks of 256*R consecutive particles (storage order).  The particles of a chunk are binned by cell
 // INSIDE the block (counting sort over the chunk's bounding box of cells: one shared-memory integer atomic per
 // particle gives count and rank at once, a block scan gives the offsets), so that afterwards every thread walks R
@@ -191,8 +106,10 @@ __device__ __forceinline__ void merge_and_flush(double *__restrict__ rho, int cu
     if (heads != 0xffffffffu) {  // warp-uniform: some run spans lanes
         const unsigned above = (lane == 31) ? 0u : (heads >> (lane + 1));
         const int end = above ? lane + __ffs(above) - 1 : 31;  // last lane of this lane's run
+        const int span = __reduce_max_sync(0xffffffffu, end - lane);
 #pragma unroll
         for (int d = 1; d < 32; d <<= 1) {
+            if (d > span) break;  // warp-uniform
             const bool take = lane + d <= end;
 #pragma unroll
             for (int k = 0; k < 8; ++k) {
@@ -208,23 +125,40 @@ template <int R>
 struct BinSmem {
     static constexpr int CH = kBinBlock * R;
     static constexpr int PAD = CH + CH / 8;  // one pad slot per 8 entries: a thread's R-entry walk is conflict-free
-    int hist[kBinCap + 1];
-    int box[2][6];  // imin, jmin, kmin, imax, jmax, kmax; double-buffered by chunk parity (no extra barrier)
+    alignas(16) int hist[kBinCap + 16];      // bins [0, ncell) = cells of the box, bin kBinCap = particles that are not binned
+    int box[2][8];  // imin, jmin, kmin, imax, jmax, kmax, lowest thread holding an inside particle; double-buffered by chunk parity
+    int anchor[4];
     int warp_tot[kBinBlock / 32];
     int key[PAD];
     double w1[3][PAD];
 };
 
+__device__ __forceinline__ void run_add(double *__restrict__ rho, int key, const double (&w)[8], int &cur, double (&acc)[8], int nx,
+                                        long long nxy) {
+    if (key != cur) {
+        flush_cell(rho, cur, acc, nx, nxy);
+        cur = key;
+#pragma unroll
+        for (int d = 0; d < 8; ++d) acc[d] = w[d];
+    } else {
+#pragma unroll
+        for (int d = 0; d < 8; ++d) acc[d] += w[d];
+    }
+}
+
 template <int R, bool VEC>
-__global__ void __launch_bounds__(kBinBlock) deposit_binned_kernel(const double *__restrict__ x, const double *__restrict__ y,
+__global__ void __launch_bounds__(kBinBlock, R >= 8 ? 2 : 3) deposit_binned_kernel(const double *__restrict__ x, const double *__restrict__ y,
                                                                    const double *__restrict__ t, long long n, GridDev g, double qw,
                                                                    double zscale, double *__restrict__ rho) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     BinSmem<R> &sm = *reinterpret_cast<BinSmem<R> *>(smem_raw);
     constexpr int CH = BinSmem<R>::CH;
+    constexpr int kBig = 0x7fffffff;
     const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
     const long long nxy = (long long)g.nx * g.ny;
     const long long nchunks = (n + CH - 1) / CH;
+    if (tid < 8) sm.box[0][tid] = (tid >= 3 && tid < 6) ? -1 : kBig;
+    __syncthreads();
     int parity = 0;
     for (long long ch = blockIdx.x; ch < nchunks; ch += gridDim.x, parity ^= 1) {
         int *box = sm.box[parity];
@@ -233,12 +167,9 @@ __global__ void __launch_bounds__(kBinBlock) deposit_binned_kernel(const double 
         load_run<R, VEC>(x, p0, n, CUDART_NAN, qx);  // NaN => outside => contributes nothing
         load_run<R, VEC>(y, p0, n, 0.0, qy);
         load_run<R, VEC>(t, p0, n, 0.0, qt);
-        if (tid < 3) box[tid] = 0x7fffffff;
-        else if (tid < 6) box[tid] = -1;
-        __syncthreads();
         Cic c[R];
         bool in[R];
-        int lo_i = 0x7fffffff, lo_j = 0x7fffffff, lo_k = 0x7fffffff, hi_i = -1, hi_j = -1, hi_k = -1;
+        int lo_i = kBig, lo_j = kBig, lo_k = kBig, hi_i = -1, hi_j = -1, hi_k = -1;
 #pragma unroll
         for (int r = 0; r < R; ++r) {
             in[r] = cic_locate(g, qx[r], qy[r], qt[r], zscale, c[r]);
@@ -248,60 +179,78 @@ __global__ void __launch_bounds__(kBinBlock) deposit_binned_kernel(const double 
                 lo_k = min(lo_k, c[r].k), hi_k = max(hi_k, c[r].k);
             }
         }
+        const int first_tid = __reduce_min_sync(0xffffffffu, hi_i >= 0 ? tid : kBig);
         lo_i = __reduce_min_sync(0xffffffffu, lo_i), hi_i = __reduce_max_sync(0xffffffffu, hi_i);
         lo_j = __reduce_min_sync(0xffffffffu, lo_j), hi_j = __reduce_max_sync(0xffffffffu, hi_j);
         lo_k = __reduce_min_sync(0xffffffffu, lo_k), hi_k = __reduce_max_sync(0xffffffffu, hi_k);
         if (lane == 0 && hi_i >= 0) {
             atomicMin(&box[0], lo_i), atomicMin(&box[1], lo_j), atomicMin(&box[2], lo_k);
             atomicMax(&box[3], hi_i), atomicMax(&box[4], hi_j), atomicMax(&box[5], hi_k);
+            atomicMin(&box[6], first_tid);
         }
-        __syncthreads();
-        const int i0 = box[0], j0 = box[1], k0 = box[2];
-        const int bx = box[3] - i0 + 1, by = box[4] - j0 + 1, bz = box[5] - k0 + 1;
-        if (box[3] < 0) continue;  // no particle of this chunk is inside the grid (block-uniform)
-        const long long ncell_ll = (long long)bx * by * bz;
-        if (ncell_ll > kBinCap) {
-            // direct path: runs in storage order
-            int cur = -1;
-            double acc[8];
-#pragma unroll
-            for (int d = 0; d < 8; ++d) acc[d] = 0.0;
-#pragma unroll
-            for (int r = 0; r < R; ++r) {
-                if (!in[r]) continue;
-                const int key = (c[r].k * g.ny + c[r].j) * g.nx + c[r].i;
-                double w[8];
-                cic_weights8(c[r], qw, w);
-                if (key != cur) {
-                    flush_cell(rho, cur, acc, g.nx, nxy);
-                    cur = key;
-#pragma unroll
-                    for (int d = 0; d < 8; ++d) acc[d] = w[d];
-                } else {
-#pragma unroll
-                    for (int d = 0; d < 8; ++d) acc[d] += w[d];
-                }
-            }
-            merge_and_flush(rho, cur, acc, g.nx, nxy);
+        __syncthreads();  // (1) box complete
+        if (tid < 8) sm.box[parity ^ 1][tid] = (tid >= 3 && tid < 6) ? -1 : kBig;  // next chunk's box (its readers passed barrier 2 of the previous chunk)
+        if (box[3] < 0) {  // no particle of this chunk is inside the grid (block-uniform)
+            __syncthreads();  // orders the re-initialisation above before the next chunk's box atomics
             continue;
         }
-        const int ncell = (int)ncell_ll;
-        for (int s = tid; s <= ncell; s += kBinBlock) sm.hist[s] = 0;
-        __syncthreads();
-        int lc[R], rank[R];
+        int i0 = box[0], j0 = box[1], k0 = box[2];
+        int bx = box[3] - i0 + 1, by = box[4] - j0 + 1, bz = box[5] - k0 + 1;
+        // A chunk that is not spatially compact (unsorted input, the thin tails): bin what falls into a fixed 16^3 box
+        // around the first inside particle -- this catches a cold core even in unsorted order -- the rest goes direct.
+        const bool big = (long long)bx * by * bz > kBinCap;
+        if (big && tid == box[6]) {
 #pragma unroll
-        for (int r = 0; r < R; ++r) {
-            lc[r] = ((c[r].k - k0) * by + (c[r].j - j0)) * bx + (c[r].i - i0);
-            rank[r] = in[r] ? atomicAdd(&sm.hist[lc[r]], 1) : 0;
+            for (int r = R - 1; r >= 0; --r)
+                if (in[r]) sm.anchor[0] = c[r].i, sm.anchor[1] = c[r].j, sm.anchor[2] = c[r].k;
         }
-        __syncthreads();
-        // exclusive scan of hist[0..ncell) in place; hist[ncell] = number of inside particles
+        const int ncell = big ? kBinCap : bx * by * bz;
         {
-            const int ipt = (ncell + kBinBlock - 1) / kBinBlock;
-            const int b0 = tid * ipt;
+            const int zr = (ncell + 15) & ~15;  // the scan's 16-entry granules
+            for (int s4 = tid * 4; s4 < zr; s4 += kBinBlock * 4) *reinterpret_cast<int4 *>(&sm.hist[s4]) = make_int4(0, 0, 0, 0);
+            if (tid == 0) sm.hist[kBinCap] = 0;  // spill bin: particles that are not binned (outside the grid / the box)
+        }
+        __syncthreads();  // (2) histogram cleared, anchor published
+        if (big) {
+            i0 = sm.anchor[0] - 8, j0 = sm.anchor[1] - 8, k0 = sm.anchor[2] - 8;
+            bx = by = bz = 16;
+        }
+        int lc[R], rank[R];
+        if (big) {
+#pragma unroll
+            for (int r = 0; r < R; ++r) {
+                const unsigned li = (unsigned)(c[r].i - i0), lj = (unsigned)(c[r].j - j0), lk = (unsigned)(c[r].k - k0);
+                const bool binned = in[r] && li < 16u && lj < 16u && lk < 16u;
+                if (in[r] && !binned) {
+                    double w[8];
+                    cic_weights8(c[r], qw, w);
+                    flush_cell(rho, (c[r].k * g.ny + c[r].j) * g.nx + c[r].i, w, g.nx, nxy);
+                }
+                in[r] = binned;
+                lc[r] = binned ? (int)((lk * 16u + lj) * 16u + li) : kBinCap;
+            }
+        } else {
+#pragma unroll
+            for (int r = 0; r < R; ++r) lc[r] = in[r] ? ((c[r].k - k0) * by + (c[r].j - j0)) * bx + (c[r].i - i0) : kBinCap;
+        }
+#pragma unroll
+        for (int r = 0; r < R; ++r) rank[r] = atomicAdd(&sm.hist[lc[r]], 1);  // count and rank within the cell in one pass
+        __syncthreads();  // (3) histogram complete
+        // exclusive scan of hist[0..ncell) in place: 16 consecutive bins per thread (4 x LDS.128), warp scan, block carry;
+        // the spill bin hist[kBinCap] is not part of it
+        int total = 0;
+        {
+            const int b0 = tid * 16;
+            const bool act = b0 < ncell;
+            int4 v[4];
             int s = 0;
-            for (int q = 0; q < ipt; ++q)
-                if (b0 + q < ncell) s += sm.hist[b0 + q];
+            if (act) {
+#pragma unroll
+                for (int q = 0; q < 4; ++q) {
+                    v[q] = *reinterpret_cast<const int4 *>(&sm.hist[b0 + 4 * q]);
+                    s += v[q].x + v[q].y + v[q].z + v[q].w;
+                }
+            }
             int incl = s;
 #pragma unroll
             for (int d = 1; d < 32; d <<= 1) {
@@ -309,18 +258,27 @@ __global__ void __launch_bounds__(kBinBlock) deposit_binned_kernel(const double 
                 if (lane >= d) incl += o;
             }
             if (lane == 31) sm.warp_tot[wid] = incl;
-            __syncthreads();
+            __syncthreads();  // (4)
             int off = incl - s;
-            for (int w = 0; w < wid; ++w) off += sm.warp_tot[w];
-            for (int q = 0; q < ipt; ++q)
-                if (b0 + q < ncell) {
-                    const int v = sm.hist[b0 + q];
-                    sm.hist[b0 + q] = off;
-                    off += v;
+#pragma unroll
+            for (int w = 0; w < kBinBlock / 32; ++w) {
+                const int wt = sm.warp_tot[w];
+                off += (w < wid) ? wt : 0;
+                total += wt;
+            }
+            if (act) {
+#pragma unroll
+                for (int q = 0; q < 4; ++q) {
+                    int4 o;
+                    o.x = off, off += v[q].x;
+                    o.y = off, off += v[q].y;
+                    o.z = off, off += v[q].z;
+                    o.w = off, off += v[q].w;
+                    *reinterpret_cast<int4 *>(&sm.hist[b0 + 4 * q]) = o;
                 }
-            if (tid == kBinBlock - 1) sm.hist[ncell] = off;
+            }
         }
-        __syncthreads();
+        __syncthreads();  // (5) offsets ready; total = number of binned particles
 #pragma unroll
         for (int r = 0; r < R; ++r)
             if (in[r]) {
@@ -331,9 +289,8 @@ __global__ void __launch_bounds__(kBinBlock) deposit_binned_kernel(const double 
                 sm.w1[1][slot] = c[r].wy1;
                 sm.w1[2][slot] = c[r].wz1;
             }
-        __syncthreads();
+        __syncthreads();  // (6) cell-ordered entry list complete
         {
-            const int total = sm.hist[ncell];
             int cur = -1;
             double acc[8];
 #pragma unroll
@@ -343,44 +300,23 @@ __global__ void __launch_bounds__(kBinBlock) deposit_binned_kernel(const double 
                 const int e = tid * R + r;
                 if (e >= total) break;
                 const int slot = e + (e >> 3);
-                const int key = sm.key[slot];
                 Cic cc;
                 cc.i = cc.j = cc.k = 0;
                 cc.wx1 = sm.w1[0][slot], cc.wy1 = sm.w1[1][slot], cc.wz1 = sm.w1[2][slot];
                 double w[8];
                 cic_weights8(cc, qw, w);
-                if (key != cur) {
-                    flush_cell(rho, cur, acc, g.nx, nxy);
-                    cur = key;
-#pragma unroll
-                    for (int d = 0; d < 8; ++d) acc[d] = w[d];
-                } else {
-#pragma unroll
-                    for (int d = 0; d < 8; ++d) acc[d] += w[d];
-                }
+                run_add(rho, sm.key[slot], w, cur, acc, g.nx, nxy);
             }
             merge_and_flush(rho, cur, acc, g.nx, nxy);
         }
-        __syncthreads();  // the next chunk reuses box/hist/entries
+        // no barrier here: the next chunk touches hist / entries only after its barrier (1), which every thread of this
+        // chunk's walk must reach first
     }
 }
 
 static int env_int_grid(const char *name, int dflt) {
     const char *v = getenv(name);
     return (v && *v) ? atoi(v) : dflt;
-}
-
-template <int R>
-static void launch_deposit_runs(Beam *b, Grid *g, const GridDev &gd, double q_weight, double zscale) {
-    const int block = 256;
-    const long long per_block = (long long)block * R;
-    long long blocks = (b->n + per_block - 1) / per_block;
-    const long long cap = (long long)b->num_sms * 8;
-    if (blocks > cap) blocks = cap;
-    if (b->aligned32)
-        deposit_runs_kernel<R, true><<<(int)blocks, block, 0, b->stream>>>(b->q[0], b->q[2], b->q[4], b->n, gd, q_weight, zscale, g->rho);
-    else
-        deposit_runs_kernel<R, false><<<(int)blocks, block, 0, b->stream>>>(b->q[0], b->q[2], b->q[4], b->n, gd, q_weight, zscale, g->rho);
 }
 
 template <int R>
@@ -408,22 +344,18 @@ static int launch_deposit_binned(Beam *b, Grid *g, const GridDev &gd, double q_w
 
 int launch_deposit(Beam *b, Grid *g, double q_weight, double zscale) {
     const GridDev gd = make_grid_dev(*g);
-    // mode 0: one particle per thread, 8 reductions each; 1: lane runs of 4; 2: lane runs of 8;
-    // 3 (default) / 4: block-local cell binning, 4 / 8 particles per thread
-    const int mode = env_int_grid("BT_DEPOSIT_MODE", 3);
-    if (mode == 3 || mode == 4) {
-        const int rc = mode == 3 ? launch_deposit_binned<4>(b, g, gd, q_weight, zscale) : launch_deposit_binned<8>(b, g, gd, q_weight, zscale);
-        if (rc != BT_OK) return rc;
-    } else if (mode == 0) {
+    // BT_DEPOSIT_MODE: 0 = one particle per thread, 8 reductions each (baseline, kept for measurements);
+    // 1 (default) = block-local cell binning, 8 particles per thread; 2 = the same with 4 particles per thread
+    const int mode = env_int_grid("BT_DEPOSIT_MODE", 1);
+    if (mode == 0) {
         const int block = 256;
         long long blocks = (b->n + block - 1) / block;
         const long long cap = (long long)b->num_sms * 16;
         if (blocks > cap) blocks = cap;
         deposit_atomic_kernel<<<(int)blocks, block, 0, b->stream>>>(b->q[0], b->q[2], b->q[4], b->n, gd, q_weight, zscale, g->rho);
-    } else if (mode == 2) {
-        launch_deposit_runs<8>(b, g, gd, q_weight, zscale);
     } else {
-        launch_deposit_runs<4>(b, g, gd, q_weight, zscale);
+        const int rc = mode == 2 ? launch_deposit_binned<4>(b, g, gd, q_weight, zscale) : launch_deposit_binned<8>(b, g, gd, q_weight, zscale);
+        if (rc != BT_OK) return rc;
     }
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return fail(BT_ERR_CUDA, std::string("bt_deposit_cic launch: ") + cudaGetErrorString(e));
@@ -510,53 +442,63 @@ __global__ void __launch_bounds__(256) gather_kick_kernel(const __grid_constant_
     }
 }
 
-// ---- S6/S7 for cell-sorted storage: lane runs of 4 consecutive particles, field of the current cell cached ----
-// Same arithmetic as gather_kick_kernel per particle.  A lane keeps the 8 node records (24 doubles) of the cell it
-// is in and reloads them only when the next particle of its run sits in another cell; particle I/O is one 256-bit
-// streaming access per array per lane (6 loads, 6 stores per 4 particles, every sector fully used), all issued
-// before the first field access, so a warp has 6 KiB of particle data in flight.
-template <bool VEC>
-__global__ void __launch_bounds__(128) gather_kick_runs_kernel(const __grid_constant__ GatherArgs a) {
-    constexpr int R = 4;
-    const int lane = threadIdx.x & 31;
-    const long long warp = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
-    const long long nwarps = ((long long)gridDim.x * blockDim.x) >> 5;
-    const long long chunk = 32LL * R;
-    for (long long c0 = warp * chunk; c0 < a.n; c0 += nwarps * chunk) {
-        const long long p0 = c0 + (long long)lane * R;
-        double x[R], px[R], y[R], py[R], t[R], pt[R];
-        load_run<R, VEC>(a.q[0], p0, a.n, CUDART_NAN, x);
-        load_run<R, VEC>(a.q[1], p0, a.n, 0.0, px);
-        load_run<R, VEC>(a.q[2], p0, a.n, 0.0, y);
-        load_run<R, VEC>(a.q[3], p0, a.n, 0.0, py);
-        load_run<R, VEC>(a.q[4], p0, a.n, 0.0, t);
-        load_run<R, VEC>(a.q[5], p0, a.n, 0.0, pt);
-        int cur = -1;
-        double fx[8], fy[8], fz[8];
+// ---- S6/S7, streaming pipeline: particle chunks ride the copy engine, the field comes through L1 ------------------
+// A persistent block cycles through kGpStages shared-memory stages of CH particles x 6 coordinates:
+//   chunk k+2 is being loaded (cp.async.bulk global->shared, completion on an mbarrier),
+//   chunk k   is updated IN PLACE in shared memory by the threads (drift, 8-node gather, kick, drift),
+//   chunk k-1 is being stored (cp.async.bulk shared->global).
+// Particle I/O therefore needs no registers and no warp ever waits on a particle load: ~96 KiB per SM are in flight in
+// each direction, independent of occupancy.  Threads address a stage with stride blockDim (conflict-free LDS/STS).  The
+// 8 node records (32 B each, one LDG.E.ENL2.256 through the read-only path) of a particle's cell are L1/L2 hits: a chunk
+// of cell-ordered particles covers a few hundred cells.  Same per-particle arithmetic as gather_kick_kernel.
+// Full chunks only; the ragged tail of the bunch (< CH particles) is done by gather_kick_kernel.
+constexpr int kGpStages = 3;
+
+template <int CH>
+struct GpSmem {
+    alignas(128) double q[kGpStages][6][CH];
+    alignas(8) uint64_t full[kGpStages];
+};
+
+template <int NT, int R>
+__global__ void __launch_bounds__(NT) gather_kick_pipe_kernel(const __grid_constant__ GatherArgs a, long long nchunks, int store_positions) {
+    constexpr int CH = NT * R;
+    constexpr uint32_t kArrBytes = CH * sizeof(double);
+    extern __shared__ __align__(128) unsigned char gp_smem_raw[];
+    GpSmem<CH> &sm = *reinterpret_cast<GpSmem<CH> *>(gp_smem_raw);
+    const int tid = threadIdx.x;
+    const auto issue_load = [&](long long ch, int s) {
+        mbar_expect_tx(&sm.full[s], 6 * kArrBytes);
+#pragma unroll
+        for (int c = 0; c < 6; ++c) bulk_g2s(sm.q[s][c], a.q[c] + ch * CH, kArrBytes, &sm.full[s]);
+    };
+    if (tid == 0) {
+#pragma unroll
+        for (int s = 0; s < kGpStages; ++s) mbar_init(&sm.full[s], 1);
+        mbar_init_fence();
+        if ((long long)blockIdx.x < nchunks) issue_load(blockIdx.x, 0);
+        if ((long long)blockIdx.x + gridDim.x < nchunks) issue_load((long long)blockIdx.x + gridDim.x, 1);
+    }
+    __syncthreads();
+    int s = 0;
+    uint32_t parity = 0;
+    for (long long ch = blockIdx.x; ch < nchunks; ch += gridDim.x) {
+        mbar_wait(&sm.full[s], parity);
+        double(*q)[CH] = sm.q[s];
 #pragma unroll
         for (int r = 0; r < R; ++r) {
+            const int e = r * NT + tid;
+            double x = q[0][e], px = q[1][e], y = q[2][e], py = q[3][e], t = q[4][e], pt = q[5][e];
             // R4 drift before the kick
-            x[r] = fma(a.hb, px[r], x[r]);
-            y[r] = fma(a.hb, py[r], y[r]);
-            t[r] = fma(a.tcb, pt[r], t[r]);
+            x = fma(a.hb, px, x);
+            y = fma(a.hb, py, y);
+            t = fma(a.tcb, pt, t);
             Cic c;
-            if (cic_locate(a.g, x[r], y[r], t[r], a.zscale, c)) {
-                const int key = (c.k * a.g.ny + c.j) * a.g.nx + c.i;
-                if (key != cur) {
-                    cur = key;
-                    const double *base = a.field + 4 * (long long)key;
-#pragma unroll
-                    for (int dz = 0; dz < 2; ++dz)
-#pragma unroll
-                        for (int dy = 0; dy < 2; ++dy)
-#pragma unroll
-                            for (int dx = 0; dx < 2; ++dx)
-                                ld_node(base + 4 * (((long long)dz * a.g.ny + dy) * a.g.nx + dx), fx[dz * 4 + dy * 2 + dx],
-                                        fy[dz * 4 + dy * 2 + dx], fz[dz * 4 + dy * 2 + dx]);
-                }
+            if (cic_locate(a.g, x, y, t, a.zscale, c)) {
                 const double wx[2] = {__dsub_rn(1.0, c.wx1), c.wx1};
                 const double wy[2] = {__dsub_rn(1.0, c.wy1), c.wy1};
                 const double wz[2] = {__dsub_rn(1.0, c.wz1), c.wz1};
+                const double *base = a.field + 4 * (((long long)c.k * a.g.ny + c.j) * a.g.nx + c.i);
                 double ex = 0.0, ey = 0.0, ez = 0.0;
 #pragma unroll
                 for (int dz = 0; dz < 2; ++dz)
@@ -565,26 +507,63 @@ __global__ void __launch_bounds__(128) gather_kick_runs_kernel(const __grid_cons
 #pragma unroll
                         for (int dx = 0; dx < 2; ++dx) {
                             const double w = __dmul_rn(__dmul_rn(wx[dx], wy[dy]), wz[dz]);
-                            ex = fma(w, fx[dz * 4 + dy * 2 + dx], ex);
-                            ey = fma(w, fy[dz * 4 + dy * 2 + dx], ey);
-                            ez = fma(w, fz[dz * 4 + dy * 2 + dx], ez);
+                            double fx, fy, fz;
+                            ld_node(base + 4 * (((long long)dz * a.g.ny + dy) * a.g.nx + dx), fx, fy, fz);
+                            ex = fma(w, fx, ex);
+                            ey = fma(w, fy, ey);
+                            ez = fma(w, fz, ez);
                         }
-                px[r] = fma(a.coef[0], ex, px[r]);
-                py[r] = fma(a.coef[1], ey, py[r]);
-                pt[r] = fma(a.coef[2], ez, pt[r]);
+                px = fma(a.coef[0], ex, px);
+                py = fma(a.coef[1], ey, py);
+                pt = fma(a.coef[2], ez, pt);
             }
             // R4 drift after the kick
-            x[r] = fma(a.ha, px[r], x[r]);
-            y[r] = fma(a.ha, py[r], y[r]);
-            t[r] = fma(a.tca, pt[r], t[r]);
+            x = fma(a.ha, px, x);
+            y = fma(a.ha, py, y);
+            t = fma(a.tca, pt, t);
+            q[0][e] = x, q[1][e] = px, q[2][e] = y, q[3][e] = py, q[4][e] = t, q[5][e] = pt;
         }
-        store_run<R, VEC>(a.q[0], p0, a.n, x);
-        store_run<R, VEC>(a.q[1], p0, a.n, px);
-        store_run<R, VEC>(a.q[2], p0, a.n, y);
-        store_run<R, VEC>(a.q[3], p0, a.n, py);
-        store_run<R, VEC>(a.q[4], p0, a.n, t);
-        store_run<R, VEC>(a.q[5], p0, a.n, pt);
+        fence_proxy_async_smem();  // this thread's shared-memory writes -> visible to the copy engine
+        __syncthreads();
+        if (tid == 0) {
+#pragma unroll
+            for (int c = 0; c < 6; ++c)
+                if (store_positions || (c & 1)) bulk_s2g(a.q[c] + ch * CH, sm.q[s][c], kArrBytes);
+            bulk_commit();
+            // the stage two chunks ahead is the one stored in the previous iteration: wait until that store has read it
+            const long long nxt = ch + 2LL * gridDim.x;
+            if (nxt < nchunks) {
+                bulk_wait_read<1>();
+                issue_load(nxt, (s + 2) % kGpStages);
+            }
+        }
+        if (++s == kGpStages) s = 0, parity ^= 1;
     }
+    if (tid == 0) bulk_wait_all<0>();  // shared memory must outlive the last stores
+}
+
+template <int NT, int R>
+static int launch_gather_pipe(Beam *b, const GatherArgs &a0) {
+    constexpr int CH = NT * R;
+    const int smem = (int)sizeof(GpSmem<CH>);
+    const long long nchunks = b->n / CH;
+    if (nchunks > 0) {
+        int per_sm = 1;
+        BT_CUDA_TRY(cudaFuncSetAttribute(gather_kick_pipe_kernel<NT, R>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+        BT_CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, gather_kick_pipe_kernel<NT, R>, NT, smem));
+        long long blocks = (long long)b->num_sms * (per_sm > 0 ? per_sm : 1);
+        if (blocks > nchunks) blocks = nchunks;
+        const int store_positions = (a0.hb != 0.0 || a0.ha != 0.0 || a0.tcb != 0.0 || a0.tca != 0.0) ? 1 : 0;
+        gather_kick_pipe_kernel<NT, R><<<(int)blocks, NT, smem, b->stream>>>(a0, nchunks, store_positions);
+    }
+    const long long done = nchunks * CH;
+    if (done < b->n) {  // ragged tail: one particle per thread
+        GatherArgs t = a0;
+        for (int c = 0; c < 6; ++c) t.q[c] = a0.q[c] + done;
+        t.n = b->n - done;
+        gather_kick_kernel<<<(int)((t.n + 255) / 256), 256, 0, b->stream>>>(t);
+    }
+    return BT_OK;
 }
 
 int launch_gather_kick(Beam *b, const Grid *g, const double coef[3], double zscale, double h_before, double tc_before,
@@ -600,18 +579,12 @@ int launch_gather_kick(Beam *b, const Grid *g, const double coef[3], double zsca
     a.tcb = tc_before;
     a.ha = h_after;
     a.tca = tc_after;
-    // cell-sorted storage (bt_beam_sort_by_cell since the last upload): lane runs with the cell's field cached;
-    // any other order: one particle per thread.  BT_GATHER_MODE=0/1 forces one of them (both are correct for any order).
-    const int mode = env_int_grid("BT_GATHER_MODE", b->permuted ? 1 : 0);
-    if (mode == 1) {
-        const int block = 128;
-        long long blocks = (b->n + block * 4LL - 1) / (block * 4LL);
-        const long long cap = (long long)b->num_sms * 16;
-        if (blocks > cap) blocks = cap;
-        if (b->aligned32)
-            gather_kick_runs_kernel<true><<<(int)blocks, block, 0, b->stream>>>(a);
-        else
-            gather_kick_runs_kernel<false><<<(int)blocks, block, 0, b->stream>>>(a);
+    // BT_GATHER_MODE: 0 = one particle per thread, everything through registers (also the path for arrays that are not
+    // 16-byte aligned); 1 (default) = streaming pipeline, 256-particle chunks; 2 / 3 = pipeline with 512 / 128-particle chunks
+    const int mode = env_int_grid("BT_GATHER_MODE", 1);
+    if (mode >= 1 && b->aligned16) {
+        const int rc = mode == 2 ? launch_gather_pipe<512, 1>(b, a) : mode == 3 ? launch_gather_pipe<128, 1>(b, a) : launch_gather_pipe<256, 1>(b, a);
+        if (rc != BT_OK) return rc;
     } else {
         const int block = 256;
         long long blocks = (b->n + block - 1) / block;
