@@ -40,6 +40,8 @@ def lib():
         L.orc_gather_kick.restype = C.c_int64
         L.orc_gather_field.argtypes = [C.c_int64] + [_dp] * 3 + [C.c_int32] * 3 + [_dp, _dp] + [_dp] * 3 + [C.c_double] + [_dp] * 3
         L.orc_gather_field.restype = C.c_int64
+        L.orc_moments.argtypes = [C.c_int64, C.POINTER(_dp), _dp, _dp]
+        L.orc_moments.restype = C.c_int
         _lib = L
     return _lib
 
@@ -134,3 +136,20 @@ def gather_field(x, y, t, shape, lo, d, E, zscale=1.0):
     lib().orc_gather_field(x.shape[0], _p(x), _p(y), _p(t), nx, ny, nz, _p(lo), _p(d),
                            _p(Ex), _p(Ey), _p(Ez), zscale, *[_p(o) for o in out])
     return out
+
+
+def moments(coords):
+    """Beam statistics: returns (mean[6], cov[6,6]) of coords = [x, px, y, py, t, pt],
+    population second moments about the mean."""
+    n = coords[0].shape[0]
+    ptrs = (_dp * 6)(*[_p(c) for c in coords])
+    mean, cov = np.zeros(6), np.zeros(36)
+    if lib().orc_moments(n, ptrs, _p(mean), _p(cov)) != 0:
+        raise ValueError("oracle: moments of an empty set")
+    return mean, cov.reshape(6, 6)
+
+
+def rms_emittances(cov):
+    """Unnormalised rms emittances of the three planes from the 6x6 second moments:
+    eps = sqrt(<q q><p p> - <q p>^2) for (x,px), (y,py), (t,pt)."""
+    return tuple(float(np.sqrt(cov[a, a] * cov[a + 1, a + 1] - cov[a, a + 1] ** 2)) for a in (0, 2, 4))
