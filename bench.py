@@ -232,6 +232,12 @@ def bench_other_configs(bt, torch, flush, peaks, nominal_peak):
         else:
             entry["roofline"] = {"bound": "hbm", "achieved": 96.0 * n * launches / t / 1e9, "peak": hbm / 1e9, "unit": "GB/s",
                                  "frac": t_hbm / t}
+        if idx in (2, 3):
+            # beam statistics: bt_beam_moments = 2 launches + a 336-byte read-back, 48 B/particle
+            beam.moments()
+            tm = statistics.mean(_event_ms(torch, beam.moments, 5, flush)) * 1e-3
+            entry["moments"] = {"ms": tm * 1e3, "roofline": {"bound": "hbm", "achieved": 48.0 * n / tm / 1e9, "peak": hbm / 1e9,
+                                                              "unit": "GB/s", "frac": 48.0 * n / tm / hbm, "traffic": None}}
         out.append(entry)
         beam.close()
         del pristine, beam
@@ -266,6 +272,9 @@ def bench_spacecharge(bt, torch, flush, peaks):
         for d, s in zip(beam.tensors, pos):
             d.copy_(s)
         del pos
+        beam.sort_by_cell(grid, sc.zscale)                         # warm-up: first call allocates the scratch
+        beam.upload(c)                                             # back to the caller's order
+        beam.track(1)
         t_sort = _event_ms(torch, lambda: beam.sort_by_cell(grid, sc.zscale), 1, flush)[0]
         t_dep, t_gat = [], []
         for step in range(sc.nsteps):

@@ -188,6 +188,21 @@ int bt_deposit_cic(bt_beam *beam, bt_grid *grid, double q_weight, double zscale,
 int bt_gather_kick(bt_beam *beam, const bt_grid *grid, const double coef[3], double zscale,
                    double half_drift_before, double half_drift_after);
 
+/* ---- beam statistics ---------------------------------------------------- */
+
+/*
+ * Means and second moments of the six coordinates (P:l.43 "beam statistics"; P:l.112 "beam second moments ...
+ * emittances"; the quantity every benchmark of the paper is judged on, and what slice-step diagnostics (P:l.61)
+ * print), order x, px, y, py, t, pt:
+ *   host_mean[i]    = (1/n) sum_p q_i[p]
+ *   host_cov[6*i+j] = (1/n) sum_p (q_i[p] - mean_i)(q_j[p] - mean_j)       (population moments, full symmetric 6x6)
+ * Both outputs are HOST arrays owned by the caller.  One pass over the particles (48 bytes each) on the beam's
+ * stream, sums taken about a provisional centre so that an offset bunch loses no digits; the call synchronises the
+ * stream.  Deterministic (fixed reduction order), independent of the storage order up to fp64 rounding.  The
+ * unnormalised rms emittance of a plane is sqrt(cov_qq*cov_pp - cov_qp^2).  NaN/Inf coordinates propagate.
+ */
+int bt_beam_moments(bt_beam *beam, double host_mean[6], double host_cov[36]);
+
 /* ---- utilities ------------------------------------------------------------------------------ */
 int bt_sync(bt_beam *beam); /* cudaStreamSynchronize on the beam's stream */
 const char *bt_last_error(void);

@@ -54,6 +54,7 @@ EXPORTS = {
     "bt_grid_download_rho": (C.c_int, [_vp, _vp]),
     "bt_deposit_cic": (C.c_int, [_vp, _vp, C.c_double, C.c_double, C.c_int]),
     "bt_gather_kick": (C.c_int, [_vp, _vp, _dp, C.c_double, C.c_double, C.c_double]),
+    "bt_beam_moments": (C.c_int, [_vp, _dp, _dp]),
     "bt_sync": (C.c_int, [_vp]),
     "bt_last_error": (C.c_char_p, []),
     "bt_version": (C.c_int, []),
@@ -211,6 +212,12 @@ class Beam:
     def gather_kick(self, grid, coef, zscale=1.0, half_drift_before=0.0, half_drift_after=0.0):
         c = (C.c_double * 3)(*coef)
         _check(lib.bt_gather_kick(self._h, grid._h, c, zscale, half_drift_before, half_drift_after), "bt_gather_kick")
+
+    def moments(self):
+        """(mean[6], cov[6, 6]) of x, px, y, py, t, pt -- computed on the device, returned as numpy arrays."""
+        mean, cov = np.zeros(6), np.zeros(36)
+        _check(lib.bt_beam_moments(self._h, mean.ctypes.data_as(_dp), cov.ctypes.data_as(_dp)), "bt_beam_moments")
+        return mean, cov.reshape(6, 6)
 
     def sort_by_cell(self, grid, zscale=1.0):
         _check(lib.bt_beam_sort_by_cell(self._h, grid._h, zscale), "bt_beam_sort_by_cell")

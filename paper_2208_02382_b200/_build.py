@@ -11,8 +11,8 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libbt.so")
-SOURCES = ["bt_api.cu", "track.cu", "grid.cu", "sort.cu", "calib.cu"]
-HEADERS = [os.path.join(CSRC, "bt_internal.h"), os.path.join(CSRC, "grid_dev.cuh"), os.path.join(HERE, "..", "include", "bt.h")]
+SOURCES = ["bt_api.cu", "track.cu", "grid.cu", "sort.cu", "moments.cu", "calib.cu"]
+HEADERS = [os.path.join(CSRC, "bt_internal.h"), os.path.join(CSRC, "grid_dev.cuh"), os.path.join(CSRC, "bulk_copy.cuh"), os.path.join(HERE, "..", "include", "bt.h")]
 
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a",

@@ -269,6 +269,7 @@ void bt_beam_destroy(bt_beam *beam) {
     for (int *p : ibufs)
         if (p) cudaFree(p);
     if (b.scratch) cudaFree(b.scratch);
+    if (b.mom_buf) cudaFree(b.mom_buf);
     delete beam;
 }
 
@@ -544,6 +545,11 @@ int bt_deposit_cic(bt_beam *beam, bt_grid *grid, double q_weight, double zscale,
     g.last_stream = b.stream;
     if (zero_first) BT_CUDA_TRY(cudaMemsetAsync(g.rho, 0, (size_t)g.nn * sizeof(double), b.stream));
     return launch_deposit(&b, &g, q_weight, zscale);
+}
+
+int bt_beam_moments(bt_beam *beam, double host_mean[6], double host_cov[36]) {
+    if (!beam || !host_mean || !host_cov) return fail(BT_ERR_INVALID, "bt_beam_moments: NULL argument");
+    return launch_moments(&beam->b, host_mean, host_cov);
 }
 
 int bt_gather_kick(bt_beam *beam, const bt_grid *grid, const double coef[3], double zscale, double half_drift_before,

@@ -90,6 +90,7 @@ struct Beam {
     int *sort_key = nullptr, *sort_dest = nullptr, *sort_count = nullptr, *sort_block_sum = nullptr;
     long long sort_count_cap = 0;
     double *scratch = nullptr;  // one array of n doubles
+    double *mom_buf = nullptr;  // beam statistics: centre[6], out[42], per-block partials, ticket (moments.cu)
 };
 
 struct Grid {
@@ -119,6 +120,7 @@ int launch_gather_kick(Beam *b, const Grid *g, const double coef[3], double zsca
                        double tc_before, double h_after, double tc_after);
 int sort_by_cell(Beam *b, const Grid *g, double zscale);
 int unpermute_to(Beam *b, int c, double *out);  // out[ids[j]] = q[c][j] on the beam's stream
+int launch_moments(Beam *b, double host_mean[6], double host_cov[36]);  // synchronises the beam's stream
 int launch_field_pack(Grid *g, const double *ex, const double *ey, const double *ez, cudaStream_t s);
 
 }  // namespace bt

@@ -1,0 +1,175 @@
+// Beam statistics ("beam statistics", l.112 "beam second moments ... emittances",
+// l.61 slice-step diagnostics): means and the 6x6 second moments about the mean, ONE pass over the particles.
+//
+//   mean_i = (1/n) sum q_i ,   cov_ij = (1/n) sum (q_i - mean_i)(q_j - mean_j)
+//
+// One pass needs a provisional centre k (a two-pass scheme would read the bunch twice): with d = q - k,
+//   S_i = sum d_i , P_ij = sum d_i d_j  =>  mean_i = k_i + S_i/n , cov_ij = P_ij/n - (S_i/n)(S_j/n),
+// which is the definition exactly (algebraically) and loses no digits as long as |k - mean| is of the order of the rms
+// size: k is the mean of the first min(n, 4096) particles (a tiny first launch), so the subtracted term is ~ cov/4096.
+// HBM-bound: 48 bytes and 33 FP64 issue slots per particle.  Deterministic: fixed partition, fixed reduction trees,
+// the per-block partials are combined in block order by the last block to finish.
+#include "bt_internal.h"
+
+namespace bt {
+
+constexpr int kMomBlock = 256;
+constexpr int kMomVals = 27;  // 6 sums + 21 products (upper triangle, row-major)
+constexpr int kCentreSample = 4096;
+
+struct MomArgs {
+    const double *q[6];
+    long long n;
+    double *centre;    // [6]
+    double *partial;   // [gridDim.x][27]
+    double *out;       // [6 mean][36 cov]
+    unsigned int *ticket;
+};
+
+__device__ __forceinline__ double block_sum(double v, double *scratch /*[kMomBlock/32]*/) {
+#pragma unroll
+    for (int d = 16; d > 0; d >>= 1) v += __shfl_xor_sync(0xffffffffu, v, d);
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    __syncthreads();  // scratch free
+    if (lane == 0) scratch[wid] = v;
+    __syncthreads();
+    double tot = 0.0;
+#pragma unroll
+    for (int w = 0; w < kMomBlock / 32; ++w) tot += scratch[w];  // same order in every thread
+    return tot;
+}
+
+__global__ void __launch_bounds__(kMomBlock) moments_centre_kernel(const __grid_constant__ MomArgs a) {
+    __shared__ double scratch[kMomBlock / 32];
+    const long long m = a.n < kCentreSample ? a.n : kCentreSample;
+    for (int c = 0; c < 6; ++c) {
+        double s = 0.0;
+        for (long long p = threadIdx.x; p < m; p += kMomBlock) s += a.q[c][p];
+        s = block_sum(s, scratch);
+        if (threadIdx.x == 0) a.centre[c] = s / (double)m;
+    }
+}
+
+__device__ __forceinline__ void accumulate(const double (&d)[6], double (&s)[6], double (&pr)[21]) {
+    int k = 0;
+#pragma unroll
+    for (int i = 0; i < 6; ++i) {
+        s[i] += d[i];
+#pragma unroll
+        for (int j = i; j < 6; ++j) pr[k] = fma(d[i], d[j], pr[k]), ++k;
+    }
+}
+
+template <bool VEC2>
+__global__ void __launch_bounds__(kMomBlock) moments_kernel(const __grid_constant__ MomArgs a) {
+    __shared__ double scratch[kMomBlock / 32];
+    __shared__ bool is_last;
+    double k[6];
+#pragma unroll
+    for (int c = 0; c < 6; ++c) k[c] = a.centre[c];
+    double s[6], pr[21];
+#pragma unroll
+    for (int c = 0; c < 6; ++c) s[c] = 0.0;
+#pragma unroll
+    for (int c = 0; c < 21; ++c) pr[c] = 0.0;
+    const long long tid = (long long)blockIdx.x * kMomBlock + threadIdx.x;
+    const long long nthreads = (long long)gridDim.x * kMomBlock;
+    if (VEC2) {  // arrays 16-byte aligned: 128-bit streaming loads, two particles per thread per trip
+        const long long n2 = a.n >> 1;
+        for (long long i = tid; i < n2; i += nthreads) {
+            double2 v[6];
+#pragma unroll
+            for (int c = 0; c < 6; ++c) v[c] = __ldcs(reinterpret_cast<const double2 *>(a.q[c]) + i);
+            double d0[6], d1[6];
+#pragma unroll
+            for (int c = 0; c < 6; ++c) d0[c] = v[c].x - k[c], d1[c] = v[c].y - k[c];
+            accumulate(d0, s, pr);
+            accumulate(d1, s, pr);
+        }
+        if ((a.n & 1) && tid == 0) {
+            double d[6];
+#pragma unroll
+            for (int c = 0; c < 6; ++c) d[c] = a.q[c][a.n - 1] - k[c];
+            accumulate(d, s, pr);
+        }
+    } else {
+        for (long long p = tid; p < a.n; p += nthreads) {
+            double d[6];
+#pragma unroll
+            for (int c = 0; c < 6; ++c) d[c] = __ldcs(a.q[c] + p) - k[c];
+            accumulate(d, s, pr);
+        }
+    }
+    // block reduction, one value at a time (27 x (5 shuffles + 8 shared reads)): once per block, negligible
+    double *mine = a.partial + (long long)blockIdx.x * kMomVals;
+#pragma unroll
+    for (int c = 0; c < 6; ++c) {
+        const double tot = block_sum(s[c], scratch);
+        if (threadIdx.x == 0) mine[c] = tot;
+    }
+#pragma unroll
+    for (int c = 0; c < 21; ++c) {
+        const double tot = block_sum(pr[c], scratch);
+        if (threadIdx.x == 0) mine[6 + c] = tot;
+    }
+    // the last block to finish combines the partials in block order
+    if (threadIdx.x == 0) {
+        __threadfence();
+        const unsigned int t = atomicAdd(a.ticket, 1u);
+        is_last = (t == gridDim.x - 1);
+    }
+    __syncthreads();
+    if (!is_last) return;
+    __threadfence();
+    __shared__ double total[kMomVals];
+    if (threadIdx.x < kMomVals) {
+        double tot = 0.0;
+        for (unsigned int b = 0; b < gridDim.x; ++b) tot += __ldcg(a.partial + (long long)b * kMomVals + threadIdx.x);
+        total[threadIdx.x] = tot;
+    }
+    __syncthreads();
+    const double inv_n = 1.0 / (double)a.n;
+    if (threadIdx.x < 6) a.out[threadIdx.x] = a.centre[threadIdx.x] + total[threadIdx.x] * inv_n;
+    if (threadIdx.x < 36) {
+        const int i = threadIdx.x / 6, j = threadIdx.x % 6;
+        const int lo = i < j ? i : j, hi = i < j ? j : i;
+        const int idx = 6 + lo * 6 - lo * (lo - 1) / 2 + (hi - lo);  // position of (lo, hi) in the packed upper triangle
+        a.out[6 + threadIdx.x] = total[idx] * inv_n - (total[lo] * inv_n) * (total[hi] * inv_n);
+    }
+    if (threadIdx.x == 0) *a.ticket = 0u;  // ready for the next call
+}
+
+int launch_moments(Beam *b, double host_mean[6], double host_cov[36]) {
+    const int max_blocks = b->num_sms * 4;
+    if (!b->mom_buf) {
+        const size_t bytes = (size_t)(6 + 42 + (size_t)max_blocks * kMomVals) * sizeof(double) + 16;
+        BT_CUDA_TRY(cudaMalloc(&b->mom_buf, bytes));
+        BT_CUDA_TRY(cudaMemsetAsync(b->mom_buf, 0, bytes, b->stream));
+    }
+    MomArgs a;
+    for (int c = 0; c < 6; ++c) a.q[c] = b->q[c];
+    a.n = b->n;
+    a.centre = b->mom_buf;
+    a.out = b->mom_buf + 6;
+    a.partial = b->mom_buf + 48;
+    a.ticket = reinterpret_cast<unsigned int *>(b->mom_buf + 48 + (size_t)max_blocks * kMomVals);
+    long long blocks = (b->n / 2 + kMomBlock - 1) / kMomBlock;
+    if (blocks > max_blocks) blocks = max_blocks;
+    if (blocks < 1) blocks = 1;
+    moments_centre_kernel<<<1, kMomBlock, 0, b->stream>>>(a);
+    if (b->aligned16)
+        moments_kernel<true><<<(int)blocks, kMomBlock, 0, b->stream>>>(a);
+    else
+        moments_kernel<false><<<(int)blocks, kMomBlock, 0, b->stream>>>(a);
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return fail(BT_ERR_CUDA, std::string("bt_beam_moments launch: ") + cudaGetErrorString(e));
+    g_launch_count.fetch_add(2);
+    double h[42];
+    BT_CUDA_TRY(cudaMemcpyAsync(h, a.out, sizeof(h), cudaMemcpyDeviceToHost, b->stream));
+    BT_CUDA_TRY(cudaStreamSynchronize(b->stream));
+    for (int i = 0; i < 6; ++i) host_mean[i] = h[i];
+    for (int i = 0; i < 36; ++i) host_cov[i] = h[6 + i];
+    return BT_OK;
+}
+
+}  // namespace bt

@@ -1,0 +1,105 @@
+"""bt_beam_moments (CUDA, through the C-ABI) against the oracle's two-pass long-double definition.
+
+Tolerance: the device sums fp64 products in a fixed tree; for N terms the error of a tree sum
+is <= ~log2(N) eps sum|terms| and |d_i d_j| sums to at most N sqrt(c_ii c_jj)(1 + 1/4096), so
+|cov - ref| <= 1e-12 sqrt(ref_ii ref_jj) and |mean - ref| <= 1e-12 sigma_i + 4 eps |ref| hold with two orders of margin."""
+import numpy as np
+import pytest
+
+import oracle as O
+import paper_2208_02382_b200 as bt
+import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+
+def check(c, beam=None):
+    own = beam is None
+    if own:
+        beam = bt.Beam(c[0].shape[0])
+        beam.upload(c)
+    mean, cov = beam.moments()
+    rm, rc = O.moments(c)
+    sig = np.sqrt(np.diag(rc))
+    assert np.all(np.abs(mean - rm) <= 1e-12 * sig + 4 * np.finfo(float).eps * np.abs(rm)), (mean - rm, sig)
+    scale = np.outer(sig, sig)
+    if np.all(scale > 0):
+        assert np.max(np.abs(cov - rc) / scale) <= 1e-12, np.max(np.abs(cov - rc) / scale)
+    else:
+        assert np.max(np.abs(cov - rc)) <= 1e-12 * max(np.max(scale), 1e-300)
+    assert np.array_equal(cov, cov.T)
+    if own:
+        beam.close()
+    return mean, cov
+
+
+@pytest.mark.parametrize("n", [1, 2, 3, 255, 4097, 100_003, 1_000_000])
+def test_moments_gaussian_sizes(n):
+    cfg = W.config(0, n=n)
+    check(W.make_bunch(cfg))
+
+
+def test_moments_offset_and_correlated_bunch():
+    """Centre 10^3 sigma away from the origin, strong x-px and t-pt correlations (the chicane's chirped bunch)."""
+    cfg = W.config(2, n=300_001)
+    c = W.make_bunch(cfg)
+    c[0] += 1.0
+    c[4] -= 3.0
+    c[1] += 0.7 * c[0]
+    check(c)
+
+
+def test_moments_unaligned_storage_and_odd_count():
+    import torch
+    cfg = W.config(0, n=70_001)
+    c = W.make_bunch(cfg)
+    backing = [torch.empty(cfg.n + 1, dtype=torch.float64, device="cuda") for _ in range(6)]
+    beam = bt.Beam(cfg.n, storage=[b[1:] for b in backing])
+    beam.upload(c)
+    check(c, beam)
+    beam.close()
+
+
+def test_moments_independent_of_storage_order_and_deterministic():
+    sc = W.spacecharge_config("A", n=200_000, shape=(32, 32, 32))
+    c = W.make_spacecharge_bunch(sc)
+    beam = bt.Beam(sc.n)
+    grid = bt.Grid(sc.shape, sc.lo, sc.d)
+    beam.upload(c)
+    m0, c0 = check(c, beam)
+    m1, c1 = beam.moments()
+    assert np.array_equal(m0, m1) and np.array_equal(c0, c1)          # bit-reproducible
+    beam.sort_by_cell(grid, sc.zscale)
+    check(c, beam)                                                     # same ensemble, other storage order
+    beam.close()
+    grid.close()
+
+
+def test_moments_after_tracking_match_and_emittance_is_conserved():
+    """second moments stay matched, emittances constant -- from the DEVICE statistics after bt_track."""
+    cfg = W.config(1, n=200_000)
+    c = W.make_bunch(cfg)
+    beam = bt.Beam(cfg.n)
+    beam.set_ref(cfg.kin_energy_MeV, cfg.mass_MeV, cfg.charge_qe)
+    beam.lattice_set(cfg.lattice[:5])            # one FODO cell of the channel
+    beam.upload(c)
+    _, cov0 = beam.moments()
+    beam.track(1)
+    _, cov1 = beam.moments()
+    ref = [a.copy() for a in c]
+    O.track(ref, cfg.lattice[:5], 1, O.ref_from_kinetic(cfg.kin_energy_MeV, cfg.mass_MeV)[0])
+    _, rc = O.moments(ref)
+    sig = np.sqrt(np.diag(rc))
+    assert np.max(np.abs(cov1 - rc) / np.outer(sig, sig)) <= 1e-11    # R14 tracking differences enter here
+    e0, e1 = O.rms_emittances(cov0), O.rms_emittances(cov1)
+    for a, b in zip(e0, e1):
+        assert abs(a - b) <= 1e-10 * a
+    assert abs(cov1[0, 0] - cov0[0, 0]) <= 2e-2 * cov0[0, 0]          # matched beam: <xx> periodic up to sampling noise ~ sqrt(2/N)
+    beam.close()
+
+
+def test_moments_argument_errors():
+    beam = bt.Beam(10)
+    assert bt.lib.bt_beam_moments(beam._h, None, None) == bt.BT_ERR_INVALID
+    assert bt.lib.bt_beam_moments(None, None, None) == bt.BT_ERR_INVALID
+    beam.close()
