@@ -233,7 +233,7 @@ def bench_other_configs(bt, torch, flush, peaks, nominal_peak):
             entry["roofline"] = {"bound": "hbm", "achieved": 96.0 * n * launches / t / 1e9, "peak": hbm / 1e9, "unit": "GB/s",
                                  "frac": t_hbm / t}
         if idx in (2, 3):
-            # beam statistics: bt_beam_moments = 2 launches + a 336-byte read-back, 48 B/particle
+            # beam statistics: bt_beam_moments = 1 launch + a 336-byte read-back, 48 B/particle
             beam.moments()
             tm = statistics.mean(_event_ms(torch, beam.moments, 5, flush)) * 1e-3
             entry["moments"] = {"ms": tm * 1e3, "roofline": {"bound": "hbm", "achieved": 48.0 * n / tm / 1e9, "peak": hbm / 1e9,

@@ -90,7 +90,7 @@ struct Beam {
     int *sort_key = nullptr, *sort_dest = nullptr, *sort_count = nullptr, *sort_block_sum = nullptr;
     long long sort_count_cap = 0;
     double *scratch = nullptr;  // one array of n doubles
-    double *mom_buf = nullptr;  // beam statistics: centre[6], out[42], per-block partials, ticket (moments.cu)
+    double *mom_buf = nullptr;  // beam statistics: out[42], pad, per-block partials, ticket (moments.cu)
 };
 
 struct Grid {

@@ -6,7 +6,7 @@
 // One pass needs a provisional centre k (a two-pass scheme would read the bunch twice): with d = q - k,
 //   S_i = sum d_i , P_ij = sum d_i d_j  =>  mean_i = k_i + S_i/n , cov_ij = P_ij/n - (S_i/n)(S_j/n),
 // which is the definition exactly (algebraically) and loses no digits as long as |k - mean| is of the order of the rms
-// size: k is the mean of the first min(n, 4096) particles (a tiny first launch), so the subtracted term is ~ cov/4096.
+// size: k is the mean of the first min(n, 256) particles (every block recomputes it), so the subtracted term is ~ cov/256.
 // HBM-bound: 48 bytes and 33 FP64 issue slots per particle.  Deterministic: fixed partition, fixed reduction trees,
 // the per-block partials are combined in block order by the last block to finish.
 #include "bt_internal.h"
@@ -15,12 +15,11 @@ namespace bt {
 
 constexpr int kMomBlock = 256;
 constexpr int kMomVals = 27;  // 6 sums + 21 products (upper triangle, row-major)
-constexpr int kCentreSample = 4096;
+constexpr int kCentreSample = kMomBlock;
 
 struct MomArgs {
     const double *q[6];
     long long n;
-    double *centre;    // [6]
     double *partial;   // [gridDim.x][27]
     double *out;       // [6 mean][36 cov]
     unsigned int *ticket;
@@ -39,17 +38,6 @@ __device__ __forceinline__ double block_sum(double v, double *scratch /*[kMomBlo
     return tot;
 }
 
-__global__ void __launch_bounds__(kMomBlock) moments_centre_kernel(const __grid_constant__ MomArgs a) {
-    __shared__ double scratch[kMomBlock / 32];
-    const long long m = a.n < kCentreSample ? a.n : kCentreSample;
-    for (int c = 0; c < 6; ++c) {
-        double s = 0.0;
-        for (long long p = threadIdx.x; p < m; p += kMomBlock) s += a.q[c][p];
-        s = block_sum(s, scratch);
-        if (threadIdx.x == 0) a.centre[c] = s / (double)m;
-    }
-}
-
 __device__ __forceinline__ void accumulate(const double (&d)[6], double (&s)[6], double (&pr)[21]) {
     int k = 0;
 #pragma unroll
@@ -64,9 +52,17 @@ template <bool VEC2>
 __global__ void __launch_bounds__(kMomBlock) moments_kernel(const __grid_constant__ MomArgs a) {
     __shared__ double scratch[kMomBlock / 32];
     __shared__ bool is_last;
+    // provisional centre: mean of the first min(n, 256) particles, computed by every block in the same order (bitwise
+    // identical everywhere; after the first block these 12 KiB are L2 hits)
     double k[6];
+    {
+        const long long m = a.n < kCentreSample ? a.n : kCentreSample;
+        double v[6];
 #pragma unroll
-    for (int c = 0; c < 6; ++c) k[c] = a.centre[c];
+        for (int c = 0; c < 6; ++c) v[c] = threadIdx.x < m ? a.q[c][threadIdx.x] : 0.0;
+#pragma unroll
+        for (int c = 0; c < 6; ++c) k[c] = block_sum(v[c], scratch) / (double)m;
+    }
     double s[6], pr[21];
 #pragma unroll
     for (int c = 0; c < 6; ++c) s[c] = 0.0;
@@ -129,7 +125,13 @@ __global__ void __launch_bounds__(kMomBlock) moments_kernel(const __grid_constan
     }
     __syncthreads();
     const double inv_n = 1.0 / (double)a.n;
-    if (threadIdx.x < 6) a.out[threadIdx.x] = a.centre[threadIdx.x] + total[threadIdx.x] * inv_n;
+    __shared__ double centre[6];
+    if (threadIdx.x == 0) {
+#pragma unroll
+        for (int c = 0; c < 6; ++c) centre[c] = k[c];
+    }
+    __syncthreads();
+    if (threadIdx.x < 6) a.out[threadIdx.x] = centre[threadIdx.x] + total[threadIdx.x] * inv_n;
     if (threadIdx.x < 36) {
         const int i = threadIdx.x / 6, j = threadIdx.x % 6;
         const int lo = i < j ? i : j, hi = i < j ? j : i;
@@ -149,21 +151,19 @@ int launch_moments(Beam *b, double host_mean[6], double host_cov[36]) {
     MomArgs a;
     for (int c = 0; c < 6; ++c) a.q[c] = b->q[c];
     a.n = b->n;
-    a.centre = b->mom_buf;
-    a.out = b->mom_buf + 6;
+    a.out = b->mom_buf;
     a.partial = b->mom_buf + 48;
     a.ticket = reinterpret_cast<unsigned int *>(b->mom_buf + 48 + (size_t)max_blocks * kMomVals);
     long long blocks = (b->n / 2 + kMomBlock - 1) / kMomBlock;
     if (blocks > max_blocks) blocks = max_blocks;
     if (blocks < 1) blocks = 1;
-    moments_centre_kernel<<<1, kMomBlock, 0, b->stream>>>(a);
     if (b->aligned16)
         moments_kernel<true><<<(int)blocks, kMomBlock, 0, b->stream>>>(a);
     else
         moments_kernel<false><<<(int)blocks, kMomBlock, 0, b->stream>>>(a);
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return fail(BT_ERR_CUDA, std::string("bt_beam_moments launch: ") + cudaGetErrorString(e));
-    g_launch_count.fetch_add(2);
+    g_launch_count.fetch_add(1);
     double h[42];
     BT_CUDA_TRY(cudaMemcpyAsync(h, a.out, sizeof(h), cudaMemcpyDeviceToHost, b->stream));
     BT_CUDA_TRY(cudaStreamSynchronize(b->stream));
