@@ -40,6 +40,10 @@ def lib():
         L.orc_gather_kick.restype = C.c_int64
         L.orc_gather_field.argtypes = [C.c_int64] + [_dp] * 3 + [C.c_int32] * 3 + [_dp, _dp] + [_dp] * 3 + [C.c_double] + [_dp] * 3
         L.orc_gather_field.restype = C.c_int64
+        L.orc_deposit_tsc.argtypes = L.orc_deposit_cic.argtypes
+        L.orc_deposit_tsc.restype = C.c_int64
+        L.orc_gather_kick_tsc.argtypes = L.orc_gather_kick.argtypes
+        L.orc_gather_kick_tsc.restype = C.c_int64
         L.orc_moments.argtypes = [C.c_int64, C.POINTER(_dp), _dp, _dp]
         L.orc_moments.restype = C.c_int
         _lib = L
@@ -100,35 +104,42 @@ def track(coords, lattice, nturns, gamma, s=0.0):
     return g.value, ss.value
 
 
-def deposit_cic(x, y, t, shape, lo, d, q_weight, zscale=1.0, rho=None):
-    """Returns (rho[nz,ny,nx] charge per node, n_inside). rho given => accumulate onto it."""
+def deposit_cic(x, y, t, shape, lo, d, q_weight, zscale=1.0, rho=None, order=1):
+    """Returns (rho[nz,ny,nx] charge per node, n_inside). rho given => accumulate onto it.
+    order = 1: CIC (R11); order = 2: quadratic B-spline (R16, PAPER.md l.60 set_particle_shape(2))."""
     nx, ny, nz = shape
     zero_first = rho is None
     if rho is None:
         rho = np.zeros((nz, ny, nx), dtype=np.float64)
     lo, d = _v3(lo), _v3(d)
-    inside = lib().orc_deposit_cic(x.shape[0], _p(x), _p(y), _p(t), nx, ny, nz, _p(lo), _p(d),
-                                   q_weight, zscale, _p(rho.reshape(-1)), int(zero_first))
+    fn = {1: lib().orc_deposit_cic, 2: lib().orc_deposit_tsc}[order]
+    inside = fn(x.shape[0], _p(x), _p(y), _p(t), nx, ny, nz, _p(lo), _p(d),
+                q_weight, zscale, _p(rho.reshape(-1)), int(zero_first))
     if inside < 0:
         raise ValueError("oracle: invalid grid")
     return rho, int(inside)
 
 
-def gather_kick(coords, shape, lo, d, E, coef, zscale=1.0):
-    """In place px,py,pt += coef * trilinear(E) ; E = (Ex,Ey,Ez) node arrays, x fastest."""
+def gather_kick(coords, shape, lo, d, E, coef, zscale=1.0, order=1):
+    """In place px,py,pt += coef * interp(E) ; E = (Ex,Ey,Ez) node arrays, x fastest; order 1 trilinear, 2 quadratic B-spline."""
     nx, ny, nz = shape
     lo, d, coef = _v3(lo), _v3(d), _v3(coef)
     x, px, y, py, t, pt = coords
     Ex, Ey, Ez = [np.ascontiguousarray(e, dtype=np.float64).reshape(-1) for e in E]
     assert Ex.size == nx * ny * nz
-    inside = lib().orc_gather_kick(x.shape[0], _p(x), _p(px), _p(y), _p(py), _p(t), _p(pt), nx, ny, nz,
-                                   _p(lo), _p(d), _p(Ex), _p(Ey), _p(Ez), _p(coef), zscale)
+    fn = {1: lib().orc_gather_kick, 2: lib().orc_gather_kick_tsc}[order]
+    inside = fn(x.shape[0], _p(x), _p(px), _p(y), _p(py), _p(t), _p(pt), nx, ny, nz,
+                _p(lo), _p(d), _p(Ex), _p(Ey), _p(Ez), _p(coef), zscale)
     if inside < 0:
         raise ValueError("oracle: invalid grid")
     return int(inside)
 
 
-def gather_field(x, y, t, shape, lo, d, E, zscale=1.0):
+def gather_field(x, y, t, shape, lo, d, E, zscale=1.0, order=1):
+    if order == 2:
+        out = [np.zeros_like(x) for _ in range(3)]
+        gather_kick([x, out[0], y, out[1], t, out[2]], shape, lo, d, E, (1.0, 1.0, 1.0), zscale, order=2)
+        return out
     nx, ny, nz = shape
     lo, d = _v3(lo), _v3(d)
     Ex, Ey, Ez = [np.ascontiguousarray(e, dtype=np.float64).reshape(-1) for e in E]
