@@ -165,6 +165,16 @@ void bt_grid_destroy(bt_grid *grid);
 /* Field at the nodes, 3 arrays of nx*ny*nz doubles, x fastest; on_device != 0: device pointers (copied
  * device-to-device), else host pointers.  The library keeps its own (internally re-laid-out) copy. */
 int bt_grid_set_field(bt_grid *grid, const double *Ex, const double *Ey, const double *Ez, int on_device);
+/*
+ * Particle shape used by bt_deposit_cic and bt_gather_kick on this grid; mirrors sim.set_particle_shape(order)
+ * (P:l.60).  order = 1 (default): CIC / trilinear, 8 nodes (R11).  order = 2: quadratic B-spline,
+ * 27 nodes (reading R16): v = u + 0.5, j = floor(v) the nearest node, delta = u - j, weights on nodes j-1, j, j+1
+ *   (1/2)(1/2 - delta)^2,  3/4 - delta^2,  (1/2)(1/2 + delta)^2     (each operation rounded once, in this order),
+ * node weight (wx*wy)*wz; inside iff 1 <= j <= n-2 on all axes (tested as v >= 1 && v < n-1), else skipped / zero
+ * field.  Needs >= 3 nodes per axis.  Other orders: BT_ERR_UNSUPPORTED.  bt_beam_sort_by_cell keeps ordering by the
+ * order-1 cell; both kernels are correct for any order of the particles.
+ */
+int bt_grid_set_particle_shape(bt_grid *grid, int32_t order);
 int bt_grid_rho(bt_grid *grid, double **dev_rho_out);    /* zero-copy device view of rho */
 int bt_grid_download_rho(bt_grid *grid, double *host_rho); /* synchronises the last beam stream used */
 

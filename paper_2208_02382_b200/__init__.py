@@ -50,6 +50,7 @@ EXPORTS = {
     "bt_grid_create": (C.c_int, [C.POINTER(_vp), C.c_int32, C.c_int32, C.c_int32, _dp, _dp]),
     "bt_grid_destroy": (None, [_vp]),
     "bt_grid_set_field": (C.c_int, [_vp, _vp, _vp, _vp, C.c_int]),
+    "bt_grid_set_particle_shape": (C.c_int, [_vp, C.c_int32]),
     "bt_grid_rho": (C.c_int, [_vp, C.POINTER(_vp)]),
     "bt_grid_download_rho": (C.c_int, [_vp, _vp]),
     "bt_deposit_cic": (C.c_int, [_vp, _vp, C.c_double, C.c_double, C.c_int]),
@@ -244,6 +245,10 @@ class Grid:
             self._h = None
 
     __del__ = close
+
+    def set_particle_shape(self, order):
+        """1 = CIC (default), 2 = quadratic B-spline."""
+        _check(lib.bt_grid_set_particle_shape(self._h, int(order)), "bt_grid_set_particle_shape")
 
     def set_field(self, Ex, Ey, Ez):
         """Host numpy arrays (any shape with nx*ny*nz elements, x fastest) or CUDA torch tensors."""

@@ -537,6 +537,15 @@ int bt_grid_download_rho(bt_grid *grid, double *host_rho) {
     return BT_OK;
 }
 
+int bt_grid_set_particle_shape(bt_grid *grid, int32_t order) {
+    if (!grid) return fail(BT_ERR_INVALID, "bt_grid_set_particle_shape: grid is NULL");
+    if (order != 1 && order != 2) return fail(BT_ERR_UNSUPPORTED, "bt_grid_set_particle_shape: order must be 1 (CIC) or 2 (quadratic B-spline)");
+    Grid &g = grid->g;
+    if (order == 2 && (g.nx < 3 || g.ny < 3 || g.nz < 3)) return fail(BT_ERR_INVALID, "bt_grid_set_particle_shape: order 2 needs >= 3 nodes per axis");
+    g.order = order;
+    return BT_OK;
+}
+
 int bt_deposit_cic(bt_beam *beam, bt_grid *grid, double q_weight, double zscale, int zero_first) {
     if (!beam || !grid) return fail(BT_ERR_INVALID, "bt_deposit_cic: NULL argument");
     if (!isfinite(q_weight) || !isfinite(zscale)) return fail(BT_ERR_INVALID, "bt_deposit_cic: q_weight or zscale not finite");

@@ -95,6 +95,7 @@ struct Beam {
 
 struct Grid {
     int32_t nx = 0, ny = 0, nz = 0;
+    int32_t order = 1;  // particle shape: 1 = CIC (R11), 2 = quadratic B-spline (R16)
     double lo[3] = {0, 0, 0}, d[3] = {0, 0, 0}, inv_d[3] = {0, 0, 0};
     int64_t nn = 0;
     double *rho = nullptr;

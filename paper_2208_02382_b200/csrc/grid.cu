@@ -15,27 +15,25 @@
 
 namespace bt {
 
-// ---- S5 deposit, mode 0: one particle per thread, 8 global fp64 reductions (RED.E.ADD.F64) --------
+// ---- S5 deposit, mode 0: one particle per thread, (ORDER+1)^3 global fp64 reductions (RED.E.ADD.F64) ----------
+template <int ORDER>
 __global__ void __launch_bounds__(256) deposit_atomic_kernel(const double *__restrict__ x, const double *__restrict__ y,
                                                              const double *__restrict__ t, long long n, GridDev g,
                                                              double qw, double zscale, double *__restrict__ rho) {
+    constexpr int NW = ORDER + 1;
     const long long stride = (long long)gridDim.x * blockDim.x;
     for (long long p = (long long)blockIdx.x * blockDim.x + threadIdx.x; p < n; p += stride) {
         Cic c;
-        if (!cic_locate(g, x[p], y[p], t[p], zscale, c)) continue;
-        const double wx[2] = {__dsub_rn(1.0, c.wx1), c.wx1};
-        const double wy[2] = {__dsub_rn(1.0, c.wy1), c.wy1};
-        const double wz[2] = {__dsub_rn(1.0, c.wz1), c.wz1};
+        if (!shape_locate<ORDER>(g, x[p], y[p], t[p], zscale, c)) continue;
+        double w[NW * NW * NW];
+        node_weights<ORDER>(c, qw, w);
         double *base = rho + ((long long)c.k * g.ny + c.j) * g.nx + c.i;
 #pragma unroll
-        for (int dz = 0; dz < 2; ++dz)
+        for (int dz = 0; dz < NW; ++dz)
 #pragma unroll
-            for (int dy = 0; dy < 2; ++dy)
+            for (int dy = 0; dy < NW; ++dy)
 #pragma unroll
-                for (int dx = 0; dx < 2; ++dx) {
-                    const double w = __dmul_rn(__dmul_rn(wx[dx], wy[dy]), wz[dz]);
-                    atomicAdd(base + ((long long)dz * g.ny + dy) * g.nx + dx, __dmul_rn(qw, w));
-                }
+                for (int dx = 0; dx < NW; ++dx) atomicAdd(base + ((long long)dz * g.ny + dy) * g.nx + dx, w[(dz * NW + dy) * NW + dx]);
     }
 }
 
@@ -56,18 +54,17 @@ __device__ __forceinline__ void load_run(const double *__restrict__ q, long long
         for (int r = 0; r < R; ++r) v[r] = (p0 + r < n) ? q[p0 + r] : fill;
     }
 }
-// ---- run flush: the 8 node sums of one cell -> 8 RED.E.ADD.F64 ------------------------------------------------
-__device__ __forceinline__ void flush_cell(double *__restrict__ rho, int key, const double (&acc)[8], int nx, long long nxy) {
+// ---- run flush: the node sums of one stencil position -> (ORDER+1)^3 RED.E.ADD.F64 ------------------------------
+template <int NW>
+__device__ __forceinline__ void flush_cell(double *__restrict__ rho, int key, const double (&acc)[NW * NW * NW], int nx, long long nxy) {
     if (key < 0) return;
-    double *base = rho + key;  // key = linear index of the lower-corner node
-    atomicAdd(base, acc[0]);
-    atomicAdd(base + 1, acc[1]);
-    atomicAdd(base + nx, acc[2]);
-    atomicAdd(base + nx + 1, acc[3]);
-    atomicAdd(base + nxy, acc[4]);
-    atomicAdd(base + nxy + 1, acc[5]);
-    atomicAdd(base + nxy + nx, acc[6]);
-    atomicAdd(base + nxy + nx + 1, acc[7]);
+    double *base = rho + key;  // key = linear index of the lowest node of the stencil
+#pragma unroll
+    for (int dz = 0; dz < NW; ++dz)
+#pragma unroll
+        for (int dy = 0; dy < NW; ++dy)
+#pragma unroll
+            for (int dx = 0; dx < NW; ++dx) atomicAdd(base + dz * nxy + dy * nx + dx, acc[(dz * NW + dy) * NW + dx]);
 }
 
 // ---- S4+S5 deposit, mode 1 (default): block-local cell binning in shared memory + run accumulation ------------
@@ -85,20 +82,9 @@ __device__ __forceinline__ void flush_cell(double *__restrict__ rho, int key, co
 constexpr int kBinBlock = 256;
 constexpr int kBinCap = 4096;  // cells of the chunk's bounding box that the shared histogram can hold
 
-__device__ __forceinline__ void cic_weights8(const Cic &c, double qw, double (&w)[8]) {
-    const double wx0 = __dsub_rn(1.0, c.wx1), wy0 = __dsub_rn(1.0, c.wy1), wz0 = __dsub_rn(1.0, c.wz1);
-    w[0] = __dmul_rn(qw, __dmul_rn(__dmul_rn(wx0, wy0), wz0));
-    w[1] = __dmul_rn(qw, __dmul_rn(__dmul_rn(c.wx1, wy0), wz0));
-    w[2] = __dmul_rn(qw, __dmul_rn(__dmul_rn(wx0, c.wy1), wz0));
-    w[3] = __dmul_rn(qw, __dmul_rn(__dmul_rn(c.wx1, c.wy1), wz0));
-    w[4] = __dmul_rn(qw, __dmul_rn(__dmul_rn(wx0, wy0), c.wz1));
-    w[5] = __dmul_rn(qw, __dmul_rn(__dmul_rn(c.wx1, wy0), c.wz1));
-    w[6] = __dmul_rn(qw, __dmul_rn(__dmul_rn(wx0, c.wy1), c.wz1));
-    w[7] = __dmul_rn(qw, __dmul_rn(__dmul_rn(c.wx1, c.wy1), c.wz1));
-}
-
 // merge the lanes' open runs (segmented suffix reduction over CONTIGUOUS equal keys), heads flush
-__device__ __forceinline__ void merge_and_flush(double *__restrict__ rho, int cur, double (&acc)[8], int nx, long long nxy) {
+template <int NW>
+__device__ __forceinline__ void merge_and_flush(double *__restrict__ rho, int cur, double (&acc)[NW * NW * NW], int nx, long long nxy) {
     const int lane = threadIdx.x & 31;
     const int prev = __shfl_up_sync(0xffffffffu, cur, 1);
     const bool head = (lane == 0) || (prev != cur);
@@ -112,13 +98,13 @@ __device__ __forceinline__ void merge_and_flush(double *__restrict__ rho, int cu
             if (d > span) break;  // warp-uniform
             const bool take = lane + d <= end;
 #pragma unroll
-            for (int k = 0; k < 8; ++k) {
+            for (int k = 0; k < NW * NW * NW; ++k) {
                 const double o = __shfl_down_sync(0xffffffffu, acc[k], d);
                 if (take) acc[k] += o;
             }
         }
     }
-    if (head) flush_cell(rho, cur, acc, nx, nxy);
+    if (head) flush_cell<NW>(rho, cur, acc, nx, nxy);
 }
 
 template <int R>
@@ -133,26 +119,28 @@ struct BinSmem {
     double w1[3][PAD];
 };
 
-__device__ __forceinline__ void run_add(double *__restrict__ rho, int key, const double (&w)[8], int &cur, double (&acc)[8], int nx,
-                                        long long nxy) {
+template <int NW>
+__device__ __forceinline__ void run_add(double *__restrict__ rho, int key, const double (&w)[NW * NW * NW], int &cur,
+                                        double (&acc)[NW * NW * NW], int nx, long long nxy) {
     if (key != cur) {
-        flush_cell(rho, cur, acc, nx, nxy);
+        flush_cell<NW>(rho, cur, acc, nx, nxy);
         cur = key;
 #pragma unroll
-        for (int d = 0; d < 8; ++d) acc[d] = w[d];
+        for (int d = 0; d < NW * NW * NW; ++d) acc[d] = w[d];
     } else {
 #pragma unroll
-        for (int d = 0; d < 8; ++d) acc[d] += w[d];
+        for (int d = 0; d < NW * NW * NW; ++d) acc[d] += w[d];
     }
 }
 
-template <int R, bool VEC>
-__global__ void __launch_bounds__(kBinBlock, R >= 8 ? 2 : 3) deposit_binned_kernel(const double *__restrict__ x, const double *__restrict__ y,
+template <int R, bool VEC, int ORDER>
+__global__ void __launch_bounds__(kBinBlock, (R >= 8 || ORDER > 1) ? 2 : 3) deposit_binned_kernel(const double *__restrict__ x, const double *__restrict__ y,
                                                                    const double *__restrict__ t, long long n, GridDev g, double qw,
                                                                    double zscale, double *__restrict__ rho) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     BinSmem<R> &sm = *reinterpret_cast<BinSmem<R> *>(smem_raw);
     constexpr int CH = BinSmem<R>::CH;
+    constexpr int NW = ORDER + 1, NN = NW * NW * NW;
     constexpr int kBig = 0x7fffffff;
     const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
     const long long nxy = (long long)g.nx * g.ny;
@@ -172,7 +160,7 @@ __global__ void __launch_bounds__(kBinBlock, R >= 8 ? 2 : 3) deposit_binned_kern
         int lo_i = kBig, lo_j = kBig, lo_k = kBig, hi_i = -1, hi_j = -1, hi_k = -1;
 #pragma unroll
         for (int r = 0; r < R; ++r) {
-            in[r] = cic_locate(g, qx[r], qy[r], qt[r], zscale, c[r]);
+            in[r] = shape_locate<ORDER>(g, qx[r], qy[r], qt[r], zscale, c[r]);
             if (in[r]) {
                 lo_i = min(lo_i, c[r].i), hi_i = max(hi_i, c[r].i);
                 lo_j = min(lo_j, c[r].j), hi_j = max(hi_j, c[r].j);
@@ -222,9 +210,9 @@ __global__ void __launch_bounds__(kBinBlock, R >= 8 ? 2 : 3) deposit_binned_kern
                 const unsigned li = (unsigned)(c[r].i - i0), lj = (unsigned)(c[r].j - j0), lk = (unsigned)(c[r].k - k0);
                 const bool binned = in[r] && li < 16u && lj < 16u && lk < 16u;
                 if (in[r] && !binned) {
-                    double w[8];
-                    cic_weights8(c[r], qw, w);
-                    flush_cell(rho, (c[r].k * g.ny + c[r].j) * g.nx + c[r].i, w, g.nx, nxy);
+                    double w[NN];
+                    node_weights<ORDER>(c[r], qw, w);
+                    flush_cell<NW>(rho, (c[r].k * g.ny + c[r].j) * g.nx + c[r].i, w, g.nx, nxy);
                 }
                 in[r] = binned;
                 lc[r] = binned ? (int)((lk * 16u + lj) * 16u + li) : kBinCap;
@@ -292,9 +280,9 @@ __global__ void __launch_bounds__(kBinBlock, R >= 8 ? 2 : 3) deposit_binned_kern
         __syncthreads();  // (6) cell-ordered entry list complete
         {
             int cur = -1;
-            double acc[8];
+            double acc[NN];
 #pragma unroll
-            for (int d = 0; d < 8; ++d) acc[d] = 0.0;
+            for (int d = 0; d < NN; ++d) acc[d] = 0.0;
 #pragma unroll
             for (int r = 0; r < R; ++r) {
                 const int e = tid * R + r;
@@ -303,11 +291,11 @@ __global__ void __launch_bounds__(kBinBlock, R >= 8 ? 2 : 3) deposit_binned_kern
                 Cic cc;
                 cc.i = cc.j = cc.k = 0;
                 cc.wx1 = sm.w1[0][slot], cc.wy1 = sm.w1[1][slot], cc.wz1 = sm.w1[2][slot];
-                double w[8];
-                cic_weights8(cc, qw, w);
-                run_add(rho, sm.key[slot], w, cur, acc, g.nx, nxy);
+                double w[NN];
+                node_weights<ORDER>(cc, qw, w);
+                run_add<NW>(rho, sm.key[slot], w, cur, acc, g.nx, nxy);
             }
-            merge_and_flush(rho, cur, acc, g.nx, nxy);
+            merge_and_flush<NW>(rho, cur, acc, g.nx, nxy);
         }
         // no barrier here: the next chunk touches hist / entries only after its barrier (1), which every thread of this
         // chunk's walk must reach first
@@ -319,44 +307,47 @@ static int env_int_grid(const char *name, int dflt) {
     return (v && *v) ? atoi(v) : dflt;
 }
 
-template <int R>
+template <int R, bool VEC, int ORDER>
 static int launch_deposit_binned(Beam *b, Grid *g, const GridDev &gd, double q_weight, double zscale) {
     const int smem = (int)sizeof(BinSmem<R>);
     const long long nchunks = (b->n + BinSmem<R>::CH - 1) / BinSmem<R>::CH;
-    long long blocks = nchunks;
     int per_sm = 1;
-    if (b->aligned32) {
-        BT_CUDA_TRY(cudaFuncSetAttribute(deposit_binned_kernel<R, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
-        BT_CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, deposit_binned_kernel<R, true>, kBinBlock, smem));
-    } else {
-        BT_CUDA_TRY(cudaFuncSetAttribute(deposit_binned_kernel<R, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
-        BT_CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, deposit_binned_kernel<R, false>, kBinBlock, smem));
-    }
-    const long long cap = (long long)b->num_sms * (per_sm > 0 ? per_sm : 1);
-    if (blocks > cap) blocks = cap;
-    if (b->aligned32) {
-        deposit_binned_kernel<R, true><<<(int)blocks, kBinBlock, smem, b->stream>>>(b->q[0], b->q[2], b->q[4], b->n, gd, q_weight, zscale, g->rho);
-    } else {
-        deposit_binned_kernel<R, false><<<(int)blocks, kBinBlock, smem, b->stream>>>(b->q[0], b->q[2], b->q[4], b->n, gd, q_weight, zscale, g->rho);
-    }
+    BT_CUDA_TRY(cudaFuncSetAttribute(deposit_binned_kernel<R, VEC, ORDER>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+    BT_CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, deposit_binned_kernel<R, VEC, ORDER>, kBinBlock, smem));
+    long long blocks = (long long)b->num_sms * (per_sm > 0 ? per_sm : 1);
+    if (blocks > nchunks) blocks = nchunks;
+    deposit_binned_kernel<R, VEC, ORDER><<<(int)blocks, kBinBlock, smem, b->stream>>>(b->q[0], b->q[2], b->q[4], b->n, gd, q_weight,
+                                                                                     zscale, g->rho);
     return BT_OK;
 }
 
-int launch_deposit(Beam *b, Grid *g, double q_weight, double zscale) {
-    const GridDev gd = make_grid_dev(*g);
-    // BT_DEPOSIT_MODE: 0 = one particle per thread, 8 reductions each (baseline, kept for measurements);
-    // 1 (default) = block-local cell binning, 8 particles per thread; 2 = the same with 4 particles per thread
+template <int ORDER>
+static int launch_deposit_order(Beam *b, Grid *g, const GridDev &gd, double q_weight, double zscale) {
+    // BT_DEPOSIT_MODE: 0 = one particle per thread, (ORDER+1)^3 reductions each (baseline, kept for measurements);
+    // 1 (default) = block-local cell binning, 8 particles per thread (4 for order 2: 27 run accumulators per thread);
+    // 2 = binning with 4 particles per thread
     const int mode = env_int_grid("BT_DEPOSIT_MODE", 1);
     if (mode == 0) {
         const int block = 256;
         long long blocks = (b->n + block - 1) / block;
         const long long cap = (long long)b->num_sms * 16;
         if (blocks > cap) blocks = cap;
-        deposit_atomic_kernel<<<(int)blocks, block, 0, b->stream>>>(b->q[0], b->q[2], b->q[4], b->n, gd, q_weight, zscale, g->rho);
-    } else {
-        const int rc = mode == 2 ? launch_deposit_binned<4>(b, g, gd, q_weight, zscale) : launch_deposit_binned<8>(b, g, gd, q_weight, zscale);
-        if (rc != BT_OK) return rc;
+        deposit_atomic_kernel<ORDER><<<(int)blocks, block, 0, b->stream>>>(b->q[0], b->q[2], b->q[4], b->n, gd, q_weight, zscale, g->rho);
+        return BT_OK;
     }
+    if constexpr (ORDER == 1) {
+        if (mode != 2)
+            return b->aligned32 ? launch_deposit_binned<8, true, ORDER>(b, g, gd, q_weight, zscale)
+                                : launch_deposit_binned<8, false, ORDER>(b, g, gd, q_weight, zscale);
+    }
+    return b->aligned32 ? launch_deposit_binned<4, true, ORDER>(b, g, gd, q_weight, zscale)
+                        : launch_deposit_binned<4, false, ORDER>(b, g, gd, q_weight, zscale);
+}
+
+int launch_deposit(Beam *b, Grid *g, double q_weight, double zscale) {
+    const GridDev gd = make_grid_dev(*g);
+    const int rc = g->order == 2 ? launch_deposit_order<2>(b, g, gd, q_weight, zscale) : launch_deposit_order<1>(b, g, gd, q_weight, zscale);
+    if (rc != BT_OK) return rc;
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return fail(BT_ERR_CUDA, std::string("bt_deposit_cic launch: ") + cudaGetErrorString(e));
     g_launch_count.fetch_add(1);
@@ -396,43 +387,53 @@ __device__ __forceinline__ void ld_node(const double *f, double &ex, double &ey,
     asm volatile("{ .reg .f64 pad; ld.global.nc.v4.f64 {%0,%1,%2,pad}, [%3]; }" : "=d"(ex), "=d"(ey), "=d"(ez) : "l"(f));
 }
 
+// One particle through [drift] -> gather over the (ORDER+1)^3 stencil -> kick -> [drift]; shared by both gather kernels.
+// Gather order dz, dy, dx (R12); weight (wx*wy)*wz with explicit roundings, field accumulated with FMAs.
+template <int ORDER>
+__device__ __forceinline__ void gather_kick_one(const GatherArgs &a, double &x, double &px, double &y, double &py, double &t, double &pt) {
+    constexpr int NW = ORDER + 1;
+    // R4 drift before the kick
+    x = fma(a.hb, px, x);
+    y = fma(a.hb, py, y);
+    t = fma(a.tcb, pt, t);
+    Cic c;
+    if (shape_locate<ORDER>(a.g, x, y, t, a.zscale, c)) {
+        double wx[NW], wy[NW], wz[NW];
+        axis_weights<ORDER>(c.wx1, wx);
+        axis_weights<ORDER>(c.wy1, wy);
+        axis_weights<ORDER>(c.wz1, wz);
+        const double *base = a.field + 4 * (((long long)c.k * a.g.ny + c.j) * a.g.nx + c.i);
+        double ex = 0.0, ey = 0.0, ez = 0.0;
+#pragma unroll
+        for (int dz = 0; dz < NW; ++dz)
+#pragma unroll
+            for (int dy = 0; dy < NW; ++dy)
+#pragma unroll
+                for (int dx = 0; dx < NW; ++dx) {
+                    const double w = __dmul_rn(__dmul_rn(wx[dx], wy[dy]), wz[dz]);
+                    double fx, fy, fz;
+                    ld_node(base + 4 * (((long long)dz * a.g.ny + dy) * a.g.nx + dx), fx, fy, fz);
+                    ex = fma(w, fx, ex);
+                    ey = fma(w, fy, ey);
+                    ez = fma(w, fz, ez);
+                }
+        px = fma(a.coef[0], ex, px);
+        py = fma(a.coef[1], ey, py);
+        pt = fma(a.coef[2], ez, pt);
+    }
+    // R4 drift after the kick
+    x = fma(a.ha, px, x);
+    y = fma(a.ha, py, y);
+    t = fma(a.tca, pt, t);
+}
+
+template <int ORDER>
 __global__ void __launch_bounds__(256) gather_kick_kernel(const __grid_constant__ GatherArgs a) {
     const long long stride = (long long)gridDim.x * blockDim.x;
     for (long long p = (long long)blockIdx.x * blockDim.x + threadIdx.x; p < a.n; p += stride) {
         double x = __ldcs(a.q[0] + p), px = __ldcs(a.q[1] + p), y = __ldcs(a.q[2] + p);
         double py = __ldcs(a.q[3] + p), t = __ldcs(a.q[4] + p), pt = __ldcs(a.q[5] + p);
-        // R4 drift before the kick
-        x = fma(a.hb, px, x);
-        y = fma(a.hb, py, y);
-        t = fma(a.tcb, pt, t);
-        Cic c;
-        if (cic_locate(a.g, x, y, t, a.zscale, c)) {
-            const double wx[2] = {__dsub_rn(1.0, c.wx1), c.wx1};
-            const double wy[2] = {__dsub_rn(1.0, c.wy1), c.wy1};
-            const double wz[2] = {__dsub_rn(1.0, c.wz1), c.wz1};
-            const double *base = a.field + 4 * (((long long)c.k * a.g.ny + c.j) * a.g.nx + c.i);
-            double ex = 0.0, ey = 0.0, ez = 0.0;
-#pragma unroll
-            for (int dz = 0; dz < 2; ++dz)
-#pragma unroll
-                for (int dy = 0; dy < 2; ++dy)
-#pragma unroll
-                    for (int dx = 0; dx < 2; ++dx) {
-                        const double w = __dmul_rn(__dmul_rn(wx[dx], wy[dy]), wz[dz]);
-                        double fx, fy, fz;
-                        ld_node(base + 4 * (((long long)dz * a.g.ny + dy) * a.g.nx + dx), fx, fy, fz);
-                        ex = fma(w, fx, ex);
-                        ey = fma(w, fy, ey);
-                        ez = fma(w, fz, ez);
-                    }
-            px = fma(a.coef[0], ex, px);
-            py = fma(a.coef[1], ey, py);
-            pt = fma(a.coef[2], ez, pt);
-        }
-        // R4 drift after the kick
-        x = fma(a.ha, px, x);
-        y = fma(a.ha, py, y);
-        t = fma(a.tca, pt, t);
+        gather_kick_one<ORDER>(a, x, px, y, py, t, pt);
         __stcs(a.q[0] + p, x);
         __stcs(a.q[1] + p, px);
         __stcs(a.q[2] + p, y);
@@ -460,7 +461,7 @@ struct GpSmem {
     alignas(8) uint64_t full[kGpStages];
 };
 
-template <int NT, int R>
+template <int NT, int R, int ORDER>
 __global__ void __launch_bounds__(NT) gather_kick_pipe_kernel(const __grid_constant__ GatherArgs a, long long nchunks, int store_positions) {
     constexpr int CH = NT * R;
     constexpr uint32_t kArrBytes = CH * sizeof(double);
@@ -489,38 +490,7 @@ __global__ void __launch_bounds__(NT) gather_kick_pipe_kernel(const __grid_const
         for (int r = 0; r < R; ++r) {
             const int e = r * NT + tid;
             double x = q[0][e], px = q[1][e], y = q[2][e], py = q[3][e], t = q[4][e], pt = q[5][e];
-            // R4 drift before the kick
-            x = fma(a.hb, px, x);
-            y = fma(a.hb, py, y);
-            t = fma(a.tcb, pt, t);
-            Cic c;
-            if (cic_locate(a.g, x, y, t, a.zscale, c)) {
-                const double wx[2] = {__dsub_rn(1.0, c.wx1), c.wx1};
-                const double wy[2] = {__dsub_rn(1.0, c.wy1), c.wy1};
-                const double wz[2] = {__dsub_rn(1.0, c.wz1), c.wz1};
-                const double *base = a.field + 4 * (((long long)c.k * a.g.ny + c.j) * a.g.nx + c.i);
-                double ex = 0.0, ey = 0.0, ez = 0.0;
-#pragma unroll
-                for (int dz = 0; dz < 2; ++dz)
-#pragma unroll
-                    for (int dy = 0; dy < 2; ++dy)
-#pragma unroll
-                        for (int dx = 0; dx < 2; ++dx) {
-                            const double w = __dmul_rn(__dmul_rn(wx[dx], wy[dy]), wz[dz]);
-                            double fx, fy, fz;
-                            ld_node(base + 4 * (((long long)dz * a.g.ny + dy) * a.g.nx + dx), fx, fy, fz);
-                            ex = fma(w, fx, ex);
-                            ey = fma(w, fy, ey);
-                            ez = fma(w, fz, ez);
-                        }
-                px = fma(a.coef[0], ex, px);
-                py = fma(a.coef[1], ey, py);
-                pt = fma(a.coef[2], ez, pt);
-            }
-            // R4 drift after the kick
-            x = fma(a.ha, px, x);
-            y = fma(a.ha, py, y);
-            t = fma(a.tca, pt, t);
+            gather_kick_one<ORDER>(a, x, px, y, py, t, pt);
             q[0][e] = x, q[1][e] = px, q[2][e] = y, q[3][e] = py, q[4][e] = t, q[5][e] = pt;
         }
         fence_proxy_async_smem();  // this thread's shared-memory writes -> visible to the copy engine
@@ -542,27 +512,42 @@ __global__ void __launch_bounds__(NT) gather_kick_pipe_kernel(const __grid_const
     if (tid == 0) bulk_wait_all<0>();  // shared memory must outlive the last stores
 }
 
-template <int NT, int R>
+template <int NT, int R, int ORDER>
 static int launch_gather_pipe(Beam *b, const GatherArgs &a0) {
     constexpr int CH = NT * R;
     const int smem = (int)sizeof(GpSmem<CH>);
     const long long nchunks = b->n / CH;
     if (nchunks > 0) {
         int per_sm = 1;
-        BT_CUDA_TRY(cudaFuncSetAttribute(gather_kick_pipe_kernel<NT, R>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
-        BT_CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, gather_kick_pipe_kernel<NT, R>, NT, smem));
+        BT_CUDA_TRY(cudaFuncSetAttribute(gather_kick_pipe_kernel<NT, R, ORDER>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+        BT_CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, gather_kick_pipe_kernel<NT, R, ORDER>, NT, smem));
         long long blocks = (long long)b->num_sms * (per_sm > 0 ? per_sm : 1);
         if (blocks > nchunks) blocks = nchunks;
         const int store_positions = (a0.hb != 0.0 || a0.ha != 0.0 || a0.tcb != 0.0 || a0.tca != 0.0) ? 1 : 0;
-        gather_kick_pipe_kernel<NT, R><<<(int)blocks, NT, smem, b->stream>>>(a0, nchunks, store_positions);
+        gather_kick_pipe_kernel<NT, R, ORDER><<<(int)blocks, NT, smem, b->stream>>>(a0, nchunks, store_positions);
     }
     const long long done = nchunks * CH;
     if (done < b->n) {  // ragged tail: one particle per thread
         GatherArgs t = a0;
         for (int c = 0; c < 6; ++c) t.q[c] = a0.q[c] + done;
         t.n = b->n - done;
-        gather_kick_kernel<<<(int)((t.n + 255) / 256), 256, 0, b->stream>>>(t);
+        gather_kick_kernel<ORDER><<<(int)((t.n + 255) / 256), 256, 0, b->stream>>>(t);
     }
+    return BT_OK;
+}
+
+template <int ORDER>
+static int launch_gather_order(Beam *b, const GatherArgs &a) {
+    // BT_GATHER_MODE: 0 = one particle per thread, everything through registers (also the path for arrays that are not
+    // 16-byte aligned); 1 (default) = streaming pipeline, 256-particle chunks; 2 / 3 = pipeline with 512 / 128-particle chunks
+    const int mode = env_int_grid("BT_GATHER_MODE", 1);
+    if (mode >= 1 && b->aligned16)
+        return mode == 2 ? launch_gather_pipe<512, 1, ORDER>(b, a) : mode == 3 ? launch_gather_pipe<128, 1, ORDER>(b, a) : launch_gather_pipe<256, 1, ORDER>(b, a);
+    const int block = 256;
+    long long blocks = (b->n + block - 1) / block;
+    const long long cap = (long long)b->num_sms * 16;
+    if (blocks > cap) blocks = cap;
+    gather_kick_kernel<ORDER><<<(int)blocks, block, 0, b->stream>>>(a);
     return BT_OK;
 }
 
@@ -579,19 +564,8 @@ int launch_gather_kick(Beam *b, const Grid *g, const double coef[3], double zsca
     a.tcb = tc_before;
     a.ha = h_after;
     a.tca = tc_after;
-    // BT_GATHER_MODE: 0 = one particle per thread, everything through registers (also the path for arrays that are not
-    // 16-byte aligned); 1 (default) = streaming pipeline, 256-particle chunks; 2 / 3 = pipeline with 512 / 128-particle chunks
-    const int mode = env_int_grid("BT_GATHER_MODE", 1);
-    if (mode >= 1 && b->aligned16) {
-        const int rc = mode == 2 ? launch_gather_pipe<512, 1>(b, a) : mode == 3 ? launch_gather_pipe<128, 1>(b, a) : launch_gather_pipe<256, 1>(b, a);
-        if (rc != BT_OK) return rc;
-    } else {
-        const int block = 256;
-        long long blocks = (b->n + block - 1) / block;
-        const long long cap = (long long)b->num_sms * 16;
-        if (blocks > cap) blocks = cap;
-        gather_kick_kernel<<<(int)blocks, block, 0, b->stream>>>(a);
-    }
+    const int rc = g->order == 2 ? launch_gather_order<2>(b, a) : launch_gather_order<1>(b, a);
+    if (rc != BT_OK) return rc;
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return fail(BT_ERR_CUDA, std::string("bt_gather_kick launch: ") + cudaGetErrorString(e));
     g_launch_count.fetch_add(1);

@@ -56,5 +56,62 @@ __device__ __forceinline__ bool cic_locate(const GridDev &g, double x, double y,
     return ix && iy && iz;
 }
 
+// ---- order-2 shape (reading R16, quadratic B-spline; P:l.60 set_particle_shape(2)) ---------------------------------
+//   v = u + 0.5, j = floor(v) (nearest node), delta = u - j; nodes j-1, j, j+1 carry
+//   (1/2)(1/2 - delta)^2, 3/4 - delta^2, (1/2)(1/2 + delta)^2, every operation rounded once in this order.
+// Inside iff 1 <= j <= n-2, tested as (v >= 1 && v < n-1).  The struct holds the BASE node j-1 and delta.
+__device__ __forceinline__ bool tsc_axis(double q, double lo, double inv_d, double umax, int &base, double &delta) {
+    const double kMagic = 6755399441055744.0;  // 1.5 * 2^52, see cic_axis
+    const double u = __dmul_rn(__dsub_rn(q, lo), inv_d);
+    const double v = __dadd_rn(u, 0.5);
+    const bool in = (v >= 1.0) && (v < umax);
+    const double tt = __dadd_rd(v, kMagic);
+    base = in ? __double2loint(tt) - 1 : 0;
+    delta = __dsub_rn(u, __dsub_rn(tt, kMagic));
+    return in;
+}
+
+// Generic view used by the templated kernels: (i, j, k) = lowest node of the stencil, (wx1, wy1, wz1) = the per-axis
+// fraction the weights are built from (order 1: w1 of R11; order 2: delta of R16).
+template <int ORDER>
+__device__ __forceinline__ bool shape_locate(const GridDev &g, double x, double y, double t, double zscale, Cic &c) {
+    if (ORDER == 1) return cic_locate(g, x, y, t, zscale, c);
+    const double zeta = __dmul_rn(zscale, t);
+    const bool ix = tsc_axis(x, g.lo[0], g.inv_d[0], g.umax[0], c.i, c.wx1);
+    const bool iy = tsc_axis(y, g.lo[1], g.inv_d[1], g.umax[1], c.j, c.wy1);
+    const bool iz = tsc_axis(zeta, g.lo[2], g.inv_d[2], g.umax[2], c.k, c.wz1);
+    return ix && iy && iz;
+}
+
+template <int ORDER>
+__device__ __forceinline__ void axis_weights(double f, double (&w)[ORDER + 1]) {
+    if (ORDER == 1) {
+        w[0] = __dsub_rn(1.0, f);
+        w[1] = f;
+    } else {
+        const double a = __dsub_rn(0.5, f), b = __dadd_rn(0.5, f);
+        w[0] = __dmul_rn(0.5, __dmul_rn(a, a));
+        w[1] = __dsub_rn(0.75, __dmul_rn(f, f));
+        w[ORDER] = __dmul_rn(0.5, __dmul_rn(b, b));
+    }
+}
+
+// q_weight * ((wx*wy)*wz) for the (ORDER+1)^3 nodes of the stencil, dz outermost, dx innermost
+template <int ORDER>
+__device__ __forceinline__ void node_weights(const Cic &c, double qw, double (&w)[(ORDER + 1) * (ORDER + 1) * (ORDER + 1)]) {
+    constexpr int NW = ORDER + 1;
+    double wx[NW], wy[NW], wz[NW];
+    axis_weights<ORDER>(c.wx1, wx);
+    axis_weights<ORDER>(c.wy1, wy);
+    axis_weights<ORDER>(c.wz1, wz);
+#pragma unroll
+    for (int dy = 0; dy < NW; ++dy)
+#pragma unroll
+        for (int dx = 0; dx < NW; ++dx) {
+            const double wxy = __dmul_rn(wx[dx], wy[dy]);
+#pragma unroll
+            for (int dz = 0; dz < NW; ++dz) w[(dz * NW + dy) * NW + dx] = __dmul_rn(qw, __dmul_rn(wxy, wz[dz]));
+        }
+}
 
 }  // namespace bt
