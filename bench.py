@@ -252,7 +252,7 @@ def bench_spacecharge(bt, torch, flush, peaks):
     gather+kick+drift 96 B/particle + 24 B/node."""
     hbm = float(peaks["hbm_gbs"])
     out = {}
-    for variant in ("A", "B"):
+    for variant, order in (("A", 1), ("B", 1), ("A", 2)):
         sc = W.spacecharge_config(variant)
         c = W.make_spacecharge_bunch(sc)
         E = W.gaussian_bunch_field(sc)
@@ -260,6 +260,7 @@ def bench_spacecharge(bt, torch, flush, peaks):
         dep_bytes, gat_bytes = 24.0 * n + 16.0 * nn, 96.0 * n + 24.0 * nn
         beam, grid = bt.Beam(n), bt.Grid(sc.shape, sc.lo, sc.d)
         beam.set_ref(sc.kin_energy_MeV, sc.mass_MeV, sc.charge_qe)
+        grid.set_particle_shape(order)                             # 1 = CIC (configs[4]); 2 = the listing's shape (S:8f NEXT-2)
         grid.set_field(*E)
         beam.lattice_set([("drift", sc.ds / 2, 1)])
         beam.upload(c)
@@ -282,8 +283,9 @@ def bench_spacecharge(bt, torch, flush, peaks):
             after = sc.ds if step < sc.nsteps - 1 else sc.ds / 2
             t_gat += _event_ms(torch, lambda: beam.gather_kick(grid, sc.kick_coef, sc.zscale, 0.0, after), 1, flush)
         md, mg = statistics.mean(t_dep) * 1e-3, statistics.mean(t_gat) * 1e-3
-        out[variant] = {
-            "workload": "configs[4] %s, %d particles, %dx%dx%d nodes, %d steps" % ((sc.name, n) + tuple(sc.shape) + (sc.nsteps,)),
+        out[variant if order == 1 else variant + "_order2"] = {
+            "workload": "configs[4] %s, %d particles, %dx%dx%d nodes, %d steps, particle shape order %d" % (
+                (sc.name, n) + tuple(sc.shape) + (sc.nsteps, order)),
             "sort_by_cell_ms_once": t_sort,
             "deposit": {"ms": md * 1e3, "ms_first_last": [t_dep[0], t_dep[-1]], "unsorted_ms": t_dep_u,
                         "roofline": {"bound": "hbm", "achieved": dep_bytes / md / 1e9, "peak": hbm, "unit": "GB/s",

@@ -398,25 +398,31 @@ __device__ __forceinline__ void gather_kick_one(const GatherArgs &a, double &x, 
     t = fma(a.tcb, pt, t);
     Cic c;
     if (shape_locate<ORDER>(a.g, x, y, t, a.zscale, c)) {
+        const double *base = a.field + 4 * (((long long)c.k * a.g.ny + c.j) * a.g.nx + c.i);
         double wx[NW], wy[NW], wz[NW];
         axis_weights<ORDER>(c.wx1, wx);
         axis_weights<ORDER>(c.wy1, wy);
         axis_weights<ORDER>(c.wz1, wz);
-        const double *base = a.field + 4 * (((long long)c.k * a.g.ny + c.j) * a.g.nx + c.i);
         double ex = 0.0, ey = 0.0, ez = 0.0;
+        // one z-plane of the stencil at a time (loads of a plane are independent of its FMAs); summation order dz, dy, dx
 #pragma unroll
-        for (int dz = 0; dz < NW; ++dz)
+        for (int dz = 0; dz < NW; ++dz) {
+            double fx[NW * NW], fy[NW * NW], fz[NW * NW];
+#pragma unroll
+            for (int dy = 0; dy < NW; ++dy)
+#pragma unroll
+                for (int dx = 0; dx < NW; ++dx)
+                    ld_node(base + 4 * (((long long)dz * a.g.ny + dy) * a.g.nx + dx), fx[dy * NW + dx], fy[dy * NW + dx], fz[dy * NW + dx]);
 #pragma unroll
             for (int dy = 0; dy < NW; ++dy)
 #pragma unroll
                 for (int dx = 0; dx < NW; ++dx) {
                     const double w = __dmul_rn(__dmul_rn(wx[dx], wy[dy]), wz[dz]);
-                    double fx, fy, fz;
-                    ld_node(base + 4 * (((long long)dz * a.g.ny + dy) * a.g.nx + dx), fx, fy, fz);
-                    ex = fma(w, fx, ex);
-                    ey = fma(w, fy, ey);
-                    ez = fma(w, fz, ez);
+                    ex = fma(w, fx[dy * NW + dx], ex);
+                    ey = fma(w, fy[dy * NW + dx], ey);
+                    ez = fma(w, fz[dy * NW + dx], ez);
                 }
+        }
         px = fma(a.coef[0], ex, px);
         py = fma(a.coef[1], ey, py);
         pt = fma(a.coef[2], ez, pt);
