@@ -16,7 +16,7 @@ stream); L2 is flushed (256 MiB write) between timed steps, outside the event in
 bracketed by barrier + torch.cuda.synchronize(); ms_per_step = sum of event intervals / K, max over ranks.
 
 The same JSON line carries: roofline (FP64-pipe issue slots), cpu_baseline (the oracle as
-it stands on a bounded sample, host cores), e2e (host pinned buffers -> bt_beam_upload -> bt_track ->
+it stands on a bounded sample, host cores), e2e (host pinned buffers -> bt_track_host = chunked upload -> bt_track ->
 bt_beam_download inside the timed region), gpu_launches, clocks.
 """
 import argparse
@@ -369,14 +369,13 @@ def run_ours(args):
     ms_sum = sum(step_ms)
 
     # ---- end to end through the C-ABI with host buffers -----------------------------------------
+    # bt_track_host = upload + walk + download with the bunch cut into chunks on three streams (copies overlap the walk)
     for _ in range(2):
-        beam.upload(pinned), beam.track(cfg.nturns), beam.download(pinned_out)
+        beam.track_host(pinned, pinned_out, cfg.nturns, args.e2e_chunks)
     barrier()
     t0 = time.perf_counter()
     for k in range(args.steps):
-        beam.upload(pinned)                  # bt_beam_upload: 6 x H2D from pinned host memory
-        beam.track(cfg.nturns)
-        beam.download(pinned_out)            # bt_beam_download: 6 x D2H, synchronises
+        beam.track_host(pinned, pinned_out, cfg.nturns, args.e2e_chunks)     # synchronous: returns when pinned_out is complete
     barrier()
     t_e2e = time.perf_counter() - t0
     clocks = sampler.stop() if rank == 0 else None
@@ -440,7 +439,9 @@ def run_ours(args):
                        "l2": "flushed between timed steps (256 MiB write)", "parallelism": "particles sharded, %d rank(s), no collective" % world},
             "roofline": roof, "cpu_baseline": cpu_baseline,
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": 48 * n, "d2h_bytes_per_step": 48 * n,
-                    "ms_per_step": t_e2e / args.steps * 1e3},
+                    "ms_per_step": t_e2e / args.steps * 1e3,
+                    "call": "bt_track_host(pinned in, pinned out, nturns, nchunks=%d): H2D / walk / D2H of the chunks overlap "
+                            "on three streams" % args.e2e_chunks},
             "gpu_launches": int(launches), "clocks": clocks,
             "step_ms_min_median_max": [min(step_ms), statistics.median(step_ms), max(step_ms)],
             "wall_s_timed_region": t_wall,
@@ -463,6 +464,7 @@ def main():
     ap.add_argument("--workload", default="fodo_channel", choices=["tiny_fodo", "fodo_channel", "chicane", "nonlinear_ring"])
     ap.add_argument("--ref-sample", type=int, default=0,
                     help="particles per step the oracle is timed on in --impl reference (0 = sized for ~60 s in total)")
+    ap.add_argument("--e2e-chunks", type=int, default=8, help="chunks of the bunch in bt_track_host (e2e leg)")
     ap.add_argument("--no-extras", action="store_true",
                     help="skip the other configs and the space-charge kernels (N=1 only; the headline is unchanged)")
     args = ap.parse_args()

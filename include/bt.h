@@ -153,6 +153,19 @@ int bt_lattice_set(bt_beam *beam, const bt_element *elems, int32_t n_elems);
  */
 int bt_track(bt_beam *beam, int32_t nturns);
 
+/*
+ * The same walk with HOST buffers on both sides: upload, bt_track(nturns), download -- what a caller whose bunch
+ * lives in host memory does per call (sim.evolve() on a host-resident container, P:l.95).  The bunch is cut into
+ * `nchunks` contiguous chunks that ride three internal streams, so the host->device copy of chunk k+1, the walk of
+ * chunk k and the device->host copy of chunk k-1 overlap; particles never interact in the walk (S:8e), so the result
+ * is bit-identical to bt_beam_upload + bt_track + bt_beam_download for any nchunks.  host_in / host_out: 6 host arrays
+ * of n doubles each (order x, px, y, py, t, pt; pinned memory for the copies to be asynchronous; host_out may alias
+ * host_in).  Synchronous: returns when host_out is complete.  The beam's device arrays hold the result too; storage
+ * order is reset as by bt_beam_upload.  nchunks in [1, 256]; lattices whose RF changes the reference energy, or with
+ * more records than one table holds, are processed as one chunk.
+ */
+int bt_track_host(bt_beam *beam, const double *const host_in[6], double *const host_out[6], int32_t nturns, int32_t nchunks);
+
 /* ---- grid, CIC deposit (S4, S5) and gather + kick (S6, S7) ---------------------------------- */
 
 /*

@@ -47,6 +47,7 @@ EXPORTS = {
     "bt_beam_ids": (C.c_int, [_vp, C.POINTER(_vp)]),
     "bt_lattice_set": (C.c_int, [_vp, _vp, C.c_int32]),
     "bt_track": (C.c_int, [_vp, C.c_int32]),
+    "bt_track_host": (C.c_int, [_vp, C.POINTER(_vp), C.POINTER(_vp), C.c_int32, C.c_int32]),
     "bt_grid_create": (C.c_int, [C.POINTER(_vp), C.c_int32, C.c_int32, C.c_int32, _dp, _dp]),
     "bt_grid_destroy": (None, [_vp]),
     "bt_grid_set_field": (C.c_int, [_vp, _vp, _vp, _vp, C.c_int]),
@@ -183,6 +184,13 @@ class Beam:
 
     def upload(self, host_arrays):
         _check(lib.bt_beam_upload(self._h, _host_ptrs(host_arrays)), "bt_beam_upload")
+
+    def track_host(self, host_in, host_out=None, nturns=1, nchunks=8):
+        """bt_track_host: host arrays in, host arrays out (in place when host_out is None), copies overlapped with the walk."""
+        if host_out is None:
+            host_out = host_in
+        _check(lib.bt_track_host(self._h, _host_ptrs(host_in), _host_ptrs(host_out), int(nturns), int(nchunks)), "bt_track_host")
+        return host_out
 
     def download(self, out=None):
         if out is None:

@@ -270,6 +270,10 @@ void bt_beam_destroy(bt_beam *beam) {
         if (p) cudaFree(p);
     if (b.scratch) cudaFree(b.scratch);
     if (b.mom_buf) cudaFree(b.mom_buf);
+    for (int i = 0; i < 3; ++i) {
+        if (b.pipe_stream[i]) cudaStreamDestroy(b.pipe_stream[i]);
+        if (b.pipe_event[i]) cudaEventDestroy(b.pipe_event[i]);
+    }
     delete beam;
 }
 
@@ -444,6 +448,70 @@ int bt_track(bt_beam *beam, int32_t nturns) {
         }
         b.gamma = gamma;
     }
+    b.s += b.lattice_length * (double)nturns;
+    b.turn += nturns;
+    return BT_OK;
+}
+
+// Host-to-host walk: chunks of the bunch ride three streams, so that the H2D copy of chunk k+1, the walk of chunk k and
+// the D2H copy of chunk k-1 overlap (PCIe is full duplex; particles are independent, so any partition is exact).
+int bt_track_host(bt_beam *beam, const double *const host_in[6], double *const host_out[6], int32_t nturns, int32_t nchunks) {
+    if (!beam || !host_in || !host_out) return fail(BT_ERR_INVALID, "bt_track_host: NULL argument");
+    for (int i = 0; i < 6; ++i)
+        if (!host_in[i] || !host_out[i]) return fail(BT_ERR_INVALID, "bt_track_host: host array list has a NULL entry");
+    if (nturns < 0) return fail(BT_ERR_INVALID, "bt_track_host: nturns < 0");
+    if (nchunks < 1 || nchunks > 256) return fail(BT_ERR_INVALID, "bt_track_host: nchunks must be in [1, 256]");
+    Beam &b = beam->b;
+    if (b.lattice.empty()) return fail(BT_ERR_STATE, "bt_track_host: bt_lattice_set not called");
+    if (!b.has_ref) return fail(BT_ERR_STATE, "bt_track_host: bt_beam_set_ref not called");
+    const size_t K = (size_t)kConstTableRecords;
+    if (!b.energy_changes && !b.table_valid) {
+        b.h_table.clear();
+        build_turn_table(b.lattice, b.gamma, b.h_table, &b.table_slots);
+        b.table_version = next_table_version();
+        b.table_valid = true;
+    }
+    // Lattices that need several tables per call (RF changing the reference energy, more records than the constant
+    // bank holds) replace the table between launches; their chunks cannot share it across streams: one chunk.
+    if (nturns == 0 || nchunks == 1 || b.energy_changes || b.h_table.size() > K) {
+        int rc = bt_beam_upload(beam, host_in);
+        if (rc == BT_OK) rc = bt_track(beam, nturns);
+        if (rc == BT_OK) rc = bt_beam_download(beam, host_out);
+        return rc;
+    }
+    for (int i = 0; i < 3; ++i) {
+        if (!b.pipe_stream[i]) BT_CUDA_TRY(cudaStreamCreateWithFlags(&b.pipe_stream[i], cudaStreamNonBlocking));
+        if (!b.pipe_event[i]) BT_CUDA_TRY(cudaEventCreateWithFlags(&b.pipe_event[i], cudaEventDisableTiming));
+    }
+    // the chunk streams start after everything already queued on the beam's stream
+    BT_CUDA_TRY(cudaEventRecord(b.pipe_event[0], b.stream));
+    for (int i = 0; i < 3; ++i) BT_CUDA_TRY(cudaStreamWaitEvent(b.pipe_stream[i], b.pipe_event[0], 0));
+    const long long gran = 1024;  // keeps every chunk's arrays as aligned as the whole arrays
+    long long len = ((b.n + nchunks - 1) / nchunks + gran - 1) / gran * gran;
+    const double spr = b.table_slots / (double)b.h_table.size();
+    int k = 0;
+    for (long long off = 0; off < b.n; off += len, ++k) {
+        const long long m = b.n - off < len ? b.n - off : len;
+        cudaStream_t st = b.pipe_stream[k % 3];
+        for (int i = 0; i < 6; ++i)
+            BT_CUDA_TRY(cudaMemcpyAsync(b.q[i] + off, host_in[i] + off, (size_t)m * sizeof(double), cudaMemcpyHostToDevice, st));
+        TrackRange r;
+        r.off = off, r.n = m, r.geom_n = b.n, r.stream = st;
+        b.range = &r;
+        const int rc = launch_track(&b, b.h_table.data(), (int32_t)b.h_table.size(), nturns, b.table_version, spr);
+        b.range = nullptr;
+        if (rc != BT_OK) return rc;
+        for (int i = 0; i < 6; ++i)
+            BT_CUDA_TRY(cudaMemcpyAsync(host_out[i] + off, b.q[i] + off, (size_t)m * sizeof(double), cudaMemcpyDeviceToHost, st));
+    }
+    for (int i = 0; i < 3; ++i) {
+        BT_CUDA_TRY(cudaEventRecord(b.pipe_event[i], b.pipe_stream[i]));
+        BT_CUDA_TRY(cudaStreamWaitEvent(b.stream, b.pipe_event[i], 0));
+    }
+    int rc = record_table_busy(&b, b.stream);
+    if (rc != BT_OK) return rc;
+    BT_CUDA_TRY(cudaStreamSynchronize(b.stream));
+    b.permuted = false;  // storage order = the caller's order
     b.s += b.lattice_length * (double)nturns;
     b.turn += nturns;
     return BT_OK;

@@ -61,6 +61,13 @@ struct TrackLaunchInfo {
     int64_t launches = 0;  // fused-walk kernels launched by this beam so far
 };
 
+// A sub-range of the beam walked on its own stream (bt_track_host): launch_track then works on [off, off + n) of the
+// arrays; the launch geometry is chosen for geom_n particles (the whole bunch), not for the chunk.
+struct TrackRange {
+    long long off = 0, n = 0, geom_n = 0;
+    cudaStream_t stream = nullptr;
+};
+
 struct Beam {
     int64_t n = 0;
     double *q[6] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
@@ -90,6 +97,9 @@ struct Beam {
     int *sort_key = nullptr, *sort_dest = nullptr, *sort_count = nullptr, *sort_block_sum = nullptr;
     long long sort_count_cap = 0;
     double *scratch = nullptr;  // one array of n doubles
+    const TrackRange *range = nullptr;  // non-NULL only inside bt_track_host
+    cudaStream_t pipe_stream[3] = {nullptr, nullptr, nullptr};  // bt_track_host: chunk streams, created on first use
+    cudaEvent_t pipe_event[3] = {nullptr, nullptr, nullptr};
     double *mom_buf = nullptr;  // beam statistics: out[42], pad, per-block partials, ticket (moments.cu)
 };
 
@@ -116,6 +126,7 @@ double build_turn_table(const std::vector<bt_element> &lat, double gamma, std::v
 int launch_track(Beam *b, const DevOp *h_table, int32_t n_ops, int32_t nturns, uint64_t version, double slots_per_record);
 uint64_t next_table_version();
 void forget_table_owner(const Beam *b);
+int record_table_busy(const Beam *b, cudaStream_t stream);  // marks `stream` as the table's last reader
 int launch_deposit(Beam *b, Grid *g, double q_weight, double zscale);
 int launch_gather_kick(Beam *b, const Grid *g, const double coef[3], double zscale, double h_before,
                        double tc_before, double h_after, double tc_after);

@@ -290,7 +290,8 @@ static int env_int(const char *name, int dflt) {
 // table is still the resident one.
 struct ConstTableState {
     std::mutex mu;
-    cudaEvent_t busy = nullptr;
+    cudaEvent_t busy = nullptr;      // recorded after the last launch that reads the table
+    cudaEvent_t uploaded = nullptr;  // recorded after the table was placed (other streams of the same beam wait on it)
     const void *owner = nullptr;
     uint64_t version = 0;
 };
@@ -309,17 +310,20 @@ int launch_track(Beam *b, const DevOp *h_table, int32_t n_ops, int32_t nturns, u
     // (per-record work negligible) P is lowered until every sub-partition gets >= 24 tasks.  Measured on B200:
     // config 1 (10^6 particles, 92 slots/record) 0.913 of the FP64 roofline at P = 4, 0.945 at P = 2; config 3
     // (12 slots/record) 0.83 at P = 4, 0.76 at P = 2.  Small blocks keep the tasks balanced over SMs.
-    const long long n = b->n;
+    const long long n = b->range ? b->range->n : b->n;
+    const long long off = b->range ? b->range->off : 0;
+    const long long geom_n = b->range ? b->range->geom_n : b->n;  // chunks of one bunch run concurrently on several streams
+    cudaStream_t stream = b->range ? b->range->stream : b->stream;
     const int sms = b->num_sms > 0 ? b->num_sms : 148;
     const long long sched = (long long)sms * 4;
-    auto tasks = [&](int p) { return n / (32LL * p) / sched; };  // tasks per sub-partition
+    auto tasks = [&](int p) { return geom_n / (32LL * p) / sched; };  // tasks per sub-partition
     int P = 1;
     if (b->aligned16) {
         if (slots_per_record < 40.0) P = tasks(4) >= 4 ? 4 : tasks(2) >= 4 ? 2 : 1;
         else P = tasks(4) >= 24 ? 4 : tasks(2) >= 12 ? 2 : 1;
     }
     int block = 64;
-    while (block > 32 && n / ((long long)P * block) < 2LL * sms) block >>= 1;
+    while (block > 32 && geom_n / ((long long)P * block) < 2LL * sms) block >>= 1;
     P = env_int("BT_TRACK_PPT", P);
     block = env_int("BT_TRACK_BLOCK", block);
     if (!(P == 1 || ((P == 2 || P == 4 || P == 8) && b->aligned16)))
@@ -327,7 +331,7 @@ int launch_track(Beam *b, const DevOp *h_table, int32_t n_ops, int32_t nturns, u
     if (block < 32 || block > kMaxBlock || (block & 31)) return fail(BT_ERR_INVALID, "BT_TRACK_BLOCK must be a multiple of 32 in [32,128]");
 
     TrackArgs a;
-    for (int c = 0; c < 6; ++c) a.q[c] = b->q[c];
+    for (int c = 0; c < 6; ++c) a.q[c] = b->q[c] + off;
     a.n = n;
     a.n_ops = n_ops;
     a.nturns = nturns;
@@ -343,22 +347,26 @@ int launch_track(Beam *b, const DevOp *h_table, int32_t n_ops, int32_t nturns, u
     ConstTableState &ct = g_ct[b->device];
     std::lock_guard<std::mutex> lock(ct.mu);
     if (!ct.busy) BT_CUDA_TRY(cudaEventCreateWithFlags(&ct.busy, cudaEventDisableTiming));
+    if (!ct.uploaded) BT_CUDA_TRY(cudaEventCreateWithFlags(&ct.uploaded, cudaEventDisableTiming));
     if (ct.owner != (const void *)b || ct.version != version) {
-        BT_CUDA_TRY(cudaStreamWaitEvent(b->stream, ct.busy, 0));  // previous readers of the table (any stream)
+        BT_CUDA_TRY(cudaStreamWaitEvent(stream, ct.busy, 0));  // previous readers of the table (any stream)
         // pageable source: the call returns after the source has been staged
-        BT_CUDA_TRY(cudaMemcpyToSymbolAsync(c_table, h_table, (size_t)n_ops * sizeof(DevOp), 0, cudaMemcpyHostToDevice, b->stream));
+        BT_CUDA_TRY(cudaMemcpyToSymbolAsync(c_table, h_table, (size_t)n_ops * sizeof(DevOp), 0, cudaMemcpyHostToDevice, stream));
+        BT_CUDA_TRY(cudaEventRecord(ct.uploaded, stream));
         ct.owner = (const void *)b;
         ct.version = version;
+    } else if (b->range) {
+        BT_CUDA_TRY(cudaStreamWaitEvent(stream, ct.uploaded, 0));  // the table was placed by another chunk's stream
     }
     switch (P) {
-        case 8: track_kernel<8><<<grid, block, 0, b->stream>>>(a); break;
-        case 4: track_kernel<4><<<grid, block, 0, b->stream>>>(a); break;
-        case 2: track_kernel<2><<<grid, block, 0, b->stream>>>(a); break;
-        default: track_kernel<1><<<grid, block, 0, b->stream>>>(a); break;
+        case 8: track_kernel<8><<<grid, block, 0, stream>>>(a); break;
+        case 4: track_kernel<4><<<grid, block, 0, stream>>>(a); break;
+        case 2: track_kernel<2><<<grid, block, 0, stream>>>(a); break;
+        default: track_kernel<1><<<grid, block, 0, stream>>>(a); break;
     }
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return fail(BT_ERR_CUDA, std::string("bt_track launch: ") + cudaGetErrorString(e));
-    BT_CUDA_TRY(cudaEventRecord(ct.busy, b->stream));
+    if (!b->range) BT_CUDA_TRY(cudaEventRecord(ct.busy, stream));  // bt_track_host records it once, after joining its streams
     g_launch_count.fetch_add(1);
     b->last_launch.grid = grid;
     b->last_launch.block = block;
@@ -369,6 +377,14 @@ int launch_track(Beam *b, const DevOp *h_table, int32_t n_ops, int32_t nturns, u
 }
 
 // A destroyed beam must not be mistaken for a later one allocated at the same address.
+int record_table_busy(const Beam *b, cudaStream_t stream) {
+    if (b->device < 0 || b->device >= kMaxDevices) return BT_OK;
+    ConstTableState &ct = g_ct[b->device];
+    std::lock_guard<std::mutex> lock(ct.mu);
+    if (ct.busy) BT_CUDA_TRY(cudaEventRecord(ct.busy, stream));
+    return BT_OK;
+}
+
 void forget_table_owner(const Beam *b) {
     if (b->device < 0 || b->device >= kMaxDevices) return;
     ConstTableState &ct = g_ct[b->device];

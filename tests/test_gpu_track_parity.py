@@ -250,3 +250,48 @@ def test_config3_full_size_sampled():
     bg0 = 1.807618289845165
     ex = rms_emittance(got[0], got[1]) * bg / bg0
     assert 0.9e-6 < ex < 1.5e-6
+
+
+@pytest.mark.parametrize("nchunks", [1, 3, 8, 64])
+def test_track_host_pipelined_is_bit_identical(nchunks):
+    """bt_track_host (chunks on three streams, copies overlapped) == upload + bt_track + download, bit for bit, and
+    within R14 of the oracle; ragged chunking (n not a multiple of anything), in-place host buffers."""
+    import torch
+    import paper_2208_02382_b200 as bt
+    cfg = W.config(1, n=70_001)
+    lat = cfg.lattice[:10]
+    c = W.make_bunch(cfg)
+    beam = bt.Beam(cfg.n)
+    beam.set_ref(cfg.kin_energy_MeV, cfg.mass_MeV, cfg.charge_qe)
+    beam.lattice_set(lat)
+    beam.upload(c)
+    beam.track(2)
+    plain = beam.download()
+    pinned = [torch.from_numpy(a.copy()).pin_memory() for a in c]
+    beam.track_host(pinned, None, nturns=2, nchunks=nchunks)           # in place
+    got = [t.numpy() for t in pinned]
+    for a, b in zip(got, plain):
+        assert np.array_equal(a, b)
+    dev = beam.download()                                               # the device copy holds the result too
+    for a, b in zip(dev, plain):
+        assert np.array_equal(a, b)
+    ref, _ = oracle_track(cfg, c, nturns=2, lattice=lat)
+    assert max(r14_error(got, ref)) <= 1e-11
+    g, s, turn = beam.get_ref()
+    assert turn == 4
+    beam.close()
+
+
+def test_track_host_with_rf_lattice_falls_back_to_one_chunk():
+    import paper_2208_02382_b200 as bt
+    cfg = W.config(3, n=20_003)
+    c = W.make_bunch(cfg)
+    beam = bt.Beam(cfg.n)
+    beam.set_ref(cfg.kin_energy_MeV, cfg.mass_MeV, cfg.charge_qe)
+    beam.lattice_set(cfg.lattice)
+    out = [np.empty_like(a) for a in c]
+    beam.track_host(c, out, nturns=2, nchunks=8)
+    ref, _ = oracle_track(cfg, c, nturns=2)
+    assert max(r14_error(out, ref)) <= 1e-11
+    assert bt.lib.bt_track_host(beam._h, None, None, 1, 8) == bt.BT_ERR_INVALID
+    beam.close()
