@@ -121,9 +121,10 @@ int64_t bt_beam_size(const bt_beam *beam);
  * Cell binning (S4; B:north_star "bins particles by cell").  Physically reorders the beam's six arrays by
  * the linear index (k*ny + j)*nx + i of each particle's lower-corner node on `grid` (R11 canonical index,
  * third axis zscale*t; particles outside the grid go last), by a counting sort on the beam's stream.
- * Opt-in and purely a performance hint: bt_deposit_cic then accumulates runs of same-cell particles in
- * registers before touching rho, and bt_gather_kick finds its nodes in L1; both remain correct for any order,
- * so the sort may be repeated at any cadence (particles move a small fraction of a cell per step).
+ * Opt-in and purely a performance hint: it makes every chunk of consecutive particles spatially compact, which is
+ * what bt_deposit_cic needs to bin a chunk by cell in shared memory and sum same-cell particles in registers before
+ * touching rho, and what lets bt_gather_kick find its nodes in L1; both remain correct for any order and stay fast
+ * while particles wander a few cells from where the sort left them, so one sort serves many steps.
  * bt_beam_download still returns the original order; bt_beam_upload resets storage to the caller's order.
  * The order of particles within one cell is not deterministic.  Needs n < 2^31; allocates 24 bytes per
  * particle of scratch on first use.
