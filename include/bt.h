@@ -59,7 +59,12 @@ typedef enum {
     BT_SBEND = 2,     /* R6 sector bend, no field index */
     BT_DIPEDGE = 3,   /* R7 thin pole-face rotation with fringe correction */
     BT_MULTIPOLE = 4, /* R8 thin multipole kick */
-    BT_SHORTRF = 5    /* R9 short RF cavity, linearised, energy kick only, updates the reference energy */
+    BT_SHORTRF = 5,   /* R9 short RF cavity, linearised, energy kick only, updates the reference energy */
+    /* non-linearised maps (P:l.168 "non-linear elements, RF-modeling"): */
+    BT_DRIFT_EXACT = 6, /* R17: ps = sqrt(1 - 2pt/beta0 + pt^2 - px^2 - py^2); x += h px/ps; y += h py/ps;
+                           t += h ((1/beta0 - pt)/ps - 1/beta0)  -- straight line with the exact time of flight */
+    BT_SHORTRF_SIN = 7  /* R18: R9 without the expansion in t: pt = r pt - (Vhat/(bg)_f)(cos(k_rf t + phi) - cos(phi)),
+                           px *= r, py *= r; same reference-energy update as R9 */
 } bt_element_type;
 
 /*
@@ -68,14 +73,15 @@ typedef enum {
  * elements.Quad(ds=1.0, k=1.0, nslice=ns) (P:l.88).
  *   type    bt_element_type
  *   nslice  >= 1; the element is applied as nslice maps of length ds/nslice (R3; P:l.47, l.87).
- *           Thin elements (DIPEDGE, MULTIPOLE, SHORTRF) must have nslice == 1.
+ *           Thin elements (DIPEDGE, MULTIPOLE, SHORTRF, SHORTRF_SIN) must have nslice == 1.
  *   ds      length [m], >= 0; ignored for the map of thin elements but still added to s.
  *   p[6]    QUAD:      p0 = k [m^-2]
  *           SBEND:     p0 = rc [m], signed bending radius, != 0
  *           DIPEDGE:   p0 = psi [rad], p1 = rc [m] (!= 0), p2 = g [m] full gap, p3 = K fringe integral
  *           MULTIPOLE: p0 = m (integer 1..10; 1 dipole, 2 quad, 3 sext, 4 oct), p1 = Kn, p2 = Ks
  *                      (integrated strengths [m^-(m-1)], MAD-X sign: Kn > 0 at m = 2 focuses x)
- *           SHORTRF:   p0 = Vhat = qV/(mc^2), p1 = frequency [Hz], p2 = phase [deg] (cosine convention)
+ *           SHORTRF, SHORTRF_SIN: p0 = Vhat = qV/(mc^2), p1 = frequency [Hz], p2 = phase [deg] (cosine convention)
+ *           DRIFT_EXACT: none
  *           unused entries are ignored.
  */
 typedef struct {

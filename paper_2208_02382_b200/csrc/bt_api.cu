@@ -32,6 +32,7 @@ static int validate_element(const bt_element &e, int idx) {
     if (!(e.ds >= 0.0) || !isfinite(e.ds)) return bad("ds < 0 or not finite");
     switch (e.type) {
         case BT_DRIFT:
+        case BT_DRIFT_EXACT:
             break;
         case BT_QUAD:
             if (!isfinite(e.p[0])) return bad("k not finite");
@@ -51,6 +52,7 @@ static int validate_element(const bt_element &e, int idx) {
             if (!isfinite(e.p[1]) || !isfinite(e.p[2])) return bad("Kn or Ks not finite");
             break;
         case BT_SHORTRF:
+        case BT_SHORTRF_SIN:
             if (e.nslice != 1) return bad("thin element needs nslice == 1");
             if (!isfinite(e.p[0]) || !isfinite(e.p[1]) || !isfinite(e.p[2])) return bad("RF parameter not finite");
             break;
@@ -193,6 +195,29 @@ double build_turn_table(const std::vector<bt_element> &lat, double gamma, std::v
                 o.c[1] = Vhat * krf * sin(phi) / bg_f;
                 gamma = gamma_f;  // S3: later elements see the new reference energy
                 nslots += 4.0;
+                out.push_back(o);
+                break;
+            }
+            case BT_DRIFT_EXACT:  // R17
+                o.op = OP_DRIFTX;
+                o.c[0] = h;
+                o.c[1] = 1.0 / beta;
+                nslots += 26.0 * e.nslice;  // 12 DFMA/DMUL/DADD + reciprocal square root (~14 FP64-pipe instructions)
+                out.push_back(o);
+                break;
+            case BT_SHORTRF_SIN: {  // R18
+                const double Vhat = e.p[0], freq = e.p[1], phi = e.p[2] * (kPi / 180.0);
+                const double cphi = cos(phi);
+                const double gamma_f = gamma + Vhat * cphi;
+                const double bg_f = sqrt(gamma_f * gamma_f - 1.0);
+                o.op = OP_RFSIN;
+                o.c[0] = bg / bg_f;
+                o.c[1] = -(Vhat / bg_f);
+                o.c[2] = 2.0 * kPi * freq / kCLight;
+                o.c[3] = phi;
+                o.c[4] = cphi;
+                gamma = gamma_f;
+                nslots += 40.0;  // fp64 cosine ~ 35 FP64-pipe instructions on the fast path
                 out.push_back(o);
                 break;
             }
@@ -365,7 +390,8 @@ int bt_lattice_set(bt_beam *beam, const bt_element *elems, int32_t n_elems) {
     for (int32_t i = 0; i < n_elems; ++i) {
         int rc = validate_element(elems[i], i);
         if (rc != BT_OK) return rc;
-        if (elems[i].type == BT_SHORTRF && elems[i].p[0] * cos(elems[i].p[2] * (kPi / 180.0)) != 0.0) energy_changes = true;
+        if ((elems[i].type == BT_SHORTRF || elems[i].type == BT_SHORTRF_SIN) && elems[i].p[0] * cos(elems[i].p[2] * (kPi / 180.0)) != 0.0)
+            energy_changes = true;
         length += elems[i].ds;
     }
     Beam &b = beam->b;

@@ -161,6 +161,27 @@ __device__ __forceinline__ void apply(Ptc<P> &p, const DevOp &r) {
             p.py[j] *= c0;
             p.pt[j] = fma(c0, p.pt[j], c1 * p.t[j]);
         }
+    } else if (op & OP_DRIFTX) {  // R17 exact drift: straight line with the exact time of flight; c0 = h, c1 = 1/beta0
+        const double c0 = r.c[0], c1 = r.c[1];
+        const int cnt = r.count;
+#pragma unroll 1
+        for (int s = 0; s < cnt; ++s) {
+            BT_FORP {
+                const double px = p.px[j], py = p.py[j], pt = p.pt[j];
+                const double a = fma(pt, pt, fma(-2.0 * pt, c1, 1.0)) - fma(px, px, py * py);
+                const double ips = 1.0 / sqrt(a);  // p0 / p_s
+                p.x[j] = fma(c0 * px, ips, p.x[j]);
+                p.y[j] = fma(c0 * py, ips, p.y[j]);
+                p.t[j] = fma(c0, fma(c1 - pt, ips, -c1), p.t[j]);
+            }
+        }
+    } else if (op & OP_RFSIN) {  // R18: the energy kick qV cos(k t + phi) without the expansion in t
+        const double c0 = r.c[0], c1 = r.c[1], c2 = r.c[2], c3 = r.c[3], c4 = r.c[4];
+        BT_FORP {
+            p.px[j] *= c0;
+            p.py[j] *= c0;
+            p.pt[j] = fma(c1, cos(fma(c2, p.t[j], c3)) - c4, c0 * p.pt[j]);
+        }
     } else if (op & OP_MULT) {  // R8 general order: repeated complex multiplication; count = m
         const double c0 = r.c[0], c1 = r.c[1];
         const int m = r.count;

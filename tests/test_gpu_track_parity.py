@@ -295,3 +295,56 @@ def test_track_host_with_rf_lattice_falls_back_to_one_chunk():
     assert max(r14_error(out, ref)) <= 1e-11
     assert bt.lib.bt_track_host(beam._h, None, None, 1, 8) == bt.BT_ERR_INVALID
     beam.close()
+
+
+def _nonlinear_ring():
+    """FODO cells with exact drifts, thin sextupoles and one sinusoidal RF cavity per turn (NEXT-3 elements)."""
+    cell = [("quad", 1.0, 5, 1.0), ("multipole", 0.0, 1, 3, 5.0, 0.0), ("drift_exact", 0.5, 3),
+            ("quad", 1.0, 5, -1.0), ("multipole", 0.0, 1, 3, -5.0, 0.0), ("drift_exact", 0.5, 1)]
+    return cell * 4 + [("shortrf_sin", 0.0, 1, 1.0 / 938.27208816, 3.4976811924685272e6 * 40, -30.0)]
+
+
+@pytest.mark.parametrize("n,nturns", [(1, 3), (10_007, 5), (300_001, 2)])
+def test_nonlinear_maps_match_oracle(n, nturns):
+    """R17 exact drift + R18 sinusoidal RF inside the fused walk (per-turn tables: the RF moves the reference energy)."""
+    cfg = W.config(3, n=n)
+    lat = _nonlinear_ring()
+    c = W.make_bunch(cfg)
+    c[4] *= 30.0                                     # spread t over a good fraction of the RF wavelength (2.1 m)
+    got, (g, s, turn), _ = gpu_track(cfg, c, nturns=nturns, lattice=lat)
+    ref, (g_ref, s_ref) = oracle_track(cfg, c, nturns=nturns, lattice=lat)
+    assert max(r14_error(got, ref)) <= 1e-11
+    assert abs(g - g_ref) <= 4e-16 * g_ref and abs(s - s_ref) <= 1e-12 and turn == nturns
+    # and they are different maps from their linearised versions (R4, R9) on this bunch
+    lin = [("drift",) + e[1:] if e[0] == "drift_exact" else ("shortrf",) + e[1:] if e[0] == "shortrf_sin" else e for e in lat]
+    ref_lin, _ = oracle_track(cfg, c, nturns=nturns, lattice=lin)
+    if n > 1:
+        assert max(r14_error(ref_lin, ref)) > 1e-6
+
+
+def test_exact_drift_only_lattice_static_table_and_host_pipeline():
+    import torch
+    import paper_2208_02382_b200 as bt
+    cfg = W.config(0, n=50_001)
+    lat = [("drift_exact", 0.25, 1), ("quad", 1.0, 10, 1.0), ("drift_exact", 0.5, 4), ("quad", 1.0, 10, -1.0), ("drift_exact", 0.25, 1)]
+    c = W.make_bunch(cfg)
+    got, _, _ = gpu_track(cfg, c, nturns=4, lattice=lat)
+    ref, _ = oracle_track(cfg, c, nturns=4, lattice=lat)
+    assert max(r14_error(got, ref)) <= 1e-11
+    beam = bt.Beam(cfg.n)
+    beam.set_ref(cfg.kin_energy_MeV, cfg.mass_MeV, cfg.charge_qe)
+    beam.lattice_set(lat)
+    out = beam.track_host(c, [np.empty_like(a) for a in c], nturns=4, nchunks=5)
+    for a, b in zip(out, got):
+        assert np.array_equal(a, b)
+    beam.close()
+
+
+def test_nonlinear_element_validation():
+    import paper_2208_02382_b200 as bt
+    beam = bt.Beam(8)
+    with pytest.raises(bt.BtError):
+        beam.lattice_set([("shortrf_sin", 0.0, 2, 1e-3, 1e8, 0.0)])
+    with pytest.raises(bt.BtError):
+        beam.lattice_set([("drift_exact", -1.0, 1)])
+    beam.close()
