@@ -44,6 +44,12 @@ def lib():
         L.orc_deposit_tsc.restype = C.c_int64
         L.orc_gather_kick_tsc.argtypes = L.orc_gather_kick.argtypes
         L.orc_gather_kick_tsc.restype = C.c_int64
+        L.orc_green_self.argtypes = [C.c_double] * 3
+        L.orc_green_self.restype = C.c_double
+        L.orc_poisson.argtypes = [C.c_int32] * 3 + [_dp, C.c_double, _dp, _dp]
+        L.orc_poisson.restype = C.c_int
+        L.orc_efield.argtypes = [C.c_int32] * 3 + [_dp, C.c_double, _dp, _dp, _dp, _dp]
+        L.orc_efield.restype = C.c_int
         L.orc_moments.argtypes = [C.c_int64, C.POINTER(_dp), _dp, _dp]
         L.orc_moments.restype = C.c_int
         _lib = L
@@ -164,3 +170,31 @@ def rms_emittances(cov):
     """Unnormalised rms emittances of the three planes from the 6x6 second moments:
     eps = sqrt(<q q><p p> - <q p>^2) for (x,px), (y,py), (t,pt)."""
     return tuple(float(np.sqrt(cov[a, a] * cov[a + 1, a + 1] - cov[a, a + 1] ** 2)) for a in (0, 2, 4))
+
+
+EPS0 = 8.8541878128e-12
+
+
+def green_self(dx, dy, dz):
+    """(1/V) * integral of 1/r over one cell dx*dy*dz centred on the origin (R19 self term)."""
+    return float(lib().orc_green_self(dx, dy, dz))
+
+
+def poisson(rho, d, gz=1.0):
+    """R19: free-space potential [V] at the nodes from rho[nz,ny,nx] (charge per node [C]); third axis spacing gz*d[2]."""
+    nz, ny, nx = rho.shape
+    rho = np.ascontiguousarray(rho, dtype=np.float64)
+    phi = np.zeros_like(rho)
+    if lib().orc_poisson(nx, ny, nz, _p(_v3(d)), gz, _p(rho.reshape(-1)), _p(phi.reshape(-1))) != 0:
+        raise ValueError("oracle: invalid grid")
+    return phi
+
+
+def efield(phi, d, gz=1.0):
+    """E = -grad phi (rest frame): centred differences inside, one-sided at the faces.  Returns (Ex, Ey, Ez)."""
+    nz, ny, nx = phi.shape
+    phi = np.ascontiguousarray(phi, dtype=np.float64)
+    E = [np.zeros_like(phi) for _ in range(3)]
+    if lib().orc_efield(nx, ny, nz, _p(_v3(d)), gz, _p(phi.reshape(-1)), *[_p(e.reshape(-1)) for e in E]) != 0:
+        raise ValueError("oracle: invalid grid")
+    return E
