@@ -196,6 +196,22 @@ int bt_grid_set_field(bt_grid *grid, const double *Ex, const double *Ey, const d
  */
 int bt_grid_set_particle_shape(bt_grid *grid, int32_t order);
 int bt_grid_rho(bt_grid *grid, double **dev_rho_out);    /* zero-copy device view of rho */
+
+/*
+ * Space-charge field from the deposited charge (P:l.49 "the Poisson equation is solved in the bunch
+ * rest frame"), reading R19: open boundaries, rho = charge per node [C],
+ *   phi_a = (1/(4 pi eps0)) sum_b q_b G(r_a - r_b),  G(r) = 1/|r| for a != b,  G(0) = (1/V) int_cell 1/|r| dV,
+ * with the third-axis spacing stretched to gz*dz (gz = gamma0 turns zeta = beta0 c dt into the rest-frame length), then
+ *   E = -grad phi  (rest frame; centred differences, one-sided first-order at the faces; third axis with gz*dz).
+ * The sum is evaluated as a zero-padded FFT convolution (Hockney) on `cuda_stream` (cudaStream_t, may be 0): rho -> phi [V]
+ * -> the grid's field (replacing any field given to bt_grid_set_field), ready for bt_gather_kick, whose coef[] carries the
+ * rest-frame -> kick factors.  Allocates ~35 x nx*ny*nz x 8 bytes on first use; the transformed Green table is cached per gz.
+ * Asynchronous.  Grids up to 2^28 nodes.
+ */
+int bt_grid_solve_poisson(bt_grid *grid, double gz, void *cuda_stream);
+int bt_grid_download_phi(bt_grid *grid, double *host_phi);   /* nx*ny*nz doubles, x fastest; synchronises */
+/* The grid's current field (from bt_grid_set_field or bt_grid_solve_poisson), 3 host arrays of nx*ny*nz doubles; synchronises. */
+int bt_grid_download_field(bt_grid *grid, double *host_Ex, double *host_Ey, double *host_Ez);
 int bt_grid_download_rho(bt_grid *grid, double *host_rho); /* synchronises the last beam stream used */
 
 /*

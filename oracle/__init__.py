@@ -48,6 +48,8 @@ def lib():
         L.orc_green_self.restype = C.c_double
         L.orc_poisson.argtypes = [C.c_int32] * 3 + [_dp, C.c_double, _dp, _dp]
         L.orc_poisson.restype = C.c_int
+        L.orc_poisson_sample.argtypes = [C.c_int32] * 3 + [_dp, C.c_double, _dp, C.c_int64, C.POINTER(C.c_int64), _dp]
+        L.orc_poisson_sample.restype = C.c_int
         L.orc_efield.argtypes = [C.c_int32] * 3 + [_dp, C.c_double, _dp, _dp, _dp, _dp]
         L.orc_efield.restype = C.c_int
         L.orc_moments.argtypes = [C.c_int64, C.POINTER(_dp), _dp, _dp]
@@ -198,3 +200,15 @@ def efield(phi, d, gz=1.0):
     if lib().orc_efield(nx, ny, nz, _p(_v3(d)), gz, _p(phi.reshape(-1)), *[_p(e.reshape(-1)) for e in E]) != 0:
         raise ValueError("oracle: invalid grid")
     return E
+
+
+def poisson_sample(rho, d, gz, targets):
+    """R19 potential at the listed linear node indices only (same sum as poisson())."""
+    nz, ny, nx = rho.shape
+    rho = np.ascontiguousarray(rho, dtype=np.float64)
+    t = np.ascontiguousarray(targets, dtype=np.int64)
+    out = np.zeros(t.size)
+    if lib().orc_poisson_sample(nx, ny, nz, _p(_v3(d)), gz, _p(rho.reshape(-1)), t.size,
+                                t.ctypes.data_as(C.POINTER(C.c_int64)), _p(out)) != 0:
+        raise ValueError("oracle: invalid grid")
+    return out

@@ -53,6 +53,9 @@ EXPORTS = {
     "bt_grid_set_field": (C.c_int, [_vp, _vp, _vp, _vp, C.c_int]),
     "bt_grid_set_particle_shape": (C.c_int, [_vp, C.c_int32]),
     "bt_grid_rho": (C.c_int, [_vp, C.POINTER(_vp)]),
+    "bt_grid_solve_poisson": (C.c_int, [_vp, C.c_double, _vp]),
+    "bt_grid_download_phi": (C.c_int, [_vp, _vp]),
+    "bt_grid_download_field": (C.c_int, [_vp, _vp, _vp, _vp]),
     "bt_grid_download_rho": (C.c_int, [_vp, _vp]),
     "bt_deposit_cic": (C.c_int, [_vp, _vp, C.c_double, C.c_double, C.c_int]),
     "bt_gather_kick": (C.c_int, [_vp, _vp, _dp, C.c_double, C.c_double, C.c_double]),
@@ -257,6 +260,21 @@ class Grid:
     def set_particle_shape(self, order):
         """1 = CIC (default), 2 = quadratic B-spline."""
         _check(lib.bt_grid_set_particle_shape(self._h, int(order)), "bt_grid_set_particle_shape")
+
+    def solve_poisson(self, gz=1.0, stream=None):
+        """rho -> phi -> E (rest frame, third axis stretched by gz) on the current torch stream; see bt_grid_solve_poisson."""
+        sp = _current_stream_ptr() if stream is None else stream
+        _check(lib.bt_grid_solve_poisson(self._h, float(gz), sp), "bt_grid_solve_poisson")
+
+    def download_phi(self):
+        out = np.empty((self.shape[2], self.shape[1], self.shape[0]), dtype=np.float64)
+        _check(lib.bt_grid_download_phi(self._h, out.ctypes.data), "bt_grid_download_phi")
+        return out
+
+    def download_field(self):
+        out = [np.empty((self.shape[2], self.shape[1], self.shape[0]), dtype=np.float64) for _ in range(3)]
+        _check(lib.bt_grid_download_field(self._h, *[o.ctypes.data for o in out]), "bt_grid_download_field")
+        return out
 
     def set_field(self, Ex, Ey, Ez):
         """Host numpy arrays (any shape with nx*ny*nz elements, x fastest) or CUDA torch tensors."""

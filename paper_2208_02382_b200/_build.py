@@ -11,7 +11,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libbt.so")
-SOURCES = ["bt_api.cu", "track.cu", "grid.cu", "sort.cu", "moments.cu", "calib.cu"]
+SOURCES = ["bt_api.cu", "track.cu", "grid.cu", "sort.cu", "moments.cu", "poisson.cu", "calib.cu"]
 HEADERS = [os.path.join(CSRC, "bt_internal.h"), os.path.join(CSRC, "grid_dev.cuh"), os.path.join(CSRC, "bulk_copy.cuh"), os.path.join(HERE, "..", "include", "bt.h")]
 
 NVCC_FLAGS = [
@@ -21,6 +21,10 @@ NVCC_FLAGS = [
     "-Xcompiler", "-fPIC,-O2,-Wall",
     "-shared", "-cudart", "shared",
 ]
+
+
+# cuFFT (the FFT of the Poisson solve is a library step); rpath so that the image's CUDA 12.9 copy is found at load time
+LINK = ["-lcufft", "-Xlinker", "-rpath=/usr/local/cuda/lib64"]
 
 
 def _nvcc():
@@ -36,7 +40,7 @@ STAMP = LIB + ".stamp"
 def _digest():
     """Content hash of sources + flags (mtimes do not survive the trip to the GPU box)."""
     import hashlib
-    h = hashlib.sha256(" ".join(NVCC_FLAGS).encode())
+    h = hashlib.sha256(" ".join(NVCC_FLAGS + LINK).encode())
     for d in [os.path.join(CSRC, s) for s in SOURCES] + HEADERS:
         with open(d, "rb") as f:
             h.update(f.read())
@@ -55,7 +59,7 @@ def build(force=False, verbose=False):
         return LIB
     tmp = LIB + ".tmp.%d" % os.getpid()
     cmd = [_nvcc()] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + \
-          ["-o", tmp] + [os.path.join(CSRC, s) for s in SOURCES]
+          ["-o", tmp] + [os.path.join(CSRC, s) for s in SOURCES] + LINK
     subprocess.check_call(cmd)
     os.replace(tmp, LIB)
     with open(STAMP, "w") as f:

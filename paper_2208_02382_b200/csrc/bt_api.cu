@@ -590,8 +590,10 @@ int bt_grid_create(bt_grid **out, int32_t nx, int32_t ny, int32_t nz, const doub
 void bt_grid_destroy(bt_grid *grid) {
     if (!grid) return;
     cudaDeviceSynchronize();
+    poisson_free(&grid->g);
     if (grid->g.rho) cudaFree(grid->g.rho);
     if (grid->g.field) cudaFree(grid->g.field);
+    if (grid->g.phi) cudaFree(grid->g.phi);
     delete grid;
 }
 
@@ -629,6 +631,39 @@ int bt_grid_download_rho(bt_grid *grid, double *host_rho) {
     BT_CUDA_TRY(cudaMemcpyAsync(host_rho, g.rho, (size_t)g.nn * sizeof(double), cudaMemcpyDeviceToHost, g.last_stream));
     BT_CUDA_TRY(cudaStreamSynchronize(g.last_stream));
     return BT_OK;
+}
+
+int bt_grid_solve_poisson(bt_grid *grid, double gz, void *cuda_stream) {
+    if (!grid) return fail(BT_ERR_INVALID, "bt_grid_solve_poisson: grid is NULL");
+    if (!(gz > 0.0) || !isfinite(gz)) return fail(BT_ERR_INVALID, "bt_grid_solve_poisson: gz must be positive and finite");
+    Grid &g = grid->g;
+    if ((int64_t)8 * g.nn > ((int64_t)1 << 31) - 1) return fail(BT_ERR_UNSUPPORTED, "bt_grid_solve_poisson: padded grid exceeds 2^31 nodes");
+    return poisson_solve(&g, gz, (cudaStream_t)cuda_stream);
+}
+
+int bt_grid_download_phi(bt_grid *grid, double *host_phi) {
+    if (!grid || !host_phi) return fail(BT_ERR_INVALID, "bt_grid_download_phi: NULL argument");
+    Grid &g = grid->g;
+    if (!g.phi) return fail(BT_ERR_STATE, "bt_grid_download_phi: bt_grid_solve_poisson not called");
+    BT_CUDA_TRY(cudaMemcpyAsync(host_phi, g.phi, (size_t)g.nn * sizeof(double), cudaMemcpyDeviceToHost, g.last_stream));
+    BT_CUDA_TRY(cudaStreamSynchronize(g.last_stream));
+    return BT_OK;
+}
+
+int bt_grid_download_field(bt_grid *grid, double *host_Ex, double *host_Ey, double *host_Ez) {
+    if (!grid || !host_Ex || !host_Ey || !host_Ez) return fail(BT_ERR_INVALID, "bt_grid_download_field: NULL argument");
+    Grid &g = grid->g;
+    if (!g.field) return fail(BT_ERR_STATE, "bt_grid_download_field: no field (bt_grid_set_field / bt_grid_solve_poisson not called)");
+    double *tmp = nullptr;
+    BT_CUDA_TRY(cudaMalloc(&tmp, (size_t)g.nn * 3 * sizeof(double)));
+    int rc = field_unpack(&g, tmp, tmp + g.nn, tmp + 2 * g.nn, g.last_stream);
+    double *host[3] = {host_Ex, host_Ey, host_Ez};
+    for (int c = 0; c < 3 && rc == BT_OK; ++c)
+        if (cudaMemcpyAsync(host[c], tmp + c * g.nn, (size_t)g.nn * sizeof(double), cudaMemcpyDeviceToHost, g.last_stream) != cudaSuccess)
+            rc = fail(BT_ERR_CUDA, "bt_grid_download_field: copy failed");
+    cudaStreamSynchronize(g.last_stream);
+    cudaFree(tmp);
+    return rc;
 }
 
 int bt_grid_set_particle_shape(bt_grid *grid, int32_t order) {

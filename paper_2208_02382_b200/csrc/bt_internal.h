@@ -112,6 +112,8 @@ struct Grid {
     int64_t nn = 0;
     double *rho = nullptr;
     double *field = nullptr;  // interleaved (Ex,Ey,Ez,pad) per node: 4*nn doubles, or nullptr
+    double *phi = nullptr;    // potential at the nodes (bt_grid_solve_poisson), or nullptr
+    void *poisson = nullptr;  // solver state (plans, padded buffers, cached Green transform), poisson.cu
     cudaStream_t last_stream = nullptr;
 };
 
@@ -135,6 +137,9 @@ int launch_gather_kick(Beam *b, const Grid *g, const double coef[3], double zsca
 int sort_by_cell(Beam *b, const Grid *g, double zscale);
 int unpermute_to(Beam *b, int c, double *out);  // out[ids[j]] = q[c][j] on the beam's stream
 int launch_moments(Beam *b, double host_mean[6], double host_cov[36]);  // synchronises the beam's stream
+int poisson_solve(Grid *g, double gz, cudaStream_t stream);  // rho -> phi -> field records
+void poisson_free(Grid *g);
+int field_unpack(Grid *g, double *ex, double *ey, double *ez, cudaStream_t stream);  // device outputs
 int launch_field_pack(Grid *g, const double *ex, const double *ey, const double *ez, cudaStream_t s);
 
 }  // namespace bt

@@ -1,0 +1,205 @@
+// Free-space Poisson solve in the bunch rest frame ("the Poisson equation is solved in
+// the bunch rest frame"), reading R19:
+//   phi_a = (1/(4 pi eps0)) sum_b q_b G(r_a - r_b),  G(r) = 1/|r| (a != b),  G(0) = cell average of 1/r,
+//   third-axis spacing dz' = gz * dz;  E = -grad phi by centred (faces: one-sided) differences.
+// The open-boundary sum is a linear convolution, evaluated exactly (up to rounding) by Hockney's zero-padding: rho is
+// embedded in a (2nx, 2ny, 2nz) box, transformed (cuFFT D2Z -- a library FFT is a step of the method, like the oracle's
+// direct sum is a loop), multiplied by the transform of the Green table, transformed back, and the physical octant is kept.
+// Everything around the two FFTs is this file's kernels: padding, Green table, spectral multiply (the table is even in every
+// index, so its transform is real and only the real part is stored), extraction, and the gradient written straight into the
+// 32-byte node records bt_gather_kick reads.  The transformed Green table is cached per (grid, gz).
+#include "bt_internal.h"
+
+#include <cufft.h>
+#include <math.h>
+
+namespace bt {
+
+static const double kEps0 = 8.8541878128e-12;
+static const double kPiP = 3.14159265358979323846264338327950288;
+
+#define BT_CUFFT_TRY(expr)                                                                              \
+    do {                                                                                                \
+        cufftResult _r = (expr);                                                                        \
+        if (_r != CUFFT_SUCCESS) return ::bt::fail(BT_ERR_CUDA, std::string(#expr) + ": cuFFT error " + std::to_string((int)_r)); \
+    } while (0)
+
+// ---- host: the self term, (1/V) int_cell 1/r dV, from the primitive F of 1/r (d^3F/dxdydz = 1/r) ---------------------
+static long double box_primitive(long double x, long double y, long double z) {
+    const long double r = sqrtl(x * x + y * y + z * z);
+    long double f = 0.0L;
+    if (x > 0 && y > 0 && z > 0)
+        f -= 0.5L * (x * x * atanl(y * z / (x * r)) + y * y * atanl(x * z / (y * r)) + z * z * atanl(x * y / (z * r)));
+    if (x > 0 && y > 0) f += x * y * logl(z + r);
+    if (y > 0 && z > 0) f += y * z * logl(x + r);
+    if (x > 0 && z > 0) f += x * z * logl(y + r);
+    return f;
+}
+static double green_self_term(double dx, double dy, double dz) {
+    const long double a = 0.5L * dx, b = 0.5L * dy, c = 0.5L * dz;
+    // one octant: F(a,b,c) - F(0,b,c) - F(a,0,c) - F(a,b,0) (the terms with two or three zeros vanish); 8 octants / volume
+    const long double oct = box_primitive(a, b, c) - box_primitive(0, b, c) - box_primitive(a, 0, c) - box_primitive(a, b, 0);
+    return (double)(oct / (a * b * c));
+}
+
+// ---- kernels ---------------------------------------------------------------------------------------------------------
+struct PadDims {
+    int nx, ny, nz, mx, my, mz;  // physical and padded (m = 2n) node counts
+};
+
+// Green table on the padded box: index i stands for the offset i (i < n) or i - m (i > n); i == n is never used.
+__global__ void __launch_bounds__(256) green_table_kernel(double *__restrict__ g, PadDims p, double dx, double dy, double dz, double g0) {
+    const long long total = (long long)p.mx * p.my * p.mz;
+    for (long long a = (long long)blockIdx.x * blockDim.x + threadIdx.x; a < total; a += (long long)gridDim.x * blockDim.x) {
+        const int i = (int)(a % p.mx), j = (int)((a / p.mx) % p.my), k = (int)(a / ((long long)p.mx * p.my));
+        const int oi = i <= p.nx ? i : i - p.mx, oj = j <= p.ny ? j : j - p.my, ok = k <= p.nz ? k : k - p.mz;
+        double v;
+        if (i == p.nx || j == p.ny || k == p.nz) v = 0.0;
+        else if (oi == 0 && oj == 0 && ok == 0) v = g0;
+        else {
+            const double rx = oi * dx, ry = oj * dy, rz = ok * dz;
+            v = 1.0 / sqrt(rx * rx + ry * ry + rz * rz);
+        }
+        g[a] = v;
+    }
+}
+
+__global__ void __launch_bounds__(256) real_part_kernel(const cufftDoubleComplex *__restrict__ spec, double *__restrict__ re, long long n) {
+    for (long long a = (long long)blockIdx.x * blockDim.x + threadIdx.x; a < n; a += (long long)gridDim.x * blockDim.x) re[a] = spec[a].x;
+}
+
+__global__ void __launch_bounds__(256) pad_rho_kernel(const double *__restrict__ rho, double *__restrict__ pad, PadDims p) {
+    const long long total = (long long)p.mx * p.my * p.mz;
+    for (long long a = (long long)blockIdx.x * blockDim.x + threadIdx.x; a < total; a += (long long)gridDim.x * blockDim.x) {
+        const int i = (int)(a % p.mx), j = (int)((a / p.mx) % p.my), k = (int)(a / ((long long)p.mx * p.my));
+        pad[a] = (i < p.nx && j < p.ny && k < p.nz) ? rho[((long long)k * p.ny + j) * p.nx + i] : 0.0;
+    }
+}
+
+__global__ void __launch_bounds__(256) spectral_multiply_kernel(cufftDoubleComplex *__restrict__ spec, const double *__restrict__ ghat,
+                                                                long long n, double scale) {
+    for (long long a = (long long)blockIdx.x * blockDim.x + threadIdx.x; a < n; a += (long long)gridDim.x * blockDim.x) {
+        const double s = ghat[a] * scale;
+        cufftDoubleComplex v = spec[a];
+        v.x *= s;
+        v.y *= s;
+        spec[a] = v;
+    }
+}
+
+__global__ void __launch_bounds__(256) extract_phi_kernel(const double *__restrict__ pad, double *__restrict__ phi, PadDims p) {
+    const long long total = (long long)p.nx * p.ny * p.nz;
+    for (long long a = (long long)blockIdx.x * blockDim.x + threadIdx.x; a < total; a += (long long)gridDim.x * blockDim.x) {
+        const int i = (int)(a % p.nx), j = (int)((a / p.nx) % p.ny), k = (int)(a / ((long long)p.nx * p.ny));
+        phi[a] = pad[((long long)k * p.my + j) * p.mx + i];
+    }
+}
+
+// E = -grad phi -> node records (Ex, Ey, Ez, 0): centred differences inside, one-sided first-order at the faces
+__global__ void __launch_bounds__(256) gradient_kernel(const double *__restrict__ phi, double4 *__restrict__ field, PadDims p, double dx,
+                                                       double dy, double dz) {
+    const long long total = (long long)p.nx * p.ny * p.nz;
+    const long long sy = p.nx, sz = (long long)p.nx * p.ny;
+    for (long long a = (long long)blockIdx.x * blockDim.x + threadIdx.x; a < total; a += (long long)gridDim.x * blockDim.x) {
+        const int i = (int)(a % p.nx), j = (int)((a / p.nx) % p.ny), k = (int)(a / sz);
+        const double c = phi[a];
+        const double gx = i == 0 ? (phi[a + 1] - c) / dx : i == p.nx - 1 ? (c - phi[a - 1]) / dx : (phi[a + 1] - phi[a - 1]) / (2.0 * dx);
+        const double gy = j == 0 ? (phi[a + sy] - c) / dy : j == p.ny - 1 ? (c - phi[a - sy]) / dy : (phi[a + sy] - phi[a - sy]) / (2.0 * dy);
+        const double gzv = k == 0 ? (phi[a + sz] - c) / dz : k == p.nz - 1 ? (c - phi[a - sz]) / dz : (phi[a + sz] - phi[a - sz]) / (2.0 * dz);
+        field[a] = make_double4(-gx, -gy, -gzv, 0.0);
+    }
+}
+
+__global__ void __launch_bounds__(256) field_unpack_kernel(const double4 *__restrict__ field, long long nn, double *__restrict__ ex,
+                                                           double *__restrict__ ey, double *__restrict__ ez) {
+    const long long a = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (a < nn) {
+        const double4 v = field[a];
+        ex[a] = v.x, ey[a] = v.y, ez[a] = v.z;
+    }
+}
+
+// ---- host side -------------------------------------------------------------------------------------------------------
+struct PoissonState {
+    cufftHandle fwd = 0, inv = 0;
+    bool plans = false;
+    double *pad = nullptr;                 // (2nz, 2ny, 2nx) reals: padded rho, then the padded potential
+    cufftDoubleComplex *spec = nullptr;    // (2nz, 2ny, nx + 1) complex
+    double *ghat = nullptr;                // real part of the Green table's transform, same shape as spec
+    double ghat_gz = 0.0;                  // gz the cached table was built for (0 = none)
+};
+
+static int grid_1d(long long n) {
+    long long b = (n + 255) / 256;
+    return (int)(b > 148 * 32 ? 148 * 32 : b);
+}
+
+void poisson_free(Grid *g) {
+    PoissonState *st = static_cast<PoissonState *>(g->poisson);
+    if (!st) return;
+    if (st->plans) {
+        cufftDestroy(st->fwd);
+        cufftDestroy(st->inv);
+    }
+    if (st->pad) cudaFree(st->pad);
+    if (st->spec) cudaFree(st->spec);
+    if (st->ghat) cudaFree(st->ghat);
+    delete st;
+    g->poisson = nullptr;
+}
+
+int poisson_solve(Grid *g, double gz, cudaStream_t stream) {
+    PadDims p;
+    p.nx = g->nx, p.ny = g->ny, p.nz = g->nz;
+    p.mx = 2 * g->nx, p.my = 2 * g->ny, p.mz = 2 * g->nz;
+    const long long nreal = (long long)p.mx * p.my * p.mz;
+    const long long nspec = (long long)p.mz * p.my * (p.mx / 2 + 1);
+    PoissonState *st = static_cast<PoissonState *>(g->poisson);
+    if (!st) {
+        st = new (std::nothrow) PoissonState();
+        if (!st) return fail(BT_ERR_OOM, "bt_grid_solve_poisson: host allocation failed");
+        g->poisson = st;
+    }
+    if (!st->pad) BT_CUDA_TRY(cudaMalloc(&st->pad, (size_t)nreal * sizeof(double)));
+    if (!st->spec) BT_CUDA_TRY(cudaMalloc(&st->spec, (size_t)nspec * sizeof(cufftDoubleComplex)));
+    if (!st->ghat) BT_CUDA_TRY(cudaMalloc(&st->ghat, (size_t)nspec * sizeof(double)));
+    if (!g->phi) BT_CUDA_TRY(cudaMalloc(&g->phi, (size_t)g->nn * sizeof(double)));
+    if (!g->field) BT_CUDA_TRY(cudaMalloc(&g->field, (size_t)g->nn * 4 * sizeof(double)));
+    if (!st->plans) {
+        BT_CUFFT_TRY(cufftPlan3d(&st->fwd, p.mz, p.my, p.mx, CUFFT_D2Z));
+        BT_CUFFT_TRY(cufftPlan3d(&st->inv, p.mz, p.my, p.mx, CUFFT_Z2D));
+        st->plans = true;
+    }
+    BT_CUFFT_TRY(cufftSetStream(st->fwd, stream));
+    BT_CUFFT_TRY(cufftSetStream(st->inv, stream));
+    const double dx = g->d[0], dy = g->d[1], dz = gz * g->d[2];
+    if (st->ghat_gz != gz) {  // Green table for this grid and this gz: built and transformed once
+        green_table_kernel<<<grid_1d(nreal), 256, 0, stream>>>(st->pad, p, dx, dy, dz, green_self_term(dx, dy, dz));
+        BT_CUFFT_TRY(cufftExecD2Z(st->fwd, st->pad, st->spec));
+        real_part_kernel<<<grid_1d(nspec), 256, 0, stream>>>(st->spec, st->ghat, nspec);
+        g_launch_count.fetch_add(2);
+        st->ghat_gz = gz;
+    }
+    pad_rho_kernel<<<grid_1d(nreal), 256, 0, stream>>>(g->rho, st->pad, p);
+    BT_CUFFT_TRY(cufftExecD2Z(st->fwd, st->pad, st->spec));
+    const double scale = 1.0 / (4.0 * kPiP * kEps0) / (double)nreal;  // Coulomb constant and the unnormalised inverse FFT
+    spectral_multiply_kernel<<<grid_1d(nspec), 256, 0, stream>>>(st->spec, st->ghat, nspec, scale);
+    BT_CUFFT_TRY(cufftExecZ2D(st->inv, st->spec, st->pad));
+    extract_phi_kernel<<<grid_1d(g->nn), 256, 0, stream>>>(st->pad, g->phi, p);
+    gradient_kernel<<<grid_1d(g->nn), 256, 0, stream>>>(g->phi, reinterpret_cast<double4 *>(g->field), p, dx, dy, dz);
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return fail(BT_ERR_CUDA, std::string("bt_grid_solve_poisson launch: ") + cudaGetErrorString(e));
+    g_launch_count.fetch_add(4);
+    g->last_stream = stream;
+    return BT_OK;
+}
+
+int field_unpack(Grid *g, double *ex, double *ey, double *ez, cudaStream_t stream) {
+    field_unpack_kernel<<<(int)((g->nn + 255) / 256), 256, 0, stream>>>(reinterpret_cast<const double4 *>(g->field), g->nn, ex, ey, ez);
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return fail(BT_ERR_CUDA, std::string("bt_grid_download_field launch: ") + cudaGetErrorString(e));
+    g_launch_count.fetch_add(1);
+    return BT_OK;
+}
+
+}  // namespace bt

@@ -113,3 +113,12 @@ def test_invalid_arguments():
         O.poisson(np.zeros((1, 4, 4)), (1, 1, 1))
     with pytest.raises(ValueError):
         O.poisson(np.zeros((4, 4, 4)), (1, 1, 1), gz=0.0)
+
+
+def test_sampled_sum_equals_the_full_sum():
+    rng = np.random.default_rng(4)
+    rho = rng.uniform(0, 1e-12, (6, 7, 5))
+    d, gz = (1e-3, 1.2e-3, 0.7e-3), 2.0
+    full = O.poisson(rho, d, gz).reshape(-1)
+    idx = np.array([0, 17, 209, 100, 3])
+    assert np.array_equal(O.poisson_sample(rho, d, gz, idx), full[idx])
