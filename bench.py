@@ -282,6 +282,21 @@ def bench_spacecharge(bt, torch, flush, peaks):
             t_dep += _event_ms(torch, lambda: beam.deposit_cic(grid, sc.q_weight, sc.zscale, True), 1, flush)
             after = sc.ds if step < sc.nsteps - 1 else sc.ds / 2
             t_gat += _event_ms(torch, lambda: beam.gather_kick(grid, sc.kick_coef, sc.zscale, 0.0, after), 1, flush)
+        poisson = None
+        if variant == "A" and order == 1:
+            # NEXT-4: rest-frame Poisson solve on the deposited rho (own kernels + 2 cuFFT transforms of the 256^3 padded
+            # box); the prescribed field is put back afterwards.  Bytes = one read and one write per array per pass if
+            # each FFT were a single pass over its data (a lower bound on HBM traffic): 1.73 GB at 128^3.
+            gz = 1.0 + sc.kin_energy_MeV / sc.mass_MeV
+            grid.solve_poisson(gz)                                 # warm-up: plans, buffers, Green transform
+            t_ps = _event_ms(torch, lambda: grid.solve_poisson(gz), 5, flush)
+            ps_bytes = 8.0 * nn * (8 + 8 + 16 + 16 + 8 + 16 + 16 + 8 + 1 + 1 + 1 + 4)
+            mp_ = statistics.mean(t_ps) * 1e-3
+            poisson = {"ms": mp_ * 1e3, "padded_box": [2 * s for s in sc.shape],
+                       "roofline": {"bound": "hbm", "achieved": ps_bytes / mp_ / 1e9, "peak": hbm, "unit": "GB/s",
+                                    "frac": ps_bytes / mp_ / 1e9 / hbm, "traffic": None,
+                                    "note": "bytes = single-pass lower bound of the pad/FFT/multiply/FFT/extract/gradient chain"}}
+            grid.set_field(*E)
         md, mg = statistics.mean(t_dep) * 1e-3, statistics.mean(t_gat) * 1e-3
         out[variant if order == 1 else variant + "_order2"] = {
             "workload": "configs[4] %s, %d particles, %dx%dx%d nodes, %d steps, particle shape order %d" % (
@@ -295,6 +310,8 @@ def bench_spacecharge(bt, torch, flush, peaks):
                                                "frac": gat_bytes / mg / 1e9 / hbm, "traffic": None}},
             "ms_per_step_incl_sort_amortised": (md + mg) * 1e3 + t_sort / sc.nsteps,
         }
+        if poisson:
+            out[variant]["poisson_solve"] = poisson
         beam.close()
         grid.close()
         del beam, grid
