@@ -263,7 +263,7 @@ def test_reference_s_and_turn_bookkeeping():
 def test_invalid_lattices_rejected():
     c = [np.zeros(1) for _ in range(6)]
     for bad in ([("quad", 1.0, 0, 1.0)], [("sbend", 1.0, 1, 0.0)], [("multipole", 0.0, 1, 11, 1.0, 0.0)],
-                [("multipole", 0.0, 2, 3, 1.0, 0.0)], [("drift", -1.0, 1)], [(7, 1.0, 1)]):
+                [("multipole", 0.0, 2, 3, 1.0, 0.0)], [("drift", -1.0, 1)], [(99, 1.0, 1)]):
         with pytest.raises(ValueError):
             O.track(c, bad, 1, GAMMA_P2GEV)
 
