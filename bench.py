@@ -286,11 +286,12 @@ def bench_spacecharge(bt, torch, flush, peaks):
         if variant == "A" and order == 1:
             # NEXT-4: rest-frame Poisson solve on the deposited rho (own kernels + 2 cuFFT transforms of the 256^3 padded
             # box); the prescribed field is put back afterwards.  Bytes = one read and one write per array per pass if
-            # each FFT were a single pass over its data (a lower bound on HBM traffic): 1.73 GB at 128^3.
+            # each FFT were a single pass over its data (a lower bound on HBM traffic): 1.0 GB at 128^3
+            # (padded box = 8 nn reals, spectrum = 4 nn complex, real Green transform = 4 nn reals).
             gz = 1.0 + sc.kin_energy_MeV / sc.mass_MeV
             grid.solve_poisson(gz)                                 # warm-up: plans, buffers, Green transform
             t_ps = _event_ms(torch, lambda: grid.solve_poisson(gz), 5, flush)
-            ps_bytes = 8.0 * nn * (8 + 8 + 16 + 16 + 8 + 16 + 16 + 8 + 1 + 1 + 1 + 4)
+            ps_bytes = 8.0 * nn * ((1 + 1) + (8 + 8) + (8 + 4 + 8) + (8 + 8) + (1 + 1 + 4))   # in doubles per node: copy, D2Z, multiply, Z2D, gradient
             mp_ = statistics.mean(t_ps) * 1e-3
             poisson = {"ms": mp_ * 1e3, "padded_box": [2 * s for s in sc.shape],
                        "roofline": {"bound": "hbm", "achieved": ps_bytes / mp_ / 1e9, "peak": hbm, "unit": "GB/s",

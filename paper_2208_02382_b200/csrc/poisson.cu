@@ -5,8 +5,8 @@
 // The open-boundary sum is a linear convolution, evaluated exactly (up to rounding) by Hockney's zero-padding: rho is
 // embedded in a (2nx, 2ny, 2nz) box, transformed (cuFFT D2Z -- a library FFT is a step of the method, like the oracle's
 // direct sum is a loop), multiplied by the transform of the Green table, transformed back, and the physical octant is kept.
-// Everything around the two FFTs is this file's kernels: padding, Green table, spectral multiply (the table is even in every
-// index, so its transform is real and only the real part is stored), extraction, and the gradient written straight into the
+// Everything around the two FFTs is this file's kernels: octant copy into a box zeroed once, Green table, spectral multiply (the table is even in every
+// index, so its transform is real and only the real part is stored), and one pass that extracts phi and writes -grad phi into the
 // 32-byte node records bt_gather_kick reads.  The transformed Green table is cached per (grid, gz).
 #include "bt_internal.h"
 
@@ -68,11 +68,12 @@ __global__ void __launch_bounds__(256) real_part_kernel(const cufftDoubleComplex
     for (long long a = (long long)blockIdx.x * blockDim.x + threadIdx.x; a < n; a += (long long)gridDim.x * blockDim.x) re[a] = spec[a].x;
 }
 
-__global__ void __launch_bounds__(256) pad_rho_kernel(const double *__restrict__ rho, double *__restrict__ pad, PadDims p) {
-    const long long total = (long long)p.mx * p.my * p.mz;
+// rho -> the physical octant of the padded input box (the other 7/8 of the box were zeroed once and are never written)
+__global__ void __launch_bounds__(256) copy_octant_kernel(const double *__restrict__ rho, double *__restrict__ pad, PadDims p) {
+    const long long total = (long long)p.nx * p.ny * p.nz;
     for (long long a = (long long)blockIdx.x * blockDim.x + threadIdx.x; a < total; a += (long long)gridDim.x * blockDim.x) {
-        const int i = (int)(a % p.mx), j = (int)((a / p.mx) % p.my), k = (int)(a / ((long long)p.mx * p.my));
-        pad[a] = (i < p.nx && j < p.ny && k < p.nz) ? rho[((long long)k * p.ny + j) * p.nx + i] : 0.0;
+        const int i = (int)(a % p.nx), j = (int)((a / p.nx) % p.ny), k = (int)(a / ((long long)p.nx * p.ny));
+        pad[((long long)k * p.my + j) * p.mx + i] = rho[a];
     }
 }
 
@@ -87,25 +88,20 @@ __global__ void __launch_bounds__(256) spectral_multiply_kernel(cufftDoubleCompl
     }
 }
 
-__global__ void __launch_bounds__(256) extract_phi_kernel(const double *__restrict__ pad, double *__restrict__ phi, PadDims p) {
+// The physical octant of the padded potential -> phi, and E = -grad phi -> node records (Ex, Ey, Ez, 0): centred
+// differences inside, one-sided first-order at the faces.  Reads the padded box directly (strides mx, mx*my).
+__global__ void __launch_bounds__(256) gradient_kernel(const double *__restrict__ pad, double *__restrict__ phi, double4 *__restrict__ field,
+                                                       PadDims p, double dx, double dy, double dz) {
     const long long total = (long long)p.nx * p.ny * p.nz;
+    const long long sy = p.mx, sz = (long long)p.mx * p.my;
     for (long long a = (long long)blockIdx.x * blockDim.x + threadIdx.x; a < total; a += (long long)gridDim.x * blockDim.x) {
         const int i = (int)(a % p.nx), j = (int)((a / p.nx) % p.ny), k = (int)(a / ((long long)p.nx * p.ny));
-        phi[a] = pad[((long long)k * p.my + j) * p.mx + i];
-    }
-}
-
-// E = -grad phi -> node records (Ex, Ey, Ez, 0): centred differences inside, one-sided first-order at the faces
-__global__ void __launch_bounds__(256) gradient_kernel(const double *__restrict__ phi, double4 *__restrict__ field, PadDims p, double dx,
-                                                       double dy, double dz) {
-    const long long total = (long long)p.nx * p.ny * p.nz;
-    const long long sy = p.nx, sz = (long long)p.nx * p.ny;
-    for (long long a = (long long)blockIdx.x * blockDim.x + threadIdx.x; a < total; a += (long long)gridDim.x * blockDim.x) {
-        const int i = (int)(a % p.nx), j = (int)((a / p.nx) % p.ny), k = (int)(a / sz);
-        const double c = phi[a];
-        const double gx = i == 0 ? (phi[a + 1] - c) / dx : i == p.nx - 1 ? (c - phi[a - 1]) / dx : (phi[a + 1] - phi[a - 1]) / (2.0 * dx);
-        const double gy = j == 0 ? (phi[a + sy] - c) / dy : j == p.ny - 1 ? (c - phi[a - sy]) / dy : (phi[a + sy] - phi[a - sy]) / (2.0 * dy);
-        const double gzv = k == 0 ? (phi[a + sz] - c) / dz : k == p.nz - 1 ? (c - phi[a - sz]) / dz : (phi[a + sz] - phi[a - sz]) / (2.0 * dz);
+        const double *q = pad + ((long long)k * p.my + j) * p.mx + i;
+        const double c = q[0];
+        const double gx = i == 0 ? (q[1] - c) / dx : i == p.nx - 1 ? (c - q[-1]) / dx : (q[1] - q[-1]) / (2.0 * dx);
+        const double gy = j == 0 ? (q[sy] - c) / dy : j == p.ny - 1 ? (c - q[-sy]) / dy : (q[sy] - q[-sy]) / (2.0 * dy);
+        const double gzv = k == 0 ? (q[sz] - c) / dz : k == p.nz - 1 ? (c - q[-sz]) / dz : (q[sz] - q[-sz]) / (2.0 * dz);
+        phi[a] = c;
         field[a] = make_double4(-gx, -gy, -gzv, 0.0);
     }
 }
@@ -123,7 +119,8 @@ __global__ void __launch_bounds__(256) field_unpack_kernel(const double4 *__rest
 struct PoissonState {
     cufftHandle fwd = 0, inv = 0;
     bool plans = false;
-    double *pad = nullptr;                 // (2nz, 2ny, 2nx) reals: padded rho, then the padded potential
+    double *pad_in = nullptr;              // (2nz, 2ny, 2nx) reals: rho in the physical octant, zeros elsewhere (zeroed once)
+    double *pad = nullptr;                 // (2nz, 2ny, 2nx) reals: the padded potential (and scratch for the Green table)
     cufftDoubleComplex *spec = nullptr;    // (2nz, 2ny, nx + 1) complex
     double *ghat = nullptr;                // real part of the Green table's transform, same shape as spec
     double ghat_gz = 0.0;                  // gz the cached table was built for (0 = none)
@@ -142,6 +139,7 @@ void poisson_free(Grid *g) {
         cufftDestroy(st->inv);
     }
     if (st->pad) cudaFree(st->pad);
+    if (st->pad_in) cudaFree(st->pad_in);
     if (st->spec) cudaFree(st->spec);
     if (st->ghat) cudaFree(st->ghat);
     delete st;
@@ -161,6 +159,10 @@ int poisson_solve(Grid *g, double gz, cudaStream_t stream) {
         g->poisson = st;
     }
     if (!st->pad) BT_CUDA_TRY(cudaMalloc(&st->pad, (size_t)nreal * sizeof(double)));
+    if (!st->pad_in) {
+        BT_CUDA_TRY(cudaMalloc(&st->pad_in, (size_t)nreal * sizeof(double)));
+        BT_CUDA_TRY(cudaMemsetAsync(st->pad_in, 0, (size_t)nreal * sizeof(double), stream));  // the D2Z transform is out of place: zeros persist
+    }
     if (!st->spec) BT_CUDA_TRY(cudaMalloc(&st->spec, (size_t)nspec * sizeof(cufftDoubleComplex)));
     if (!st->ghat) BT_CUDA_TRY(cudaMalloc(&st->ghat, (size_t)nspec * sizeof(double)));
     if (!g->phi) BT_CUDA_TRY(cudaMalloc(&g->phi, (size_t)g->nn * sizeof(double)));
@@ -180,16 +182,15 @@ int poisson_solve(Grid *g, double gz, cudaStream_t stream) {
         g_launch_count.fetch_add(2);
         st->ghat_gz = gz;
     }
-    pad_rho_kernel<<<grid_1d(nreal), 256, 0, stream>>>(g->rho, st->pad, p);
-    BT_CUFFT_TRY(cufftExecD2Z(st->fwd, st->pad, st->spec));
+    copy_octant_kernel<<<grid_1d(g->nn), 256, 0, stream>>>(g->rho, st->pad_in, p);
+    BT_CUFFT_TRY(cufftExecD2Z(st->fwd, st->pad_in, st->spec));
     const double scale = 1.0 / (4.0 * kPiP * kEps0) / (double)nreal;  // Coulomb constant and the unnormalised inverse FFT
     spectral_multiply_kernel<<<grid_1d(nspec), 256, 0, stream>>>(st->spec, st->ghat, nspec, scale);
     BT_CUFFT_TRY(cufftExecZ2D(st->inv, st->spec, st->pad));
-    extract_phi_kernel<<<grid_1d(g->nn), 256, 0, stream>>>(st->pad, g->phi, p);
-    gradient_kernel<<<grid_1d(g->nn), 256, 0, stream>>>(g->phi, reinterpret_cast<double4 *>(g->field), p, dx, dy, dz);
+    gradient_kernel<<<grid_1d(g->nn), 256, 0, stream>>>(st->pad, g->phi, reinterpret_cast<double4 *>(g->field), p, dx, dy, dz);
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return fail(BT_ERR_CUDA, std::string("bt_grid_solve_poisson launch: ") + cudaGetErrorString(e));
-    g_launch_count.fetch_add(4);
+    g_launch_count.fetch_add(3);
     g->last_stream = stream;
     return BT_OK;
 }
