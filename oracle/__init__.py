@@ -12,9 +12,9 @@ import numpy as np
 
 from . import build as _build
 
-DRIFT, QUAD, SBEND, DIPEDGE, MULTIPOLE, SHORTRF, DRIFT_EXACT, SHORTRF_SIN = range(8)
+DRIFT, QUAD, SBEND, DIPEDGE, MULTIPOLE, SHORTRF, DRIFT_EXACT, SHORTRF_SIN, QUAD_CHROMATIC = range(9)
 _TYPE_BY_NAME = {"drift": DRIFT, "quad": QUAD, "sbend": SBEND, "dipedge": DIPEDGE,
-                 "multipole": MULTIPOLE, "shortrf": SHORTRF, "drift_exact": DRIFT_EXACT, "shortrf_sin": SHORTRF_SIN}
+                 "multipole": MULTIPOLE, "shortrf": SHORTRF, "drift_exact": DRIFT_EXACT, "shortrf_sin": SHORTRF_SIN, "quad_chromatic": QUAD_CHROMATIC}
 
 ELEMENT_DTYPE = np.dtype([("type", "<i4"), ("nslice", "<i4"), ("ds", "<f8"), ("p", "<f8", (6,))])
 assert ELEMENT_DTYPE.itemsize == 64

@@ -2,6 +2,8 @@
 PAPER.md l.168 "non-linear elements, RF-modeling").  Independent of the oracle's formulas: relativistic kinematics of a
 free particle / of an energy kick written out in 50-digit arithmetic from (E, P), the linear limits R4 and R9,
 symplecticity of numerical Jacobians, slice composition, periodicity."""
+import math
+
 import mpmath as mp
 import numpy as np
 import pytest
@@ -159,3 +161,85 @@ def test_nonlinear_elements_argument_checks():
         O.track(c, [("shortrf_sin", 0.0, 2, VHAT, FREQ, PHI)], 1, G0)       # thin element: nslice must be 1
     with pytest.raises(ValueError):
         O.track(c, [("drift_exact", -1.0, 1)], 1, G0)
+
+
+# ---- R20 chromatic quadrupole ----------------------------------------------------------------------------------------
+def ode_quad(v, h, k, expanded):
+    """40-digit integration of Hamilton's equations in s.  expanded=True: H with the square root expanded in (px, py) only
+    (the reading's Hamiltonian); False: the full square root (SURVEY 8(c) derivation sketch with a quadrupole term)."""
+    mp.mp.dps = 40
+    x, px, y, py, t, pt = [mp.mpf(a) for a in v]
+    g0 = mp.mpf(G0)
+    b0 = mp.sqrt(g0 * g0 - 1) / g0
+    opd = mp.sqrt(1 - 2 * pt / b0 + pt * pt)
+
+    def rhs(s, u):
+        X, PX, Y, PY, T = u
+        if expanded:
+            inv = 1 / opd
+            tdot = (1 / b0 - pt) / opd * (1 + (PX * PX + PY * PY) / (2 * opd * opd)) - 1 / b0
+        else:
+            ps = mp.sqrt(opd * opd - PX * PX - PY * PY)
+            inv = 1 / ps
+            tdot = (1 / b0 - pt) / ps - 1 / b0
+        return [PX * inv, -k * X, PY * inv, k * Y, tdot]
+
+    sol = mp.odefun(rhs, 0, [x, px, y, py, t])
+    out = sol(mp.mpf(h))
+    mp.mp.dps = 50
+    return [out[0], out[1], out[2], out[3], out[4], pt]
+
+
+@pytest.mark.parametrize("k", [1.3, -0.8])
+@pytest.mark.parametrize("v", [(1e-3, 2e-3, -1e-3, 1e-3, 5e-4, 1e-2), (2e-3, -1e-3, 1e-3, 2e-3, 0.0, -3e-2)])
+def test_chromatic_quad_is_the_flow_of_its_hamiltonian(k, v):
+    h = 0.6
+    got, g = one(v, [("quad_chromatic", h, 1, k)])
+    ref = ode_quad(v, h, k, expanded=True)
+    assert g == G0
+    for i, (a, b) in enumerate(zip(got, ref)):
+        tol = 4e-16 * h if i == 4 else 4e-16 * max(abs(b), 1e-3)      # t: difference of two O(h/beta0) numbers
+        assert abs(mp.mpf(a) - b) <= tol, (i, a, b)
+    # and that Hamiltonian is the full square-root one up to fourth order in the transverse momenta: the velocities
+    # px/ps and px/(1+d) differ by a relative p_perp^2/2, i.e. the coordinates by O(h p_perp^3); t by O(h p_perp^4)
+    exact = ode_quad(v, h, k, expanded=False)
+    pperp = math.hypot(max(abs(v[1]), abs(float(exact[1]))), max(abs(v[3]), abs(float(exact[3]))))
+    for i in (0, 1, 2, 3):
+        assert abs(mp.mpf(got[i]) - exact[i]) <= 2.0 * h * pperp ** 3 * max(1.0, abs(k) * h)
+        assert abs(mp.mpf(got[i]) - exact[i]) > 0
+    assert abs(mp.mpf(got[4]) - exact[4]) <= 2.0 * h * pperp ** 4 + 4e-16 * h
+
+
+def test_chromatic_quad_limits_and_plane_exchange():
+    h, k = 0.8, 1.1
+    v = (1e-3, 2e-3, -1e-3, 1e-3, 5e-4, 0.0)
+    a, _ = one(v, [("quad_chromatic", h, 1, k)])
+    b, _ = one(v, [("quad", h, 1, k)])
+    for i in range(4):                                   # on momentum: the transverse map is R5
+        assert abs(a[i] - b[i]) <= 4e-16 * max(abs(b[i]), 1e-3)
+    assert a[4] > b[4]                                   # ... but the path is longer than the reference's
+    off = (1e-3, 2e-3, -1e-3, 1e-3, 5e-4, 2e-2)          # off momentum (pt > 0: lower energy): stronger focusing
+    c, _ = one(off, [("quad_chromatic", h, 1, k)])
+    d, _ = one(off, [("quad", h, 1, k)])
+    assert abs(c[0] - d[0]) > 1e-3 * abs(d[0])
+    # k < 0 is k > 0 with the planes exchanged
+    sw = (v[2], v[3], v[0], v[1], v[4], 1e-2)
+    e, _ = one((v[0], v[1], v[2], v[3], v[4], 1e-2), [("quad_chromatic", h, 1, -k)])
+    f, _ = one(sw, [("quad_chromatic", h, 1, k)])
+    assert [e[0], e[1], e[2], e[3], e[4]] == [f[2], f[3], f[0], f[1], f[4]]
+    # k = 0: paraxial chromatic drift, continuous limit of small k
+    z, _ = one(off, [("quad_chromatic", h, 1, 0.0)])
+    s_, _ = one(off, [("quad_chromatic", h, 1, 1e-12)])
+    for i in range(5):
+        assert abs(z[i] - s_[i]) <= 1e-12 * max(abs(z[i]), 1e-3)
+
+
+def test_chromatic_quad_jacobian_is_symplectic_and_slices_compose():
+    v0 = (1e-3, 2e-3, -1e-3, 1e-3, 5e-4, 1e-2)
+    M = numerical_jacobian([("quad_chromatic", 0.7, 1, 1.4)], v0, [1e-6] * 6)
+    assert np.max(np.abs(M.T @ J6 @ M - J6)) <= 1e-8
+    assert abs(M[0, 5]) > 1e-5                            # chromatic coupling: x depends on pt
+    a, _ = one(v0, [("quad_chromatic", 0.7, 1, 1.4)])
+    b, _ = one(v0, [("quad_chromatic", 0.7, 5, 1.4)])
+    for i in range(6):
+        assert abs(a[i] - b[i]) <= (5 * 4e-16 * 0.7 if i == 4 else 2e-15 * max(abs(a[i]), 1e-3))   # t: eps h per slice
