@@ -386,6 +386,8 @@ def run_ours(args):
     step_ms = [a.elapsed_time(b) for a, b in ev]
     ms_sum = sum(step_ms)
 
+    launch_info = beam.last_launch()         # geometry of the timed launches (the e2e leg below launches per chunk)
+
     # ---- end to end through the C-ABI with host buffers -----------------------------------------
     # bt_track_host = upload + walk + download with the bunch cut into chunks on three streams (copies overlap the walk)
     for _ in range(2):
@@ -401,7 +403,6 @@ def run_ours(args):
     # max over ranks
     from paper_2208_02382_b200.shard import max_over_ranks
     ms_sum, t_e2e, t_wall = max_over_ranks([ms_sum, t_e2e, t_wall], device="cuda")
-    launch_info = beam.last_launch()
 
     result = None
     if rank == 0:

@@ -63,6 +63,8 @@ typedef enum {
     /* non-linearised maps (P:l.168 "non-linear elements, RF-modeling"): */
     BT_DRIFT_EXACT = 6, /* R17: ps = sqrt(1 - 2pt/beta0 + pt^2 - px^2 - py^2); x += h px/ps; y += h py/ps;
                            t += h ((1/beta0 - pt)/ps - 1/beta0)  -- straight line with the exact time of flight */
+    BT_QUAD_CHROMATIC = 8, /* R20: thick quad with focusing k/(1+delta) per particle and the second-order path length;
+                              closed-form flow of H = -(1+d) + (px^2+py^2)/(2(1+d)) + k(x^2-y^2)/2 - pt/beta0; p0 = k */
     BT_SHORTRF_SIN = 7  /* R18: R9 without the expansion in t: pt = r pt - (Vhat/(bg)_f)(cos(k_rf t + phi) - cos(phi)),
                            px *= r, py *= r; same reference-energy update as R9 */
 } bt_element_type;
@@ -75,7 +77,7 @@ typedef enum {
  *   nslice  >= 1; the element is applied as nslice maps of length ds/nslice (R3; P:l.47, l.87).
  *           Thin elements (DIPEDGE, MULTIPOLE, SHORTRF, SHORTRF_SIN) must have nslice == 1.
  *   ds      length [m], >= 0; ignored for the map of thin elements but still added to s.
- *   p[6]    QUAD:      p0 = k [m^-2]
+ *   p[6]    QUAD, QUAD_CHROMATIC: p0 = k [m^-2]
  *           SBEND:     p0 = rc [m], signed bending radius, != 0
  *           DIPEDGE:   p0 = psi [rad], p1 = rc [m] (!= 0), p2 = g [m] full gap, p3 = K fringe integral
  *           MULTIPOLE: p0 = m (integer 1..10; 1 dipole, 2 quad, 3 sext, 4 oct), p1 = Kn, p2 = Ks

@@ -22,9 +22,9 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libbt.so")
 
 BT_OK, BT_ERR_INVALID, BT_ERR_CUDA, BT_ERR_OOM, BT_ERR_STATE, BT_ERR_UNSUPPORTED = 0, -1, -2, -3, -4, -5
-BT_DRIFT, BT_QUAD, BT_SBEND, BT_DIPEDGE, BT_MULTIPOLE, BT_SHORTRF, BT_DRIFT_EXACT, BT_SHORTRF_SIN = range(8)
+BT_DRIFT, BT_QUAD, BT_SBEND, BT_DIPEDGE, BT_MULTIPOLE, BT_SHORTRF, BT_DRIFT_EXACT, BT_SHORTRF_SIN, BT_QUAD_CHROMATIC = range(9)
 _KIND = {"drift": BT_DRIFT, "quad": BT_QUAD, "sbend": BT_SBEND, "dipedge": BT_DIPEDGE,
-         "multipole": BT_MULTIPOLE, "shortrf": BT_SHORTRF, "drift_exact": BT_DRIFT_EXACT, "shortrf_sin": BT_SHORTRF_SIN}
+         "multipole": BT_MULTIPOLE, "shortrf": BT_SHORTRF, "drift_exact": BT_DRIFT_EXACT, "shortrf_sin": BT_SHORTRF_SIN, "quad_chromatic": BT_QUAD_CHROMATIC}
 
 # bt_element: 64 bytes
 ELEMENT_DTYPE = np.dtype([("type", "<i4"), ("nslice", "<i4"), ("ds", "<f8"), ("p", "<f8", (6,))])

@@ -34,6 +34,7 @@ static int validate_element(const bt_element &e, int idx) {
         case BT_DRIFT:
         case BT_DRIFT_EXACT:
             break;
+        case BT_QUAD_CHROMATIC:
         case BT_QUAD:
             if (!isfinite(e.p[0])) return bad("k not finite");
             break;
@@ -203,6 +204,15 @@ double build_turn_table(const std::vector<bt_element> &lat, double gamma, std::v
                 o.c[0] = h;
                 o.c[1] = 1.0 / beta;
                 nslots += 26.0 * e.nslice;  // 12 DFMA/DMUL/DADD + reciprocal square root (~14 FP64-pipe instructions)
+                out.push_back(o);
+                break;
+            case BT_QUAD_CHROMATIC:  // R20
+                o.op = OP_QUADCHR;
+                o.c[0] = h;
+                o.c[1] = 1.0 / beta;
+                o.c[2] = fabs(e.p[0]);
+                o.c[3] = e.p[0] > 0.0 ? 1.0 : e.p[0] < 0.0 ? -1.0 : 0.0;
+                nslots += 200.0 * e.nslice;  // two square roots, sincos, exp, a reciprocal and ~60 DFMA/DMUL: order of magnitude
                 out.push_back(o);
                 break;
             case BT_SHORTRF_SIN: {  // R18

@@ -43,6 +43,7 @@ enum Op : int32_t {
     OP_MULT = 1 << 10,    // general thin multipole: count = m, c0 = Kn/(m-1)!, c1 = Ks/(m-1)!
     OP_RF = 1 << 11,      // px *= c0 ; py *= c0 ; pt = c0 pt + c1 t
     OP_DRIFTX = 1 << 13,  // exact drift (R17), count slices: c0 = h, c1 = 1/beta0
+    OP_QUADCHR = 1 << 15, // chromatic quad (R20), count slices: c0 = h, c1 = 1/beta0, c2 = |k|, c3 = +1 (k > 0: x focusing) / -1 / 0 (k = 0)
     OP_RFSIN = 1 << 14,   // sinusoidal short RF (R18): px *= c0; py *= c0; pt = c0 pt + c1 (cos(c2 t + c3) - c4)
     OP_TAILDRIFT = 1 << 12  // modifier of SEXT/OCT/SEXTOCT: the single-slice drift that follows the kick rides in the
                             // same record (c3 = h, c4 = h/(b0 g0)^2); same arithmetic, same order, one dispatch less

@@ -97,8 +97,50 @@ __device__ __forceinline__ void oct_kick(Ptc<P> &p, double c) {
     }
 }
 
+// R20 chromatic quad for ONE particle: per-particle focusing strength k/(1+delta), closed-form flow of
+// H = -(1+d) + (px^2+py^2)/(2(1+d)) + k(x^2-y^2)/2 - pt/beta0.  Deliberately NOT inlined: two square roots, sincos, exp and
+// a reciprocal need ~100 registers of their own; as a real call they do not weigh on the register allocation of the
+// DFMA-only maps that share the kernel (inlined, the P = 4 instantiation spilled 800 bytes).
+struct ChrOut {
+    double x, px, y, py, t;
+};
+__device__ __noinline__ ChrOut quadchr_one(double x, double px, double y, double py, double t, double pt, double h, double ib, double ak,
+                                           double sgn) {
+    const double opd = sqrt(fma(pt, pt, fma(-2.0 * pt, ib, 1.0)));  // 1 + delta = P/p0
+    double integral;
+    ChrOut o;
+    if (sgn == 0.0) {
+        integral = fma(px, px, py * py) * h;
+        o.x = fma(h / opd, px, x), o.px = px;
+        o.y = fma(h / opd, py, y), o.py = py;
+    } else {
+        const double w = sqrt(ak / opd), a = opd * w, wh = w * h;
+        double sn, cs;
+        sincos(wh, &sn, &cs);
+        const double ex = exp(wh), exi = 1.0 / ex;
+        const double ch = 0.5 * (ex + exi), sh = 0.5 * (ex - exi);
+        const bool fx = sgn > 0.0;
+        const double qf = fx ? x : y, pf = fx ? px : py;
+        const double qd = fx ? y : x, pd = fx ? py : px;
+        const double A = pf, B = -a * qf, C = pd, D = a * qd;
+        // sin(2wh) = 2 s c, sinh(2wh) = 2 sh ch
+        const double IF = 0.5 * h * fma(A, A, B * B) + (fma(A, A, -B * B) * (0.5 * sn * cs) + A * B * (sn * sn)) / w;
+        const double ID = 0.5 * h * fma(C, C, -D * D) + (fma(C, C, D * D) * (0.5 * sh * ch) + C * D * (sh * sh)) / w;
+        integral = IF + ID;
+        const double qf1 = fma(sn / a, pf, cs * qf), pf1 = fma(-a * sn, qf, cs * pf);
+        const double qd1 = fma(sh / a, pd, ch * qd), pd1 = fma(a * sh, qd, ch * pd);
+        o.x = fx ? qf1 : qd1, o.px = fx ? pf1 : pd1;
+        o.y = fx ? qd1 : qf1, o.py = fx ? pd1 : pf1;
+    }
+    o.t = t + (((ib - pt) / opd) * fma(integral, 0.5 / (opd * opd), h) - h * ib);
+    return o;
+}
+
 // ---- one record applied to the P particles of this thread -----------------------------------------
-template <int P>
+// NL: this instantiation also knows the non-linearised maps (R17, R18, R20).  They need square roots, sincos and exp;
+// compiled into the same kernel they cost the DFMA-only maps registers (configs[1]: 2.61 -> 3.19 ms per step, measured), so
+// lattices without them run the NL = false kernel, which is the linear walk exactly as before.
+template <int P, bool NL>
 __device__ __forceinline__ void apply(Ptc<P> &p, const DevOp &r) {
     const int op = r.op;
     if (op & (OP_QUAD5 | OP_QUAD1 | OP_QUAD)) {
@@ -161,7 +203,7 @@ __device__ __forceinline__ void apply(Ptc<P> &p, const DevOp &r) {
             p.py[j] *= c0;
             p.pt[j] = fma(c0, p.pt[j], c1 * p.t[j]);
         }
-    } else if (op & OP_DRIFTX) {  // R17 exact drift: straight line with the exact time of flight; c0 = h, c1 = 1/beta0
+    } else if (NL && (op & OP_DRIFTX)) {  // R17 exact drift: straight line with the exact time of flight; c0 = h, c1 = 1/beta0
         const double c0 = r.c[0], c1 = r.c[1];
         const int cnt = r.count;
 #pragma unroll 1
@@ -175,7 +217,17 @@ __device__ __forceinline__ void apply(Ptc<P> &p, const DevOp &r) {
                 p.t[j] = fma(c0, fma(c1 - pt, ips, -c1), p.t[j]);
             }
         }
-    } else if (op & OP_RFSIN) {  // R18: the energy kick qV cos(k t + phi) without the expansion in t
+    } else if (NL && (op & OP_QUADCHR)) {  // R20 chromatic quad: a call per particle (see quadchr_one)
+        const double h = r.c[0], ib = r.c[1], ak = r.c[2], sgn = r.c[3];
+        const int cnt = r.count;
+#pragma unroll 1
+        for (int s = 0; s < cnt; ++s) {
+            BT_FORP {
+                const ChrOut o = quadchr_one(p.x[j], p.px[j], p.y[j], p.py[j], p.t[j], p.pt[j], h, ib, ak, sgn);
+                p.x[j] = o.x, p.px[j] = o.px, p.y[j] = o.y, p.py[j] = o.py, p.t[j] = o.t;
+            }
+        }
+    } else if (NL && (op & OP_RFSIN)) {  // R18: the energy kick qV cos(k t + phi) without the expansion in t
         const double c0 = r.c[0], c1 = r.c[1], c2 = r.c[2], c3 = r.c[3], c4 = r.c[4];
         BT_FORP {
             p.px[j] *= c0;
@@ -201,12 +253,12 @@ __device__ __forceinline__ void apply(Ptc<P> &p, const DevOp &r) {
     }
 }
 
-template <int P>
+template <int P, bool NL>
 __device__ __forceinline__ void walk(Ptc<P> &p, const int n_ops, const int nturns) {
 #pragma unroll 1
     for (int turn = 0; turn < nturns; ++turn) {
 #pragma unroll 1
-        for (int e = 0; e < n_ops; ++e) apply<P>(p, c_table[e]);
+        for (int e = 0; e < n_ops; ++e) apply<P, NL>(p, c_table[e]);
     }
 }
 
@@ -227,7 +279,7 @@ __device__ __forceinline__ double ld_stream1(const double *p) {
 __device__ __forceinline__ void st_stream1(double *p, double v) { asm volatile("st.global.cs.f64 [%0], %1;" ::"l"(p), "d"(v) : "memory"); }
 
 // P particles per thread (P even: 16-byte vector access; requires 16-byte aligned arrays).
-template <int P>
+template <int P, bool NL>
 __global__ void __launch_bounds__(kMaxBlock, kMinBlocks<P>) track_kernel(const __grid_constant__ TrackArgs a) {
     const int tid = threadIdx.x;
     const int B = blockDim.x;
@@ -251,7 +303,7 @@ __global__ void __launch_bounds__(kMaxBlock, kMinBlocks<P>) track_kernel(const _
                 v = ld_stream2(q[4] + off), p.t[2 * j] = v.x, p.t[2 * j + 1] = v.y;
                 v = ld_stream2(q[5] + off), p.pt[2 * j] = v.x, p.pt[2 * j + 1] = v.y;
             }
-            walk<P>(p, a.n_ops, a.nturns);
+            walk<P, NL>(p, a.n_ops, a.nturns);
 #pragma unroll
             for (int j = 0; j < P / 2; ++j) {
                 const int off = j * 2 * B;
@@ -270,7 +322,7 @@ __global__ void __launch_bounds__(kMaxBlock, kMinBlocks<P>) track_kernel(const _
             p.py[0] = ld_stream1(a.q[3] + i);
             p.t[0] = ld_stream1(a.q[4] + i);
             p.pt[0] = ld_stream1(a.q[5] + i);
-            walk<P>(p, a.n_ops, a.nturns);
+            walk<P, NL>(p, a.n_ops, a.nturns);
             st_stream1(a.q[0] + i, p.x[0]);
             st_stream1(a.q[1] + i, p.px[0]);
             st_stream1(a.q[2] + i, p.y[0]);
@@ -289,7 +341,7 @@ __global__ void __launch_bounds__(kMaxBlock, kMinBlocks<P>) track_kernel(const _
         p.py[0] = ld_stream1(a.q[3] + i);
         p.t[0] = ld_stream1(a.q[4] + i);
         p.pt[0] = ld_stream1(a.q[5] + i);
-        walk<1>(p, a.n_ops, a.nturns);
+        walk<1, NL>(p, a.n_ops, a.nturns);
         st_stream1(a.q[0] + i, p.x[0]);
         st_stream1(a.q[1] + i, p.px[0]);
         st_stream1(a.q[2] + i, p.y[0]);
@@ -379,11 +431,13 @@ int launch_track(Beam *b, const DevOp *h_table, int32_t n_ops, int32_t nturns, u
     } else if (b->range) {
         BT_CUDA_TRY(cudaStreamWaitEvent(stream, ct.uploaded, 0));  // the table was placed by another chunk's stream
     }
+    bool nl = false;  // any non-linearised record in this table?
+    for (int32_t e = 0; e < n_ops; ++e) nl = nl || (h_table[e].op & (OP_DRIFTX | OP_RFSIN | OP_QUADCHR));
     switch (P) {
-        case 8: track_kernel<8><<<grid, block, 0, stream>>>(a); break;
-        case 4: track_kernel<4><<<grid, block, 0, stream>>>(a); break;
-        case 2: track_kernel<2><<<grid, block, 0, stream>>>(a); break;
-        default: track_kernel<1><<<grid, block, 0, stream>>>(a); break;
+        case 8: nl ? track_kernel<8, true><<<grid, block, 0, stream>>>(a) : track_kernel<8, false><<<grid, block, 0, stream>>>(a); break;
+        case 4: nl ? track_kernel<4, true><<<grid, block, 0, stream>>>(a) : track_kernel<4, false><<<grid, block, 0, stream>>>(a); break;
+        case 2: nl ? track_kernel<2, true><<<grid, block, 0, stream>>>(a) : track_kernel<2, false><<<grid, block, 0, stream>>>(a); break;
+        default: nl ? track_kernel<1, true><<<grid, block, 0, stream>>>(a) : track_kernel<1, false><<<grid, block, 0, stream>>>(a); break;
     }
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return fail(BT_ERR_CUDA, std::string("bt_track launch: ") + cudaGetErrorString(e));

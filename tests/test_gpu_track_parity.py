@@ -348,3 +348,21 @@ def test_nonlinear_element_validation():
     with pytest.raises(bt.BtError):
         beam.lattice_set([("drift_exact", -1.0, 1)])
     beam.close()
+
+
+@pytest.mark.parametrize("n,nturns", [(1, 2), (20_011, 3), (200_001, 1)])
+def test_chromatic_quad_matches_oracle(n, nturns):
+    """R20 chromatic quadrupole (both signs, k = 0, sliced) mixed with exact drifts and linear elements in one walk."""
+    cfg = W.config(0, n=n)
+    lat = [("drift_exact", 0.25, 1), ("quad_chromatic", 1.0, 4, 1.0), ("drift", 0.5, 2), ("quad_chromatic", 1.0, 3, -1.0),
+           ("quad_chromatic", 0.3, 1, 0.0), ("quad", 0.2, 2, 0.7), ("drift_exact", 0.25, 1)]
+    c = W.make_bunch(cfg)
+    c[5] *= 10.0                                       # percent-level momentum spread: the chromatic effect is visible
+    got, (g, s, turn), _ = gpu_track(cfg, c, nturns=nturns, lattice=lat)
+    ref, (g_ref, s_ref) = oracle_track(cfg, c, nturns=nturns, lattice=lat)
+    assert max(r14_error(got, ref)) <= 1e-11
+    assert g == g_ref and abs(s - s_ref) <= 1e-12
+    if n > 1:
+        lin = [("quad",) + e[1:] if e[0] == "quad_chromatic" else e for e in lat]
+        ref_lin, _ = oracle_track(cfg, c, nturns=nturns, lattice=lin)
+        assert max(r14_error(ref_lin, ref)) > 1e-4      # a different map from R5 on this bunch
