@@ -366,3 +366,43 @@ def test_chromatic_quad_matches_oracle(n, nturns):
         lin = [("quad",) + e[1:] if e[0] == "quad_chromatic" else e for e in lat]
         ref_lin, _ = oracle_track(cfg, c, nturns=nturns, lattice=lin)
         assert max(r14_error(ref_lin, ref)) > 1e-4      # a different map from R5 on this bunch
+
+
+@pytest.mark.parametrize("seed", [0, 1, 2, 3, 4, 5])
+def test_random_lattices_of_all_element_kinds(seed):
+    """Seeded random lattices mixing all nine element kinds (random order, parameters, slice counts; with and without
+    energy-changing cavities), several turns: exercises every opcode, the peephole fusions and the per-turn tables."""
+    rng = np.random.default_rng(1000 + seed)
+    cfg = W.config(0, n=3001 + 64 * seed)
+    lat = []
+    for _ in range(int(rng.integers(8, 24))):
+        kind = int(rng.integers(0, 9))
+        ns = int(rng.integers(1, 8))
+        L = float(rng.uniform(0.05, 0.6))
+        if kind == 0:
+            lat.append(("drift", L, ns))
+        elif kind == 1:
+            lat.append(("quad", L, ns, float(rng.choice([-0.6, -0.3, 0.0, 0.4, 0.7]))))
+        elif kind == 2:
+            lat.append(("sbend", L, ns, float(rng.choice([-8.0, 5.0, 12.0]))))
+        elif kind == 3:
+            lat.append(("dipedge", 0.0, 1, float(rng.uniform(-0.2, 0.2)), float(rng.choice([-8.0, 5.0])), 0.02, 0.5))
+        elif kind == 4:
+            m = int(rng.integers(1, 7))
+            lat.append(("multipole", 0.0, 1, m, float(rng.uniform(-0.5, 0.5)) * (1e-3 if m == 1 else 1.0),
+                        float(rng.choice([0.0, rng.uniform(-0.3, 0.3)])) * (1e-3 if m == 1 else 1.0)))
+        elif kind == 5 and seed % 2 == 0:
+            lat.append(("shortrf", 0.0, 1, 1e-3, 2e8, float(rng.choice([-90.0, -30.0, 20.0]))))
+        elif kind == 6:
+            lat.append(("drift_exact", L, ns))
+        elif kind == 7 and seed % 2 == 0:
+            lat.append(("shortrf_sin", 0.0, 1, 5e-4, 1e8, float(rng.choice([-90.0, -45.0, 10.0]))))
+        else:
+            lat.append(("quad_chromatic", L, ns, float(rng.choice([-1.0, 0.0, 0.8]))))
+    c = W.make_bunch(cfg)
+    nturns = 2
+    got, (g, s, turn), _ = gpu_track(cfg, c, nturns=nturns, lattice=lat)
+    ref, (g_ref, s_ref) = oracle_track(cfg, c, nturns=nturns, lattice=lat)
+    assert all(np.all(np.isfinite(a)) for a in ref), lat        # the lattices are tame enough for the bunch to survive
+    assert max(r14_error(got, ref)) <= 1e-11, lat
+    assert abs(g - g_ref) <= 8e-16 * g_ref and abs(s - s_ref) <= 1e-10 and turn == nturns
