@@ -346,3 +346,51 @@ def test_gather_modes(mode, offset, monkeypatch):
     assert max(r14_error([a[ok] for a in got], [a[ok] for a in ref])) <= 1e-11
     beam.close()
     grid.close()
+
+
+@pytest.mark.parametrize("seed", range(8))
+def test_random_grids_shapes_orders_and_clouds(seed):
+    """Seeded random grids (anisotropic, non-cubic, offset), particle clouds that partly leave the grid, both shape orders,
+    random zscale, sorted or not: deposit (R15 isolated) and gather + kick with drifts (R14) against the oracle."""
+    rng = np.random.default_rng(500 + seed)
+    shape = tuple(int(v) for v in rng.integers(3, 40, 3))
+    d = tuple(float(v) for v in rng.uniform(0.2e-3, 2e-3, 3))
+    lo = tuple(float(v) for v in rng.uniform(-5e-3, 0.0, 3))
+    order = 1 + seed % 2
+    zscale = float(rng.choice([1.0, -1.0, 0.37, 2.5]))
+    n = int(rng.integers(1, 60_000))
+    centre = [lo[a] + 0.5 * d[a] * (shape[a] - 1) for a in range(3)]
+    width = [0.35 * d[a] * (shape[a] - 1) for a in range(3)]
+    c = [np.zeros(n) for _ in range(6)]
+    c[0] = centre[0] + width[0] * rng.standard_normal(n)
+    c[2] = centre[1] + width[1] * rng.standard_normal(n)
+    c[4] = (centre[2] + width[2] * rng.standard_normal(n)) / zscale
+    for a in (1, 3, 5):
+        c[a] = 1e-3 * rng.standard_normal(n)
+    nn = shape[0] * shape[1] * shape[2]
+    E = [rng.standard_normal((shape[2], shape[1], shape[0])) * 1e5 for _ in range(3)]
+    coef, qw, ds = (1e-9, -2e-9, 0.5e-9), 1e-9 / n, 0.01
+    beam = bt.Beam(n)
+    grid = bt.Grid(shape, lo, d)
+    grid.set_particle_shape(order)
+    beam.set_ref(1000.0, W.MASS_PROTON_MEV, 1.0)
+    grid.set_field(*E)
+    beam.upload(c)
+    if seed % 3 == 0:
+        beam.sort_by_cell(grid, zscale)
+    beam.deposit_cic(grid, qw, zscale, True)
+    rho = grid.download_rho()
+    ref_rho, n_in = O.deposit_cic(c[0], c[2], c[4], shape, lo, d, qw, zscale, order=order)
+    assert r15_isolated(rho, ref_rho) <= 1e-12
+    assert abs(math.fsum(rho.ravel()) - qw * n_in) <= 1e-13 * qw * max(n_in, 1)
+    beam.gather_kick(grid, coef, zscale, ds / 2, ds)
+    got = beam.download()
+    g0 = O.ref_from_kinetic(1000.0, W.MASS_PROTON_MEV)[0]
+    ref = [a.copy() for a in c]
+    O.track(ref, [("drift", ds / 2, 1)], 1, g0)
+    O.gather_kick(ref, shape, lo, d, E, coef, zscale, order=order)
+    O.track(ref, [("drift", ds, 1)], 1, g0)
+    assert max(r14_error(got, ref)) <= 1e-11
+    assert nn > 0
+    beam.close()
+    grid.close()
