@@ -68,7 +68,9 @@ __device__ __forceinline__ void flush_cell(double *__restrict__ rho, int key, co
 }
 
 // ---- S4+S5 deposit, mode 1 (default): block-local cell binning in shared memory + run accumulation ------------
-// A block owns chunks of 256*R consecutive particles (storage order).  The particles of a chunk are binned by cell
+// A block of NT threads owns chunks of NT*R consecutive particles (storage order); NT = 256, R = 8 measured best on B200
+// (10-step mean on 4A: 256x8 131 us, 128x8 134, 256x4 134, 512x4 140, 512x8 152, 1024x4 164: block barriers over many
+// warps cost more than the extra warps hide).  The particles of a chunk are binned by cell
 // INSIDE the block (counting sort over the chunk's bounding box of cells: one shared-memory integer atomic per
 // particle gives count and rank at once, a block scan gives the offsets), so that afterwards every thread walks R
 // entries of the cell-ordered list and sums same-cell particles in registers; a run is flushed with 8 RED.E.ADD.F64
@@ -79,7 +81,6 @@ __device__ __forceinline__ void flush_cell(double *__restrict__ rho, int key, co
 // 32-byte sectors (measured: 0.6-0.8 SM-cycles per RED lane against 1.55 for scattered sectors).
 // A chunk whose box exceeds kBinCap cells (unsorted input, the thin tails of the bunch) takes the direct path:
 // per-lane runs in storage order, as in mode 1.  Weights are the canonical R11 expression on every path.
-constexpr int kBinBlock = 256;
 constexpr int kBinCap = 4096;  // cells of the chunk's bounding box that the shared histogram can hold
 
 // merge the lanes' open runs (segmented suffix reduction over CONTIGUOUS equal keys), heads flush
@@ -107,17 +108,23 @@ __device__ __forceinline__ void merge_and_flush(double *__restrict__ rho, int cu
     if (head) flush_cell<NW>(rho, cur, acc, nx, nxy);
 }
 
-template <int R>
+template <int NT, int R>
 struct BinSmem {
-    static constexpr int CH = kBinBlock * R;
+    static constexpr int CH = NT * R;
     static constexpr int PAD = CH + CH / 8;  // one pad slot per 8 entries: a thread's R-entry walk is conflict-free
     alignas(16) int hist[kBinCap + 16];      // bins [0, ncell) = cells of the box, bin kBinCap = particles that are not binned
     int box[2][8];  // imin, jmin, kmin, imax, jmax, kmax, lowest thread holding an inside particle; double-buffered by chunk parity
     int anchor[4];
-    int warp_tot[kBinBlock / 32];
+    int warp_tot[NT / 32];
     int key[PAD];
     double w1[3][PAD];
 };
+
+// register budget per thread: 128 for 8 particles per thread or 27 run accumulators, else 80 (64 in blocks of >= 512 threads)
+template <int NT, int R, int ORDER>
+constexpr int kBinRegs = (R >= 8 || ORDER > 1) ? 128 : (NT >= 512 ? 64 : 80);
+template <int NT, int R, int ORDER>
+constexpr int kBinMinBlocks = (65536 / NT) / kBinRegs<NT, R, ORDER> > 0 ? (65536 / NT) / kBinRegs<NT, R, ORDER> : 1;
 
 template <int NW>
 __device__ __forceinline__ void run_add(double *__restrict__ rho, int key, const double (&w)[NW * NW * NW], int &cur,
@@ -133,13 +140,14 @@ __device__ __forceinline__ void run_add(double *__restrict__ rho, int key, const
     }
 }
 
-template <int R, bool VEC, int ORDER>
-__global__ void __launch_bounds__(kBinBlock, (R >= 8 || ORDER > 1) ? 2 : 3) deposit_binned_kernel(const double *__restrict__ x, const double *__restrict__ y,
+template <int NT, int R, bool VEC, int ORDER>
+__global__ void __launch_bounds__(NT, kBinMinBlocks<NT, R, ORDER>) deposit_binned_kernel(const double *__restrict__ x, const double *__restrict__ y,
                                                                    const double *__restrict__ t, long long n, GridDev g, double qw,
                                                                    double zscale, double *__restrict__ rho) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    BinSmem<R> &sm = *reinterpret_cast<BinSmem<R> *>(smem_raw);
-    constexpr int CH = BinSmem<R>::CH;
+    BinSmem<NT, R> &sm = *reinterpret_cast<BinSmem<NT, R> *>(smem_raw);
+    constexpr int CH = BinSmem<NT, R>::CH;
+    constexpr int BPT = kBinCap / NT;  // histogram bins per thread in the scan (a multiple of 4)
     constexpr int NW = ORDER + 1, NN = NW * NW * NW;
     constexpr int kBig = 0x7fffffff;
     const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
@@ -195,7 +203,7 @@ __global__ void __launch_bounds__(kBinBlock, (R >= 8 || ORDER > 1) ? 2 : 3) depo
         const int ncell = big ? kBinCap : bx * by * bz;
         {
             const int zr = (ncell + 15) & ~15;  // the scan's 16-entry granules
-            for (int s4 = tid * 4; s4 < zr; s4 += kBinBlock * 4) *reinterpret_cast<int4 *>(&sm.hist[s4]) = make_int4(0, 0, 0, 0);
+            for (int s4 = tid * 4; s4 < zr; s4 += NT * 4) *reinterpret_cast<int4 *>(&sm.hist[s4]) = make_int4(0, 0, 0, 0);
             if (tid == 0) sm.hist[kBinCap] = 0;  // spill bin: particles that are not binned (outside the grid / the box)
         }
         __syncthreads();  // (2) histogram cleared, anchor published
@@ -224,17 +232,17 @@ __global__ void __launch_bounds__(kBinBlock, (R >= 8 || ORDER > 1) ? 2 : 3) depo
 #pragma unroll
         for (int r = 0; r < R; ++r) rank[r] = atomicAdd(&sm.hist[lc[r]], 1);  // count and rank within the cell in one pass
         __syncthreads();  // (3) histogram complete
-        // exclusive scan of hist[0..ncell) in place: 16 consecutive bins per thread (4 x LDS.128), warp scan, block carry;
+        // exclusive scan of hist[0..ncell) in place: BPT consecutive bins per thread (LDS.128), warp scan, block carry;
         // the spill bin hist[kBinCap] is not part of it
         int total = 0;
         {
-            const int b0 = tid * 16;
+            const int b0 = tid * BPT;
             const bool act = b0 < ncell;
-            int4 v[4];
+            int4 v[BPT / 4];
             int s = 0;
             if (act) {
 #pragma unroll
-                for (int q = 0; q < 4; ++q) {
+                for (int q = 0; q < BPT / 4; ++q) {
                     v[q] = *reinterpret_cast<const int4 *>(&sm.hist[b0 + 4 * q]);
                     s += v[q].x + v[q].y + v[q].z + v[q].w;
                 }
@@ -249,14 +257,14 @@ __global__ void __launch_bounds__(kBinBlock, (R >= 8 || ORDER > 1) ? 2 : 3) depo
             __syncthreads();  // (4)
             int off = incl - s;
 #pragma unroll
-            for (int w = 0; w < kBinBlock / 32; ++w) {
+            for (int w = 0; w < NT / 32; ++w) {
                 const int wt = sm.warp_tot[w];
                 off += (w < wid) ? wt : 0;
                 total += wt;
             }
             if (act) {
 #pragma unroll
-                for (int q = 0; q < 4; ++q) {
+                for (int q = 0; q < BPT / 4; ++q) {
                     int4 o;
                     o.x = off, off += v[q].x;
                     o.y = off, off += v[q].y;
@@ -307,16 +315,16 @@ static int env_int_grid(const char *name, int dflt) {
     return (v && *v) ? atoi(v) : dflt;
 }
 
-template <int R, bool VEC, int ORDER>
+template <int NT, int R, bool VEC, int ORDER>
 static int launch_deposit_binned(Beam *b, Grid *g, const GridDev &gd, double q_weight, double zscale) {
-    const int smem = (int)sizeof(BinSmem<R>);
-    const long long nchunks = (b->n + BinSmem<R>::CH - 1) / BinSmem<R>::CH;
+    const int smem = (int)sizeof(BinSmem<NT, R>);
+    const long long nchunks = (b->n + BinSmem<NT, R>::CH - 1) / BinSmem<NT, R>::CH;
     int per_sm = 1;
-    BT_CUDA_TRY(cudaFuncSetAttribute(deposit_binned_kernel<R, VEC, ORDER>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
-    BT_CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, deposit_binned_kernel<R, VEC, ORDER>, kBinBlock, smem));
+    BT_CUDA_TRY(cudaFuncSetAttribute(deposit_binned_kernel<NT, R, VEC, ORDER>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+    BT_CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, deposit_binned_kernel<NT, R, VEC, ORDER>, NT, smem));
     long long blocks = (long long)b->num_sms * (per_sm > 0 ? per_sm : 1);
     if (blocks > nchunks) blocks = nchunks;
-    deposit_binned_kernel<R, VEC, ORDER><<<(int)blocks, kBinBlock, smem, b->stream>>>(b->q[0], b->q[2], b->q[4], b->n, gd, q_weight,
+    deposit_binned_kernel<NT, R, VEC, ORDER><<<(int)blocks, NT, smem, b->stream>>>(b->q[0], b->q[2], b->q[4], b->n, gd, q_weight,
                                                                                      zscale, g->rho);
     return BT_OK;
 }
@@ -337,11 +345,11 @@ static int launch_deposit_order(Beam *b, Grid *g, const GridDev &gd, double q_we
     }
     if constexpr (ORDER == 1) {
         if (mode != 2)
-            return b->aligned32 ? launch_deposit_binned<8, true, ORDER>(b, g, gd, q_weight, zscale)
-                                : launch_deposit_binned<8, false, ORDER>(b, g, gd, q_weight, zscale);
+            return b->aligned32 ? launch_deposit_binned<256, 8, true, ORDER>(b, g, gd, q_weight, zscale)
+                                : launch_deposit_binned<256, 8, false, ORDER>(b, g, gd, q_weight, zscale);
     }
-    return b->aligned32 ? launch_deposit_binned<4, true, ORDER>(b, g, gd, q_weight, zscale)
-                        : launch_deposit_binned<4, false, ORDER>(b, g, gd, q_weight, zscale);
+    return b->aligned32 ? launch_deposit_binned<256, 4, true, ORDER>(b, g, gd, q_weight, zscale)
+                        : launch_deposit_binned<256, 4, false, ORDER>(b, g, gd, q_weight, zscale);
 }
 
 int launch_deposit(Beam *b, Grid *g, double q_weight, double zscale) {
