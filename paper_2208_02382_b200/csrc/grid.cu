@@ -154,6 +154,7 @@ __global__ void __launch_bounds__(NT, kBinMinBlocks<NT, R, ORDER>) deposit_binne
     const long long nxy = (long long)g.nx * g.ny;
     const long long nchunks = (n + CH - 1) / CH;
     if (tid < 8) sm.box[0][tid] = (tid >= 3 && tid < 6) ? -1 : kBig;
+    for (int s4 = tid * 4; s4 < kBinCap + 16; s4 += NT * 4) *reinterpret_cast<int4 *>(&sm.hist[s4]) = make_int4(0, 0, 0, 0);
     __syncthreads();
     int parity = 0;
     for (long long ch = blockIdx.x; ch < nchunks; ch += gridDim.x, parity ^= 1) {
@@ -195,19 +196,14 @@ __global__ void __launch_bounds__(NT, kBinMinBlocks<NT, R, ORDER>) deposit_binne
         // A chunk that is not spatially compact (unsorted input, the thin tails): bin what falls into a fixed 16^3 box
         // around the first inside particle -- this catches a cold core even in unsorted order -- the rest goes direct.
         const bool big = (long long)bx * by * bz > kBinCap;
-        if (big && tid == box[6]) {
-#pragma unroll
-            for (int r = R - 1; r >= 0; --r)
-                if (in[r]) sm.anchor[0] = c[r].i, sm.anchor[1] = c[r].j, sm.anchor[2] = c[r].k;
-        }
         const int ncell = big ? kBinCap : bx * by * bz;
-        {
-            const int zr = (ncell + 15) & ~15;  // the scan's 16-entry granules
-            for (int s4 = tid * 4; s4 < zr; s4 += NT * 4) *reinterpret_cast<int4 *>(&sm.hist[s4]) = make_int4(0, 0, 0, 0);
-            if (tid == 0) sm.hist[kBinCap] = 0;  // spill bin: particles that are not binned (outside the grid / the box)
-        }
-        __syncthreads();  // (2) histogram cleared, anchor published
-        if (big) {
+        if (big) {  // block-uniform; compact chunks skip this barrier (the histogram was cleared during the previous walk)
+            if (tid == box[6]) {
+#pragma unroll
+                for (int r = R - 1; r >= 0; --r)
+                    if (in[r]) sm.anchor[0] = c[r].i, sm.anchor[1] = c[r].j, sm.anchor[2] = c[r].k;
+            }
+            __syncthreads();  // (2) anchor published
             i0 = sm.anchor[0] - 8, j0 = sm.anchor[1] - 8, k0 = sm.anchor[2] - 8;
             bx = by = bz = 16;
         }
@@ -286,6 +282,8 @@ __global__ void __launch_bounds__(NT, kBinMinBlocks<NT, R, ORDER>) deposit_binne
                 sm.w1[2][slot] = c[r].wz1;
             }
         __syncthreads();  // (6) cell-ordered entry list complete
+        // the histogram is dead from here on: clear it for the next chunk (whose first access follows its barrier (1))
+        for (int s4 = tid * 4; s4 < kBinCap + 16; s4 += NT * 4) *reinterpret_cast<int4 *>(&sm.hist[s4]) = make_int4(0, 0, 0, 0);
         {
             int cur = -1;
             double acc[NN];
