@@ -251,6 +251,15 @@ int bt_gather_kick(bt_beam *beam, const bt_grid *grid, const double coef[3], dou
  */
 int bt_beam_moments(bt_beam *beam, double host_mean[6], double host_cov[36]);
 
+/*
+ * Element-step diagnostics (mirrors sim.set_slice_step_diagnostics(True), P:l.61, at element granularity): the same walk
+ * as bt_track(nturns) -- bit-identical final coordinates, reference energy, s and turn -- but one launch per element, each
+ * followed by bt_beam_moments.  host_moments receives nturns * n_elems records of 42 doubles (mean[6], then cov[36] row-major)
+ * in walk order: record (turn * n_elems + e) is the beam right after element e of that turn.  Costs 144 bytes of HBM
+ * traffic per particle and element instead of 96 per call, and synchronises after every element: a diagnostics mode.
+ */
+int bt_track_diagnostics(bt_beam *beam, int32_t nturns, double *host_moments);
+
 /* ---- utilities ------------------------------------------------------------------------------ */
 int bt_sync(bt_beam *beam); /* cudaStreamSynchronize on the beam's stream */
 const char *bt_last_error(void);

@@ -489,6 +489,40 @@ int bt_track(bt_beam *beam, int32_t nturns) {
     return BT_OK;
 }
 
+// Element-step diagnostics (P:l.61 set_slice_step_diagnostics; SURVEY 8(f) NEXT-1 "callable between elements"): the same walk,
+// one launch per element, with the beam statistics taken after every element.
+int bt_track_diagnostics(bt_beam *beam, int32_t nturns, double *host_moments) {
+    if (!beam || !host_moments) return fail(BT_ERR_INVALID, "bt_track_diagnostics: NULL argument");
+    if (nturns < 0) return fail(BT_ERR_INVALID, "bt_track_diagnostics: nturns < 0");
+    Beam &b = beam->b;
+    if (b.lattice.empty()) return fail(BT_ERR_STATE, "bt_track_diagnostics: bt_lattice_set not called");
+    if (!b.has_ref) return fail(BT_ERR_STATE, "bt_track_diagnostics: bt_beam_set_ref not called");
+    std::vector<bt_element> one(1);
+    std::vector<DevOp> ops;
+    double *out = host_moments;
+    for (int32_t t = 0; t < nturns; ++t) {
+        for (size_t e = 0; e < b.lattice.size(); ++e) {
+            one[0] = b.lattice[e];
+            ops.clear();
+            double slots = 0.0;
+            const double gamma_after = build_turn_table(one, b.gamma, ops, &slots);
+            for (size_t lo = 0; lo < ops.size(); lo += (size_t)kConstTableRecords) {
+                const size_t len = ops.size() - lo < (size_t)kConstTableRecords ? ops.size() - lo : (size_t)kConstTableRecords;
+                const int rc = launch_track(&b, ops.data() + lo, (int32_t)len, 1, next_table_version(), slots / (double)ops.size());
+                if (rc != BT_OK) return rc;
+            }
+            b.gamma = gamma_after;
+            b.s += b.lattice[e].ds;
+            const int rc = launch_moments(&b, out, out + 6);
+            if (rc != BT_OK) return rc;
+            out += 42;
+        }
+        b.turn += 1;
+    }
+    b.table_valid = false;  // the constant bank no longer holds this beam's whole-lattice table
+    return BT_OK;
+}
+
 // Host-to-host walk: chunks of the bunch ride three streams, so that the H2D copy of chunk k+1, the walk of chunk k and
 // the D2H copy of chunk k-1 overlap (PCIe is full duplex; particles are independent, so any partition is exact).
 int bt_track_host(bt_beam *beam, const double *const host_in[6], double *const host_out[6], int32_t nturns, int32_t nchunks) {

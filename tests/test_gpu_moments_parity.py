@@ -103,3 +103,36 @@ def test_moments_argument_errors():
     assert bt.lib.bt_beam_moments(beam._h, None, None) == bt.BT_ERR_INVALID
     assert bt.lib.bt_beam_moments(None, None, None) == bt.BT_ERR_INVALID
     beam.close()
+
+
+@pytest.mark.parametrize("idx", [0, 3])
+def test_track_diagnostics_moments_after_every_element(idx):
+    """bt_track_diagnostics: final state bit-identical to bt_track; every per-element record equals the oracle's moments of
+    the oracle's bunch at that point of the walk (config 0: FODO cell; config 3: ring with kicks and an RF cavity)."""
+    cfg = W.config(idx, n=20_000)
+    lat = cfg.lattice if idx == 0 else cfg.lattice[:16] + cfg.lattice[-1:]
+    nturns = 2
+    c = W.make_bunch(cfg)
+    beam = bt.Beam(cfg.n)
+    beam.set_ref(cfg.kin_energy_MeV, cfg.mass_MeV, cfg.charge_qe)
+    beam.lattice_set(lat)
+    beam.upload(c)
+    beam.track(nturns)
+    plain, ref_state = beam.download(), beam.get_ref()
+    beam.set_ref(cfg.kin_energy_MeV, cfg.mass_MeV, cfg.charge_qe)
+    beam.upload(c)
+    mean, cov = beam.track_diagnostics(nturns, len(lat))
+    got = beam.download()
+    for a, b in zip(got, plain):
+        assert np.array_equal(a, b)
+    assert beam.get_ref() == ref_state
+    ref = [a.copy() for a in c]
+    g = O.ref_from_kinetic(cfg.kin_energy_MeV, cfg.mass_MeV)[0]
+    for t in range(nturns):
+        for e, el in enumerate(lat):
+            g, _ = O.track(ref, [el], 1, g)
+            rm, rc = O.moments(ref)
+            sig = np.sqrt(np.diag(rc))
+            assert np.max(np.abs(cov[t, e] - rc) / np.outer(sig, sig)) <= 1e-11, (t, e)
+            assert np.all(np.abs(mean[t, e] - rm) <= 1e-11 * sig + 1e-15 * np.abs(rm)), (t, e)
+    beam.close()
