@@ -420,7 +420,12 @@ def run_ours(args):
         bound = "alu" if alu_time_ms >= hbm_time_ms else "hbm"
         if bound == "alu":
             roof = {"bound": "alu", "achieved": achieved / 1e12, "peak": nominal_peak / 1e12, "unit": "Tslot/s",
-                    "frac": achieved / nominal_peak, "traffic": None,
+                    "frac": achieved / nominal_peak,
+                    # dram__bytes_read.sum + dram__bytes_write.sum of one launch on configs[1] from the ncu --set full capture in
+                    # profiles/r01_summary.md (48.0 MB read + 1.1 MB written: the 48 MB result stays in the 126 MB L2);
+                    # algorithmic bytes 96 B/particle = 96 MB per launch.  null for any other workload (not captured).
+                    "traffic": 49.1e6 if (args.workload == "fodo_channel" and n == 1_000_000) else None,
+                    "traffic_unit": "bytes per launch (ncu, profiles/r01_summary.md)",
                     "peak_kind": "derived: 148 SMs x 64 FP64 lanes x %s sm_max_mhz (DESIGN.md s7)" % peaks_kind,
                     "peak_measured_dfma_chain": measured_fp64 / 1e12, "frac_of_measured_dfma_chain": achieved / measured_fp64,
                     "slots_per_particle": slots_pp, "tflops": None}
