@@ -71,16 +71,17 @@ __device__ __forceinline__ void flush_cell(double *__restrict__ rho, int key, co
 // A block of NT threads owns chunks of NT*R consecutive particles (storage order); NT = 256, R = 8 measured best on B200
 // (10-step mean on 4A: 256x8 131 us, 128x8 134, 256x4 134, 512x4 140, 512x8 152, 1024x4 164: block barriers over many
 // warps cost more than the extra warps hide).  The particles of a chunk are binned by cell
-// INSIDE the block (counting sort over the chunk's bounding box of cells: one shared-memory integer atomic per
-// particle gives count and rank at once, a block scan gives the offsets), so that afterwards every thread walks R
+// INSIDE the block (counting sort over the chunk's bounding box of cells: one shared-memory integer atomic per run of
+// same-cell particles of a thread gives count and rank at once, a block scan gives the offsets), so that afterwards every thread walks R
 // entries of the cell-ordered list and sums same-cell particles in registers; a run is flushed with 8 RED.E.ADD.F64
 // when the cell changes, and the lanes' open runs are merged by a segmented shuffle reduction first.  Global
 // reductions per chunk = 8 x (distinct cells + warp seams) instead of 8 x particles, for ANY order in which a chunk
 // is spatially compact (bt_beam_sort_by_cell once, then many drift/kick steps: particles wander a few cells, the
 // chunk's box stays small).  Consecutive lanes flush x-adjacent cells, so the REDs of one instruction share
 // 32-byte sectors (measured: 0.6-0.8 SM-cycles per RED lane against 1.55 for scattered sectors).
-// A chunk whose box exceeds kBinCap cells (unsorted input, the thin tails of the bunch) takes the direct path:
-// per-lane runs in storage order, as in mode 1.  Weights are the canonical R11 expression on every path.
+// A chunk whose box exceeds kBinCap cells (unsorted input, the thin tails of the bunch) bins what falls into a fixed 16^3
+// box around its first inside particle and sends the rest straight to RED.  Weights are the canonical R11 / R16
+// expression on every path.
 constexpr int kBinCap = 4096;  // cells of the chunk's bounding box that the shared histogram can hold
 
 // merge the lanes' open runs (segmented suffix reduction over CONTIGUOUS equal keys), heads flush
