@@ -562,11 +562,187 @@ static int launch_gather_pipe(Beam *b, const GatherArgs &a0) {
     return BT_OK;
 }
 
+// ---- S6/S7, streaming pipeline with the chunk's field tile staged in shared memory ---------------------------------
+// B:north_star's gather: "stages the field tile in shared memory".  Same particle pipeline as gather_kick_pipe_kernel
+// (bulk copies in, in-place update, bulk copies out); in addition the block finds the bounding box of its chunk's stencils
+// (warp REDUX + shared atomics), loads the box's node records ONCE, coalesced row by row, into three planar shared arrays
+// (Ex, Ey, Ez: 24 bytes per node, no pad) and every particle then reads its (ORDER+1)^3 nodes with LDS.64.  Why it pays:
+// the L1 -> register return path delivers ~64 B/clk/SM and every lane needs its own copy of every node record
+// ((ORDER+1)^3 x 32 B per particle: 864 B at order 2, where the L1 path is flat at 0.23 of the HBM bound even when all
+// lanes read the same records), while shared memory returns 128 B/clk and lanes that share a node are served by one
+// broadcast wavefront.  A chunk whose box exceeds kTileCap nodes (unsorted input, thin tails) reads through L1 as before.
+constexpr int kTileCap = 1280;  // nodes: 30 KiB of shared memory; a drifted 256-particle chunk of configs[4] needs ~1200 at order 2
+
+template <int CH>
+struct GtSmem {
+    alignas(128) double q[kGpStages][6][CH];
+    alignas(16) double tile[3][kTileCap];
+    int box[2][8];
+    alignas(8) uint64_t full[kGpStages];
+};
+
+template <int ORDER>
+__global__ void __launch_bounds__(256, 3) gather_kick_tile_kernel(const __grid_constant__ GatherArgs a, long long nchunks, int store_positions) {
+    constexpr int NT = 256, CH = 256, NW = ORDER + 1;
+    constexpr uint32_t kArrBytes = CH * sizeof(double);
+    constexpr int kBig = 0x7fffffff;
+    extern __shared__ __align__(128) unsigned char gt_smem_raw[];
+    GtSmem<CH> &sm = *reinterpret_cast<GtSmem<CH> *>(gt_smem_raw);
+    const int tid = threadIdx.x, lane = tid & 31;
+    const auto issue_load = [&](long long ch, int s) {
+        mbar_expect_tx(&sm.full[s], 6 * kArrBytes);
+#pragma unroll
+        for (int c = 0; c < 6; ++c) bulk_g2s(sm.q[s][c], a.q[c] + ch * CH, kArrBytes, &sm.full[s]);
+    };
+    if (tid == 0) {
+#pragma unroll
+        for (int s = 0; s < kGpStages; ++s) mbar_init(&sm.full[s], 1);
+        mbar_init_fence();
+        if ((long long)blockIdx.x < nchunks) issue_load(blockIdx.x, 0);
+        if ((long long)blockIdx.x + gridDim.x < nchunks) issue_load((long long)blockIdx.x + gridDim.x, 1);
+    }
+    if (tid < 8) sm.box[0][tid] = (tid >= 3 && tid < 6) ? -1 : kBig;
+    __syncthreads();
+    int s = 0, bpar = 0;
+    uint32_t parity = 0;
+    for (long long ch = blockIdx.x; ch < nchunks; ch += gridDim.x, bpar ^= 1) {
+        mbar_wait(&sm.full[s], parity);
+        double(*q)[CH] = sm.q[s];
+        int *box = sm.box[bpar];
+        double x = q[0][tid], px = q[1][tid], y = q[2][tid], py = q[3][tid], t = q[4][tid], pt = q[5][tid];
+        // R4 drift before the kick
+        x = fma(a.hb, px, x);
+        y = fma(a.hb, py, y);
+        t = fma(a.tcb, pt, t);
+        Cic c;
+        const bool in = shape_locate<ORDER>(a.g, x, y, t, a.zscale, c);
+        {   // bounding box of the chunk's stencil bases
+            int lo_i = in ? c.i : kBig, lo_j = in ? c.j : kBig, lo_k = in ? c.k : kBig;
+            int hi_i = in ? c.i : -1, hi_j = in ? c.j : -1, hi_k = in ? c.k : -1;
+            lo_i = __reduce_min_sync(0xffffffffu, lo_i), hi_i = __reduce_max_sync(0xffffffffu, hi_i);
+            lo_j = __reduce_min_sync(0xffffffffu, lo_j), hi_j = __reduce_max_sync(0xffffffffu, hi_j);
+            lo_k = __reduce_min_sync(0xffffffffu, lo_k), hi_k = __reduce_max_sync(0xffffffffu, hi_k);
+            if (lane == 0 && hi_i >= 0) {
+                atomicMin(&box[0], lo_i), atomicMin(&box[1], lo_j), atomicMin(&box[2], lo_k);
+                atomicMax(&box[3], hi_i), atomicMax(&box[4], hi_j), atomicMax(&box[5], hi_k);
+            }
+        }
+        __syncthreads();  // (1) box complete
+        if (tid < 8) sm.box[bpar ^ 1][tid] = (tid >= 3 && tid < 6) ? -1 : kBig;  // next chunk's box
+        const int i0 = box[0], j0 = box[1], k0 = box[2];
+        const int tx = box[3] - i0 + NW, ty = box[4] - j0 + NW, tz = box[5] - k0 + NW;  // nodes per axis of the tile
+        const bool staged = box[3] >= 0 && (long long)tx * ty * tz <= kTileCap;  // block-uniform
+        if (staged) {
+            // rows of tx consecutive node records (x fastest): 16 lanes per row, 16 rows per sweep
+            const int rows = ty * tz;
+            for (int row = tid >> 4; row < rows; row += NT / 16) {
+                const int iz = row / ty, iy = row - iz * ty;
+                const double *src = a.field + 4 * ((((long long)(k0 + iz)) * a.g.ny + (j0 + iy)) * a.g.nx + i0);
+                for (int xx = tid & 15; xx < tx; xx += 16) {
+                    double fx, fy, fz;
+                    ld_node(src + 4 * xx, fx, fy, fz);
+                    const int idx = row * tx + xx;
+                    sm.tile[0][idx] = fx, sm.tile[1][idx] = fy, sm.tile[2][idx] = fz;
+                }
+            }
+        }
+        __syncthreads();  // (2) tile staged
+        if (in) {
+            double wx[NW], wy[NW], wz[NW];
+            axis_weights<ORDER>(c.wx1, wx);
+            axis_weights<ORDER>(c.wy1, wy);
+            axis_weights<ORDER>(c.wz1, wz);
+            double ex = 0.0, ey = 0.0, ez = 0.0;
+            if (staged) {
+                const int base = ((c.k - k0) * ty + (c.j - j0)) * tx + (c.i - i0);
+#pragma unroll
+                for (int dz = 0; dz < NW; ++dz)
+#pragma unroll
+                    for (int dy = 0; dy < NW; ++dy)
+#pragma unroll
+                        for (int dx = 0; dx < NW; ++dx) {
+                            const double w = __dmul_rn(__dmul_rn(wx[dx], wy[dy]), wz[dz]);
+                            const int idx = base + (dz * ty + dy) * tx + dx;
+                            ex = fma(w, sm.tile[0][idx], ex);
+                            ey = fma(w, sm.tile[1][idx], ey);
+                            ez = fma(w, sm.tile[2][idx], ez);
+                        }
+            } else {
+                const double *gbase = a.field + 4 * (((long long)c.k * a.g.ny + c.j) * a.g.nx + c.i);
+#pragma unroll
+                for (int dz = 0; dz < NW; ++dz)
+#pragma unroll
+                    for (int dy = 0; dy < NW; ++dy)
+#pragma unroll
+                        for (int dx = 0; dx < NW; ++dx) {
+                            const double w = __dmul_rn(__dmul_rn(wx[dx], wy[dy]), wz[dz]);
+                            double fx, fy, fz;
+                            ld_node(gbase + 4 * (((long long)dz * a.g.ny + dy) * a.g.nx + dx), fx, fy, fz);
+                            ex = fma(w, fx, ex);
+                            ey = fma(w, fy, ey);
+                            ez = fma(w, fz, ez);
+                        }
+            }
+            px = fma(a.coef[0], ex, px);
+            py = fma(a.coef[1], ey, py);
+            pt = fma(a.coef[2], ez, pt);
+        }
+        // R4 drift after the kick
+        x = fma(a.ha, px, x);
+        y = fma(a.ha, py, y);
+        t = fma(a.tca, pt, t);
+        q[0][tid] = x, q[1][tid] = px, q[2][tid] = y, q[3][tid] = py, q[4][tid] = t, q[5][tid] = pt;
+        fence_proxy_async_smem();  // this thread's shared-memory writes -> visible to the copy engine
+        __syncthreads();           // (3) stage complete; everyone is done with the tile
+        if (tid == 0) {
+#pragma unroll
+            for (int cc = 0; cc < 6; ++cc)
+                if (store_positions || (cc & 1)) bulk_s2g(a.q[cc] + ch * CH, sm.q[s][cc], kArrBytes);
+            bulk_commit();
+            const long long nxt = ch + 2LL * gridDim.x;
+            if (nxt < nchunks) {
+                bulk_wait_read<1>();
+                issue_load(nxt, (s + 2) % kGpStages);
+            }
+        }
+        if (++s == kGpStages) s = 0, parity ^= 1;
+    }
+    if (tid == 0) bulk_wait_all<0>();  // shared memory must outlive the last stores
+}
+
+template <int ORDER>
+static int launch_gather_tile(Beam *b, const GatherArgs &a0) {
+    constexpr int CH = 256;
+    const int smem = (int)sizeof(GtSmem<CH>);
+    const long long nchunks = b->n / CH;
+    if (nchunks > 0) {
+        int per_sm = 1;
+        BT_CUDA_TRY(cudaFuncSetAttribute(gather_kick_tile_kernel<ORDER>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+        BT_CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, gather_kick_tile_kernel<ORDER>, 256, smem));
+        long long blocks = (long long)b->num_sms * (per_sm > 0 ? per_sm : 1);
+        if (blocks > nchunks) blocks = nchunks;
+        const int store_positions = (a0.hb != 0.0 || a0.ha != 0.0 || a0.tcb != 0.0 || a0.tca != 0.0) ? 1 : 0;
+        gather_kick_tile_kernel<ORDER><<<(int)blocks, 256, smem, b->stream>>>(a0, nchunks, store_positions);
+    }
+    const long long done = nchunks * CH;
+    if (done < b->n) {  // ragged tail: one particle per thread
+        GatherArgs t = a0;
+        for (int c = 0; c < 6; ++c) t.q[c] = a0.q[c] + done;
+        t.n = b->n - done;
+        gather_kick_kernel<ORDER><<<(int)((t.n + 255) / 256), 256, 0, b->stream>>>(t);
+    }
+    return BT_OK;
+}
+
 template <int ORDER>
 static int launch_gather_order(Beam *b, const GatherArgs &a) {
     // BT_GATHER_MODE: 0 = one particle per thread, everything through registers (also the path for arrays that are not
-    // 16-byte aligned); 1 (default) = streaming pipeline, 256-particle chunks; 2 / 3 = pipeline with 512 / 128-particle chunks
+    // 16-byte aligned); 1 (default) = streaming pipeline, 256-particle chunks, field through L1 (order 1) or staged in shared
+    // memory (order 2); 2 / 3 = L1 pipeline with 512 / 128-particle chunks; 4 = shared-memory tile at any order
     const int mode = env_int_grid("BT_GATHER_MODE", 1);
+    // field tile staged in shared memory: the default at order 2 (measured 4A 10-step mean 547 -> 477 us, 4B 529 -> 430 us),
+    // selectable at order 1 (BT_GATHER_MODE=4), where the L1 path is faster (181 against 216 us)
+    if ((mode == 4 || (mode == 1 && ORDER == 2)) && b->aligned16) return launch_gather_tile<ORDER>(b, a);
     if (mode >= 1 && b->aligned16)
         return mode == 2 ? launch_gather_pipe<512, 1, ORDER>(b, a) : mode == 3 ? launch_gather_pipe<128, 1, ORDER>(b, a) : launch_gather_pipe<256, 1, ORDER>(b, a);
     const int block = 256;
