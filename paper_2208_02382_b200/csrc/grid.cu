@@ -742,7 +742,9 @@ static int launch_gather_order(Beam *b, const GatherArgs &a) {
     const int mode = env_int_grid("BT_GATHER_MODE", 1);
     // field tile staged in shared memory: the default at order 2 (measured 4A 10-step mean 547 -> 477 us, 4B 529 -> 430 us),
     // selectable at order 1 (BT_GATHER_MODE=4), where the L1 path is faster (181 against 216 us)
-    if ((mode == 4 || (mode == 1 && ORDER == 2)) && b->aligned16) return launch_gather_tile<ORDER>(b, a);
+    // only on cell-sorted beams: in the caller's order no chunk's box fits the tile and the pass through L1 is faster from
+    // the plain pipeline (order 2, unsorted kick: 0.79 against 1.51 ms)
+    if ((mode == 4 || (mode == 1 && ORDER == 2 && b->permuted)) && b->aligned16) return launch_gather_tile<ORDER>(b, a);
     if (mode >= 1 && b->aligned16)
         return mode == 2 ? launch_gather_pipe<512, 1, ORDER>(b, a) : mode == 3 ? launch_gather_pipe<128, 1, ORDER>(b, a) : launch_gather_pipe<256, 1, ORDER>(b, a);
     const int block = 256;
