@@ -449,6 +449,18 @@ def run_ours(args):
         cpu_baseline = {"value": cb_pushes / cb_t, "unit": UNIT, "cores": cores, "kind": "oracle",
                         "sample": "%d of %d particles, full lattice (%d slice maps), %d turn(s); %d repetitions, %.1f s of CPU work in total"
                                   % (n_cb, n, cfg.slice_maps_per_turn, cfg.nturns, len(cb_times), sum(cb_times))}
+        # the same oracle on ONE thread (SURVEY 8d asks for both), on a smaller sample of the same workload (~3 s)
+        try:
+            import oracle as _O
+            nthr = _O.num_threads()
+            _O.set_num_threads(1)
+            n_st = min(n_cb, 100_000)
+            st_pushes, st_times, _ = oracle_rate(cb_cfg, n_st)
+            _O.set_num_threads(nthr)
+            cpu_baseline["single_thread"] = {"value": st_pushes / st_times[0], "unit": UNIT, "cores": 1,
+                                             "sample": "%d of %d particles, full lattice, %d turn(s), one run" % (n_st, n, cfg.nturns)}
+        except Exception as exc:  # the all-cores number above is the contract; this one is extra
+            cpu_baseline["single_thread"] = {"unavailable": repr(exc)}
         extras = {}
         if world == 1 and not args.no_extras:
             extras["other_configs"] = bench_other_configs(bt, torch, flush, peaks, nominal_peak)
