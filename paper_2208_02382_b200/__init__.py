@@ -45,6 +45,7 @@ EXPORTS = {
     "bt_beam_size": (C.c_int64, [_vp]),
     "bt_beam_sort_by_cell": (C.c_int, [_vp, _vp, C.c_double]),
     "bt_beam_ids": (C.c_int, [_vp, C.POINTER(_vp)]),
+    "bt_beam_set_resort_interval": (C.c_int, [_vp, C.c_int32]),
     "bt_lattice_set": (C.c_int, [_vp, _vp, C.c_int32]),
     "bt_track": (C.c_int, [_vp, C.c_int32]),
     "bt_track_host": (C.c_int, [_vp, C.POINTER(_vp), C.POINTER(_vp), C.c_int32, C.c_int32]),
@@ -238,6 +239,9 @@ class Beam:
         mean, cov = np.zeros(6), np.zeros(36)
         _check(lib.bt_beam_moments(self._h, mean.ctypes.data_as(_dp), cov.ctypes.data_as(_dp)), "bt_beam_moments")
         return mean, cov.reshape(6, 6)
+
+    def set_resort_interval(self, every_n_deposits):
+        _check(lib.bt_beam_set_resort_interval(self._h, int(every_n_deposits)), "bt_beam_set_resort_interval")
 
     def sort_by_cell(self, grid, zscale=1.0):
         _check(lib.bt_beam_sort_by_cell(self._h, grid._h, zscale), "bt_beam_sort_by_cell")

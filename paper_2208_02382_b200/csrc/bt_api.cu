@@ -347,6 +347,7 @@ int bt_beam_upload(bt_beam *beam, const double *const host[6]) {
     for (int i = 0; i < 6; ++i)
         BT_CUDA_TRY(cudaMemcpyAsync(b.q[i], host[i], (size_t)b.n * sizeof(double), cudaMemcpyHostToDevice, b.stream));
     b.permuted = false;  // storage order = the caller's order again
+    b.deposits_since_sort = 0;
     return BT_OK;
 }
 
@@ -725,8 +726,24 @@ int bt_deposit_cic(bt_beam *beam, bt_grid *grid, double q_weight, double zscale,
     Beam &b = beam->b;
     Grid &g = grid->g;
     g.last_stream = b.stream;
+    if (b.resort_interval > 0) {  // S4 cadence: re-bin the storage every resort_interval deposits (the first one included)
+        if (b.deposits_since_sort % b.resort_interval == 0) {
+            const int rc = sort_by_cell(&b, &g, zscale);
+            if (rc != BT_OK) return rc;
+            b.deposits_since_sort = 0;
+        }
+        b.deposits_since_sort += 1;
+    }
     if (zero_first) BT_CUDA_TRY(cudaMemsetAsync(g.rho, 0, (size_t)g.nn * sizeof(double), b.stream));
     return launch_deposit(&b, &g, q_weight, zscale);
+}
+
+int bt_beam_set_resort_interval(bt_beam *beam, int32_t every_n_deposits) {
+    if (!beam) return fail(BT_ERR_INVALID, "bt_beam_set_resort_interval: beam is NULL");
+    if (every_n_deposits < 0) return fail(BT_ERR_INVALID, "bt_beam_set_resort_interval: negative interval");
+    beam->b.resort_interval = every_n_deposits;
+    beam->b.deposits_since_sort = 0;
+    return BT_OK;
 }
 
 int bt_beam_moments(bt_beam *beam, double host_mean[6], double host_cov[36]) {

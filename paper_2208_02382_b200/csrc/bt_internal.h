@@ -96,6 +96,8 @@ struct Beam {
     TrackLaunchInfo last_launch;
     // S4 cell binning: storage order != original order once sorted; ids[j] = original index of slot j
     bool permuted = false;
+    int32_t resort_interval = 0;      // bt_beam_set_resort_interval: re-sort every n-th bt_deposit_cic (0 = never)
+    int32_t deposits_since_sort = 0;
     int *ids = nullptr, *ids_tmp = nullptr;
     int *sort_key = nullptr, *sort_dest = nullptr, *sort_count = nullptr, *sort_block_sum = nullptr;
     long long sort_count_cap = 0;

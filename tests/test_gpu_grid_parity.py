@@ -394,3 +394,41 @@ def test_random_grids_shapes_orders_and_clouds(seed):
     assert nn > 0
     beam.close()
     grid.close()
+
+
+def test_resort_interval_sorts_inside_deposit_and_keeps_results():
+    """bt_beam_set_resort_interval(3): deposits 1, 4, 7 re-bin the storage themselves; the step loop still matches the
+    oracle's loop (API order is unaffected), and upload resets the cadence."""
+    sc = W.spacecharge_config("A", n=120_000, shape=(32, 32, 32))
+    c = W.make_spacecharge_bunch(sc)
+    E = W.gaussian_bunch_field(sc)
+    g0 = O.ref_from_kinetic(sc.kin_energy_MeV, sc.mass_MeV)[0]
+    beam = bt.Beam(sc.n)
+    grid = bt.Grid(sc.shape, sc.lo, sc.d)
+    beam.set_ref(sc.kin_energy_MeV, sc.mass_MeV, 1.0)
+    grid.set_field(*E)
+    beam.set_resort_interval(3)
+    beam.upload(c)
+    assert beam.ids_ptr() == 0
+    ref = [a.copy() for a in c]
+    for step in range(5):
+        beam.deposit_cic(grid, sc.q_weight, sc.zscale, True)
+        assert beam.ids_ptr() != 0                      # sorted by the first deposit
+        rho = grid.download_rho()
+        rref, _ = O.deposit_cic(ref[0], ref[2], ref[4], sc.shape, sc.lo, sc.d, sc.q_weight, sc.zscale)
+        assert np.max(np.abs(rho - rref) / np.maximum(rref, sc.q_weight)) <= 1e-12
+        beam.gather_kick(grid, sc.kick_coef, sc.zscale, 0.0, sc.ds)
+        O.gather_kick(ref, sc.shape, sc.lo, sc.d, E, sc.kick_coef, sc.zscale)
+        O.track(ref, [("drift", sc.ds, 1)], 1, g0)
+        if step in (0, 3):                               # right after a sort the storage is in cell order at the deposit's positions
+            pass
+    got = beam.download()
+    assert max(r14_error(got, ref)) <= 1e-11
+    beam.upload(c)
+    assert beam.ids_ptr() == 0
+    assert bt.lib.bt_beam_set_resort_interval(beam._h, -1) == bt.BT_ERR_INVALID
+    beam.set_resort_interval(0)
+    beam.deposit_cic(grid, sc.q_weight, sc.zscale, True)
+    assert beam.ids_ptr() == 0                           # interval 0: the deposit never sorts
+    beam.close()
+    grid.close()
