@@ -264,7 +264,8 @@ int bt_beam_moments(bt_beam *beam, double host_mean[6], double host_cov[36]);
  * as bt_track(nturns) -- bit-identical final coordinates, reference energy, s and turn -- but one launch per element, each
  * followed by bt_beam_moments.  host_moments receives nturns * n_elems records of 42 doubles (mean[6], then cov[36] row-major)
  * in walk order: record (turn * n_elems + e) is the beam right after element e of that turn.  Costs 144 bytes of HBM
- * traffic per particle and element instead of 96 per call, and synchronises after every element: a diagnostics mode.
+ * traffic per particle and element instead of 96 per call (two launches per element, no synchronisation until the end,
+ * where the records are copied to the host): a diagnostics mode.
  */
 int bt_track_diagnostics(bt_beam *beam, int32_t nturns, double *host_moments);
 

@@ -500,8 +500,13 @@ int bt_track_diagnostics(bt_beam *beam, int32_t nturns, double *host_moments) {
     if (!b.has_ref) return fail(BT_ERR_STATE, "bt_track_diagnostics: bt_beam_set_ref not called");
     std::vector<bt_element> one(1);
     std::vector<DevOp> ops;
-    double *out = host_moments;
-    for (int32_t t = 0; t < nturns; ++t) {
+    const size_t nrec = (size_t)nturns * b.lattice.size();
+    if (nrec == 0) return BT_OK;
+    double *dev = nullptr;  // all records stay on the device until the end: no synchronisation inside the walk
+    BT_CUDA_TRY(cudaMalloc(&dev, nrec * 42 * sizeof(double)));
+    double *out = dev;
+    int rc_all = BT_OK;
+    for (int32_t t = 0; t < nturns && rc_all == BT_OK; ++t) {
         for (size_t e = 0; e < b.lattice.size(); ++e) {
             one[0] = b.lattice[e];
             ops.clear();
@@ -509,19 +514,24 @@ int bt_track_diagnostics(bt_beam *beam, int32_t nturns, double *host_moments) {
             const double gamma_after = build_turn_table(one, b.gamma, ops, &slots);
             for (size_t lo = 0; lo < ops.size(); lo += (size_t)kConstTableRecords) {
                 const size_t len = ops.size() - lo < (size_t)kConstTableRecords ? ops.size() - lo : (size_t)kConstTableRecords;
-                const int rc = launch_track(&b, ops.data() + lo, (int32_t)len, 1, next_table_version(), slots / (double)ops.size());
-                if (rc != BT_OK) return rc;
+                rc_all = launch_track(&b, ops.data() + lo, (int32_t)len, 1, next_table_version(), slots / (double)ops.size());
+                if (rc_all != BT_OK) break;
             }
+            if (rc_all != BT_OK) break;
             b.gamma = gamma_after;
             b.s += b.lattice[e].ds;
-            const int rc = launch_moments(&b, out, out + 6);
-            if (rc != BT_OK) return rc;
+            rc_all = launch_moments_async(&b, out);
+            if (rc_all != BT_OK) break;
             out += 42;
         }
-        b.turn += 1;
+        if (rc_all == BT_OK) b.turn += 1;
     }
     b.table_valid = false;  // the constant bank no longer holds this beam's whole-lattice table
-    return BT_OK;
+    if (rc_all == BT_OK && cudaMemcpyAsync(host_moments, dev, nrec * 42 * sizeof(double), cudaMemcpyDeviceToHost, b.stream) != cudaSuccess)
+        rc_all = fail(BT_ERR_CUDA, "bt_track_diagnostics: copy of the records failed");
+    cudaStreamSynchronize(b.stream);
+    cudaFree(dev);
+    return rc_all;
 }
 
 // Host-to-host walk: chunks of the bunch ride three streams, so that the H2D copy of chunk k+1, the walk of chunk k and

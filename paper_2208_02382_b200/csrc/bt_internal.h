@@ -140,6 +140,7 @@ int launch_gather_kick(Beam *b, const Grid *g, const double coef[3], double zsca
 int sort_by_cell(Beam *b, const Grid *g, double zscale);
 int unpermute_to(Beam *b, int c, double *out);  // out[ids[j]] = q[c][j] on the beam's stream
 int launch_moments(Beam *b, double host_mean[6], double host_cov[36]);  // synchronises the beam's stream
+int launch_moments_async(Beam *b, double *dev_out);                      // 42 doubles to device memory, no synchronisation
 int poisson_solve(Grid *g, double gz, cudaStream_t stream);  // rho -> phi -> field records
 void poisson_free(Grid *g);
 int field_unpack(Grid *g, double *ex, double *ey, double *ez, cudaStream_t stream);  // device outputs

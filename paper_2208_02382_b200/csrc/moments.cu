@@ -141,7 +141,8 @@ __global__ void __launch_bounds__(kMomBlock) moments_kernel(const __grid_constan
     if (threadIdx.x == 0) *a.ticket = 0u;  // ready for the next call
 }
 
-int launch_moments(Beam *b, double host_mean[6], double host_cov[36]) {
+// Enqueues the reduction; the 42 results (mean[6], cov[36]) land in dev_out (device memory) on the beam's stream.
+int launch_moments_async(Beam *b, double *dev_out) {
     const int max_blocks = b->num_sms * 4;
     if (!b->mom_buf) {
         const size_t bytes = (size_t)(6 + 42 + (size_t)max_blocks * kMomVals) * sizeof(double) + 16;
@@ -151,7 +152,7 @@ int launch_moments(Beam *b, double host_mean[6], double host_cov[36]) {
     MomArgs a;
     for (int c = 0; c < 6; ++c) a.q[c] = b->q[c];
     a.n = b->n;
-    a.out = b->mom_buf;
+    a.out = dev_out ? dev_out : b->mom_buf;
     a.partial = b->mom_buf + 48;
     a.ticket = reinterpret_cast<unsigned int *>(b->mom_buf + 48 + (size_t)max_blocks * kMomVals);
     long long blocks = (b->n / 2 + kMomBlock - 1) / kMomBlock;
@@ -164,8 +165,14 @@ int launch_moments(Beam *b, double host_mean[6], double host_cov[36]) {
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return fail(BT_ERR_CUDA, std::string("bt_beam_moments launch: ") + cudaGetErrorString(e));
     g_launch_count.fetch_add(1);
+    return BT_OK;
+}
+
+int launch_moments(Beam *b, double host_mean[6], double host_cov[36]) {
+    const int rc = launch_moments_async(b, nullptr);
+    if (rc != BT_OK) return rc;
     double h[42];
-    BT_CUDA_TRY(cudaMemcpyAsync(h, a.out, sizeof(h), cudaMemcpyDeviceToHost, b->stream));
+    BT_CUDA_TRY(cudaMemcpyAsync(h, b->mom_buf, sizeof(h), cudaMemcpyDeviceToHost, b->stream));
     BT_CUDA_TRY(cudaStreamSynchronize(b->stream));
     for (int i = 0; i < 6; ++i) host_mean[i] = h[i];
     for (int i = 0; i < 36; ++i) host_cov[i] = h[6 + i];
