@@ -142,3 +142,53 @@ def test_shape_argument_errors():
     small = bt.Grid((2, 8, 8), (0, 0, 0), (1, 1, 1))
     assert bt.lib.bt_grid_set_particle_shape(small._h, 2) == bt.BT_ERR_INVALID
     small.close()
+
+
+@pytest.mark.parametrize("order", [1, 2])
+@pytest.mark.parametrize("n", [1, 255, 256, 257, 513])
+def test_gather_small_counts_around_the_chunk_size(order, n, monkeypatch):
+    """Pipeline chunks are 256 particles: counts below, at and just above one chunk (ragged tail kernel), tile mode forced."""
+    monkeypatch.setenv("BT_GATHER_MODE", "4")
+    sc = W.spacecharge_config("A", n=n, shape=(16, 16, 16))
+    c = W.make_spacecharge_bunch(sc)
+    E = W.gaussian_bunch_field(sc)
+    beam = bt.Beam(n)
+    grid = bt.Grid(sc.shape, sc.lo, sc.d)
+    grid.set_particle_shape(order)
+    beam.set_ref(sc.kin_energy_MeV, sc.mass_MeV, 1.0)
+    grid.set_field(*E)
+    beam.upload(c)
+    beam.sort_by_cell(grid, sc.zscale)
+    beam.gather_kick(grid, sc.kick_coef, sc.zscale, sc.ds / 2, sc.ds / 2)
+    got = beam.download()
+    g0 = O.ref_from_kinetic(sc.kin_energy_MeV, sc.mass_MeV)[0]
+    ref = [a.copy() for a in c]
+    O.track(ref, [("drift", sc.ds / 2, 1)], 1, g0)
+    O.gather_kick(ref, sc.shape, sc.lo, sc.d, E, sc.kick_coef, sc.zscale, order=order)
+    O.track(ref, [("drift", sc.ds / 2, 1)], 1, g0)
+    assert max(r14_error(got, ref)) <= 1e-11
+    beam.close()
+    grid.close()
+
+
+def test_everything_outside_the_grid_is_a_no_op():
+    sc = W.spacecharge_config("A", n=3000, shape=(8, 8, 8))
+    c = W.make_spacecharge_bunch(sc)
+    c[0] += 1.0                                     # the whole bunch is a metre away from the grid
+    E = W.gaussian_bunch_field(sc)
+    for order in (1, 2):
+        beam = bt.Beam(sc.n)
+        grid = bt.Grid(sc.shape, sc.lo, sc.d)
+        grid.set_particle_shape(order)
+        beam.set_ref(sc.kin_energy_MeV, sc.mass_MeV, 1.0)
+        grid.set_field(*E)
+        beam.upload(c)
+        beam.sort_by_cell(grid, sc.zscale)
+        beam.deposit_cic(grid, sc.q_weight, sc.zscale, True)
+        assert not grid.download_rho().any()
+        beam.gather_kick(grid, sc.kick_coef, sc.zscale, 0.0, 0.0)
+        got = beam.download()
+        for a, b in zip(got, c):
+            assert np.array_equal(a, b)
+        beam.close()
+        grid.close()

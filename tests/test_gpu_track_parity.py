@@ -406,3 +406,21 @@ def test_random_lattices_of_all_element_kinds(seed):
     assert all(np.all(np.isfinite(a)) for a in ref), lat        # the lattices are tame enough for the bunch to survive
     assert max(r14_error(got, ref)) <= 1e-11, lat
     assert abs(g - g_ref) <= 8e-16 * g_ref and abs(s - s_ref) <= 1e-10 and turn == nturns
+
+
+def test_track_host_edge_cases():
+    """nturns = 0 copies through unchanged; more chunks than 1024-particle granules; tiny bunch."""
+    import paper_2208_02382_b200 as bt
+    cfg = W.config(0, n=1500)
+    c = W.make_bunch(cfg)
+    beam = bt.Beam(cfg.n)
+    beam.set_ref(cfg.kin_energy_MeV, cfg.mass_MeV, cfg.charge_qe)
+    beam.lattice_set(cfg.lattice)
+    out = beam.track_host(c, [np.empty_like(a) for a in c], nturns=0, nchunks=4)
+    for a, b in zip(out, c):
+        assert np.array_equal(a, b)
+    out = beam.track_host(c, [np.empty_like(a) for a in c], nturns=2, nchunks=200)
+    ref, _ = oracle_track(cfg, c, nturns=2)
+    assert max(r14_error(out, ref)) <= 1e-11
+    assert bt.lib.bt_track_host(beam._h, None, None, 1, 0) == bt.BT_ERR_INVALID
+    beam.close()
