@@ -116,12 +116,16 @@ __global__ void __launch_bounds__(256) field_unpack_kernel(const double4 *__rest
 }
 
 // ---- host side -------------------------------------------------------------------------------------------------------
+// The 3-D transforms are done as a batch of 2-D transforms over (y, x) for the planes that matter plus one strided 1-D pass
+// over z: rho is zero on the planes z >= nz of the padded box and only the planes z < nz of the result are used, so both the
+// forward and the inverse (y, x) passes run on nz instead of 2 nz planes -- a pruned FFT, a third of the work saved.
 struct PoissonState {
-    cufftHandle fwd = 0, inv = 0;
+    cufftHandle fwd2d = 0, zpass = 0, inv2d = 0;
     bool plans = false;
-    double *pad_in = nullptr;              // (2nz, 2ny, 2nx) reals: rho in the physical octant, zeros elsewhere (zeroed once)
-    double *pad = nullptr;                 // (2nz, 2ny, 2nx) reals: the padded potential (and scratch for the Green table)
-    cufftDoubleComplex *spec = nullptr;    // (2nz, 2ny, nx + 1) complex
+    double *in2d = nullptr;                // (nz, 2ny, 2nx) reals: rho in x < nx, y < ny; zeros elsewhere (zeroed once)
+    cufftDoubleComplex *half = nullptr;    // (2nz, 2ny, nx + 1): the (y, x) transforms of the planes z < nz; planes z >= nz stay zero
+    cufftDoubleComplex *spec = nullptr;    // (2nz, 2ny, nx + 1): full spectrum (z pass out of place, so `half` keeps its zeros)
+    double *out2d = nullptr;               // (nz, 2ny, 2nx) reals: the potential on the planes z < nz of the padded box
     double *ghat = nullptr;                // real part of the Green table's transform, same shape as spec
     double ghat_gz = 0.0;                  // gz the cached table was built for (0 = none)
 };
@@ -135,59 +139,92 @@ void poisson_free(Grid *g) {
     PoissonState *st = static_cast<PoissonState *>(g->poisson);
     if (!st) return;
     if (st->plans) {
-        cufftDestroy(st->fwd);
-        cufftDestroy(st->inv);
+        cufftDestroy(st->fwd2d);
+        cufftDestroy(st->zpass);
+        cufftDestroy(st->inv2d);
     }
-    if (st->pad) cudaFree(st->pad);
-    if (st->pad_in) cudaFree(st->pad_in);
+    if (st->in2d) cudaFree(st->in2d);
+    if (st->half) cudaFree(st->half);
     if (st->spec) cudaFree(st->spec);
+    if (st->out2d) cudaFree(st->out2d);
     if (st->ghat) cudaFree(st->ghat);
     delete st;
     g->poisson = nullptr;
+}
+
+// Transform of the (dense) Green table: a plain 3-D D2Z with a temporary plan and buffer, once per gz.
+static int build_green_transform(PoissonState *st, const PadDims &p, double dx, double dy, double dz, cudaStream_t stream) {
+    const long long nreal = (long long)p.mx * p.my * p.mz;
+    const long long nspec = (long long)p.mz * p.my * (p.mx / 2 + 1);
+    double *table = nullptr;
+    BT_CUDA_TRY(cudaMalloc(&table, (size_t)nreal * sizeof(double)));
+    cufftHandle plan3d = 0;
+    cufftResult r = cufftPlan3d(&plan3d, p.mz, p.my, p.mx, CUFFT_D2Z);
+    if (r == CUFFT_SUCCESS) r = cufftSetStream(plan3d, stream);
+    if (r == CUFFT_SUCCESS) {
+        green_table_kernel<<<grid_1d(nreal), 256, 0, stream>>>(table, p, dx, dy, dz, green_self_term(dx, dy, dz));
+        r = cufftExecD2Z(plan3d, table, st->spec);
+    }
+    if (r == CUFFT_SUCCESS) real_part_kernel<<<grid_1d(nspec), 256, 0, stream>>>(st->spec, st->ghat, nspec);
+    cudaStreamSynchronize(stream);  // the temporaries go away
+    if (plan3d) cufftDestroy(plan3d);
+    cudaFree(table);
+    if (r != CUFFT_SUCCESS) return fail(BT_ERR_CUDA, "bt_grid_solve_poisson: cuFFT error " + std::to_string((int)r) + " while transforming the Green table");
+    g_launch_count.fetch_add(2);
+    return BT_OK;
 }
 
 int poisson_solve(Grid *g, double gz, cudaStream_t stream) {
     PadDims p;
     p.nx = g->nx, p.ny = g->ny, p.nz = g->nz;
     p.mx = 2 * g->nx, p.my = 2 * g->ny, p.mz = 2 * g->nz;
+    const int hx = p.mx / 2 + 1;
     const long long nreal = (long long)p.mx * p.my * p.mz;
-    const long long nspec = (long long)p.mz * p.my * (p.mx / 2 + 1);
+    const long long nplane_r = (long long)p.my * p.mx, nplane_c = (long long)p.my * hx;
+    const long long nspec = (long long)p.mz * nplane_c;
     PoissonState *st = static_cast<PoissonState *>(g->poisson);
     if (!st) {
         st = new (std::nothrow) PoissonState();
         if (!st) return fail(BT_ERR_OOM, "bt_grid_solve_poisson: host allocation failed");
         g->poisson = st;
     }
-    if (!st->pad) BT_CUDA_TRY(cudaMalloc(&st->pad, (size_t)nreal * sizeof(double)));
-    if (!st->pad_in) {
-        BT_CUDA_TRY(cudaMalloc(&st->pad_in, (size_t)nreal * sizeof(double)));
-        BT_CUDA_TRY(cudaMemsetAsync(st->pad_in, 0, (size_t)nreal * sizeof(double), stream));  // the D2Z transform is out of place: zeros persist
+    if (!st->in2d) {
+        BT_CUDA_TRY(cudaMalloc(&st->in2d, (size_t)(p.nz * nplane_r) * sizeof(double)));
+        BT_CUDA_TRY(cudaMemsetAsync(st->in2d, 0, (size_t)(p.nz * nplane_r) * sizeof(double), stream));  // transforms are out of place: zeros persist
     }
+    if (!st->half) {
+        BT_CUDA_TRY(cudaMalloc(&st->half, (size_t)nspec * sizeof(cufftDoubleComplex)));
+        BT_CUDA_TRY(cudaMemsetAsync(st->half, 0, (size_t)nspec * sizeof(cufftDoubleComplex), stream));
+    }
+    if (!st->out2d) BT_CUDA_TRY(cudaMalloc(&st->out2d, (size_t)(p.nz * nplane_r) * sizeof(double)));
     if (!st->spec) BT_CUDA_TRY(cudaMalloc(&st->spec, (size_t)nspec * sizeof(cufftDoubleComplex)));
     if (!st->ghat) BT_CUDA_TRY(cudaMalloc(&st->ghat, (size_t)nspec * sizeof(double)));
     if (!g->phi) BT_CUDA_TRY(cudaMalloc(&g->phi, (size_t)g->nn * sizeof(double)));
     if (!g->field) BT_CUDA_TRY(cudaMalloc(&g->field, (size_t)g->nn * 4 * sizeof(double)));
     if (!st->plans) {
-        BT_CUFFT_TRY(cufftPlan3d(&st->fwd, p.mz, p.my, p.mx, CUFFT_D2Z));
-        BT_CUFFT_TRY(cufftPlan3d(&st->inv, p.mz, p.my, p.mx, CUFFT_Z2D));
+        int n2[2] = {p.my, p.mx}, emb_r[2] = {p.my, p.mx}, emb_c[2] = {p.my, hx}, n1[1] = {p.mz}, emb_z[1] = {p.mz};
+        BT_CUFFT_TRY(cufftPlanMany(&st->fwd2d, 2, n2, emb_r, 1, (int)nplane_r, emb_c, 1, (int)nplane_c, CUFFT_D2Z, p.nz));
+        BT_CUFFT_TRY(cufftPlanMany(&st->zpass, 1, n1, emb_z, (int)nplane_c, 1, emb_z, (int)nplane_c, 1, CUFFT_Z2Z, (int)nplane_c));
+        BT_CUFFT_TRY(cufftPlanMany(&st->inv2d, 2, n2, emb_c, 1, (int)nplane_c, emb_r, 1, (int)nplane_r, CUFFT_Z2D, p.nz));
         st->plans = true;
     }
-    BT_CUFFT_TRY(cufftSetStream(st->fwd, stream));
-    BT_CUFFT_TRY(cufftSetStream(st->inv, stream));
+    BT_CUFFT_TRY(cufftSetStream(st->fwd2d, stream));
+    BT_CUFFT_TRY(cufftSetStream(st->zpass, stream));
+    BT_CUFFT_TRY(cufftSetStream(st->inv2d, stream));
     const double dx = g->d[0], dy = g->d[1], dz = gz * g->d[2];
     if (st->ghat_gz != gz) {  // Green table for this grid and this gz: built and transformed once
-        green_table_kernel<<<grid_1d(nreal), 256, 0, stream>>>(st->pad, p, dx, dy, dz, green_self_term(dx, dy, dz));
-        BT_CUFFT_TRY(cufftExecD2Z(st->fwd, st->pad, st->spec));
-        real_part_kernel<<<grid_1d(nspec), 256, 0, stream>>>(st->spec, st->ghat, nspec);
-        g_launch_count.fetch_add(2);
+        const int rc = build_green_transform(st, p, dx, dy, dz, stream);
+        if (rc != BT_OK) return rc;
         st->ghat_gz = gz;
     }
-    copy_octant_kernel<<<grid_1d(g->nn), 256, 0, stream>>>(g->rho, st->pad_in, p);
-    BT_CUFFT_TRY(cufftExecD2Z(st->fwd, st->pad_in, st->spec));
+    copy_octant_kernel<<<grid_1d(g->nn), 256, 0, stream>>>(g->rho, st->in2d, p);
+    BT_CUFFT_TRY(cufftExecD2Z(st->fwd2d, st->in2d, st->half));                    // (y, x) on the planes z < nz
+    BT_CUFFT_TRY(cufftExecZ2Z(st->zpass, st->half, st->spec, CUFFT_FORWARD));     // z
     const double scale = 1.0 / (4.0 * kPiP * kEps0) / (double)nreal;  // Coulomb constant and the unnormalised inverse FFT
     spectral_multiply_kernel<<<grid_1d(nspec), 256, 0, stream>>>(st->spec, st->ghat, nspec, scale);
-    BT_CUFFT_TRY(cufftExecZ2D(st->inv, st->spec, st->pad));
-    gradient_kernel<<<grid_1d(g->nn), 256, 0, stream>>>(st->pad, g->phi, reinterpret_cast<double4 *>(g->field), p, dx, dy, dz);
+    BT_CUFFT_TRY(cufftExecZ2Z(st->zpass, st->spec, st->spec, CUFFT_INVERSE));     // z, in place
+    BT_CUFFT_TRY(cufftExecZ2D(st->inv2d, st->spec, st->out2d));                   // (y, x) on the planes z < nz
+    gradient_kernel<<<grid_1d(g->nn), 256, 0, stream>>>(st->out2d, g->phi, reinterpret_cast<double4 *>(g->field), p, dx, dy, dz);
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return fail(BT_ERR_CUDA, std::string("bt_grid_solve_poisson launch: ") + cudaGetErrorString(e));
     g_launch_count.fetch_add(3);
