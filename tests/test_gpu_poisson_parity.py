@@ -58,6 +58,23 @@ def test_poisson_matches_direct_sum(shape, d, gz):
     check(rho, d, gz)
 
 
+@pytest.mark.parametrize("shape", [(32, 32, 32), (16, 24, 128), (40, 12, 32)])
+def test_poisson_more_grid_shapes(shape):
+    """Non-cubic grids with power-of-two and other plane counts; the 128-plane case on sampled nodes."""
+    rng = np.random.default_rng(7)
+    nx, ny, nz = shape
+    rho = rng.uniform(-1e-12, 3e-12, (nz, ny, nx))
+    rho[rng.uniform(size=rho.shape) < 0.5] = 0.0
+    d, gz = (1e-3, 0.8e-3, 0.5e-3), 1.7
+    if nz <= 32:
+        check(rho, d, gz)
+    else:
+        phi, E = gpu_solve(rho, (0.0, 0.0, 0.0), d, gz)
+        idx = rng.integers(0, rho.size, 64)
+        ref = O.poisson_sample(rho, d, gz, idx)
+        assert np.max(np.abs(phi.reshape(-1)[idx] - ref)) <= 1e-12 * np.max(np.abs(phi))
+
+
 def test_point_charge_and_resolve_with_another_gz():
     """Coulomb potential of one node charge; the cached Green transform is rebuilt when gz changes."""
     rho = np.zeros((9, 10, 11))
