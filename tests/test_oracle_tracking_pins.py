@@ -364,15 +364,144 @@ def test_rectangular_magnet_geometry():
 
 
 def test_dipedge_fringe_correction_direction():
-    """Finite gap (g, K > 0) weakens the vertical edge focusing; g = 0 or K = 0 removes the correction."""
+    """Finite gap (g, K > 0) weakens the vertical edge focusing; g = 0 or K = 0 removes the correction.
+    (Limits and sign only; the size of the correction is pinned by test_dipedge_fringe_term_vs_maxwell_ray_tracing.)"""
     psi, rho = 0.05, 10.0
     hard = M_of([("dipedge", 0.0, 1, psi, rho, 0.0, 0.5)], GAMMA_E5GEV)[3, 2]
     soft = M_of([("dipedge", 0.0, 1, psi, rho, 0.02, 0.5)], GAMMA_E5GEV)[3, 2]
     k0 = M_of([("dipedge", 0.0, 1, psi, rho, 0.02, 0.0)], GAMMA_E5GEV)[3, 2]
     assert hard == k0 == -math.tan(psi) / rho
     assert hard < soft < 0.0
-    psi_c = 0.5 * (0.02 / rho) * (1 + math.sin(psi) ** 2) / math.cos(psi)
-    assert abs(soft + math.tan(psi - psi_c) / rho) < 1e-17
+
+
+# ---- R7 fringe term psi_c: pinned by ray tracing through an extended, Maxwell-consistent fringe field ----------
+# Nothing below knows the expression for psi_c.  A pole face with normal e_n (pointing into the magnet at an entrance,
+# out of it at an exit), e_tau along the face, e_y vertical, (e_n, e_tau, e_y) right-handed.  The mid-plane field falls
+# off along the normal only: B_y(n, 0) = B0 f(n).  curl B = 0 then fixes the field off the mid-plane to first order in y:
+#     B = B0 ( y f'(n), 0, f(n) )        (dB_n/dy = dB_y/dn; div B = 0 only adds -y^2 f''/2 to B_y, second order in y).
+# A particle of momentum p and charge q obeys the Lorentz force, with path length s as the independent variable:
+#     dr/ds = u,   du/ds = h u x b,   h = q B0 / p = 1/rho,   b = B / B0,   |u| = 1.
+# The reference ray moves in the plane y = 0 and makes the angle psi with e_n where the field has vanished; rays started
+# with a tiny vertical offset / slope give the 2 x 2 vertical transfer matrix M of the fringe region.  The hard-edge
+# model of the same region (what a lattice of Sbend + DipEdge + Drift elements represents) is
+#     M_model = D(L_body) . Edge . D(L_drift),
+# the edge sitting where the field integral puts it (int f dn = length of full field), D(L) the vertical map of a drift
+# or of a gradient-free sector-bend body of arc length L.  Hence Edge = D(-L_body) M D(-L_drift), and its (2,1) element is
+# what the oracle's R43 = -tan(psi - psi_c)/rho has to equal, up to terms of second order in g/rho.  The fringe integral
+# K = int f (1 - f) dn / g is computed from the profile by quadrature (its definition, include/bt.h).
+def _fringe_profile(kind, g):
+    if kind == "ramp":      # linear fall-off over 3 g  ->  K = 1/2, the value configs[2] uses
+        w = 3.0 * g
+        return (lambda n: min(max(n / w, 0.0), 1.0)), (lambda n: 1.0 / w if 0.0 < n < w else 0.0), [0.0, w], (0.0, w)
+    lam = 0.7 * g           # smooth (tanh) fall-off: K = lam / (2 g) = 0.35
+    return (lambda n: 0.5 * (1.0 + math.tanh(n / lam))), (lambda n: 0.5 / (lam * math.cosh(n / lam) ** 2)), [], (-22.0 * lam, 22.0 * lam)
+
+
+def _trace_fringe(f, fp, breaks, span, h, theta0, y0, yp0):
+    from scipy.integrate import solve_ivp
+
+    def rhs(_s, w):
+        n, _tau, y, un, ut, uy = w
+        bn, bt, by = y * fp(n), 0.0, f(n)
+        return [un, ut, uy, h * (ut * by - uy * bt), h * (uy * bn - un * by), h * (un * bt - ut * bn)]
+
+    na, nb = span
+    norm = math.sqrt(1.0 + yp0 * yp0)
+    w = [na, 0.0, y0, math.cos(theta0) / norm, math.sin(theta0) / norm, yp0 / norm]
+    s = 0.0
+    for c in [b for b in breaks if na < b < nb] + [nb]:      # integrate from kink to kink of the profile
+        def hit(_s, w, c=c):
+            return w[0] - c
+        hit.terminal, hit.direction = True, 1
+        sol = solve_ivp(rhs, (s, s + 10.0 * (c - w[0]) + 1.0), w, method="DOP853", rtol=1e-13, atol=1e-18, events=hit,
+                        max_step=(nb - na) / 50.0)
+        assert sol.t_events[0].size == 1
+        s, w = float(sol.t_events[0][0]), list(sol.y_events[0][0])
+    return w
+
+
+def _edge_matrix_from_ray_tracing(kind, g, rho, psi, face):
+    """(Edge 2x2, K) for a face of a magnet with bending radius rho and TRANSPORT-sign edge angle psi (psi > 0 at both
+    faces of a rectangular magnet)."""
+    from scipy.integrate import quad
+    h = 1.0 / rho
+    f, fp, breaks, (na, nb) = _fringe_profile(kind, g)
+    pts = breaks or None
+    full = quad(f, na, nb, points=pts, epsabs=1e-15, epsrel=1e-13)[0]           # length of full field in the region
+    K = quad(lambda n: f(n) * (1.0 - f(n)), na, nb, points=pts, epsabs=1e-15, epsrel=1e-13)[0] / g
+    if face == "entrance":                      # field-free at na, full field at nb; the ray bends towards the normal
+        theta0 = psi
+        l_drift, arc = ((nb - full) - na) / math.cos(psi), None
+    else:                                       # mirror image: full field at the start, the ray leaves at angle -psi
+        f, fp = (lambda n, f=f: f(-n)), (lambda n, fp=fp: -fp(-n))
+        breaks, (na, nb) = [-b for b in reversed(breaks)], (-nb, -na)
+        theta0 = math.asin(-math.sin(psi) + h * full)    # d sin(theta)/dn = -h f  integrated over the region
+        l_drift = (nb - (na + full)) / math.cos(psi)
+    eps = 1e-7
+    w0 = _trace_fringe(f, fp, breaks, (na, nb), h, theta0, 0.0, 0.0)
+    wa = _trace_fringe(f, fp, breaks, (na, nb), h, theta0, eps, 0.0)
+    wb = _trace_fringe(f, fp, breaks, (na, nb), h, theta0, 0.0, eps)
+    assert w0[2] == 0.0 and w0[5] == 0.0                                        # the reference ray stays in the mid-plane
+    M = np.array([[wa[2], wb[2]], [wa[5] / math.hypot(wa[3], wa[4]), wb[5] / math.hypot(wb[3], wb[4])]]) / eps
+    theta1 = math.atan2(w0[4], w0[3])
+    l_body = (theta0 - theta1) / h if face == "entrance" else (theta0 - (-psi)) / h   # arc of the hard-edge orbit in full field
+    if face == "exit":
+        assert abs(theta1 + psi) < 1e-9                                         # it does leave at -psi
+    D = lambda L: np.array([[1.0, L], [0.0, 1.0]])
+    E = D(-l_body) @ M @ D(-l_drift) if face == "entrance" else D(-l_drift) @ M @ D(-l_body)
+    return E, K
+
+
+def _oracle_r43(psi, rho, g, K):
+    c = [np.zeros(1) for _ in range(6)]
+    c[2][0] = 1e-3
+    O.track(c, [("dipedge", 0.0, 1, psi, rho, g, K)], 1, GAMMA_E5GEV)
+    return c[3][0] / 1e-3
+
+
+@pytest.mark.parametrize("rho,g", [(10.0, 0.02), (10.0, 0.005), (2.5, 0.02), (-4.0, 0.01)])
+@pytest.mark.parametrize("psi", [0.5, -0.4, 0.05, -0.05, 0.0])
+@pytest.mark.parametrize("kind", ["ramp", "tanh"])
+def test_dipedge_fringe_term_vs_maxwell_ray_tracing(rho, g, psi, kind):
+    """R7's fringe term against the Lorentz force in an extended fringe field (see the comment block above): the
+    vertical focusing of the oracle's thin edge must equal that of the ray-traced fringe region, once the drift and
+    the bend body of the hard-edge model are divided out, to within 2 % of the fringe correction itself (the remainder
+    is second order in g/rho: it measures 0.2 % at g/rho = 0.002 and 0.7 % at 0.008) -- for both signs of psi and of
+    rho, configs[2]'s values (rho = 10, g = 0.02, K = 1/2, psi = +-0.05) included, two field profiles with different K.
+
+    Mutants of oracle/bt_oracle.c:pass_dipedge that these pins kill (each was applied to a copy of the oracle and
+    `pytest -k dipedge_fringe_term` run against it; `fail` = failing cases of 41 = 40 here + the remainder test below;
+    the unmutated oracle passes all 41):
+        (1 + sp*sp)  ->  (1 + cp*cp)                                                        fail 41
+        (1 + sp*sp)  ->  1   (tan(theta(n)) averaged over the fringe, double-kick term lost) fail 17  (all with |psi| >= 0.4)
+        "/ cp" dropped                                                                      fail 17  (all with |psi| >= 0.4)
+        K  ->  2 K                                                                          fail 41
+        g / rho  ->  g / (rho * rho)                                                        fail 41
+        tan(psi - psi_c)  ->  tan(psi + psi_c)                                              fail 41
+        tan(psi - psi_c)  ->  tan(psi) - psi_c                                              fail 17  (all with |psi| >= 0.4)
+    """
+    face = "entrance" if psi >= 0.0 or kind == "tanh" else "exit"              # both faces are exercised
+    E, K = _edge_matrix_from_ray_tracing(kind, g, rho, psi, face)
+    assert abs(K - (0.5 if kind == "ramp" else 0.35)) < 1e-9
+    hard = -math.tan(psi) / rho
+    got = _oracle_r43(psi, rho, g, K)
+    corr = abs(got - hard)
+    assert corr > 0.2 * K * g / rho ** 2                                        # there is a correction to compare
+    assert abs(E[1, 0] - got) <= 0.02 * corr, (E[1, 0], got, hard)
+    # the rest of the ray-traced edge is the identity to first order in g: a thin element at the effective edge
+    assert abs(E[0, 0] - 1.0) < 1e-4 and abs(E[1, 1] - 1.0) < 1e-4
+    assert abs(E[0, 1]) < 1e-4
+    assert abs(np.linalg.det(E) - 1.0) < 1e-9
+
+
+def test_dipedge_fringe_term_remainder_is_second_order():
+    """Halving g quarters the distance between the ray-traced edge focusing and the oracle's first-order expression."""
+    rho, psi = 2.5, 0.5
+    d = []
+    for g in (0.02, 0.01, 0.005):
+        E, K = _edge_matrix_from_ray_tracing("ramp", g, rho, psi, "entrance")
+        d.append(abs(E[1, 0] - _oracle_r43(psi, rho, g, K)))
+    assert 3.5 < d[0] / d[1] < 4.5 and 3.5 < d[1] / d[2] < 4.5
 
 
 # ------------------------------------------------------------------------------------------------
