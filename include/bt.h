@@ -154,8 +154,9 @@ int bt_beam_ids(bt_beam *beam, int32_t **dev_ids_out);
 /*
  * Validate and copy the element list (n_elems >= 1).  Mirrors sim.lattice.extend([...]) (P:l.93).
  * The per-slice map coefficients are computed on the host from (type, params, beta0, beta0*gamma0)
- * when bt_track needs them, packed into 64-byte device records and uploaded once per bt_track call
- * (once per turn-chunk if an RF cavity changes the reference energy).
+ * when bt_track needs them and packed into 64-byte records; a launch of the walk carries its records as kernel
+ * parameters (<= 510 records; constant bank 0), so nothing on the device is shared between beams or streams:
+ * beams may be used concurrently from different host threads / streams (one thread per beam at a time).
  */
 int bt_lattice_set(bt_beam *beam, const bt_element *elems, int32_t n_elems);
 
@@ -164,7 +165,8 @@ int bt_lattice_set(bt_beam *beam, const bt_element *elems, int32_t n_elems);
  * apply the element's map of length ds/nslice to every particle.  ONE kernel: each particle is
  * loaded once, every element map and slice is applied in registers, and it is stored once per launch
  * (96 bytes of HBM traffic per particle per launch).  Lattices whose RF cavities change the reference
- * energy are processed in chunks of turns (one launch per chunk, per-turn coefficient tables).
+ * energy are processed in chunks of whole turns (one launch per <= 510 records, per-turn coefficient tables),
+ * lattices with more than 510 records per turn in several launches per turn.
  * Updates the reference gamma, s and turn.  Bit-reproducible run to run.  nturns >= 0.
  * Mirrors sim.evolve() (P:l.95) without space charge.
  */
@@ -178,8 +180,9 @@ int bt_track(bt_beam *beam, int32_t nturns);
  * is bit-identical to bt_beam_upload + bt_track + bt_beam_download for any nchunks.  host_in / host_out: 6 host arrays
  * of n doubles each (order x, px, y, py, t, pt; pinned memory for the copies to be asynchronous; host_out may alias
  * host_in).  Synchronous: returns when host_out is complete.  The beam's device arrays hold the result too; storage
- * order is reset as by bt_beam_upload.  nchunks in [1, 256]; lattices whose RF changes the reference energy, or with
- * more records than one table holds, are processed as one chunk.
+ * order is reset as by bt_beam_upload.  nchunks in [1, 256].  Any lattice is pipelined, including those whose RF changes
+ * the reference energy (P:l.82-83 reference particle; S3): every chunk runs the same sequence of launches, each launch
+ * carrying its own coefficient table.
  */
 int bt_track_host(bt_beam *beam, const double *const host_in[6], double *const host_out[6], int32_t nturns, int32_t nchunks);
 
@@ -273,11 +276,25 @@ int bt_track_diagnostics(bt_beam *beam, int32_t nturns, double *host_moments);
 int bt_sync(bt_beam *beam); /* cudaStreamSynchronize on the beam's stream */
 const char *bt_last_error(void);
 int bt_version(void);
+
+/* ==== diagnostics and measurement helpers: NOT part of the method, no passage of the paper behind them ================
+ * They exist for bench.py (launch counts, roofline denominators measured on the box) and for the tests (forcing every
+ * kernel variant).  A caller of the method never needs them. */
 /* Number of CUDA kernels this library has launched in this process (all beams/grids). */
 int64_t bt_launch_count(void);
-/* Name and launch geometry of the last fused-walk launch (diagnostic; any out may be NULL). */
+/* Name and launch geometry of the last fused-walk launch (any out may be NULL). */
 int bt_track_last_launch(const bt_beam *beam, int32_t *grid_dim, int32_t *block_dim,
                          int32_t *particles_per_thread, int32_t *smem_bytes);
+/*
+ * Force a kernel variant, process-wide (typed replacement of round 1's BT_* environment variables; nothing in the library
+ * reads the environment).  value < 0 restores the measured default.  Results never depend on a knob; speed does.
+ *   "track_ppt"     particles per thread of the fused walk: 1, 2, 4
+ *   "track_block"   threads per block of the fused walk: 32, 64, 96, 128
+ *   "track_fuse"    0: one record per lattice element (no peephole fusion of records)
+ *   "deposit_mode"  0: one particle per thread, plain reductions; 1: default; 2: 4 particles per thread
+ *   "gather_mode"   0: registers; 1: default; 2 / 3: 512- / 128-particle chunks; 4: field tile in shared memory
+ */
+int bt_debug_knob(const char *name, int32_t value);
 
 /*
  * Measurement utilities (roofline denominators measured on the box):

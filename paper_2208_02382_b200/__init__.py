@@ -16,7 +16,7 @@ import numpy as np
 from . import _build
 
 __all__ = ["lib", "BtError", "Beam", "Grid", "pack_lattice", "ELEMENT_DTYPE", "EXPORTS",
-           "calib_fp64", "calib_rw6", "launch_count", "version"]
+           "calib_fp64", "calib_rw6", "launch_count", "debug_knob", "version"]
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libbt.so")
@@ -66,6 +66,7 @@ EXPORTS = {
     "bt_last_error": (C.c_char_p, []),
     "bt_version": (C.c_int, []),
     "bt_launch_count": (C.c_int64, []),
+    "bt_debug_knob": (C.c_int, [C.c_char_p, C.c_int32]),
     "bt_track_last_launch": (C.c_int, [_vp] + [C.POINTER(C.c_int32)] * 4),
     "bt_calib_fp64": (C.c_int, [_vp, C.c_double, _dp]),
     "bt_calib_rw6": (C.c_int, [_vp, C.c_int64, C.c_int32, _dp]),
@@ -111,6 +112,11 @@ def version():
 
 def launch_count():
     return int(lib.bt_launch_count())
+
+
+def debug_knob(name, value):
+    """bt_debug_knob: force a kernel variant (tests, A/B measurements); value -1 restores the measured default."""
+    _check(lib.bt_debug_knob(name.encode(), int(value)), "bt_debug_knob")
 
 
 def pack_lattice(lattice):

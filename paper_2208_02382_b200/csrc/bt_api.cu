@@ -63,11 +63,38 @@ static int validate_element(const bt_element &e, int idx) {
     return BT_OK;
 }
 
+// ---- debug knobs (bt_debug_knob): process-wide, typed, default -1 = "the measured default" ---------------------------
+std::atomic<int32_t> g_knob[KNOB_COUNT] = {{-1}, {-1}, {-1}, {-1}, {-1}};
+static const char *const kKnobNames[KNOB_COUNT] = {"track_ppt", "track_block", "track_fuse", "deposit_mode", "gather_mode"};
+
+// Runs of half cells [QUAD1][SEXTOCT|TAILDRIFT] among the records appended since `start` become one dispatch: the first
+// record of a run is relabelled OP_HALFCELL with count = pairs in the run; the coefficients stay where they are, so the
+// table keeps its size and the walk applies exactly the same maps in the same order.  A run never crosses a multiple of
+// kTableRecords counted from `start` (where bt_track cuts a turn that is longer than one launch's table).
+static void fuse_halfcell_runs(std::vector<DevOp> &out, size_t start) {
+    const size_t K = (size_t)kTableRecords;
+    size_t i = start;
+    while (i + 1 < out.size()) {
+        size_t head = i, pairs = 0;
+        while (i + 1 < out.size() && out[i].op == OP_QUAD1 && out[i + 1].op == (OP_SEXTOCT | OP_TAILDRIFT) &&
+               (i - start) / K == (i + 1 - start) / K && (i - start) / K == (head - start) / K) {
+            ++pairs;
+            i += 2;
+        }
+        if (pairs >= 1) {
+            out[head].op = OP_HALFCELL;
+            out[head].count = (int32_t)pairs;
+        } else {
+            ++i;
+        }
+    }
+}
+
 // ---- S1/S3: coefficients of one slice map per element, for one pass at reference gamma ----------
 double build_turn_table(const std::vector<bt_element> &lat, double gamma, std::vector<DevOp> &out, double *slots) {
     double nslots = 0.0;
-    const char *fuse_env = getenv("BT_TRACK_FUSE");  // 0: one record per element (debugging / A-B measurements)
-    const bool fuse = !(fuse_env && fuse_env[0] == '0');
+    const bool fuse = g_knob[KNOB_TRACK_FUSE].load() != 0;  // 0: one record per element (A/B measurements, bit-identity test)
+    const size_t start = out.size();
     for (size_t i = 0; i < lat.size(); ++i) {
         const bt_element &e = lat[i];
         DevOp o;
@@ -233,8 +260,94 @@ double build_turn_table(const std::vector<bt_element> &lat, double gamma, std::v
             }
         }
     }
+    if (fuse) fuse_halfcell_runs(out, start);
     if (slots) *slots = nslots;
     return gamma;
+}
+
+// ---- grids are shared between streams: order their operations with one event ------------------------------------------
+int grid_acquire(Grid *g, cudaStream_t s) {
+    if (g->done_valid && s != g->last_stream) BT_CUDA_TRY(cudaStreamWaitEvent(s, g->done, 0));
+    return BT_OK;
+}
+int grid_release(Grid *g, cudaStream_t s) {
+    if (!g->done) BT_CUDA_TRY(cudaEventCreateWithFlags(&g->done, cudaEventDisableTiming));
+    BT_CUDA_TRY(cudaEventRecord(g->done, s));
+    g->done_valid = true;
+    g->last_stream = s;
+    return BT_OK;
+}
+
+// ---- the launches of one bt_track(nturns) call ---------------------------------------------------------------------
+// A plan is a list of (records, passes) launches over record storage it owns or borrows.  Static lattices: one table,
+// walked nturns times by one launch (or, when a turn needs more than kTableRecords records, its segments turn after turn).
+// Lattices whose RF changes the reference energy (S3): every turn has its own coefficients; as many whole turns as fit
+// one launch's table go into it.  The same plan serves every chunk of bt_track_host.
+struct WalkPlan {
+    struct Launch {
+        size_t lo;
+        int32_t len, nturns;
+        double spr;  // FP64 slots per record (geometry heuristic)
+    };
+    const std::vector<DevOp> *ops = nullptr;
+    std::vector<DevOp> own;
+    std::vector<Launch> launches;
+    double gamma_after = 0.0;
+};
+
+static void plan_walk(Beam &b, int32_t nturns, WalkPlan &plan) {
+    const size_t K = (size_t)kTableRecords;
+    auto add_segments = [&](size_t lo, size_t len, double spr) {
+        for (size_t o = 0; o < len; o += K) plan.launches.push_back({lo + o, (int32_t)(len - o < K ? len - o : K), 1, spr});
+    };
+    if (!b.energy_changes) {
+        if (!b.table_valid) {
+            b.h_table.clear();
+            build_turn_table(b.lattice, b.gamma, b.h_table, &b.table_slots);
+            b.table_valid = true;
+        }
+        plan.ops = &b.h_table;
+        plan.gamma_after = b.gamma;
+        const double spr = b.table_slots / (double)b.h_table.size();
+        if (b.h_table.size() <= K) {
+            plan.launches.push_back({0, (int32_t)b.h_table.size(), nturns, spr});
+        } else {
+            for (int32_t t = 0; t < nturns; ++t) add_segments(0, b.h_table.size(), spr);
+        }
+        return;
+    }
+    plan.ops = &plan.own;
+    double gamma = b.gamma;
+    size_t pend_lo = 0;  // records [pend_lo, own.size()) = whole turns not yet assigned to a launch
+    double pend_spr = 0.0;
+    for (int32_t t = 0; t < nturns; ++t) {
+        const size_t turn_lo = plan.own.size();
+        double slots = 0.0;
+        gamma = build_turn_table(b.lattice, gamma, plan.own, &slots);
+        const size_t turn_len = plan.own.size() - turn_lo;
+        const double spr = slots / (double)turn_len;
+        if (turn_len > K) {  // a single turn exceeds one table: flush what is pending, then its segments
+            if (turn_lo > pend_lo) plan.launches.push_back({pend_lo, (int32_t)(turn_lo - pend_lo), 1, pend_spr});
+            add_segments(turn_lo, turn_len, spr);
+            pend_lo = plan.own.size();
+            continue;
+        }
+        if (plan.own.size() - pend_lo > K) {  // this turn no longer fits with the pending ones
+            plan.launches.push_back({pend_lo, (int32_t)(turn_lo - pend_lo), 1, pend_spr});
+            pend_lo = turn_lo;
+        }
+        pend_spr = spr;
+    }
+    if (plan.own.size() > pend_lo) plan.launches.push_back({pend_lo, (int32_t)(plan.own.size() - pend_lo), 1, pend_spr});
+    plan.gamma_after = gamma;
+}
+
+static int run_plan(Beam &b, const WalkPlan &plan) {  // on b.range's stream when set, else on the beam's
+    for (const WalkPlan::Launch &l : plan.launches) {
+        const int rc = launch_track(&b, plan.ops->data() + l.lo, l.len, l.nturns, l.spr);
+        if (rc != BT_OK) return rc;
+    }
+    return BT_OK;
 }
 
 }  // namespace bt
@@ -244,6 +357,16 @@ using namespace bt;
 extern "C" {
 
 const char *bt_last_error(void) { return t_last_error.c_str(); }
+
+int bt_debug_knob(const char *name, int32_t value) {
+    if (!name) return fail(BT_ERR_INVALID, "bt_debug_knob: name is NULL");
+    for (int k = 0; k < KNOB_COUNT; ++k)
+        if (strcmp(name, kKnobNames[k]) == 0) {
+            g_knob[k].store(value < 0 ? -1 : value);
+            return BT_OK;
+        }
+    return fail(BT_ERR_INVALID, std::string("bt_debug_knob: unknown knob ") + name);
+}
 int bt_version(void) { return BT_VERSION; }
 int64_t bt_launch_count(void) { return g_launch_count.load(); }
 
@@ -299,7 +422,6 @@ void bt_beam_destroy(bt_beam *beam) {
     Beam &b = beam->b;
     cudaStreamSynchronize(b.stream);
     if (b.owns && b.q[0]) cudaFree(b.q[0]);
-    forget_table_owner(&b);
     int *ibufs[] = {b.ids, b.ids_tmp, b.sort_key, b.sort_dest, b.sort_count, b.sort_block_sum};
     for (int *p : ibufs)
         if (p) cudaFree(p);
@@ -420,71 +542,11 @@ int bt_track(bt_beam *beam, int32_t nturns) {
     if (b.lattice.empty()) return fail(BT_ERR_STATE, "bt_track: bt_lattice_set not called");
     if (!b.has_ref) return fail(BT_ERR_STATE, "bt_track: bt_beam_set_ref not called");
     if (nturns == 0) return BT_OK;
-    const size_t K = (size_t)kConstTableRecords;
-    // records [lo, hi) of one turn's table, in launches of at most K records
-    auto launch_segments = [&](const std::vector<DevOp> &ops, double spr) -> int {
-        for (size_t lo = 0; lo < ops.size(); lo += K) {
-            const size_t len = ops.size() - lo < K ? ops.size() - lo : K;
-            int rc = launch_track(&b, ops.data() + lo, (int32_t)len, 1, next_table_version(), spr);
-            if (rc != BT_OK) return rc;
-        }
-        return BT_OK;
-    };
-
-    if (!b.energy_changes) {
-        // one table serves every turn: "uploaded once", resident until the lattice, the reference or another
-        // beam's table replaces it
-        if (!b.table_valid) {
-            b.h_table.clear();
-            build_turn_table(b.lattice, b.gamma, b.h_table, &b.table_slots);
-            b.table_version = next_table_version();
-            b.table_valid = true;
-        }
-        const double spr = b.table_slots / (double)b.h_table.size();
-        if (b.h_table.size() <= K) {
-            int rc = launch_track(&b, b.h_table.data(), (int32_t)b.h_table.size(), nturns, b.table_version, spr);
-            if (rc != BT_OK) return rc;
-        } else {  // lattice longer than the constant bank: several launches per turn
-            for (int32_t t = 0; t < nturns; ++t) {
-                int rc = launch_segments(b.h_table, spr);
-                if (rc != BT_OK) return rc;
-            }
-        }
-    } else {
-        // S3: the reference energy changes at RF passages -> every turn has its own coefficients; as many whole
-        // turns as fit the constant bank go into one launch
-        b.table_valid = false;
-        std::vector<DevOp> buf, turn_ops;
-        double gamma = b.gamma, buf_spr = 0.0;
-        for (int32_t t = 0; t < nturns; ++t) {
-            turn_ops.clear();
-            double slots = 0.0;
-            gamma = build_turn_table(b.lattice, gamma, turn_ops, &slots);
-            const double spr = slots / (double)turn_ops.size();
-            if (turn_ops.size() > K) {  // a single turn exceeds the bank: flush what is pending, then its segments
-                if (!buf.empty()) {
-                    int rc = launch_track(&b, buf.data(), (int32_t)buf.size(), 1, next_table_version(), buf_spr);
-                    if (rc != BT_OK) return rc;
-                    buf.clear();
-                }
-                int rc = launch_segments(turn_ops, spr);
-                if (rc != BT_OK) return rc;
-                continue;
-            }
-            if (buf.size() + turn_ops.size() > K) {
-                int rc = launch_track(&b, buf.data(), (int32_t)buf.size(), 1, next_table_version(), buf_spr);
-                if (rc != BT_OK) return rc;
-                buf.clear();
-            }
-            buf.insert(buf.end(), turn_ops.begin(), turn_ops.end());
-            buf_spr = spr;
-        }
-        if (!buf.empty()) {
-            int rc = launch_track(&b, buf.data(), (int32_t)buf.size(), 1, next_table_version(), buf_spr);
-            if (rc != BT_OK) return rc;
-        }
-        b.gamma = gamma;
-    }
+    WalkPlan plan;
+    plan_walk(b, nturns, plan);
+    const int rc = run_plan(b, plan);
+    if (rc != BT_OK) return rc;
+    b.gamma = plan.gamma_after;  // S3
     b.s += b.lattice_length * (double)nturns;
     b.turn += nturns;
     return BT_OK;
@@ -512,9 +574,9 @@ int bt_track_diagnostics(bt_beam *beam, int32_t nturns, double *host_moments) {
             ops.clear();
             double slots = 0.0;
             const double gamma_after = build_turn_table(one, b.gamma, ops, &slots);
-            for (size_t lo = 0; lo < ops.size(); lo += (size_t)kConstTableRecords) {
-                const size_t len = ops.size() - lo < (size_t)kConstTableRecords ? ops.size() - lo : (size_t)kConstTableRecords;
-                rc_all = launch_track(&b, ops.data() + lo, (int32_t)len, 1, next_table_version(), slots / (double)ops.size());
+            for (size_t lo = 0; lo < ops.size(); lo += (size_t)kTableRecords) {
+                const size_t len = ops.size() - lo < (size_t)kTableRecords ? ops.size() - lo : (size_t)kTableRecords;
+                rc_all = launch_track(&b, ops.data() + lo, (int32_t)len, 1, slots / (double)ops.size());
                 if (rc_all != BT_OK) break;
             }
             if (rc_all != BT_OK) break;
@@ -535,7 +597,9 @@ int bt_track_diagnostics(bt_beam *beam, int32_t nturns, double *host_moments) {
 }
 
 // Host-to-host walk: chunks of the bunch ride three streams, so that the H2D copy of chunk k+1, the walk of chunk k and
-// the D2H copy of chunk k-1 overlap (PCIe is full duplex; particles are independent, so any partition is exact).
+// the D2H copy of chunk k-1 overlap (PCIe is full duplex; particles are independent, so any partition is exact).  Every
+// chunk runs the same plan of launches; a launch carries its record table as kernel parameters, so chunks on different
+// streams may be at different launches of the plan (lattices whose RF changes the reference energy included).
 int bt_track_host(bt_beam *beam, const double *const host_in[6], double *const host_out[6], int32_t nturns, int32_t nchunks) {
     if (!beam || !host_in || !host_out) return fail(BT_ERR_INVALID, "bt_track_host: NULL argument");
     for (int i = 0; i < 6; ++i)
@@ -545,16 +609,7 @@ int bt_track_host(bt_beam *beam, const double *const host_in[6], double *const h
     Beam &b = beam->b;
     if (b.lattice.empty()) return fail(BT_ERR_STATE, "bt_track_host: bt_lattice_set not called");
     if (!b.has_ref) return fail(BT_ERR_STATE, "bt_track_host: bt_beam_set_ref not called");
-    const size_t K = (size_t)kConstTableRecords;
-    if (!b.energy_changes && !b.table_valid) {
-        b.h_table.clear();
-        build_turn_table(b.lattice, b.gamma, b.h_table, &b.table_slots);
-        b.table_version = next_table_version();
-        b.table_valid = true;
-    }
-    // Lattices that need several tables per call (RF changing the reference energy, more records than the constant
-    // bank holds) replace the table between launches; their chunks cannot share it across streams: one chunk.
-    if (nturns == 0 || nchunks == 1 || b.energy_changes || b.h_table.size() > K) {
+    if (nturns == 0 || nchunks == 1) {
         int rc = bt_beam_upload(beam, host_in);
         if (rc == BT_OK) rc = bt_track(beam, nturns);
         if (rc == BT_OK) rc = bt_beam_download(beam, host_out);
@@ -564,35 +619,41 @@ int bt_track_host(bt_beam *beam, const double *const host_in[6], double *const h
         if (!b.pipe_stream[i]) BT_CUDA_TRY(cudaStreamCreateWithFlags(&b.pipe_stream[i], cudaStreamNonBlocking));
         if (!b.pipe_event[i]) BT_CUDA_TRY(cudaEventCreateWithFlags(&b.pipe_event[i], cudaEventDisableTiming));
     }
+    WalkPlan plan;
+    plan_walk(b, nturns, plan);
     // the chunk streams start after everything already queued on the beam's stream
     BT_CUDA_TRY(cudaEventRecord(b.pipe_event[0], b.stream));
     for (int i = 0; i < 3; ++i) BT_CUDA_TRY(cudaStreamWaitEvent(b.pipe_stream[i], b.pipe_event[0], 0));
     const long long gran = 1024;  // keeps every chunk's arrays as aligned as the whole arrays
-    long long len = ((b.n + nchunks - 1) / nchunks + gran - 1) / gran * gran;
-    const double spr = b.table_slots / (double)b.h_table.size();
+    const long long len = ((b.n + nchunks - 1) / nchunks + gran - 1) / gran * gran;
+    int rc = BT_OK;
+    cudaError_t ce = cudaSuccess;
     int k = 0;
-    for (long long off = 0; off < b.n; off += len, ++k) {
+    for (long long off = 0; off < b.n && rc == BT_OK && ce == cudaSuccess; off += len, ++k) {
         const long long m = b.n - off < len ? b.n - off : len;
         cudaStream_t st = b.pipe_stream[k % 3];
-        for (int i = 0; i < 6; ++i)
-            BT_CUDA_TRY(cudaMemcpyAsync(b.q[i] + off, host_in[i] + off, (size_t)m * sizeof(double), cudaMemcpyHostToDevice, st));
+        for (int i = 0; i < 6 && ce == cudaSuccess; ++i)
+            ce = cudaMemcpyAsync(b.q[i] + off, host_in[i] + off, (size_t)m * sizeof(double), cudaMemcpyHostToDevice, st);
+        if (ce != cudaSuccess) break;
         TrackRange r;
         r.off = off, r.n = m, r.geom_n = b.n, r.stream = st;
         b.range = &r;
-        const int rc = launch_track(&b, b.h_table.data(), (int32_t)b.h_table.size(), nturns, b.table_version, spr);
+        rc = run_plan(b, plan);
         b.range = nullptr;
-        if (rc != BT_OK) return rc;
-        for (int i = 0; i < 6; ++i)
-            BT_CUDA_TRY(cudaMemcpyAsync(host_out[i] + off, b.q[i] + off, (size_t)m * sizeof(double), cudaMemcpyDeviceToHost, st));
+        for (int i = 0; i < 6 && rc == BT_OK && ce == cudaSuccess; ++i)
+            ce = cudaMemcpyAsync(host_out[i] + off, b.q[i] + off, (size_t)m * sizeof(double), cudaMemcpyDeviceToHost, st);
     }
+    // join the chunk streams on every path (an error above must not leave them running behind the caller's back)
     for (int i = 0; i < 3; ++i) {
-        BT_CUDA_TRY(cudaEventRecord(b.pipe_event[i], b.pipe_stream[i]));
-        BT_CUDA_TRY(cudaStreamWaitEvent(b.stream, b.pipe_event[i], 0));
+        if (cudaEventRecord(b.pipe_event[i], b.pipe_stream[i]) == cudaSuccess) cudaStreamWaitEvent(b.stream, b.pipe_event[i], 0);
     }
-    int rc = record_table_busy(&b, b.stream);
-    if (rc != BT_OK) return rc;
-    BT_CUDA_TRY(cudaStreamSynchronize(b.stream));
+    const cudaError_t se = cudaStreamSynchronize(b.stream);
     b.permuted = false;  // storage order = the caller's order
+    b.deposits_since_sort = 0;
+    if (rc != BT_OK) return rc;
+    if (ce != cudaSuccess) return fail(BT_ERR_CUDA, std::string("bt_track_host: copy: ") + cudaGetErrorString(ce));
+    if (se != cudaSuccess) return fail(BT_ERR_CUDA, std::string("bt_track_host: ") + cudaGetErrorString(se));
+    b.gamma = plan.gamma_after;
     b.s += b.lattice_length * (double)nturns;
     b.turn += nturns;
     return BT_OK;
@@ -649,6 +710,7 @@ void bt_grid_destroy(bt_grid *grid) {
     if (grid->g.rho) cudaFree(grid->g.rho);
     if (grid->g.field) cudaFree(grid->g.field);
     if (grid->g.phi) cudaFree(grid->g.phi);
+    if (grid->g.done) cudaEventDestroy(grid->g.done);
     delete grid;
 }
 
@@ -657,8 +719,11 @@ int bt_grid_set_field(bt_grid *grid, const double *Ex, const double *Ey, const d
     Grid &g = grid->g;
     const size_t bytes = (size_t)g.nn * sizeof(double);
     if (!g.field) BT_CUDA_TRY(cudaMalloc(&g.field, bytes * 4));
-    cudaStream_t s = g.last_stream;
-    if (on_device) return launch_field_pack(&g, Ex, Ey, Ez, s);
+    cudaStream_t s = g.last_stream;  // ordered after whatever used the grid last; the caller's Ex/Ey/Ez must be ready on it
+    if (on_device) {
+        const int rc = launch_field_pack(&g, Ex, Ey, Ez, s);
+        return rc != BT_OK ? rc : grid_release(&g, s);
+    }
     double *tmp = nullptr;
     BT_CUDA_TRY(cudaMalloc(&tmp, bytes * 3));
     cudaError_t e = cudaMemcpyAsync(tmp, Ex, bytes, cudaMemcpyHostToDevice, s);
@@ -671,7 +736,7 @@ int bt_grid_set_field(bt_grid *grid, const double *Ex, const double *Ey, const d
         rc = launch_field_pack(&g, tmp, tmp + g.nn, tmp + 2 * g.nn, s);
     cudaStreamSynchronize(s);
     cudaFree(tmp);
-    return rc;
+    return rc != BT_OK ? rc : grid_release(&g, s);
 }
 
 int bt_grid_rho(bt_grid *grid, double **dev_rho_out) {
@@ -693,7 +758,9 @@ int bt_grid_solve_poisson(bt_grid *grid, double gz, void *cuda_stream) {
     if (!(gz > 0.0) || !isfinite(gz)) return fail(BT_ERR_INVALID, "bt_grid_solve_poisson: gz must be positive and finite");
     Grid &g = grid->g;
     if ((int64_t)8 * g.nn > ((int64_t)1 << 31) - 1) return fail(BT_ERR_UNSUPPORTED, "bt_grid_solve_poisson: padded grid exceeds 2^31 nodes");
-    return poisson_solve(&g, gz, (cudaStream_t)cuda_stream);
+    int rc = grid_acquire(&g, (cudaStream_t)cuda_stream);  // rho may still be in flight on a beam's stream
+    if (rc == BT_OK) rc = poisson_solve(&g, gz, (cudaStream_t)cuda_stream);
+    return rc != BT_OK ? rc : grid_release(&g, (cudaStream_t)cuda_stream);
 }
 
 int bt_grid_download_phi(bt_grid *grid, double *host_phi) {
@@ -735,7 +802,8 @@ int bt_deposit_cic(bt_beam *beam, bt_grid *grid, double q_weight, double zscale,
     if (!isfinite(q_weight) || !isfinite(zscale)) return fail(BT_ERR_INVALID, "bt_deposit_cic: q_weight or zscale not finite");
     Beam &b = beam->b;
     Grid &g = grid->g;
-    g.last_stream = b.stream;
+    int arc = grid_acquire(&g, b.stream);
+    if (arc != BT_OK) return arc;
     if (b.resort_interval > 0) {  // S4 cadence: re-bin the storage every resort_interval deposits (the first one included)
         if (b.deposits_since_sort % b.resort_interval == 0) {
             const int rc = sort_by_cell(&b, &g, zscale);
@@ -745,7 +813,8 @@ int bt_deposit_cic(bt_beam *beam, bt_grid *grid, double q_weight, double zscale,
         b.deposits_since_sort += 1;
     }
     if (zero_first) BT_CUDA_TRY(cudaMemsetAsync(g.rho, 0, (size_t)g.nn * sizeof(double), b.stream));
-    return launch_deposit(&b, &g, q_weight, zscale);
+    arc = launch_deposit(&b, &g, q_weight, zscale);
+    return arc != BT_OK ? arc : grid_release(&g, b.stream);
 }
 
 int bt_beam_set_resort_interval(bt_beam *beam, int32_t every_n_deposits) {
@@ -769,13 +838,16 @@ int bt_gather_kick(bt_beam *beam, const bt_grid *grid, const double coef[3], dou
     if (!(half_drift_before >= 0.0) || !(half_drift_after >= 0.0) || !isfinite(half_drift_before) || !isfinite(half_drift_after))
         return fail(BT_ERR_INVALID, "bt_gather_kick: negative or non-finite drift length");
     Beam &b = beam->b;
-    const Grid &g = grid->g;
+    Grid &g = const_cast<Grid &>(grid->g);  // const for the caller: the field is only read; the ordering event is bookkeeping
     if (!g.field) return fail(BT_ERR_STATE, "bt_gather_kick: bt_grid_set_field not called");
     if (!b.has_ref) return fail(BT_ERR_STATE, "bt_gather_kick: bt_beam_set_ref not called");
+    int rc = grid_acquire(&g, b.stream);  // the field may still be in flight on the stream of bt_grid_solve_poisson
+    if (rc != BT_OK) return rc;
     const double bg2 = b.gamma * b.gamma - 1.0;
     const double bg = sqrt(bg2);
     const double tcb = half_drift_before / (bg * bg), tca = half_drift_after / (bg * bg);  // R4
-    int rc = launch_gather_kick(&b, &g, coef, zscale, half_drift_before, tcb, half_drift_after, tca);
+    rc = launch_gather_kick(&b, &g, coef, zscale, half_drift_before, tcb, half_drift_after, tca);
+    if (rc == BT_OK) rc = grid_release(&g, b.stream);
     if (rc != BT_OK) return rc;
     b.s += half_drift_before + half_drift_after;
     return BT_OK;

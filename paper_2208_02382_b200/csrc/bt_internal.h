@@ -17,6 +17,14 @@ void set_error(const std::string &msg);
 int fail(int code, const std::string &msg);
 extern std::atomic<int64_t> g_launch_count;
 
+// Debug knobs (bt_debug_knob): A/B measurements and the tests that exercise every kernel variant.  -1 = measured default.
+enum Knob { KNOB_TRACK_PPT = 0, KNOB_TRACK_BLOCK, KNOB_TRACK_FUSE, KNOB_DEPOSIT_MODE, KNOB_GATHER_MODE, KNOB_COUNT };
+extern std::atomic<int32_t> g_knob[KNOB_COUNT];
+static inline int knob(Knob k, int dflt) {
+    const int v = g_knob[k].load(std::memory_order_relaxed);
+    return v < 0 ? dflt : v;
+}
+
 #define BT_CUDA_TRY(expr)                                                                        \
     do {                                                                                         \
         cudaError_t _e = (expr);                                                                 \
@@ -45,8 +53,11 @@ enum Op : int32_t {
     OP_DRIFTX = 1 << 13,  // exact drift (R17), count slices: c0 = h, c1 = 1/beta0
     OP_QUADCHR = 1 << 15, // chromatic quad (R20), count slices: c0 = h, c1 = 1/beta0, c2 = |k|, c3 = +1 (k > 0: x focusing) / -1 / 0 (k = 0)
     OP_RFSIN = 1 << 14,   // sinusoidal short RF (R18): px *= c0; py *= c0; pt = c0 pt + c1 (cos(c2 t + c3) - c4)
-    OP_TAILDRIFT = 1 << 12  // modifier of SEXT/OCT/SEXTOCT: the single-slice drift that follows the kick rides in the
-                            // same record (c3 = h, c4 = h/(b0 g0)^2); same arithmetic, same order, one dispatch less
+    OP_TAILDRIFT = 1 << 12,  // modifier of SEXT/OCT/SEXTOCT: the single-slice drift that follows the kick rides in the
+                             // same record (c3 = h, c4 = h/(b0 g0)^2); same arithmetic, same order, one dispatch less
+    OP_HALFCELL = 1 << 16   // head of a run of `count` half cells [QUAD1][SEXTOCT|TAILDRIFT]: this record holds the first quad's
+                            // coefficients (c0..c6 as QUAD1), the next one the kicks' and the drift's (as SEXTOCT|TAILDRIFT), and so
+                            // on for 2*count records, which the walk consumes in one dispatch
 };
 
 struct alignas(16) DevOp {
@@ -56,7 +67,9 @@ struct alignas(16) DevOp {
 };
 static_assert(sizeof(DevOp) == 64, "DevOp must be 64 bytes");
 
-constexpr int kConstTableRecords = 1024;  // 64 KiB constant bank / 64 B
+// The record table of a launch travels in the kernel's parameter space (32 764 bytes on sm_70+; constant bank 0).
+constexpr int kTableRecords = 510;      // 80-byte launch header + 510 x 64 B = 32 720 B
+constexpr int kTableRecordsSmall = 30;  // short lattices: 2 000 B of parameters
 constexpr int kMaxDevices = 64;
 
 struct TrackLaunchInfo {
@@ -91,7 +104,6 @@ struct Beam {
     double lattice_length = 0.0;
     std::vector<DevOp> h_table;  // single-turn record table for the current lattice and gamma (static lattices)
     bool table_valid = false;    // h_table is up to date
-    uint64_t table_version = 0;  // identifies h_table's contents in the device's constant bank (track.cu)
     double table_slots = 0.0;    // FP64 slots per particle per turn of that table
     TrackLaunchInfo last_launch;
     // S4 cell binning: storage order != original order once sorted; ids[j] = original index of slot j
@@ -117,7 +129,11 @@ struct Grid {
     double *field = nullptr;  // interleaved (Ex,Ey,Ez,pad) per node: 4*nn doubles, or nullptr
     double *phi = nullptr;    // potential at the nodes (bt_grid_solve_poisson), or nullptr
     void *poisson = nullptr;  // solver state (plans, padded buffers, cached Green transform), poisson.cu
+    // cross-stream ordering: every operation on the grid's arrays waits for `done` of the previous one when it runs on
+    // another stream (deposit on the beam's stream, solve on the caller's, gather on the beam's again, ...)
     cudaStream_t last_stream = nullptr;
+    cudaEvent_t done = nullptr;
+    bool done_valid = false;
 };
 
 // ---- host precompute (S1/S3), in bt_api.cu ------------------------------------------------------
@@ -126,14 +142,13 @@ struct Grid {
 // FP64 instruction slots one particle spends in this pass (minimal DFMA/DMUL sequences).
 double build_turn_table(const std::vector<bt_element> &lat, double gamma, std::vector<DevOp> &out, double *slots);
 
+int grid_acquire(Grid *g, cudaStream_t s);  // make `s` wait for the last operation enqueued on the grid (no-op on the same stream)
+int grid_release(Grid *g, cudaStream_t s);  // record that the grid's latest operation was enqueued on `s`
+
 // ---- launchers --------------------------------------------------------------------------------
-// One fused-walk launch: n_ops (<= kConstTableRecords) host records are placed in the constant bank (skipped when
-// `version` of this beam is already resident) and walked nturns times.  slots_per_record (FP64 slots per particle per
-// record, averaged) steers the particles-per-thread choice.
-int launch_track(Beam *b, const DevOp *h_table, int32_t n_ops, int32_t nturns, uint64_t version, double slots_per_record);
-uint64_t next_table_version();
-void forget_table_owner(const Beam *b);
-int record_table_busy(const Beam *b, cudaStream_t stream);  // marks `stream` as the table's last reader
+// One fused-walk launch: n_ops (<= kTableRecords) host records travel as kernel parameters and are walked nturns times.
+// slots_per_record (FP64 slots per particle per record, averaged) steers the particles-per-thread choice.
+int launch_track(Beam *b, const DevOp *h_table, int32_t n_ops, int32_t nturns, double slots_per_record);
 int launch_deposit(Beam *b, Grid *g, double q_weight, double zscale);
 int launch_gather_kick(Beam *b, const Grid *g, const double coef[3], double zscale, double h_before,
                        double tc_before, double h_after, double tc_after);

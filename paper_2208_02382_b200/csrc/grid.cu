@@ -322,9 +322,20 @@ __global__ void __launch_bounds__(NT, kBinMinBlocks<NT, R, ORDER>) deposit_binne
     }
 }
 
-static int env_int_grid(const char *name, int dflt) {
-    const char *v = getenv(name);
-    return (v && *v) ? atoi(v) : dflt;
+// cudaFuncSetAttribute + the occupancy query, once per (kernel instantiation, device)
+template <auto kernel>
+static int blocks_per_sm(int threads, int smem, int device, int *out) {
+    static std::atomic<int> cache[kMaxDevices];  // 0 = not queried yet; one array per kernel instantiation
+    if (device < 0 || device >= kMaxDevices) return fail(BT_ERR_UNSUPPORTED, "device index too large");
+    int v = cache[device].load(std::memory_order_acquire);
+    if (v == 0) {
+        BT_CUDA_TRY(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+        BT_CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&v, kernel, threads, smem));
+        if (v < 1) v = 1;
+        cache[device].store(v, std::memory_order_release);
+    }
+    *out = v;
+    return BT_OK;
 }
 
 template <int NT, int R, bool VEC, int ORDER>
@@ -332,8 +343,8 @@ static int launch_deposit_binned(Beam *b, Grid *g, const GridDev &gd, double q_w
     const int smem = (int)sizeof(BinSmem<NT, R>);
     const long long nchunks = (b->n + BinSmem<NT, R>::CH - 1) / BinSmem<NT, R>::CH;
     int per_sm = 1;
-    BT_CUDA_TRY(cudaFuncSetAttribute(deposit_binned_kernel<NT, R, VEC, ORDER>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
-    BT_CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, deposit_binned_kernel<NT, R, VEC, ORDER>, NT, smem));
+    const int qrc = blocks_per_sm<deposit_binned_kernel<NT, R, VEC, ORDER>>(NT, smem, b->device, &per_sm);
+    if (qrc != BT_OK) return qrc;
     long long blocks = (long long)b->num_sms * (per_sm > 0 ? per_sm : 1);
     if (blocks > nchunks) blocks = nchunks;
     deposit_binned_kernel<NT, R, VEC, ORDER><<<(int)blocks, NT, smem, b->stream>>>(b->q[0], b->q[2], b->q[4], b->n, gd, q_weight,
@@ -343,10 +354,10 @@ static int launch_deposit_binned(Beam *b, Grid *g, const GridDev &gd, double q_w
 
 template <int ORDER>
 static int launch_deposit_order(Beam *b, Grid *g, const GridDev &gd, double q_weight, double zscale) {
-    // BT_DEPOSIT_MODE: 0 = one particle per thread, (ORDER+1)^3 reductions each (baseline, kept for measurements);
+    // knob deposit_mode: 0 = one particle per thread, (ORDER+1)^3 reductions each (baseline, kept for measurements);
     // 1 (default) = block-local cell binning, 8 particles per thread (4 for order 2: 27 run accumulators per thread);
     // 2 = binning with 4 particles per thread
-    const int mode = env_int_grid("BT_DEPOSIT_MODE", 1);
+    const int mode = knob(KNOB_DEPOSIT_MODE, 1);
     if (mode == 0) {
         const int block = 256;
         long long blocks = (b->n + block - 1) / block;
@@ -412,10 +423,12 @@ __device__ __forceinline__ void ld_node(const double *f, double &ex, double &ey,
 template <int ORDER>
 __device__ __forceinline__ void gather_kick_one(const GatherArgs &a, double &x, double &px, double &y, double &py, double &t, double &pt) {
     constexpr int NW = ORDER + 1;
-    // R4 drift before the kick
-    x = fma(a.hb, px, x);
-    y = fma(a.hb, py, y);
-    t = fma(a.tcb, pt, t);
+    // R4 drift before the kick (a zero-length drift is no map at all: positions stay bit-identical, also for non-finite momenta)
+    if (a.hb != 0.0 || a.tcb != 0.0) {
+        x = fma(a.hb, px, x);
+        y = fma(a.hb, py, y);
+        t = fma(a.tcb, pt, t);
+    }
     Cic c;
     if (shape_locate<ORDER>(a.g, x, y, t, a.zscale, c)) {
         const double *base = a.field + 4 * (((long long)c.k * a.g.ny + c.j) * a.g.nx + c.i);
@@ -448,9 +461,11 @@ __device__ __forceinline__ void gather_kick_one(const GatherArgs &a, double &x, 
         pt = fma(a.coef[2], ez, pt);
     }
     // R4 drift after the kick
-    x = fma(a.ha, px, x);
-    y = fma(a.ha, py, y);
-    t = fma(a.tca, pt, t);
+    if (a.ha != 0.0 || a.tca != 0.0) {
+        x = fma(a.ha, px, x);
+        y = fma(a.ha, py, y);
+        t = fma(a.tca, pt, t);
+    }
 }
 
 template <int ORDER>
@@ -545,8 +560,8 @@ static int launch_gather_pipe(Beam *b, const GatherArgs &a0) {
     const long long nchunks = b->n / CH;
     if (nchunks > 0) {
         int per_sm = 1;
-        BT_CUDA_TRY(cudaFuncSetAttribute(gather_kick_pipe_kernel<NT, R, ORDER>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
-        BT_CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, gather_kick_pipe_kernel<NT, R, ORDER>, NT, smem));
+        const int qrc = blocks_per_sm<gather_kick_pipe_kernel<NT, R, ORDER>>(NT, smem, b->device, &per_sm);
+        if (qrc != BT_OK) return qrc;
         long long blocks = (long long)b->num_sms * (per_sm > 0 ? per_sm : 1);
         if (blocks > nchunks) blocks = nchunks;
         const int store_positions = (a0.hb != 0.0 || a0.ha != 0.0 || a0.tcb != 0.0 || a0.tca != 0.0) ? 1 : 0;
@@ -610,10 +625,12 @@ __global__ void __launch_bounds__(256, 3) gather_kick_tile_kernel(const __grid_c
         double(*q)[CH] = sm.q[s];
         int *box = sm.box[bpar];
         double x = q[0][tid], px = q[1][tid], y = q[2][tid], py = q[3][tid], t = q[4][tid], pt = q[5][tid];
-        // R4 drift before the kick
-        x = fma(a.hb, px, x);
-        y = fma(a.hb, py, y);
-        t = fma(a.tcb, pt, t);
+        // R4 drift before the kick (skipped when zero-length, as in gather_kick_one)
+        if (a.hb != 0.0 || a.tcb != 0.0) {
+            x = fma(a.hb, px, x);
+            y = fma(a.hb, py, y);
+            t = fma(a.tcb, pt, t);
+        }
         Cic c;
         const bool in = shape_locate<ORDER>(a.g, x, y, t, a.zscale, c);
         {   // bounding box of the chunk's stencil bases
@@ -688,9 +705,11 @@ __global__ void __launch_bounds__(256, 3) gather_kick_tile_kernel(const __grid_c
             pt = fma(a.coef[2], ez, pt);
         }
         // R4 drift after the kick
-        x = fma(a.ha, px, x);
-        y = fma(a.ha, py, y);
-        t = fma(a.tca, pt, t);
+        if (a.ha != 0.0 || a.tca != 0.0) {
+            x = fma(a.ha, px, x);
+            y = fma(a.ha, py, y);
+            t = fma(a.tca, pt, t);
+        }
         q[0][tid] = x, q[1][tid] = px, q[2][tid] = y, q[3][tid] = py, q[4][tid] = t, q[5][tid] = pt;
         fence_proxy_async_smem();  // this thread's shared-memory writes -> visible to the copy engine
         __syncthreads();           // (3) stage complete; everyone is done with the tile
@@ -717,8 +736,8 @@ static int launch_gather_tile(Beam *b, const GatherArgs &a0) {
     const long long nchunks = b->n / CH;
     if (nchunks > 0) {
         int per_sm = 1;
-        BT_CUDA_TRY(cudaFuncSetAttribute(gather_kick_tile_kernel<ORDER>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
-        BT_CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, gather_kick_tile_kernel<ORDER>, 256, smem));
+        const int qrc = blocks_per_sm<gather_kick_tile_kernel<ORDER>>(256, smem, b->device, &per_sm);
+        if (qrc != BT_OK) return qrc;
         long long blocks = (long long)b->num_sms * (per_sm > 0 ? per_sm : 1);
         if (blocks > nchunks) blocks = nchunks;
         const int store_positions = (a0.hb != 0.0 || a0.ha != 0.0 || a0.tcb != 0.0 || a0.tca != 0.0) ? 1 : 0;
@@ -736,12 +755,12 @@ static int launch_gather_tile(Beam *b, const GatherArgs &a0) {
 
 template <int ORDER>
 static int launch_gather_order(Beam *b, const GatherArgs &a) {
-    // BT_GATHER_MODE: 0 = one particle per thread, everything through registers (also the path for arrays that are not
+    // knob gather_mode: 0 = one particle per thread, everything through registers (also the path for arrays that are not
     // 16-byte aligned); 1 (default) = streaming pipeline, 256-particle chunks, field through L1 (order 1) or staged in shared
     // memory (order 2); 2 / 3 = L1 pipeline with 512 / 128-particle chunks; 4 = shared-memory tile at any order
-    const int mode = env_int_grid("BT_GATHER_MODE", 1);
+    const int mode = knob(KNOB_GATHER_MODE, 1);
     // field tile staged in shared memory: the default at order 2 (measured 4A 10-step mean 547 -> 477 us, 4B 529 -> 430 us),
-    // selectable at order 1 (BT_GATHER_MODE=4), where the L1 path is faster (181 against 216 us)
+    // selectable at order 1 (knob gather_mode = 4), where the L1 path is faster (181 against 216 us)
     // only on cell-sorted beams: in the caller's order no chunk's box fits the tile and the pass through L1 is faster from
     // the plain pipeline (order 2, unsorted kick: 0.79 against 1.51 ms)
     if ((mode == 4 || (mode == 1 && ORDER == 2 && b->permuted)) && b->aligned16) return launch_gather_tile<ORDER>(b, a);

@@ -6,7 +6,8 @@
 // One pass needs a provisional centre k (a two-pass scheme would read the bunch twice): with d = q - k,
 //   S_i = sum d_i , P_ij = sum d_i d_j  =>  mean_i = k_i + S_i/n , cov_ij = P_ij/n - (S_i/n)(S_j/n),
 // which is the definition exactly (algebraically) and loses no digits as long as |k - mean| is of the order of the rms
-// size: k is the mean of the first min(n, 256) particles (every block recomputes it), so the subtracted term is ~ cov/256.
+// size: k is the mean of min(n, 256) particles sampled at a stride of n/256 through the storage (every block recomputes
+// it), so the subtracted term is ~ cov/256 in any storage order, cell-sorted included.
 // HBM-bound: 48 bytes and 33 FP64 issue slots per particle.  Deterministic: fixed partition, fixed reduction trees,
 // the per-block partials are combined in block order by the last block to finish.
 #include "bt_internal.h"
@@ -52,14 +53,17 @@ template <bool VEC2>
 __global__ void __launch_bounds__(kMomBlock) moments_kernel(const __grid_constant__ MomArgs a) {
     __shared__ double scratch[kMomBlock / 32];
     __shared__ bool is_last;
-    // provisional centre: mean of the first min(n, 256) particles, computed by every block in the same order (bitwise
-    // identical everywhere; after the first block these 12 KiB are L2 hits)
+    // provisional centre: mean of min(n, 256) particles taken at a stride of n/256 through the storage -- representative in
+    // any storage order (after bt_beam_sort_by_cell the FIRST 256 particles all sit in one corner of the grid, several
+    // sigma from the mean) -- computed by every block in the same order (bitwise identical everywhere; L2 hits after the
+    // first block)
     double k[6];
     {
         const long long m = a.n < kCentreSample ? a.n : kCentreSample;
+        const long long stride = a.n / m;
         double v[6];
 #pragma unroll
-        for (int c = 0; c < 6; ++c) v[c] = threadIdx.x < m ? a.q[c][threadIdx.x] : 0.0;
+        for (int c = 0; c < 6; ++c) v[c] = threadIdx.x < m ? a.q[c][threadIdx.x * stride] : 0.0;
 #pragma unroll
         for (int c = 0; c < 6; ++c) k[c] = block_sum(v[c], scratch) / (double)m;
     }

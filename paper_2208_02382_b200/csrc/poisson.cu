@@ -228,7 +228,6 @@ int poisson_solve(Grid *g, double gz, cudaStream_t stream) {
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return fail(BT_ERR_CUDA, std::string("bt_grid_solve_poisson launch: ") + cudaGetErrorString(e));
     g_launch_count.fetch_add(3);
-    g->last_stream = stream;
     return BT_OK;
 }
 

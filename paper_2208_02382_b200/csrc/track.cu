@@ -4,46 +4,54 @@
 // particle per launch.  Arithmetic is pure FP64 DFMA/DMUL: every transcendental is an element
 // parameter and was folded into the per-slice coefficients on the host (bt_api.cu: build_turn_table).
 //
-// Thread mapping: each thread owns P particles (P = 1, 2, 4 or 8); one warp = one task of 32*P particles
+// Thread mapping: each thread owns P particles (P = 1, 2 or 4); one warp = one task of 32*P particles
 // that walks the whole record table.
 //
-// Record table: the CONSTANT bank (64 KiB = 1024 records of 64 B).  The walk is warp-uniform, so every
-// record word is fetched with a uniform-datapath constant load (LDCU) straight into a uniform register and
-// used as the UR operand of the DFMAs -- no vector-register traffic, no R2UR moves, and the dispatch is
-// uniform compares + uniform branches.  Measured on B200 against the alternatives (shared-memory table,
-// global table through L1, either with software-prefetched records in vector registers): vector-register
-// coefficients cost FP64 issue rate (three 64-bit vector operands per DFMA), and R2UR of loaded words sits
-// on the dependency chain of every element; the constant-bank walk keeps the FP64 pipe busiest.
+// Record table: KERNEL PARAMETER space (a __grid_constant__ struct of up to 32 764 bytes = 510 records of 64 B).
+// Parameters live in constant bank 0, so -- exactly as with a __constant__ array -- the warp-uniform walk fetches every
+// record word with a uniform-datapath constant load (SASS: LDCU UR, c[0x0][UR+off]) straight into a uniform register and
+// uses it as the UR operand of the DFMAs: no vector-register traffic, no R2UR moves, and the dispatch is uniform
+// compares + uniform branches.  Unlike a __constant__ array the table belongs to the LAUNCH: nothing on the device is
+// shared between beams, streams or launches, so beams on different streams / host threads and the chunk streams of
+// bt_track_host need no serialisation, and a lattice whose RF changes the reference energy simply passes a different
+// table with every launch.  (Round 1 kept one 64 KiB __constant__ table per device behind a mutex and an event.)
+// Measured on B200 against the alternatives (shared-memory table, global table through L1, either with
+// software-prefetched records in vector registers): vector-register coefficients cost FP64 issue rate (three 64-bit
+// vector operands per DFMA), and R2UR of loaded words sits on the dependency chain of every element.
 // Lattices x turns longer than one table are walked in several launches (bt_api.cu plans them).
 //
 // Opcodes are one-hot bits, tested with a short uniform compare tree ordered by how often the kinds occur;
-// the host specialises single-slice elements (no loop control) and groups of five quad slices (unrolled).
+// the host specialises single-slice elements (no loop control), groups of five quad slices (unrolled) and runs of
+// [single-slice quad, sextupole, octupole, single-slice drift] half cells (one dispatch for the whole run).
 #include "bt_internal.h"
 
 #include <stdlib.h>
-
-#include <mutex>
+#include <string.h>
 
 namespace bt {
 
 constexpr int kMaxBlock = 128;  // launch bound; the default block is 64 threads (fine-grained balance over SMs)
 
-__constant__ DevOp c_table[kConstTableRecords];
-
 // Register budget per instantiation (128-thread blocks per SM the compiler must allow): the per-record latency
 // (constant loads, compare tree, branch) is covered by other warps, so P <= 4 is held to 80 registers
-// (6 warps per sub-partition); P = 8 needs 96 registers for the particles alone.
+// (6 warps per sub-partition).
 template <int P>
-constexpr int kMinBlocks = P <= 2 ? 8 : P == 4 ? 6 : 3;
+constexpr int kMinBlocks = P <= 2 ? 8 : 6;
 
+// Kernel parameters: launch geometry + the record table itself.  Two capacities, so that short lattices (configs[0]:
+// 5 records) do not push 32 KiB of parameters through every launch.
+template <int NREC>
 struct TrackArgs {
     double *q[6];
     long long n;
     long long tail_start;  // first particle handled by the guarded P=1 blocks
     int n_full_blocks;     // blocks [0, n_full_blocks) run the unguarded P-particle path
-    int n_ops;             // records in c_table for this launch
+    int n_ops;             // records of tab[] in use
     int nturns;            // passes over those records
+    int pad_;
+    DevOp tab[NREC];
 };
+static_assert(sizeof(TrackArgs<kTableRecords>) <= 32764, "kernel parameter space is 32 764 bytes");
 
 template <int P>
 struct Ptc {
@@ -136,14 +144,31 @@ __device__ __noinline__ ChrOut quadchr_one(double x, double px, double y, double
     return o;
 }
 
-// ---- one record applied to the P particles of this thread -----------------------------------------
+// ---- the record at tab[e] applied to the P particles of this thread; returns how many records it consumed ----------
 // NL: this instantiation also knows the non-linearised maps (R17, R18, R20).  They need square roots, sincos and exp;
 // compiled into the same kernel they cost the DFMA-only maps registers (configs[1]: 2.61 -> 3.19 ms per step, measured), so
 // lattices without them run the NL = false kernel, which is the linear walk exactly as before.
 template <int P, bool NL>
-__device__ __forceinline__ void apply(Ptc<P> &p, const DevOp &r) {
+__device__ __forceinline__ int apply(Ptc<P> &p, const DevOp *__restrict__ tab, const int e) {
+    const DevOp &r = tab[e];
     const int op = r.op;
-    if (op & (OP_QUAD5 | OP_QUAD1 | OP_QUAD)) {
+    if (op & (OP_HALFCELL | OP_QUAD5 | OP_QUAD1 | OP_QUAD)) {
+        if (op & OP_HALFCELL) {
+            // a run of `count` half cells [quad (one slice), sextupole, octupole, drift (one slice)]: records e, e+1 hold the
+            // first one (quad coefficients; kick and drift coefficients), e+2, e+3 the second, ...  Same arithmetic and order
+            // as the four maps dispatched one by one; one dispatch for the whole run.
+            const int cnt = r.count;
+#pragma unroll 1
+            for (int s = 0; s < cnt; ++s) {
+                const DevOp &qa = tab[e + 2 * s];
+                const DevOp &kb = tab[e + 2 * s + 1];
+                quad_slice<P>(p, qa.c[0], qa.c[1], qa.c[2], qa.c[3], qa.c[4], qa.c[5], qa.c[6]);
+                sext_kick<P>(p, kb.c[0], kb.c[1]);
+                oct_kick<P>(p, kb.c[2]);
+                drift_slice<P>(p, kb.c[3], kb.c[4]);
+            }
+            return 2 * cnt;
+        }
         const double c0 = r.c[0], c1 = r.c[1], c2 = r.c[2], c3 = r.c[3], c4 = r.c[4], c5 = r.c[5], c6 = r.c[6];
         if (op & OP_QUAD5) {  // count groups of five slices
             const int cnt = r.count;
@@ -251,14 +276,15 @@ __device__ __forceinline__ void apply(Ptc<P> &p, const DevOp &r) {
             p.py[j] += fma(c1, zr, c0 * zi);
         }
     }
+    return 1;
 }
 
 template <int P, bool NL>
-__device__ __forceinline__ void walk(Ptc<P> &p, const int n_ops, const int nturns) {
+__device__ __forceinline__ void walk(Ptc<P> &p, const DevOp *__restrict__ tab, const int n_ops, const int nturns) {
 #pragma unroll 1
     for (int turn = 0; turn < nturns; ++turn) {
 #pragma unroll 1
-        for (int e = 0; e < n_ops; ++e) apply<P, NL>(p, c_table[e]);
+        for (int e = 0; e < n_ops;) e += apply<P, NL>(p, tab, e);
     }
 }
 
@@ -278,104 +304,99 @@ __device__ __forceinline__ double ld_stream1(const double *p) {
 }
 __device__ __forceinline__ void st_stream1(double *p, double v) { asm volatile("st.global.cs.f64 [%0], %1;" ::"l"(p), "d"(v) : "memory"); }
 
+template <int P>
+__device__ __forceinline__ void load_ptc(Ptc<P> &p, double *const (&q)[6], const int B) {
+    if constexpr (P >= 2) {  // q[] already point at this thread's first pair
+#pragma unroll
+        for (int j = 0; j < P / 2; ++j) {
+            const int off = j * 2 * B;
+            double2 v;
+            v = ld_stream2(q[0] + off), p.x[2 * j] = v.x, p.x[2 * j + 1] = v.y;
+            v = ld_stream2(q[1] + off), p.px[2 * j] = v.x, p.px[2 * j + 1] = v.y;
+            v = ld_stream2(q[2] + off), p.y[2 * j] = v.x, p.y[2 * j + 1] = v.y;
+            v = ld_stream2(q[3] + off), p.py[2 * j] = v.x, p.py[2 * j + 1] = v.y;
+            v = ld_stream2(q[4] + off), p.t[2 * j] = v.x, p.t[2 * j + 1] = v.y;
+            v = ld_stream2(q[5] + off), p.pt[2 * j] = v.x, p.pt[2 * j + 1] = v.y;
+        }
+    } else {
+        p.x[0] = ld_stream1(q[0]);
+        p.px[0] = ld_stream1(q[1]);
+        p.y[0] = ld_stream1(q[2]);
+        p.py[0] = ld_stream1(q[3]);
+        p.t[0] = ld_stream1(q[4]);
+        p.pt[0] = ld_stream1(q[5]);
+    }
+}
+template <int P>
+__device__ __forceinline__ void store_ptc(const Ptc<P> &p, double *const (&q)[6], const int B) {
+    if constexpr (P >= 2) {
+#pragma unroll
+        for (int j = 0; j < P / 2; ++j) {
+            const int off = j * 2 * B;
+            st_stream2(q[0] + off, make_double2(p.x[2 * j], p.x[2 * j + 1]));
+            st_stream2(q[1] + off, make_double2(p.px[2 * j], p.px[2 * j + 1]));
+            st_stream2(q[2] + off, make_double2(p.y[2 * j], p.y[2 * j + 1]));
+            st_stream2(q[3] + off, make_double2(p.py[2 * j], p.py[2 * j + 1]));
+            st_stream2(q[4] + off, make_double2(p.t[2 * j], p.t[2 * j + 1]));
+            st_stream2(q[5] + off, make_double2(p.pt[2 * j], p.pt[2 * j + 1]));
+        }
+    } else {
+        st_stream1(q[0], p.x[0]);
+        st_stream1(q[1], p.px[0]);
+        st_stream1(q[2], p.y[0]);
+        st_stream1(q[3], p.py[0]);
+        st_stream1(q[4], p.t[0]);
+        st_stream1(q[5], p.pt[0]);
+    }
+}
+
 // P particles per thread (P even: 16-byte vector access; requires 16-byte aligned arrays).
-template <int P, bool NL>
-__global__ void __launch_bounds__(kMaxBlock, kMinBlocks<P>) track_kernel(const __grid_constant__ TrackArgs a) {
+template <int P, bool NL, int NREC>
+__global__ void __launch_bounds__(kMaxBlock, kMinBlocks<P>) track_kernel(const __grid_constant__ TrackArgs<NREC> a) {
     const int tid = threadIdx.x;
     const int B = blockDim.x;
-
     if ((int)blockIdx.x < a.n_full_blocks) {
         // ---- unguarded path: this block owns particles [blk*P*B, (blk+1)*P*B) ----
         Ptc<P> p;
-        const long long base = (long long)blockIdx.x * (P * B);
-        if constexpr (P >= 2) {
-            double *q[6];
+        const long long first = (long long)blockIdx.x * (P * B) + (P >= 2 ? 2 * tid : tid);
+        double *q[6];
 #pragma unroll
-            for (int c = 0; c < 6; ++c) q[c] = a.q[c] + base + 2 * tid;
-#pragma unroll
-            for (int j = 0; j < P / 2; ++j) {
-                const int off = j * 2 * B;
-                double2 v;
-                v = ld_stream2(q[0] + off), p.x[2 * j] = v.x, p.x[2 * j + 1] = v.y;
-                v = ld_stream2(q[1] + off), p.px[2 * j] = v.x, p.px[2 * j + 1] = v.y;
-                v = ld_stream2(q[2] + off), p.y[2 * j] = v.x, p.y[2 * j + 1] = v.y;
-                v = ld_stream2(q[3] + off), p.py[2 * j] = v.x, p.py[2 * j + 1] = v.y;
-                v = ld_stream2(q[4] + off), p.t[2 * j] = v.x, p.t[2 * j + 1] = v.y;
-                v = ld_stream2(q[5] + off), p.pt[2 * j] = v.x, p.pt[2 * j + 1] = v.y;
-            }
-            walk<P, NL>(p, a.n_ops, a.nturns);
-#pragma unroll
-            for (int j = 0; j < P / 2; ++j) {
-                const int off = j * 2 * B;
-                st_stream2(q[0] + off, make_double2(p.x[2 * j], p.x[2 * j + 1]));
-                st_stream2(q[1] + off, make_double2(p.px[2 * j], p.px[2 * j + 1]));
-                st_stream2(q[2] + off, make_double2(p.y[2 * j], p.y[2 * j + 1]));
-                st_stream2(q[3] + off, make_double2(p.py[2 * j], p.py[2 * j + 1]));
-                st_stream2(q[4] + off, make_double2(p.t[2 * j], p.t[2 * j + 1]));
-                st_stream2(q[5] + off, make_double2(p.pt[2 * j], p.pt[2 * j + 1]));
-            }
-        } else {
-            const long long i = base + tid;
-            p.x[0] = ld_stream1(a.q[0] + i);
-            p.px[0] = ld_stream1(a.q[1] + i);
-            p.y[0] = ld_stream1(a.q[2] + i);
-            p.py[0] = ld_stream1(a.q[3] + i);
-            p.t[0] = ld_stream1(a.q[4] + i);
-            p.pt[0] = ld_stream1(a.q[5] + i);
-            walk<P, NL>(p, a.n_ops, a.nturns);
-            st_stream1(a.q[0] + i, p.x[0]);
-            st_stream1(a.q[1] + i, p.px[0]);
-            st_stream1(a.q[2] + i, p.y[0]);
-            st_stream1(a.q[3] + i, p.py[0]);
-            st_stream1(a.q[4] + i, p.t[0]);
-            st_stream1(a.q[5] + i, p.pt[0]);
-        }
+        for (int c = 0; c < 6; ++c) q[c] = a.q[c] + first;
+        load_ptc<P>(p, q, B);
+        walk<P, NL>(p, a.tab, a.n_ops, a.nturns);
+        store_ptc<P>(p, q, B);
     } else {
         // ---- guarded tail: one particle per thread ----
         Ptc<1> p;
         const long long i = a.tail_start + (long long)((int)blockIdx.x - a.n_full_blocks) * B + tid;
         if (i >= a.n) return;
-        p.x[0] = ld_stream1(a.q[0] + i);
-        p.px[0] = ld_stream1(a.q[1] + i);
-        p.y[0] = ld_stream1(a.q[2] + i);
-        p.py[0] = ld_stream1(a.q[3] + i);
-        p.t[0] = ld_stream1(a.q[4] + i);
-        p.pt[0] = ld_stream1(a.q[5] + i);
-        walk<1, NL>(p, a.n_ops, a.nturns);
-        st_stream1(a.q[0] + i, p.x[0]);
-        st_stream1(a.q[1] + i, p.px[0]);
-        st_stream1(a.q[2] + i, p.y[0]);
-        st_stream1(a.q[3] + i, p.py[0]);
-        st_stream1(a.q[4] + i, p.t[0]);
-        st_stream1(a.q[5] + i, p.pt[0]);
+        double *q[6];
+#pragma unroll
+        for (int c = 0; c < 6; ++c) q[c] = a.q[c] + i;
+        load_ptc<1>(p, q, B);
+        walk<1, NL>(p, a.tab, a.n_ops, a.nturns);
+        store_ptc<1>(p, q, B);
     }
 }
 
-static int env_int(const char *name, int dflt) {
-    const char *v = getenv(name);
-    return (v && *v) ? atoi(v) : dflt;
+template <int P, bool NL, int NREC>
+static cudaError_t launch_one(const TrackArgs<NREC> &a, int grid, int block, cudaStream_t stream) {
+    track_kernel<P, NL, NREC><<<grid, block, 0, stream>>>(a);
+    return cudaGetLastError();
 }
 
-// ---- the constant table is one per device: serialise its users -----------------------------------
-// An upload (stream-ordered copy into the constant bank) must not overtake the kernels of another beam
-// (another stream) that still read the previous contents.  Every launch records `busy` after its kernel; an
-// upload first makes its stream wait for `busy`.  `owner`/`version` let a beam skip the upload while its
-// table is still the resident one.
-struct ConstTableState {
-    std::mutex mu;
-    cudaEvent_t busy = nullptr;      // recorded after the last launch that reads the table
-    cudaEvent_t uploaded = nullptr;  // recorded after the table was placed (other streams of the same beam wait on it)
-    const void *owner = nullptr;
-    uint64_t version = 0;
-};
-static ConstTableState g_ct[kMaxDevices];
-static std::atomic<uint64_t> g_table_version{1};
+template <int NREC>
+static cudaError_t launch_sized(TrackArgs<NREC> &a, const DevOp *h_table, int n_ops, int P, bool nl, int grid, int block, cudaStream_t stream) {
+    memcpy(a.tab, h_table, (size_t)n_ops * sizeof(DevOp));
+    switch (P) {
+        case 4: return nl ? launch_one<4, true, NREC>(a, grid, block, stream) : launch_one<4, false, NREC>(a, grid, block, stream);
+        case 2: return nl ? launch_one<2, true, NREC>(a, grid, block, stream) : launch_one<2, false, NREC>(a, grid, block, stream);
+        default: return nl ? launch_one<1, true, NREC>(a, grid, block, stream) : launch_one<1, false, NREC>(a, grid, block, stream);
+    }
+}
 
-uint64_t next_table_version() { return g_table_version.fetch_add(1); }
-
-int launch_track(Beam *b, const DevOp *h_table, int32_t n_ops, int32_t nturns, uint64_t version, double slots_per_record) {
-    if (n_ops < 1 || n_ops > kConstTableRecords) return fail(BT_ERR_INVALID, "launch_track: table size");
-    if (b->device < 0 || b->device >= kMaxDevices) return fail(BT_ERR_UNSUPPORTED, "bt_track: device index too large");
+int launch_track(Beam *b, const DevOp *h_table, int32_t n_ops, int32_t nturns, double slots_per_record) {
+    if (n_ops < 1 || n_ops > kTableRecords) return fail(BT_ERR_INVALID, "launch_track: table size");
     // ---- launch geometry -------------------------------------------------------------------------
     // One warp = one task of 32*P particles walking the whole table.  P amortises the interpreter's per-record
     // work (what matters when records are short: slots_per_record small) but coarsens the tasks: the last tasks
@@ -397,51 +418,42 @@ int launch_track(Beam *b, const DevOp *h_table, int32_t n_ops, int32_t nturns, u
     }
     int block = 64;
     while (block > 32 && geom_n / ((long long)P * block) < 2LL * sms) block >>= 1;
-    P = env_int("BT_TRACK_PPT", P);
-    block = env_int("BT_TRACK_BLOCK", block);
-    if (!(P == 1 || ((P == 2 || P == 4 || P == 8) && b->aligned16)))
-        return fail(BT_ERR_INVALID, "BT_TRACK_PPT must be 1, 2, 4 or 8 (2, 4, 8 need 16-byte aligned arrays)");
-    if (block < 32 || block > kMaxBlock || (block & 31)) return fail(BT_ERR_INVALID, "BT_TRACK_BLOCK must be a multiple of 32 in [32,128]");
+    P = knob(KNOB_TRACK_PPT, P);
+    block = knob(KNOB_TRACK_BLOCK, block);
+    if (!(P == 1 || ((P == 2 || P == 4) && b->aligned16)))
+        return fail(BT_ERR_INVALID, "knob track_ppt must be 1, 2 or 4 (2, 4 need 16-byte aligned arrays)");
+    if (block < 32 || block > kMaxBlock || (block & 31)) return fail(BT_ERR_INVALID, "knob track_block must be a multiple of 32 in [32,128]");
 
-    TrackArgs a;
-    for (int c = 0; c < 6; ++c) a.q[c] = b->q[c] + off;
-    a.n = n;
-    a.n_ops = n_ops;
-    a.nturns = nturns;
     const long long per_block = (long long)P * block;
     const long long full = n / per_block;
-    a.n_full_blocks = (int)full;
-    a.tail_start = full * per_block;
-    const long long rem = n - a.tail_start;
+    const long long tail_start = full * per_block;
+    const long long rem = n - tail_start;
     const long long grid_ll = full + (rem + block - 1) / block;
     if (grid_ll > 0x7fffffffLL) return fail(BT_ERR_UNSUPPORTED, "bt_track: grid too large");
     const int grid = (int)grid_ll;
-
-    ConstTableState &ct = g_ct[b->device];
-    std::lock_guard<std::mutex> lock(ct.mu);
-    if (!ct.busy) BT_CUDA_TRY(cudaEventCreateWithFlags(&ct.busy, cudaEventDisableTiming));
-    if (!ct.uploaded) BT_CUDA_TRY(cudaEventCreateWithFlags(&ct.uploaded, cudaEventDisableTiming));
-    if (ct.owner != (const void *)b || ct.version != version) {
-        BT_CUDA_TRY(cudaStreamWaitEvent(stream, ct.busy, 0));  // previous readers of the table (any stream)
-        // pageable source: the call returns after the source has been staged
-        BT_CUDA_TRY(cudaMemcpyToSymbolAsync(c_table, h_table, (size_t)n_ops * sizeof(DevOp), 0, cudaMemcpyHostToDevice, stream));
-        BT_CUDA_TRY(cudaEventRecord(ct.uploaded, stream));
-        ct.owner = (const void *)b;
-        ct.version = version;
-    } else if (b->range) {
-        BT_CUDA_TRY(cudaStreamWaitEvent(stream, ct.uploaded, 0));  // the table was placed by another chunk's stream
-    }
     bool nl = false;  // any non-linearised record in this table?
     for (int32_t e = 0; e < n_ops; ++e) nl = nl || (h_table[e].op & (OP_DRIFTX | OP_RFSIN | OP_QUADCHR));
-    switch (P) {
-        case 8: nl ? track_kernel<8, true><<<grid, block, 0, stream>>>(a) : track_kernel<8, false><<<grid, block, 0, stream>>>(a); break;
-        case 4: nl ? track_kernel<4, true><<<grid, block, 0, stream>>>(a) : track_kernel<4, false><<<grid, block, 0, stream>>>(a); break;
-        case 2: nl ? track_kernel<2, true><<<grid, block, 0, stream>>>(a) : track_kernel<2, false><<<grid, block, 0, stream>>>(a); break;
-        default: nl ? track_kernel<1, true><<<grid, block, 0, stream>>>(a) : track_kernel<1, false><<<grid, block, 0, stream>>>(a); break;
+
+    auto fill = [&](auto &a) {
+        for (int c = 0; c < 6; ++c) a.q[c] = b->q[c] + off;
+        a.n = n;
+        a.tail_start = tail_start;
+        a.n_full_blocks = (int)full;
+        a.n_ops = n_ops;
+        a.nturns = nturns;
+        a.pad_ = 0;
+    };
+    cudaError_t e;
+    if (n_ops <= kTableRecordsSmall) {
+        TrackArgs<kTableRecordsSmall> a;
+        fill(a);
+        e = launch_sized(a, h_table, n_ops, P, nl, grid, block, stream);
+    } else {
+        TrackArgs<kTableRecords> a;
+        fill(a);
+        e = launch_sized(a, h_table, n_ops, P, nl, grid, block, stream);
     }
-    cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return fail(BT_ERR_CUDA, std::string("bt_track launch: ") + cudaGetErrorString(e));
-    if (!b->range) BT_CUDA_TRY(cudaEventRecord(ct.busy, stream));  // bt_track_host records it once, after joining its streams
     g_launch_count.fetch_add(1);
     b->last_launch.grid = grid;
     b->last_launch.block = block;
@@ -449,22 +461,6 @@ int launch_track(Beam *b, const DevOp *h_table, int32_t n_ops, int32_t nturns, u
     b->last_launch.smem = 0;
     b->last_launch.launches += 1;
     return BT_OK;
-}
-
-// A destroyed beam must not be mistaken for a later one allocated at the same address.
-int record_table_busy(const Beam *b, cudaStream_t stream) {
-    if (b->device < 0 || b->device >= kMaxDevices) return BT_OK;
-    ConstTableState &ct = g_ct[b->device];
-    std::lock_guard<std::mutex> lock(ct.mu);
-    if (ct.busy) BT_CUDA_TRY(cudaEventRecord(ct.busy, stream));
-    return BT_OK;
-}
-
-void forget_table_owner(const Beam *b) {
-    if (b->device < 0 || b->device >= kMaxDevices) return;
-    ConstTableState &ct = g_ct[b->device];
-    std::lock_guard<std::mutex> lock(ct.mu);
-    if (ct.owner == (const void *)b) ct.owner = nullptr;
 }
 
 }  // namespace bt

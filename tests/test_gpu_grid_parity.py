@@ -297,9 +297,9 @@ def test_sorted_tracking_still_matches():
 
 @pytest.mark.parametrize("mode", [0, 1, 2])
 @pytest.mark.parametrize("variant", ["A", "B"])
-def test_deposit_modes_unaligned(mode, variant, monkeypatch):
+def test_deposit_modes_unaligned(mode, variant, knobs):
     import torch
-    monkeypatch.setenv("BT_DEPOSIT_MODE", str(mode))
+    knobs("deposit_mode", mode)
     sc = W.spacecharge_config(variant, n=70_001, shape=(32, 32, 32))
     c = W.make_spacecharge_bunch(sc)
     backing = [torch.empty(sc.n + 1, dtype=torch.float64, device="cuda") for _ in range(6)]
@@ -316,12 +316,12 @@ def test_deposit_modes_unaligned(mode, variant, monkeypatch):
 
 @pytest.mark.parametrize("mode", [0, 1, 2, 3, 4])
 @pytest.mark.parametrize("offset", [0, 1])
-def test_gather_modes(mode, offset, monkeypatch):
+def test_gather_modes(mode, offset, knobs):
     """Every gather path (registers / streaming pipeline with 256-, 512-, 128-particle chunks), on aligned and on
     8-byte-offset storage (the pipeline needs 16-byte alignment: offset storage must take the register path), with a
     ragged tail, sorted storage, drifts on both sides and a kick-only call."""
     import torch
-    monkeypatch.setenv("BT_GATHER_MODE", str(mode))
+    knobs("gather_mode", mode)
     sc = W.spacecharge_config("A", n=70_001, shape=(32, 32, 32))
     c = W.make_spacecharge_bunch(sc)
     c[0][:5] = [1.0, np.nan, -1.0, 5.9e-3, -5.9e-3]

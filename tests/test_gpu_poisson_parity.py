@@ -111,14 +111,23 @@ def test_full_size_grid_on_sampled_nodes():
     grid.close()
 
 
-def test_closed_space_charge_step_deposit_solve_gather():
+@pytest.mark.parametrize("side_stream", [False, True])
+def test_closed_space_charge_step_deposit_solve_gather(side_stream):
     """The paper's split-operator step with its own field (P:l.49): deposit -> Poisson (rest frame) -> gather + kick + drift,
-    two steps, against the oracle chain.  The kick coefficients are the caller's (R12); any finite values test the plumbing."""
-    sc = W.spacecharge_config("A", n=60_000, shape=(24, 24, 24))
+    two steps, against the oracle chain.  The kick coefficients are the caller's (R12); any finite values test the plumbing.
+    side_stream: the beam lives on a non-blocking side stream while the solve runs on the default stream -- the grid's
+    operations must be ordered across the two (deposit -> solve -> gather hand the grid over with an event)."""
+    import torch
+    n, shape = (60_000, (24, 24, 24)) if not side_stream else (1_500_000, (48, 48, 48))   # long enough kernels to race
+    sc = W.spacecharge_config("A", n=n, shape=shape)
     c = W.make_spacecharge_bunch(sc)
     g0 = O.ref_from_kinetic(sc.kin_energy_MeV, sc.mass_MeV)[0]
     coef = (2.0e-9, 2.0e-9, -1.0e-9)
-    beam = bt.Beam(sc.n)
+    if side_stream:
+        cs = torch.cuda.Stream()                     # torch side streams are non-blocking w.r.t. the default stream
+        beam = bt.Beam(sc.n, storage="library", stream=cs.cuda_stream)
+    else:
+        beam = bt.Beam(sc.n)
     grid = bt.Grid(sc.shape, sc.lo, sc.d)
     beam.set_ref(sc.kin_energy_MeV, sc.mass_MeV, 1.0)
     beam.upload(c)

@@ -37,8 +37,8 @@ def run_deposit(c, sc, zscale=None, sort=False, storage=None, twice=False):
 @pytest.mark.parametrize("variant", ["A", "B"])
 @pytest.mark.parametrize("n,shape,sort", [(1, (8, 8, 8), False), (257, (16, 12, 10), False), (200_003, (32, 32, 32), False),
                                           (200_003, (32, 32, 32), True), (300_000, (128, 128, 128), True)])
-def test_deposit_order2(mode, variant, n, shape, sort, monkeypatch):
-    monkeypatch.setenv("BT_DEPOSIT_MODE", str(mode))
+def test_deposit_order2(mode, variant, n, shape, sort, knobs):
+    knobs("deposit_mode", mode)
     sc = W.spacecharge_config(variant, n=n, shape=shape)
     c = W.make_spacecharge_bunch(sc)
     rho = run_deposit(c, sc, sort=sort)
@@ -69,9 +69,9 @@ def test_deposit_order2_boundaries_zscale_unaligned_accumulate():
 
 @pytest.mark.parametrize("mode", [0, 1, 2, 3, 4])
 @pytest.mark.parametrize("offset", [0, 1])
-def test_gather_order2(mode, offset, monkeypatch):
+def test_gather_order2(mode, offset, knobs):
     import torch
-    monkeypatch.setenv("BT_GATHER_MODE", str(mode))
+    knobs("gather_mode", mode)
     sc = W.spacecharge_config("A", n=70_001, shape=(32, 32, 32))
     c = W.make_spacecharge_bunch(sc)
     c[0][:5] = [1.0, np.nan, -1.0, 5.9e-3, -5.9e-3]
@@ -146,9 +146,9 @@ def test_shape_argument_errors():
 
 @pytest.mark.parametrize("order", [1, 2])
 @pytest.mark.parametrize("n", [1, 255, 256, 257, 513])
-def test_gather_small_counts_around_the_chunk_size(order, n, monkeypatch):
+def test_gather_small_counts_around_the_chunk_size(order, n, knobs):
     """Pipeline chunks are 256 particles: counts below, at and just above one chunk (ragged tail kernel), tile mode forced."""
-    monkeypatch.setenv("BT_GATHER_MODE", "4")
+    knobs("gather_mode", 4)
     sc = W.spacecharge_config("A", n=n, shape=(16, 16, 16))
     c = W.make_spacecharge_bunch(sc)
     E = W.gaussian_bunch_field(sc)

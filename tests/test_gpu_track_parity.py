@@ -44,12 +44,12 @@ def test_config1_fodo_channel_reduced(n):
     check(got, ref)
 
 
-@pytest.mark.parametrize("ppt,block", [(1, 32), (1, 128), (2, 64), (2, 128), (4, 128), (4, 96), (4, 32), (8, 64), (8, 32)])
-def test_all_kernel_variants_agree(ppt, block, monkeypatch):
+@pytest.mark.parametrize("ppt,block", [(1, 32), (1, 128), (2, 64), (2, 128), (4, 128), (4, 96), (4, 32), (4, 64)])
+def test_all_kernel_variants_agree(ppt, block, knobs):
     """Every (particles-per-thread, block size) instantiation against the oracle, config-3 ring (all op kinds except
     sbend/edge; 7 turns of per-turn tables = 2 launches) and the chicane."""
-    monkeypatch.setenv("BT_TRACK_PPT", str(ppt))
-    monkeypatch.setenv("BT_TRACK_BLOCK", str(block))
+    knobs("track_ppt", ppt)
+    knobs("track_block", block)
     n = 4 * 128 * 3 + 201
     cfg = W.config(3, n=n)
     c = W.make_bunch(cfg)
@@ -65,19 +65,20 @@ def test_all_kernel_variants_agree(ppt, block, monkeypatch):
     check(got, ref)
 
 
-def test_record_fusion_is_bit_identical(monkeypatch):
+def test_record_fusion_is_bit_identical(knobs):
     """Peephole fusion of adjacent thin kicks / trailing drift into one record changes the dispatch count, not the
-    arithmetic: BT_TRACK_FUSE=0 (one record per element) must give the same bits."""
+    arithmetic: with the knob track_fuse = 0 (one record per element) the walk must give the same bits.  configs[3]'s ring
+    exercises all three fusions: SEXTOCT, TAILDRIFT and the half-cell runs (one dispatch per 25 half cells)."""
     cfg = W.config(3, n=5000)
     c = W.make_bunch(cfg)
     fused, _, _ = gpu_track(cfg, c, nturns=3)
-    monkeypatch.setenv("BT_TRACK_FUSE", "0")
+    knobs("track_fuse", 0)
     plain, _, _ = gpu_track(cfg, c, nturns=3)
     assert all(np.array_equal(a, b) for a, b in zip(fused, plain))
 
 
-def test_lattice_longer_than_the_constant_bank():
-    """> 1024 records per turn: the walk is split into several launches per turn (static and per-turn tables)."""
+def test_lattice_longer_than_one_launch_table():
+    """> 510 records per turn: the walk is split into several launches per turn (static and per-turn tables)."""
     cell = [("quad", 0.2, 1, 1.3), ("multipole", 0.0, 1, 3, 0.2, 0.0), ("drift", 0.1, 1), ("quad", 0.2, 7, -1.3),
             ("multipole", 0.0, 1, 4, 2.0, 0.0), ("multipole", 0.0, 1, 3, -0.2, 0.0), ("multipole", 0.0, 1, 4, 0.9, 0.0), ("drift", 0.1, 2)]
     lat = cell * 300                                   # 2400 elements -> 2400 records (one fused pair, one split quad per cell)
@@ -93,8 +94,8 @@ def test_lattice_longer_than_the_constant_bank():
     assert abs(g - g_ref) <= 1e-15 * g_ref
 
 
-def test_two_beams_share_the_constant_bank():
-    """The record table lives in the device's single constant bank: beams with different lattices on different
+def test_two_beams_with_different_lattices_interleaved():
+    """The record table travels with each launch (kernel parameters): beams with different lattices on different
     streams, interleaved, must each see their own table."""
     import torch
     import paper_2208_02382_b200 as bt
@@ -282,17 +283,36 @@ def test_track_host_pipelined_is_bit_identical(nchunks):
     beam.close()
 
 
-def test_track_host_with_rf_lattice_falls_back_to_one_chunk():
+@pytest.mark.parametrize("nchunks", [3, 8])
+def test_track_host_with_rf_lattice_is_pipelined_and_bit_identical(nchunks):
+    """A lattice whose RF changes the reference energy (per-turn tables, 7 turns = 2 launches per chunk) through the chunked
+    host path: every launch carries its own table, so the chunk streams need no serialisation.  Bit-identical to
+    upload + bt_track + download, same reference energy, one walk launch per (chunk, plan launch)."""
+    import torch
     import paper_2208_02382_b200 as bt
     cfg = W.config(3, n=20_003)
     c = W.make_bunch(cfg)
     beam = bt.Beam(cfg.n)
     beam.set_ref(cfg.kin_energy_MeV, cfg.mass_MeV, cfg.charge_qe)
     beam.lattice_set(cfg.lattice)
-    out = [np.empty_like(a) for a in c]
-    beam.track_host(c, out, nturns=2, nchunks=8)
-    ref, _ = oracle_track(cfg, c, nturns=2)
-    assert max(r14_error(out, ref)) <= 1e-11
+    beam.upload(c)
+    n0 = bt.launch_count()
+    beam.track(7)
+    per_call = bt.launch_count() - n0
+    plain, g_plain = beam.download(), beam.get_ref()[0]
+    beam.set_ref(cfg.kin_energy_MeV, cfg.mass_MeV, cfg.charge_qe)
+    pinned = [torch.from_numpy(a.copy()).pin_memory() for a in c]
+    out = [torch.empty(cfg.n, dtype=torch.float64).pin_memory() for _ in range(6)]
+    n0 = bt.launch_count()
+    beam.track_host(pinned, out, nturns=7, nchunks=nchunks)
+    chunk_len = -(-(-(-cfg.n // nchunks)) // 1024) * 1024               # chunks are whole 1024-particle granules
+    assert per_call == 2 and bt.launch_count() - n0 == per_call * -(-cfg.n // chunk_len)
+    for a, b in zip(out, plain):
+        assert np.array_equal(a.numpy(), b)
+    g, s, turn = beam.get_ref()
+    assert g == g_plain and turn == 7
+    ref, _ = oracle_track(cfg, c, nturns=7)
+    assert max(r14_error([t.numpy() for t in out], ref)) <= 1e-11
     assert bt.lib.bt_track_host(beam._h, None, None, 1, 8) == bt.BT_ERR_INVALID
     beam.close()
 
