@@ -1,25 +1,31 @@
 #!/usr/bin/env python
 """bench.py -- the driver's measurement contract for the B200 beam-tracking hot path.
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload fodo_channel|...]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload nonlinear_ring|...]
 
 Metric (BASELINE.json): particle-element pushes/s (fp64).  One *element push* = one particle through one
-lattice element (all its slices).  Workload at N=1 = BASELINE configs[1] ("Linear FODO channel": 10^6
-particles, the FODO cell x100 = 500 elements / 5300 slice maps, 1 pass), synthetic seeded input from
-workloads/.  A *step* = one pass of the hot path over the bunch = one bt_track(1) call = ONE kernel launch.
+lattice element (all its slices).  BASELINE.json's `metric` names no config, so the N=1 workload is the largest
+single-GPU tracking config, configs[3] ("Nonlinear ring": 64e6 seeded particles, 201 elements, 100 turns -- the
+stand-in for the paper's only performance run), synthetic input from workloads/.
+A *step* = one pass of the hot path over the bunch = one bt_track(nturns) call (20 launches of the fused walk for
+configs[3]: the RF cavity changes the reference energy every turn, five turns of coefficients travel with a launch).
 
 N > 1 (torchrun): particles are independent, so the path shards with no data-path collective; every rank
-tracks its own 10^6-particle bunch (seed + rank) -> "scaling": "weak"; value = all ranks' pushes / max-over-ranks time.
+tracks its own bunch (seed + 1000 rank) -> "scaling": "weak"; value = all ranks' pushes / max-over-ranks time.
 
 Timing: W >= 3 warm-up steps; every timed step is bracketed by CUDA events on the beam's stream (torch's current
-stream); L2 is flushed (256 MiB write) between timed steps, outside the event intervals; the K-step region is
-bracketed by barrier + torch.cuda.synchronize(); ms_per_step = sum of event intervals / K, max over ranks.
+stream); inputs are larger than L2 (3.07 GB of SoA state against 126 MB) and are restored from a pristine device copy
+between timed steps, outside the event intervals; the K-step region is bracketed by barrier +
+torch.cuda.synchronize(); ms_per_step = sum of event intervals / K, max over ranks.
 
 The same JSON line carries: roofline (FP64-pipe issue slots), cpu_baseline (the oracle as
-it stands on a bounded sample, host cores), e2e (host pinned buffers -> bt_track_host = chunked upload -> bt_track ->
-bt_beam_download inside the timed region), gpu_launches, clocks.
+it stands on a bounded sample, host cores, all cores and one thread), e2e (host pinned buffers -> bt_track_host =
+chunked upload -> walk -> download inside the timed region), gpu_launches, clocks; at N=1 also `other_configs`
+(configs 0, 1, 2) and `spacecharge` (configs[4] A, B and A with the order-2 shape), each with its roofline and its
+CPU baselines.
 """
 import argparse
+import csv
 import json
 import os
 import statistics
@@ -37,6 +43,7 @@ import workloads as W  # noqa: E402
 
 METRIC = "particle-element pushes/s (fp64)"
 UNIT = "pushes/s"
+WORKLOADS = {"tiny_fodo": 0, "fodo_channel": 1, "chicane": 2, "nonlinear_ring": 3}
 
 # FP64 issue slots per slice map (DESIGN.md section 7 / SURVEY 8d): minimal DFMA/DMUL sequences.
 SLOTS = {"drift": 3, "quad": 9, "sbend": 10, "dipedge": 2, "shortrf": 4}
@@ -63,6 +70,42 @@ def load_peaks():
         with open(path) as f:
             return json.load(f), "measured"
     return {"hbm_gbs": 6650.0, "sm_max_mhz": 1965.0}, "fallback"
+
+
+def load_traffic():
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch from the ncu --set full captures summarised under
+    profiles/ (text, written by hand from `ncu -i ... --page raw --csv`): {key: (bytes, source)}."""
+    out = {}
+    path = os.path.join(ROOT, "profiles", "r02_traffic.csv")
+    if os.path.exists(path):
+        with open(path) as f:
+            for row in csv.DictReader(f):
+                out[row["key"]] = (float(row["dram_read_bytes"]) + float(row["dram_write_bytes"]), row["source"])
+    return out
+
+
+def traffic_of(table, key):
+    return table[key][0] if key in table else None
+
+
+def cpu_model():
+    try:
+        with open("/proc/cpuinfo") as f:
+            for line in f:
+                if line.startswith("model name"):
+                    return line.split(":", 1)[1].strip()
+    except OSError:
+        pass
+    return "unknown"
+
+
+def config_dict(cfg, world):
+    """The workload description: identical in both arms (`--impl ours` and `--impl reference`)."""
+    return {"workload": "configs[%d] %s" % (cfg.index, cfg.name), "particles_per_gpu": cfg.n, "elements": cfg.n_elements,
+            "slice_maps_per_turn": cfg.slice_maps_per_turn, "turns_per_step": cfg.nturns,
+            "l2": "inputs larger than L2 (%.2f GB of particle state), restored from a pristine copy between timed steps"
+                  % (48.0 * cfg.n / 1e9) if 48.0 * cfg.n > 512e6 else "flushed between timed steps (256 MiB write)",
+            "parallelism": "particles sharded, %d rank(s), no collective" % world}
 
 
 class ClockSampler:
@@ -115,15 +158,13 @@ class ClockSampler:
 
 
 def get_workload(name, rank):
-    idx = {"tiny_fodo": 0, "fodo_channel": 1, "chicane": 2, "nonlinear_ring": 3}[name]
-    cfg = W.config(idx)
-    from paper_2208_02382_b200.shard import rank_seed
-    cfg.seed = rank_seed(cfg.seed, rank)   # every rank its own bunch (weak scaling)
+    cfg = W.config(WORKLOADS[name])
+    cfg.seed = W.rank_seed(cfg.seed, rank)   # every rank its own bunch (weak scaling)
     return cfg
 
 
 # ---------------------------------------------------------------------------------------------------
-# reference arm: the oracle as it stands, on the host cores, on a bounded sample of the same workload
+# the oracle as it stands, on the host cores, on a bounded sample of a workload
 # ---------------------------------------------------------------------------------------------------
 def oracle_rate(cfg, n_sample, reps=1):
     import oracle as O
@@ -139,6 +180,66 @@ def oracle_rate(cfg, n_sample, reps=1):
     return pushes, times, O.num_threads()
 
 
+def oracle_track_baseline(cfg, budget_s=12.0, single_budget_s=4.0):
+    """cpu_baseline object for a tracking config: all cores on a sample sized for ~budget_s, one thread for ~single_budget_s."""
+    import oracle as O
+    n_cal = min(cfg.n, 20_000)
+    _p, tms, cores = oracle_rate(cfg, n_cal)
+    rate = n_cal / tms[0]                                       # particles through the whole call per second (cold)
+    n_all = int(max(1000, min(cfg.n, rate * budget_s, 2_000_000)))
+    pushes, tms, cores = oracle_rate(cfg, n_all, reps=2 if n_all == cfg.n and tms[0] * cfg.n / n_cal < budget_s / 3 else 1)
+    t = min(tms)
+    out = {"value": pushes / t, "unit": UNIT, "cores": cores, "cpu": cpu_model(), "kind": "oracle",
+           "sample": "%d of %d particles (same seeded recipe), full lattice (%d elements, %d slice maps), %d turn(s); %.1f s of CPU work"
+                     % (n_all, cfg.n, cfg.n_elements, cfg.slice_maps_per_turn, cfg.nturns, sum(tms))}
+    nthr = O.num_threads()
+    try:
+        O.set_num_threads(1)
+        n_st = int(max(500, min(n_all, rate / max(cores, 1) * single_budget_s * 1.5)))
+        st_pushes, st_times, _ = oracle_rate(cfg, n_st)
+        out["single_thread"] = {"value": st_pushes / st_times[0], "unit": UNIT, "cores": 1,
+                                "sample": "%d of %d particles, full lattice, %d turn(s), one run, %.1f s" % (n_st, cfg.n, cfg.nturns, st_times[0])}
+    finally:
+        O.set_num_threads(nthr)
+    return out
+
+
+def oracle_grid_baseline(sc, c, E):
+    """CPU baselines of the two particle-grid steps on configs[4]: the oracle's deposit and gather+kick on the full bunch
+    (all cores; the deposit's long-double node sums are a serial loop by definition) and on one thread (1/8 sample)."""
+    import oracle as O
+    nn = sc.shape[0] * sc.shape[1] * sc.shape[2]
+    dep_bytes, gat_bytes = 24.0 * sc.n + 16.0 * nn, 96.0 * sc.n + 24.0 * nn
+    out = {}
+    t0 = time.perf_counter()
+    O.deposit_cic(c[0], c[2], c[4], sc.shape, sc.lo, sc.d, sc.q_weight, sc.zscale)
+    td = time.perf_counter() - t0
+    ref = [a.copy() for a in c]
+    t0 = time.perf_counter()
+    O.gather_kick(ref, sc.shape, sc.lo, sc.d, E, sc.kick_coef, sc.zscale)
+    tg = time.perf_counter() - t0
+    cores = O.num_threads()
+    out["all_cores"] = {"cores": cores, "cpu": cpu_model(), "kind": "oracle", "sample": "all %d particles, one call each" % sc.n,
+                        "deposit_ms": td * 1e3, "deposit_gbs": dep_bytes / td / 1e9,
+                        "gather_kick_ms": tg * 1e3, "gather_kick_gbs": (72.0 * sc.n + 24.0 * nn) / tg / 1e9}
+    m = sc.n // 8
+    try:
+        O.set_num_threads(1)
+        t0 = time.perf_counter()
+        O.deposit_cic(c[0][:m].copy(), c[2][:m].copy(), c[4][:m].copy(), sc.shape, sc.lo, sc.d, sc.q_weight, sc.zscale)
+        td1 = time.perf_counter() - t0
+        ref = [a[:m].copy() for a in c]
+        t0 = time.perf_counter()
+        O.gather_kick(ref, sc.shape, sc.lo, sc.d, E, sc.kick_coef, sc.zscale)
+        tg1 = time.perf_counter() - t0
+    finally:
+        O.set_num_threads(cores)
+    out["single_thread"] = {"cores": 1, "sample": "first %d of %d particles, one call each" % (m, sc.n),
+                            "deposit_ms_per_particle_scaled": td1 * 8e3, "deposit_gbs": (24.0 * m + 16.0 * nn) / td1 / 1e9,
+                            "gather_kick_ms_scaled": tg1 * 8e3, "gather_kick_gbs": (72.0 * m + 24.0 * nn) / tg1 / 1e9}
+    return out
+
+
 def run_reference(args):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
@@ -147,7 +248,7 @@ def run_reference(args):
     # W warm-up steps on a small sample also calibrate the rate; the per-step sample is then sized so that the
     # K timed steps take about REF_BUDGET_S seconds in total (bounded sample of the same workload).
     REF_BUDGET_S = 60.0
-    n_cal = min(cfg.n, 20_000)
+    n_cal = min(cfg.n, 10_000)
     rate = None
     for _ in range(max(1, args.warmup)):
         p, tms, _c = oracle_rate(cfg, n_cal)
@@ -157,15 +258,13 @@ def run_reference(args):
     pushes, times, cores = oracle_rate(cfg, n_sample, reps=max(1, args.steps))
     t = sum(times) / len(times)
     value = pushes / t
-    sample = "%d of %d particles (seed %d), full lattice (%d elements, %d slice maps), %d turn(s) per step" % (
+    sample = "%d of %d particles per step (same seeded recipe, seed %d), full lattice (%d elements, %d slice maps), %d turn(s) per step" % (
         n_sample, cfg.n, cfg.seed, cfg.n_elements, cfg.slice_maps_per_turn, cfg.nturns)
     line = {
         "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": len(times),
         "warmup": max(1, args.warmup), "ms_per_step": t * 1e3, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-        "dtype": "f64", "data": "synthetic",
-        "config": {"workload": "configs[1] " + cfg.name + " (bounded sample)", "particles": n_sample,
-                   "elements": cfg.n_elements, "slice_maps_per_turn": cfg.slice_maps_per_turn, "turns": cfg.nturns},
-        "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+        "dtype": "f64", "data": "synthetic", "config": config_dict(cfg, args.gpus),
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "cpu": cpu_model(), "kind": "oracle", "sample": sample},
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
     }
@@ -192,24 +291,32 @@ def _event_ms(torch, fn, reps, flush, pre=None):
     return ts
 
 
-def bench_other_configs(bt, torch, flush, peaks, nominal_peak):
-    """bt_track on configs[0], [2], [3] at full size (one call = the config's nturns).  configs[3]'s 64e6-particle
-    bunch is a seeded 10^6-particle draw tiled 64 times on the device (timing does not depend on the values)."""
+def walk_roofline(n, lattice, nturns, launches, t_s, peaks, nominal_peak):
+    hbm = float(peaks["hbm_gbs"]) * 1e9
+    slots = float(n) * slots_per_particle_per_turn(lattice) * nturns
+    t_alu, t_hbm = slots / nominal_peak, 96.0 * n * launches / hbm
+    if t_alu >= t_hbm:
+        return {"bound": "alu", "achieved": slots / t_s / 1e12, "peak": nominal_peak / 1e12, "unit": "Tslot/s", "frac": t_alu / t_s,
+                "slots_per_particle": slots / n, "roofline_time_ms": t_alu * 1e3}
+    return {"bound": "hbm", "achieved": 96.0 * n * launches / t_s / 1e9, "peak": hbm / 1e9, "unit": "GB/s", "frac": t_hbm / t_s,
+            "roofline_time_ms": t_hbm * 1e3}
+
+
+def bench_other_configs(bt, torch, flush, peaks, nominal_peak, traffic):
+    """bt_track on configs[0], [1], [2] at full size (one call = the config's nturns), each with the oracle timed beside it."""
     out = []
     hbm = float(peaks["hbm_gbs"]) * 1e9
-    for idx, reps in ((0, 5), (2, 5), (3, 2)):
+    for idx, reps in ((0, 5), (1, 10), (2, 5)):
         cfg = W.config(idx)
         n = cfg.n
-        base = W.make_bunch(cfg, n=min(n, 1_000_000))
-        tile = -(-n // len(base[0]))
-        pristine = [torch.from_numpy(a).cuda().repeat(tile)[:n].contiguous() for a in base]
+        pristine = [torch.from_numpy(a).cuda() for a in W.make_bunch(cfg)]
         beam = bt.Beam(n)
         beam.lattice_set(cfg.lattice)
 
         def restore():
             for d, s in zip(beam.tensors, pristine):
                 d.copy_(s)
-            beam.set_ref(cfg.kin_energy_MeV, cfg.mass_MeV, cfg.charge_qe)   # RF lattices: same energy every repetition
+            beam.set_ref(cfg.kin_energy_MeV, cfg.mass_MeV, cfg.charge_qe)
 
         restore()
         beam.track(cfg.nturns)
@@ -217,27 +324,25 @@ def bench_other_configs(bt, torch, flush, peaks, nominal_peak):
         ts = _event_ms(torch, lambda: beam.track(cfg.nturns), reps, flush, restore)
         launches = (bt.launch_count() - launches0) // reps
         t = statistics.mean(ts) * 1e-3
-        slots = float(n) * slots_per_particle_per_turn(cfg.lattice) * cfg.nturns
-        t_alu, t_hbm = slots / nominal_peak, 96.0 * n * launches / hbm
         li = beam.last_launch()
         entry = {"workload": "configs[%d] %s" % (idx, cfg.name), "particles": n, "elements": cfg.n_elements, "turns": cfg.nturns,
                  "ms_per_call": t * 1e3, "pushes_per_s": n * cfg.n_elements * cfg.nturns / t, "launches_per_call": launches,
                  "kernel": "bt::track_kernel<P=%d> grid=%d block=%d" % (li["particles_per_thread"], li["grid"], li["block"])}
+        roof = walk_roofline(n, cfg.lattice, cfg.nturns, launches, t, peaks, nominal_peak)
         if idx == 0:
-            entry["roofline"] = {"bound": "latency", "note": "10^4 particles = 313 warps on 148 SMs: neither pipe nor HBM can be filled "
-                                 "(SURVEY 8d); roofline time %.2f us shown for information" % (max(t_alu, t_hbm) * 1e6)}
-        elif t_alu >= t_hbm:
-            entry["roofline"] = {"bound": "alu", "achieved": slots / t / 1e12, "peak": nominal_peak / 1e12, "unit": "Tslot/s",
-                                 "frac": t_alu / t}
+            roof = {"bound": "latency", "note": "10^4 particles = 313 warps on 148 SMs: neither pipe nor HBM can be filled "
+                    "(SURVEY 8d); roofline time %.2f us shown for information" % (roof["roofline_time_ms"] * 1e3)}
         else:
-            entry["roofline"] = {"bound": "hbm", "achieved": 96.0 * n * launches / t / 1e9, "peak": hbm / 1e9, "unit": "GB/s",
-                                 "frac": t_hbm / t}
-        if idx in (2, 3):
+            roof["traffic"] = traffic_of(traffic, "walk:" + cfg.name)
+        entry["roofline"] = roof
+        if idx == 2:
             # beam statistics: bt_beam_moments = 1 launch + a 336-byte read-back, 48 B/particle
             beam.moments()
             tm = statistics.mean(_event_ms(torch, beam.moments, 5, flush)) * 1e-3
             entry["moments"] = {"ms": tm * 1e3, "roofline": {"bound": "hbm", "achieved": 48.0 * n / tm / 1e9, "peak": hbm / 1e9,
-                                                              "unit": "GB/s", "frac": 48.0 * n / tm / hbm, "traffic": None}}
+                                                              "unit": "GB/s", "frac": 48.0 * n / tm / hbm,
+                                                              "traffic": traffic_of(traffic, "moments:%d" % n)}}
+        entry["cpu_baseline"] = oracle_track_baseline(cfg, budget_s=6.0, single_budget_s=3.0)
         out.append(entry)
         beam.close()
         del pristine, beam
@@ -245,10 +350,11 @@ def bench_other_configs(bt, torch, flush, peaks, nominal_peak):
     return out
 
 
-def bench_spacecharge(bt, torch, flush, peaks):
-    """configs[4] A and B at full size (8e6 particles, 128^3 nodes): bt_beam_sort_by_cell once, then 10 steps of
-    bt_deposit_cic + bt_gather_kick(0, ds) (SURVEY 8d call sequence), every call timed with CUDA events, L2 flushed
-    before each.  GB/s = ALGORITHMIC bytes / time: deposit 24 B/particle + 2 x 8 B/node (zeroing + result);
+def bench_spacecharge(bt, torch, flush, peaks, traffic, interval):
+    """configs[4] A and B at full size (8e6 particles, 128^3 nodes): 10 steps of bt_deposit_cic + bt_gather_kick(0, ds)
+    (SURVEY 8d call sequence) with the library's own re-sort cadence (bt_beam_set_resort_interval: every sort the run
+    needs is inside the timed deposit calls), every call timed with CUDA events, L2 flushed before each.
+    GB/s = ALGORITHMIC bytes / time: deposit 24 B/particle + 2 x 8 B/node (zeroing + result);
     gather+kick+drift 96 B/particle + 24 B/node."""
     hbm = float(peaks["hbm_gbs"])
     out = {}
@@ -274,14 +380,22 @@ def bench_spacecharge(bt, torch, flush, peaks):
             d.copy_(s)
         del pos
         beam.sort_by_cell(grid, sc.zscale)                         # warm-up: first call allocates the scratch
+        t_resort = _event_ms(torch, lambda: beam.sort_by_cell(grid, sc.zscale), 2, flush)   # re-sort of a sorted beam
         beam.upload(c)                                             # back to the caller's order
         beam.track(1)
-        t_sort = _event_ms(torch, lambda: beam.sort_by_cell(grid, sc.zscale), 1, flush)[0]
+        t_sort = _event_ms(torch, lambda: beam.sort_by_cell(grid, sc.zscale), 1, flush)[0]  # cold: from the caller's order
+        # the timed run: the library re-sorts by itself every `interval` deposits, inside the timed deposit calls
+        beam.upload(c)
+        beam.track(1)
+        beam.set_resort_interval(interval)
         t_dep, t_gat = [], []
         for step in range(sc.nsteps):
             t_dep += _event_ms(torch, lambda: beam.deposit_cic(grid, sc.q_weight, sc.zscale, True), 1, flush)
             after = sc.ds if step < sc.nsteps - 1 else sc.ds / 2
             t_gat += _event_ms(torch, lambda: beam.gather_kick(grid, sc.kick_coef, sc.zscale, 0.0, after), 1, flush)
+        beam.set_resort_interval(0)
+        is_sort_step = [s % interval == 0 for s in range(sc.nsteps)]
+        dep_plain = [t for t, srt in zip(t_dep, is_sort_step) if not srt]
         poisson = None
         if variant == "A" and order == 1:
             # NEXT-4: rest-frame Poisson solve on the deposited rho (own kernels + 2 cuFFT transforms of the 256^3 padded
@@ -295,24 +409,33 @@ def bench_spacecharge(bt, torch, flush, peaks):
             mp_ = statistics.mean(t_ps) * 1e-3
             poisson = {"ms": mp_ * 1e3, "padded_box": [2 * s for s in sc.shape],
                        "roofline": {"bound": "hbm", "achieved": ps_bytes / mp_ / 1e9, "peak": hbm, "unit": "GB/s",
-                                    "frac": ps_bytes / mp_ / 1e9 / hbm, "traffic": None,
+                                    "frac": ps_bytes / mp_ / 1e9 / hbm, "traffic": traffic_of(traffic, "poisson:128"),
                                     "note": "bytes = single-pass lower bound of the pad/FFT/multiply/FFT/extract/gradient chain"}}
             grid.set_field(*E)
-        md, mg = statistics.mean(t_dep) * 1e-3, statistics.mean(t_gat) * 1e-3
-        out[variant if order == 1 else variant + "_order2"] = {
+        md_all, mg = statistics.mean(t_dep) * 1e-3, statistics.mean(t_gat) * 1e-3
+        md = statistics.mean(dep_plain) * 1e-3 if dep_plain else md_all
+        key = variant if order == 1 else variant + "_order2"
+        out[key] = {
             "workload": "configs[4] %s, %d particles, %dx%dx%d nodes, %d steps, particle shape order %d" % (
                 (sc.name, n) + tuple(sc.shape) + (sc.nsteps, order)),
-            "sort_by_cell_ms_once": t_sort,
-            "deposit": {"ms": md * 1e3, "ms_first_last": [t_dep[0], t_dep[-1]], "unsorted_ms": t_dep_u,
+            "resort_interval": interval,
+            "sort_by_cell_ms": {"cold_from_callers_order": t_sort, "resort_of_sorted_beam": min(t_resort)},
+            "deposit": {"ms": md * 1e3, "ms_incl_resorts": md_all * 1e3, "ms_per_step": t_dep, "unsorted_ms": t_dep_u,
+                        "note": "ms = mean over the steps without a re-sort; ms_incl_resorts = mean over all 10 timed calls "
+                                "(steps 0, %d, ... contain bt_beam_sort_by_cell)" % interval,
                         "roofline": {"bound": "hbm", "achieved": dep_bytes / md / 1e9, "peak": hbm, "unit": "GB/s",
-                                     "frac": dep_bytes / md / 1e9 / hbm, "traffic": None}},
-            "gather_kick_drift": {"ms": mg * 1e3, "ms_first_last": [t_gat[0], t_gat[-1]], "unsorted_kick_only_ms": t_gat_u,
+                                     "frac": dep_bytes / md / 1e9 / hbm, "frac_incl_resorts": dep_bytes / md_all / 1e9 / hbm,
+                                     "traffic": traffic_of(traffic, "deposit:%s:%d" % (variant, order))}},
+            "gather_kick_drift": {"ms": mg * 1e3, "ms_per_step": t_gat, "unsorted_kick_only_ms": t_gat_u,
                                   "roofline": {"bound": "hbm", "achieved": gat_bytes / mg / 1e9, "peak": hbm, "unit": "GB/s",
-                                               "frac": gat_bytes / mg / 1e9 / hbm, "traffic": None}},
-            "ms_per_step_incl_sort_amortised": (md + mg) * 1e3 + t_sort / sc.nsteps,
+                                               "frac": gat_bytes / mg / 1e9 / hbm,
+                                               "traffic": traffic_of(traffic, "gather:%s:%d" % (variant, order))}},
+            "ms_per_step_incl_sort_amortised": (md_all + mg) * 1e3,
         }
         if poisson:
-            out[variant]["poisson_solve"] = poisson
+            out[key]["poisson_solve"] = poisson
+        if order == 1:
+            out[key]["cpu_baseline"] = oracle_grid_baseline(sc, c, E)
         beam.close()
         grid.close()
         del beam, grid
@@ -327,6 +450,7 @@ def run_ours(args):
     import torch
     import torch.distributed as dist
     import paper_2208_02382_b200 as bt
+    from paper_2208_02382_b200.shard import max_over_ranks
 
     world = int(os.environ.get("WORLD_SIZE", "1"))
     rank = int(os.environ.get("RANK", "0"))
@@ -344,27 +468,30 @@ def run_ours(args):
         torch.cuda.synchronize()
 
     cfg = get_workload(args.workload, rank)
-    coords = W.make_bunch(cfg)
     n = cfg.n
+    pinned = []
+    for a in W.make_bunch(cfg):                      # seeded draw of the whole bunch (64e6 particles for configs[3])
+        pinned.append(torch.from_numpy(a).pin_memory())
+        del a
+    pinned_out = [torch.empty(n, dtype=torch.float64).pin_memory() for _ in range(6)]
     pushes_per_step = n * cfg.n_elements * cfg.nturns
     slots_pp = slots_per_particle_per_turn(cfg.lattice) * cfg.nturns
-    slots_per_launch = float(n) * slots_pp
 
     beam = bt.Beam(n)                       # six torch.float64 CUDA tensors lent to the library
     beam.set_ref(cfg.kin_energy_MeV, cfg.mass_MeV, cfg.charge_qe)
     beam.lattice_set(cfg.lattice)
-    pinned = [torch.from_numpy(a).pin_memory() for a in coords]
-    pinned_out = [torch.empty(n, dtype=torch.float64).pin_memory() for _ in range(6)]
     pristine = [t.to("cuda", non_blocking=True) for t in pinned]
+    big = 48.0 * n > 512e6                  # inputs larger than L2 by a wide margin: no flush needed
     flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
 
     def restore():
         for dst, src in zip(beam.tensors, pristine):
             dst.copy_(src, non_blocking=True)
+        beam.set_ref(cfg.kin_energy_MeV, cfg.mass_MeV, cfg.charge_qe)    # RF lattices: same reference energy every step
 
     # ---- device-resident timing ----------------------------------------------------------------
-    restore()
     for _ in range(max(args.warmup, 3)):
+        restore()
         beam.track(cfg.nturns)
     torch.cuda.synchronize()
     ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
@@ -376,108 +503,85 @@ def run_ours(args):
     t_wall0 = time.perf_counter()
     for k in range(args.steps):
         restore()                            # same input every step (outside the event interval)
-        flush.zero_()                        # L2 flush between timed iterations (outside the event interval)
+        if not big:
+            flush.zero_()                    # L2 flush between timed iterations (outside the event interval)
         ev[k][0].record()
-        beam.track(cfg.nturns)               # ONE fused-walk launch
+        beam.track(cfg.nturns)               # the whole hot path of this workload: the fused walk
         ev[k][1].record()
     barrier()
     t_wall = time.perf_counter() - t_wall0
     launches = bt.launch_count() - launches0
     step_ms = [a.elapsed_time(b) for a, b in ev]
     ms_sum = sum(step_ms)
-
     launch_info = beam.last_launch()         # geometry of the timed launches (the e2e leg below launches per chunk)
 
     # ---- end to end through the C-ABI with host buffers -----------------------------------------
     # bt_track_host = upload + walk + download with the bunch cut into chunks on three streams (copies overlap the walk)
+    def e2e_step():
+        beam.set_ref(cfg.kin_energy_MeV, cfg.mass_MeV, cfg.charge_qe)
+        beam.track_host(pinned, pinned_out, cfg.nturns, args.e2e_chunks)    # synchronous: returns when pinned_out is complete
+
     for _ in range(2):
-        beam.track_host(pinned, pinned_out, cfg.nturns, args.e2e_chunks)
+        e2e_step()
     barrier()
     t0 = time.perf_counter()
     for k in range(args.steps):
-        beam.track_host(pinned, pinned_out, cfg.nturns, args.e2e_chunks)     # synchronous: returns when pinned_out is complete
+        e2e_step()
     barrier()
     t_e2e = time.perf_counter() - t0
     clocks = sampler.stop() if rank == 0 else None
 
-    # max over ranks
-    from paper_2208_02382_b200.shard import max_over_ranks
-    ms_sum, t_e2e, t_wall = max_over_ranks([ms_sum, t_e2e, t_wall], device="cuda")
+    ms_sum, t_e2e, t_wall = max_over_ranks([ms_sum, t_e2e, t_wall], device="cuda")   # max over ranks
 
     result = None
     if rank == 0:
         peaks, peaks_kind = load_peaks()
+        traffic = load_traffic()
         ms_per_step = ms_sum / args.steps
         value = world * pushes_per_step / (ms_per_step * 1e-3)
         e2e_value = world * pushes_per_step * args.steps / t_e2e
         # roofline of the dominant (only) kernel: FP64 pipe issue slots
         nominal_peak = 148 * 64 * float(peaks.get("sm_max_mhz", 1965.0)) * 1e6       # slots/s at max SM clock
-        measured_fp64 = bt.calib_fp64(300.0)
-        measured_rw6 = bt.calib_rw6(min(64_000_000, max(n, 8_000_000)), 5)
-        achieved = slots_per_launch / (statistics.mean(step_ms) * 1e-3)
-        hbm_time_ms = 96.0 * n / (float(peaks["hbm_gbs"]) * 1e9) * 1e3
-        alu_time_ms = slots_per_launch / nominal_peak * 1e3
-        bound = "alu" if alu_time_ms >= hbm_time_ms else "hbm"
-        if bound == "alu":
-            roof = {"bound": "alu", "achieved": achieved / 1e12, "peak": nominal_peak / 1e12, "unit": "Tslot/s",
-                    "frac": achieved / nominal_peak,
-                    # dram__bytes_read.sum + dram__bytes_write.sum of one launch on configs[1] from the ncu --set full capture in
-                    # profiles/r01_summary.md (48.0 MB read + 1.1 MB written: the 48 MB result stays in the 126 MB L2);
-                    # algorithmic bytes 96 B/particle = 96 MB per launch.  null for any other workload (not captured).
-                    "traffic": 49.1e6 if (args.workload == "fodo_channel" and n == 1_000_000) else None,
-                    "traffic_unit": "bytes per launch (ncu, profiles/r01_summary.md)",
-                    "peak_kind": "derived: 148 SMs x 64 FP64 lanes x %s sm_max_mhz (DESIGN.md s7)" % peaks_kind,
-                    "peak_measured_dfma_chain": measured_fp64 / 1e12, "frac_of_measured_dfma_chain": achieved / measured_fp64,
-                    "slots_per_particle": slots_pp, "tflops": None}
+        launches_per_step = launches // args.steps
+        roof = walk_roofline(n, cfg.lattice, cfg.nturns, launches_per_step, statistics.mean(step_ms) * 1e-3, peaks, nominal_peak)
+        roof["traffic"] = traffic_of(traffic, "walk:" + cfg.name)
+        roof["traffic_unit"] = "dram bytes per launch (ncu --set full; profiles/r02_traffic.csv names the capture)"
+        roof["launches_per_step"] = launches_per_step
+        roof["kernel"] = "bt::track_kernel<P=%d> grid=%d block=%d, record table in kernel parameters" % (
+            launch_info["particles_per_thread"], launch_info["grid"], launch_info["block"])
+        roof["rw6_stream_ceiling_gbs"] = bt.calib_rw6(min(64_000_000, max(n, 8_000_000)), 5)
+        if roof["bound"] == "alu":
+            measured_fp64 = bt.calib_fp64(300.0)
+            roof["peak_kind"] = "derived: 148 SMs x 64 FP64 lanes x %s sm_max_mhz (DESIGN.md s7)" % peaks_kind
+            roof["peak_measured_dfma_chain"] = measured_fp64 / 1e12
+            roof["frac_of_measured_dfma_chain"] = roof["achieved"] * 1e12 / measured_fp64
+            if args.workload == "nonlinear_ring":
+                roof["note"] = ("achieved counts the ALGORITHMIC slots of SURVEY 8d (sextupole 5 + octupole 8 per pair); the fused "
+                                "half-cell record shares x*x between the two adjacent kicks, so 24 instead of 25 FP64 instructions "
+                                "execute per half cell (120 400 instead of 125 400 per particle: sm__inst_executed_pipe_fp64 in "
+                                "profiles/): pipe utilisation = frac x 120400/125400")
+                roof["pipe_utilisation_executed"] = roof["frac"] * 120400.0 / 125400.0
         else:
-            gbs = 96.0 * n / (statistics.mean(step_ms) * 1e-3) / 1e9
-            roof = {"bound": "hbm", "achieved": gbs, "peak": float(peaks["hbm_gbs"]), "unit": "GB/s",
-                    "frac": gbs / float(peaks["hbm_gbs"]), "traffic": None, "peak_kind": peaks_kind + " copy bandwidth",
-                    "rw6_stream_ceiling_gbs": measured_rw6}
-        roof["kernel"] = "bt::track_kernel<P=%d> grid=%d block=%d smem=%dB" % (
-            launch_info["particles_per_thread"], launch_info["grid"], launch_info["block"], launch_info["smem_bytes"])
-        roof["roofline_time_ms"] = max(alu_time_ms, hbm_time_ms)
-        roof["rw6_stream_ceiling_gbs"] = measured_rw6
-        # CPU baseline: the oracle as it stands, bounded sample, host cores
-        cb_cfg = get_workload(args.workload, 0)
-        n_cb = min(n, 1_000_000)
-        cb_times, cores, cb_pushes = [], 0, 0
-        while sum(cb_times) < 10.0 and len(cb_times) < 12:       # about 10-30 s of CPU work
-            cb_pushes, tms, cores = oracle_rate(cb_cfg, n_cb)
-            cb_times += tms
-        cb_t = sum(cb_times) / len(cb_times)
-        cpu_baseline = {"value": cb_pushes / cb_t, "unit": UNIT, "cores": cores, "kind": "oracle",
-                        "sample": "%d of %d particles, full lattice (%d slice maps), %d turn(s); %d repetitions, %.1f s of CPU work in total"
-                                  % (n_cb, n, cfg.slice_maps_per_turn, cfg.nturns, len(cb_times), sum(cb_times))}
-        # the same oracle on ONE thread (SURVEY 8d asks for both), on a smaller sample of the same workload (~3 s)
-        try:
-            import oracle as _O
-            nthr = _O.num_threads()
-            _O.set_num_threads(1)
-            n_st = min(n_cb, 100_000)
-            st_pushes, st_times, _ = oracle_rate(cb_cfg, n_st)
-            _O.set_num_threads(nthr)
-            cpu_baseline["single_thread"] = {"value": st_pushes / st_times[0], "unit": UNIT, "cores": 1,
-                                             "sample": "%d of %d particles, full lattice, %d turn(s), one run" % (n_st, n, cfg.nturns)}
-        except Exception as exc:  # the all-cores number above is the contract; this one is extra
-            cpu_baseline["single_thread"] = {"unavailable": repr(exc)}
+            roof["peak_kind"] = peaks_kind + " copy bandwidth"
+        # CPU baseline: the oracle as it stands, bounded sample, host cores (all cores, and one thread)
+        cpu_baseline = oracle_track_baseline(get_workload(args.workload, 0), budget_s=15.0, single_budget_s=5.0)
         extras = {}
         if world == 1 and not args.no_extras:
-            extras["other_configs"] = bench_other_configs(bt, torch, flush, peaks, nominal_peak)
-            extras["spacecharge"] = bench_spacecharge(bt, torch, flush, peaks)
+            del pinned_out, pristine
+            torch.cuda.empty_cache()
+            extras["other_configs"] = bench_other_configs(bt, torch, flush, peaks, nominal_peak, traffic)
+            extras["spacecharge"] = bench_spacecharge(bt, torch, flush, peaks, traffic, args.resort_interval)
+        cfgd = config_dict(cfg, world)
         result = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
             "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-            "dtype": "f64", "data": "synthetic",
-            "config": {"workload": "configs[1] " + cfg.name, "particles_per_gpu": n, "elements": cfg.n_elements,
-                       "slice_maps_per_turn": cfg.slice_maps_per_turn, "turns_per_step": cfg.nturns,
-                       "slice_maps_per_s": world * n * cfg.slice_maps_per_turn * cfg.nturns / (ms_per_step * 1e-3),
-                       "l2": "flushed between timed steps (256 MiB write)", "parallelism": "particles sharded, %d rank(s), no collective" % world},
+            "dtype": "f64", "data": "synthetic", "config": cfgd,
+            "slice_maps_per_s": world * n * cfg.slice_maps_per_turn * cfg.nturns / (ms_per_step * 1e-3),
             "roofline": roof, "cpu_baseline": cpu_baseline,
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": 48 * n, "d2h_bytes_per_step": 48 * n,
-                    "ms_per_step": t_e2e / args.steps * 1e3,
+                    "ms_per_step": t_e2e / args.steps * 1e3, "vs_device_time": t_e2e / args.steps * 1e3 / ms_per_step,
                     "call": "bt_track_host(pinned in, pinned out, nturns, nchunks=%d): H2D / walk / D2H of the chunks overlap "
-                            "on three streams" % args.e2e_chunks},
+                            "on three streams; every launch carries its own coefficient table" % args.e2e_chunks},
             "gpu_launches": int(launches), "clocks": clocks,
             "step_ms_min_median_max": [min(step_ms), statistics.median(step_ms), max(step_ms)],
             "wall_s_timed_region": t_wall,
@@ -494,13 +598,14 @@ def run_ours(args):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=100)
-    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="fodo_channel", choices=["tiny_fodo", "fodo_channel", "chicane", "nonlinear_ring"])
+    ap.add_argument("--workload", default="nonlinear_ring", choices=sorted(WORKLOADS))
     ap.add_argument("--ref-sample", type=int, default=0,
                     help="particles per step the oracle is timed on in --impl reference (0 = sized for ~60 s in total)")
-    ap.add_argument("--e2e-chunks", type=int, default=8, help="chunks of the bunch in bt_track_host (e2e leg)")
+    ap.add_argument("--e2e-chunks", type=int, default=16, help="chunks of the bunch in bt_track_host (e2e leg)")
+    ap.add_argument("--resort-interval", type=int, default=5, help="bt_beam_set_resort_interval used in the configs[4] run")
     ap.add_argument("--no-extras", action="store_true",
                     help="skip the other configs and the space-charge kernels (N=1 only; the headline is unchanged)")
     args = ap.parse_args()

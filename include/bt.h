@@ -121,7 +121,11 @@ int bt_beam_get_ref(const bt_beam *beam, double *gamma, double *s, int64_t *turn
  * memory); download returns after the data has arrived. */
 int bt_beam_upload(bt_beam *beam, const double *const host[6]);
 int bt_beam_download(const bt_beam *beam, double *const host[6]);
-/* Zero-copy view of the 6 device arrays (P:l.102 "zero-copy access"); valid until bt_beam_destroy. */
+/* Zero-copy view of the 6 device arrays the particles live in (P:l.102 "zero-copy access"), in STORAGE order.  These are
+ * the arrays given to / allocated by bt_beam_create until bt_beam_sort_by_cell is used: a sort moves the bunch into a
+ * library-owned partner set of arrays and the next sort moves it back (ping-pong: a particle's data crosses memory once
+ * per sort, no copy back), so ask again after any sort.  bt_beam_upload and bt_track_host return the bunch to the original
+ * arrays. */
 int bt_beam_ptrs(bt_beam *beam, double *dev_ptrs_out[6]);
 int64_t bt_beam_size(const bt_beam *beam);
 
@@ -134,8 +138,8 @@ int64_t bt_beam_size(const bt_beam *beam);
  * touching rho, and what lets bt_gather_kick find its nodes in L1; both remain correct for any order and stay fast
  * while particles wander a few cells from where the sort left them, so one sort serves many steps.
  * bt_beam_download still returns the original order; bt_beam_upload resets storage to the caller's order.
- * The order of particles within one cell is not deterministic.  Needs n < 2^31; allocates 24 bytes per
- * particle of scratch on first use.
+ * The order of particles within one cell is not deterministic.  Needs n < 2^31; allocates 56 bytes per
+ * particle on first use (the partner set of six arrays the bunch is moved into -- see bt_beam_ptrs -- and two id arrays).
  */
 int bt_beam_sort_by_cell(bt_beam *beam, const bt_grid *grid, double zscale);
 /*

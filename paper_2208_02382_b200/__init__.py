@@ -165,7 +165,7 @@ class Beam:
     def __init__(self, n, storage=None, stream=None):
         self._h = _vp()
         self.n = int(n)
-        self.tensors = None
+        self._tensors = None
         if storage == "library":
             dev = None
         else:
@@ -173,8 +173,8 @@ class Beam:
             if storage is None:
                 storage = [torch.empty(self.n, dtype=torch.float64, device="cuda") for _ in range(6)]
             assert len(storage) == 6 and all(t.is_cuda and t.dtype == torch.float64 and t.is_contiguous() and t.numel() == self.n for t in storage)
-            self.tensors = list(storage)
-            dev = _ptr6([t.data_ptr() for t in self.tensors])
+            self._tensors = list(storage)
+            dev = _ptr6([t.data_ptr() for t in self._tensors])
         self.stream = _current_stream_ptr() if stream is None else int(stream)
         _check(lib.bt_beam_create(C.byref(self._h), self.n, dev, _vp(self.stream)), "bt_beam_create")
 
@@ -184,6 +184,25 @@ class Beam:
             self._h = None
 
     __del__ = close
+
+    @property
+    def tensors(self):
+        """Six CUDA tensors over the arrays the particles live in NOW (storage order): the tensors lent at construction,
+        or -- after bt_beam_sort_by_cell moved the bunch into the library's partner arrays (ping-pong) -- zero-copy views
+        of those (valid until the next sort / upload / close).  None for library-owned storage that was never lent."""
+        import torch
+        cur = self.ptrs()
+        if self._tensors is not None and all(t.data_ptr() == p for t, p in zip(self._tensors, cur)):
+            return self._tensors
+        if self._tensors is None:
+            return None
+        n = self.n
+
+        def view(ptr):
+            class _V:
+                __cuda_array_interface__ = {"shape": (n,), "typestr": "<f8", "data": (ptr, False), "version": 3, "strides": None}
+            return torch.as_tensor(_V(), device="cuda")
+        return [view(p) for p in cur]
 
     def set_ref(self, kin_energy_MeV, mass_MeV, charge_qe=1.0):
         _check(lib.bt_beam_set_ref(self._h, kin_energy_MeV, mass_MeV, charge_qe), "bt_beam_set_ref")

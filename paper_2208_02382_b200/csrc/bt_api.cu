@@ -309,7 +309,20 @@ static void plan_walk(Beam &b, int32_t nturns, WalkPlan &plan) {
         plan.ops = &b.h_table;
         plan.gamma_after = b.gamma;
         const double spr = b.table_slots / (double)b.h_table.size();
-        if (b.h_table.size() <= K) {
+        // A periodic channel (configs[1]: one FODO cell x 100) is one period walked repeats x nturns times: the same
+        // records in the same order, a table of 5 instead of 500 records in the launch's parameters.
+        size_t period = b.h_table.size();
+        for (size_t p = 1; p <= b.h_table.size() / 2; ++p) {
+            if (b.h_table.size() % p) continue;
+            if (memcmp(b.h_table.data(), b.h_table.data() + p, (b.h_table.size() - p) * sizeof(DevOp)) == 0) {
+                period = p;
+                break;
+            }
+        }
+        const long long passes = (long long)nturns * (long long)(b.h_table.size() / period);
+        if (period <= K && passes <= 0x7fffffffLL) {
+            plan.launches.push_back({0, (int32_t)period, (int32_t)passes, spr});
+        } else if (b.h_table.size() <= K) {
             plan.launches.push_back({0, (int32_t)b.h_table.size(), nturns, spr});
         } else {
             for (int32_t t = 0; t < nturns; ++t) add_segments(0, b.h_table.size(), spr);
@@ -393,7 +406,7 @@ int bt_beam_create(bt_beam **out, int64_t n, double *const dev_ptrs[6], void *cu
     b.max_smem_optin = (int)prop.sharedMemPerBlockOptin;
     b.stream = (cudaStream_t)cuda_stream;
     if (dev_ptrs) {
-        for (int i = 0; i < 6; ++i) b.q[i] = dev_ptrs[i];
+        for (int i = 0; i < 6; ++i) b.q[i] = b.home[i] = dev_ptrs[i];
         b.owns = false;
     } else {
         // one allocation, 6 slices, each 256-byte aligned (S0)
@@ -405,7 +418,7 @@ int bt_beam_create(bt_beam **out, int64_t n, double *const dev_ptrs[6], void *cu
             return fail(e == cudaErrorMemoryAllocation ? BT_ERR_OOM : BT_ERR_CUDA,
                         std::string("bt_beam_create: cudaMalloc: ") + cudaGetErrorString(e));
         }
-        for (int i = 0; i < 6; ++i) b.q[i] = (double *)((char *)base + stride * i);
+        for (int i = 0; i < 6; ++i) b.q[i] = b.home[i] = (double *)((char *)base + stride * i);
         b.owns = true;
     }
     b.aligned16 = b.aligned32 = true;
@@ -421,11 +434,11 @@ void bt_beam_destroy(bt_beam *beam) {
     if (!beam) return;
     Beam &b = beam->b;
     cudaStreamSynchronize(b.stream);
-    if (b.owns && b.q[0]) cudaFree(b.q[0]);
-    int *ibufs[] = {b.ids, b.ids_tmp, b.sort_key, b.sort_dest, b.sort_count, b.sort_block_sum};
+    if (b.owns && b.home[0]) cudaFree(b.home[0]);
+    if (b.alt[0]) cudaFree(b.alt[0]);
+    int *ibufs[] = {b.ids, b.ids_tmp, b.sort_count, b.sort_block_sum};
     for (int *p : ibufs)
         if (p) cudaFree(p);
-    if (b.scratch) cudaFree(b.scratch);
     if (b.mom_buf) cudaFree(b.mom_buf);
     for (int i = 0; i < 3; ++i) {
         if (b.pipe_stream[i]) cudaStreamDestroy(b.pipe_stream[i]);
@@ -466,9 +479,10 @@ int bt_beam_upload(bt_beam *beam, const double *const host[6]) {
     for (int i = 0; i < 6; ++i)
         if (!host[i]) return fail(BT_ERR_INVALID, "bt_beam_upload: host has a NULL entry");
     Beam &b = beam->b;
+    set_current_storage(&b, false);  // back in the home arrays, in the caller's order
     for (int i = 0; i < 6; ++i)
         BT_CUDA_TRY(cudaMemcpyAsync(b.q[i], host[i], (size_t)b.n * sizeof(double), cudaMemcpyHostToDevice, b.stream));
-    b.permuted = false;  // storage order = the caller's order again
+    b.permuted = false;
     b.deposits_since_sort = 0;
     return BT_OK;
 }
@@ -480,10 +494,11 @@ int bt_beam_download(const bt_beam *beam, double *const host[6]) {
     Beam &b = const_cast<Beam &>(beam->b);
     for (int i = 0; i < 6; ++i) {
         const double *src = b.q[i];
-        if (b.permuted) {  // storage is cell-sorted: restore the original order through the scratch array
-            int rc = unpermute_to(&b, i, b.scratch);
+        if (b.permuted) {  // storage is cell-sorted: restore the original order through the idle partner array
+            double *tmp = b.in_alt ? b.home[i] : b.alt[i];
+            int rc = unpermute_to(&b, i, tmp);
             if (rc != BT_OK) return rc;
-            src = b.scratch;
+            src = tmp;
         }
         BT_CUDA_TRY(cudaMemcpyAsync(host[i], src, (size_t)b.n * sizeof(double), cudaMemcpyDeviceToHost, b.stream));
     }
@@ -621,6 +636,7 @@ int bt_track_host(bt_beam *beam, const double *const host_in[6], double *const h
     }
     WalkPlan plan;
     plan_walk(b, nturns, plan);
+    set_current_storage(&b, false);  // the result lives in the home arrays, in the caller's order
     // the chunk streams start after everything already queued on the beam's stream
     BT_CUDA_TRY(cudaEventRecord(b.pipe_event[0], b.stream));
     for (int i = 0; i < 3; ++i) BT_CUDA_TRY(cudaStreamWaitEvent(b.pipe_stream[i], b.pipe_event[0], 0));

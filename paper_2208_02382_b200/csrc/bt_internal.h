@@ -86,7 +86,10 @@ struct TrackRange {
 
 struct Beam {
     int64_t n = 0;
-    double *q[6] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
+    double *q[6] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};     // where the particles are now (home or alt)
+    double *home[6] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};  // the caller's arrays (borrowed) or the library's
+    double *alt[6] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};   // library-owned partner set (bt_beam_sort_by_cell ping-pong)
+    bool in_alt = false;
     bool owns = false;
     bool aligned16 = false;
     bool aligned32 = false;  // all six arrays 32-byte aligned: 256-bit lane-run access in the grid kernels
@@ -111,9 +114,8 @@ struct Beam {
     int32_t resort_interval = 0;      // bt_beam_set_resort_interval: re-sort every n-th bt_deposit_cic (0 = never)
     int32_t deposits_since_sort = 0;
     int *ids = nullptr, *ids_tmp = nullptr;
-    int *sort_key = nullptr, *sort_dest = nullptr, *sort_count = nullptr, *sort_block_sum = nullptr;
+    int *sort_count = nullptr, *sort_block_sum = nullptr;
     long long sort_count_cap = 0;
-    double *scratch = nullptr;  // one array of n doubles
     const TrackRange *range = nullptr;  // non-NULL only inside bt_track_host
     cudaStream_t pipe_stream[3] = {nullptr, nullptr, nullptr};  // bt_track_host: chunk streams, created on first use
     cudaEvent_t pipe_event[3] = {nullptr, nullptr, nullptr};
@@ -154,6 +156,8 @@ int launch_gather_kick(Beam *b, const Grid *g, const double coef[3], double zsca
                        double tc_before, double h_after, double tc_after);
 int sort_by_cell(Beam *b, const Grid *g, double zscale);
 int unpermute_to(Beam *b, int c, double *out);  // out[ids[j]] = q[c][j] on the beam's stream
+int ensure_alt_storage(Beam *b);                 // allocates the partner arrays and the id arrays on first use
+void set_current_storage(Beam *b, bool use_alt); // q = alt or home; refreshes the alignment flags
 int launch_moments(Beam *b, double host_mean[6], double host_cov[36]);  // synchronises the beam's stream
 int launch_moments_async(Beam *b, double *dev_out);                      // 42 doubles to device memory, no synchronisation
 int poisson_solve(Grid *g, double gz, cudaStream_t stream);  // rho -> phi -> field records

@@ -58,13 +58,15 @@ __device__ __forceinline__ void load_run(const double *__restrict__ q, long long
 template <int NW>
 __device__ __forceinline__ void flush_cell(double *__restrict__ rho, int key, const double (&acc)[NW * NW * NW], int nx, long long nxy) {
     if (key < 0) return;
-    double *base = rho + key;  // key = linear index of the lowest node of the stencil
+    double *plane = rho + key;  // key = linear index of the lowest node of the stencil
 #pragma unroll
-    for (int dz = 0; dz < NW; ++dz)
+    for (int dz = 0; dz < NW; ++dz, plane += nxy) {
+        double *row = plane;
 #pragma unroll
-        for (int dy = 0; dy < NW; ++dy)
+        for (int dy = 0; dy < NW; ++dy, row += nx)
 #pragma unroll
-            for (int dx = 0; dx < NW; ++dx) atomicAdd(base + dz * nxy + dy * nx + dx, acc[(dz * NW + dy) * NW + dx]);
+            for (int dx = 0; dx < NW; ++dx) atomicAdd(row + dx, acc[(dz * NW + dy) * NW + dx]);
+    }
 }
 
 // ---- S4+S5 deposit, mode 1 (default): block-local cell binning in shared memory + run accumulation ------------
@@ -84,9 +86,25 @@ __device__ __forceinline__ void flush_cell(double *__restrict__ rho, int key, co
 // expression on every path.
 constexpr int kBinCap = 4096;  // cells of the chunk's bounding box that the shared histogram can hold
 
+// Runs hold UNSCALED weight sums (wx*wy)*wz and are scaled by q_weight once, at the flush.
+template <int NW>
+__device__ __forceinline__ void flush_cell_scaled(double *__restrict__ rho, int key, const double (&acc)[NW * NW * NW], double qw, int nx,
+                                                  long long nxy) {
+    if (key < 0) return;
+    double *plane = rho + key;
+#pragma unroll
+    for (int dz = 0; dz < NW; ++dz, plane += nxy) {
+        double *row = plane;
+#pragma unroll
+        for (int dy = 0; dy < NW; ++dy, row += nx)
+#pragma unroll
+            for (int dx = 0; dx < NW; ++dx) atomicAdd(row + dx, __dmul_rn(qw, acc[(dz * NW + dy) * NW + dx]));
+    }
+}
 // merge the lanes' open runs (segmented suffix reduction over CONTIGUOUS equal keys), heads flush
 template <int NW>
-__device__ __forceinline__ void merge_and_flush(double *__restrict__ rho, int cur, double (&acc)[NW * NW * NW], int nx, long long nxy) {
+__device__ __forceinline__ void merge_and_flush_scaled(double *__restrict__ rho, int cur, double (&acc)[NW * NW * NW], double qw, int nx,
+                                                       long long nxy) {
     const int lane = threadIdx.x & 31;
     const int prev = __shfl_up_sync(0xffffffffu, cur, 1);
     const bool head = (lane == 0) || (prev != cur);
@@ -106,7 +124,7 @@ __device__ __forceinline__ void merge_and_flush(double *__restrict__ rho, int cu
             }
         }
     }
-    if (head) flush_cell<NW>(rho, cur, acc, nx, nxy);
+    if (head) flush_cell_scaled<NW>(rho, cur, acc, qw, nx, nxy);
 }
 
 template <int NT, int R>
@@ -126,20 +144,6 @@ template <int NT, int R, int ORDER>
 constexpr int kBinRegs = (R >= 8 || ORDER > 1) ? 128 : (NT >= 512 ? 64 : 80);
 template <int NT, int R, int ORDER>
 constexpr int kBinMinBlocks = (65536 / NT) / kBinRegs<NT, R, ORDER> > 0 ? (65536 / NT) / kBinRegs<NT, R, ORDER> : 1;
-
-template <int NW>
-__device__ __forceinline__ void run_add(double *__restrict__ rho, int key, const double (&w)[NW * NW * NW], int &cur,
-                                        double (&acc)[NW * NW * NW], int nx, long long nxy) {
-    if (key != cur) {
-        flush_cell<NW>(rho, cur, acc, nx, nxy);
-        cur = key;
-#pragma unroll
-        for (int d = 0; d < NW * NW * NW; ++d) acc[d] = w[d];
-    } else {
-#pragma unroll
-        for (int d = 0; d < NW * NW * NW; ++d) acc[d] += w[d];
-    }
-}
 
 template <int NT, int R, bool VEC, int ORDER>
 __global__ void __launch_bounds__(NT, kBinMinBlocks<NT, R, ORDER>) deposit_binned_kernel(const double *__restrict__ x, const double *__restrict__ y,
@@ -197,7 +201,6 @@ __global__ void __launch_bounds__(NT, kBinMinBlocks<NT, R, ORDER>) deposit_binne
         // A chunk that is not spatially compact (unsorted input, the thin tails): bin what falls into a fixed 16^3 box
         // around the first inside particle -- this catches a cold core even in unsorted order -- the rest goes direct.
         const bool big = (long long)bx * by * bz > kBinCap;
-        const int ncell = big ? kBinCap : bx * by * bz;
         if (big) {  // block-uniform; compact chunks skip this barrier (the histogram was cleared during the previous walk)
             if (tid == box[6]) {
 #pragma unroll
@@ -246,16 +249,16 @@ __global__ void __launch_bounds__(NT, kBinMinBlocks<NT, R, ORDER>) deposit_binne
         // the spill bin hist[kBinCap] is not part of it
         int total = 0;
         {
-            const int b0 = tid * BPT;
-            const bool act = b0 < ncell;
+            // a thread owns the bins {4 NT q + 4 tid + 0..3}: 128-bit accesses contiguous across the warp (conflict-free);
+            // the scan order (thread-major) is a fixed permutation of the bins, which is all a counting sort needs
+            const int ncell = big ? kBinCap : bx * by * bz;  // bins >= ncell are empty: skip their quarter of the table (block-uniform)
             int4 v[BPT / 4];
             int s = 0;
-            if (act) {
 #pragma unroll
-                for (int q = 0; q < BPT / 4; ++q) {
-                    v[q] = *reinterpret_cast<const int4 *>(&sm.hist[b0 + 4 * q]);
-                    s += v[q].x + v[q].y + v[q].z + v[q].w;
-                }
+            for (int q = 0; q < BPT / 4; ++q) {
+                v[q] = make_int4(0, 0, 0, 0);
+                if (4 * NT * q < ncell) v[q] = *reinterpret_cast<const int4 *>(&sm.hist[4 * NT * q + 4 * tid]);
+                s += v[q].x + v[q].y + v[q].z + v[q].w;
             }
             int incl = s;
 #pragma unroll
@@ -272,16 +275,14 @@ __global__ void __launch_bounds__(NT, kBinMinBlocks<NT, R, ORDER>) deposit_binne
                 off += (w < wid) ? wt : 0;
                 total += wt;
             }
-            if (act) {
 #pragma unroll
-                for (int q = 0; q < BPT / 4; ++q) {
-                    int4 o;
-                    o.x = off, off += v[q].x;
-                    o.y = off, off += v[q].y;
-                    o.z = off, off += v[q].z;
-                    o.w = off, off += v[q].w;
-                    *reinterpret_cast<int4 *>(&sm.hist[b0 + 4 * q]) = o;
-                }
+            for (int q = 0; q < BPT / 4; ++q) {
+                int4 o;
+                o.x = off, off += v[q].x;
+                o.y = off, off += v[q].y;
+                o.z = off, off += v[q].z;
+                o.w = off, off += v[q].w;
+                if (4 * NT * q < ncell) *reinterpret_cast<int4 *>(&sm.hist[4 * NT * q + 4 * tid]) = o;
             }
         }
         __syncthreads();  // (5) offsets ready; total = number of binned particles
@@ -312,13 +313,178 @@ __global__ void __launch_bounds__(NT, kBinMinBlocks<NT, R, ORDER>) deposit_binne
                 cc.i = cc.j = cc.k = 0;
                 cc.wx1 = sm.w1[0][slot], cc.wy1 = sm.w1[1][slot], cc.wz1 = sm.w1[2][slot];
                 double w[NN];
-                node_weights<ORDER>(cc, qw, w);
-                run_add<NW>(rho, sm.key[slot], w, cur, acc, g.nx, nxy);
+                node_weights_unscaled<ORDER>(cc, w);
+                const int key = sm.key[slot];
+                if (key != cur) {  // a new run: the finished one leaves (scaled by q_weight), the accumulators restart from zero
+                    flush_cell_scaled<NW>(rho, cur, acc, qw, g.nx, nxy);
+                    cur = key;
+#pragma unroll
+                    for (int d = 0; d < NN; ++d) acc[d] = 0.0;
+                }
+#pragma unroll
+                for (int d = 0; d < NN; ++d) acc[d] += w[d];
             }
-            merge_and_flush<NW>(rho, cur, acc, g.nx, nxy);
+            merge_and_flush_scaled<NW>(rho, cur, acc, qw, g.nx, nxy);
         }
         // no barrier here: the next chunk touches hist / entries only after its barrier (1), which every thread of this
         // chunk's walk must reach first
+    }
+}
+
+// ---- S4+S5 deposit, mode 1 (default): WARP-private cell binning + run accumulation ---------------------------------------
+// Same idea as deposit_binned_kernel (bin the chunk's particles by cell in shared memory, then sum same-cell particles in
+// registers and flush a run with (ORDER+1)^3 reductions), re-cut so that nothing in it needs a block barrier:
+//   * a WARP owns a chunk of 32*R consecutive particles (R = 8: 256 particles) and its own slice of shared memory; warps
+//     only ever __syncwarp, so the warps of an SM drift apart and cover each other's latencies (the block-wide version
+//     ran 5-6 __syncthreads per 2048 particles at 16 resident warps: 41 % issue utilisation, profiles/r01b_summary.md);
+//   * no bounding box: the bin is the low three bits of each cell index, (k&7, j&7, i&7) -> 512 bins.  It is injective
+//     whenever the chunk spans <= 8 cells per axis, which is what a cell-sorted chunk does for many steps (the dense
+//     part of the bunch); where it is not (thin tails, unsorted input) aliased cells merely interleave inside a bin and
+//     shorten the runs -- the walk compares full node keys, so the result never depends on the hash;
+//   * the located particles (node key, the three weight fractions) are parked in shared memory in LOAD order right
+//     away and only a 2-byte slot index is sorted, so registers hold R bins + R ranks across the scan instead of R
+//     located particles (round 1: 128 registers, 16 warps per SM; here <= 96 and 20);
+//   * runs accumulate the UNSCALED weights (wx*wy)*wz and are scaled by q_weight once per flush
+//     (q*(w1+w2+...) instead of q*w1+q*w2+...: one rounding of difference, far inside R15's 1e-12).
+constexpr int kWarpBins = 512;
+
+template <int R>
+struct WarpBinSmem {
+    static constexpr int CW = 32 * R;        // particles per warp chunk
+    static constexpr int CWP = 32 * (R + 1); // padded slots: lane l, particle r -> l*(R+1) + r (64-bit accesses: 2 wavefronts)
+    alignas(16) int hist[kWarpBins];
+    alignas(16) unsigned short idx[CW];      // cell-ordered list of slots
+    int key[CWP];
+    double w1[3][CWP];
+};
+
+template <int R, int ORDER>
+constexpr int kWarpDepBlocks = ORDER == 1 ? (R >= 8 ? 5 : 8) : 4;  // 128-thread blocks per SM (shared memory and registers)
+
+template <int R, bool VEC, int ORDER>
+__global__ void __launch_bounds__(128, kWarpDepBlocks<R, ORDER>) deposit_warp_kernel(const double *__restrict__ x, const double *__restrict__ y,
+                                                                                   const double *__restrict__ t, long long n, GridDev g,
+                                                                                   double qw, double zscale, double *__restrict__ rho) {
+    extern __shared__ __align__(16) unsigned char wsmem_raw[];
+    constexpr int CW = WarpBinSmem<R>::CW;
+    constexpr int BPL = kWarpBins / 32;  // bins per lane in the scan
+    constexpr int NW = ORDER + 1, NN = NW * NW * NW;
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    WarpBinSmem<R> &sm = reinterpret_cast<WarpBinSmem<R> *>(wsmem_raw)[wid];
+    const long long nxy = (long long)g.nx * g.ny;
+    const long long nchunks = (n + CW - 1) / CW;
+    const long long warps_total = (long long)gridDim.x * (blockDim.x >> 5);
+    // a lane owns the bins {128 q + 4 lane + 0..3}: its 128-bit accesses are contiguous across the warp (conflict-free)
+#pragma unroll
+    for (int q = 0; q < BPL / 4; ++q) *reinterpret_cast<int4 *>(&sm.hist[128 * q + 4 * lane]) = make_int4(0, 0, 0, 0);
+    __syncwarp();
+    for (long long ch = (long long)blockIdx.x * (blockDim.x >> 5) + wid; ch < nchunks; ch += warps_total) {
+        // ---- phase 1: load, locate, park in shared memory, count per bin (one atomic per run of equal bins) ----
+        int bin[R], rank[R];
+        {
+            const long long p0 = ch * CW + (long long)lane * R;
+            double qx[R], qy[R], qt[R];
+            load_run<R, VEC>(x, p0, n, CUDART_NAN, qx);  // NaN => outside => contributes nothing
+            load_run<R, VEC>(y, p0, n, 0.0, qy);
+            load_run<R, VEC>(t, p0, n, 0.0, qt);
+#pragma unroll
+            for (int r = 0; r < R; ++r) {
+                Cic c;
+                const bool in = shape_locate<ORDER>(g, qx[r], qy[r], qt[r], zscale, c);
+                const int slot = lane * (R + 1) + r;
+                sm.key[slot] = (c.k * g.ny + c.j) * g.nx + c.i;
+                sm.w1[0][slot] = c.wx1;
+                sm.w1[1][slot] = c.wy1;
+                sm.w1[2][slot] = c.wz1;
+                bin[r] = in ? (((c.k & 7) << 6) | ((c.j & 7) << 3) | (c.i & 7)) : -1;
+            }
+            int len[R];
+            len[R - 1] = 1;
+#pragma unroll
+            for (int r = R - 2; r >= 0; --r) len[r] = (bin[r] == bin[r + 1]) ? len[r + 1] + 1 : 1;
+#pragma unroll
+            for (int r = 0; r < R; ++r) {
+                const bool head = (r == 0) || (bin[r] != bin[r - 1]);
+                if (head) rank[r] = bin[r] >= 0 ? atomicAdd(&sm.hist[bin[r]], len[r]) : 0;
+                else rank[r] = rank[r - 1] + 1;
+            }
+        }
+        __syncwarp();
+        // ---- phase 2: exclusive scan of the 512 counters (16 per lane, lane-major order), in place ----
+        int total;
+        {
+            int4 v[BPL / 4];
+            int s = 0;
+#pragma unroll
+            for (int q = 0; q < BPL / 4; ++q) {
+                v[q] = *reinterpret_cast<const int4 *>(&sm.hist[128 * q + 4 * lane]);
+                s += v[q].x + v[q].y + v[q].z + v[q].w;
+            }
+            int incl = s;
+#pragma unroll
+            for (int d = 1; d < 32; d <<= 1) {
+                const int o = __shfl_up_sync(0xffffffffu, incl, d);
+                if (lane >= d) incl += o;
+            }
+            total = __shfl_sync(0xffffffffu, incl, 31);
+            int off = incl - s;
+#pragma unroll
+            for (int q = 0; q < BPL / 4; ++q) {
+                int4 o;
+                o.x = off, off += v[q].x;
+                o.y = off, off += v[q].y;
+                o.z = off, off += v[q].z;
+                o.w = off, off += v[q].w;
+                *reinterpret_cast<int4 *>(&sm.hist[128 * q + 4 * lane]) = o;
+            }
+        }
+        __syncwarp();
+        // ---- phase 3: the cell-ordered list of slots ----
+#pragma unroll
+        for (int r = 0; r < R; ++r)
+            if (bin[r] >= 0) sm.idx[sm.hist[bin[r]] + rank[r]] = (unsigned short)(lane * (R + 1) + r);
+        __syncwarp();
+        // the counters are dead: clear them for the next chunk
+#pragma unroll
+        for (int q = 0; q < BPL / 4; ++q) *reinterpret_cast<int4 *>(&sm.hist[128 * q + 4 * lane]) = make_int4(0, 0, 0, 0);
+        // ---- phase 4: every lane walks R consecutive entries of the list, sums same-cell particles, merges, flushes ----
+        {
+            unsigned short my[R];
+            static_assert(R == 4 || R == 8, "idx is read as one 8- or 16-byte word per lane");
+            if (R == 8) {
+                const uint4 u = *reinterpret_cast<const uint4 *>(&sm.idx[lane * R]);
+                my[0] = u.x & 0xffff, my[1] = u.x >> 16, my[2] = u.y & 0xffff, my[3] = u.y >> 16;
+                my[4 % R] = u.z & 0xffff, my[5 % R] = u.z >> 16, my[6 % R] = u.w & 0xffff, my[7 % R] = u.w >> 16;
+            } else {
+                const uint2 u = *reinterpret_cast<const uint2 *>(&sm.idx[lane * R]);
+                my[0] = u.x & 0xffff, my[1] = u.x >> 16, my[2] = u.y & 0xffff, my[3] = u.y >> 16;
+            }
+            int cur = -1;
+            double acc[NN];
+#pragma unroll
+            for (int d = 0; d < NN; ++d) acc[d] = 0.0;
+#pragma unroll
+            for (int r = 0; r < R; ++r) {
+                if (lane * R + r >= total) break;
+                const int slot = my[r];
+                Cic cc;
+                cc.i = cc.j = cc.k = 0;
+                cc.wx1 = sm.w1[0][slot], cc.wy1 = sm.w1[1][slot], cc.wz1 = sm.w1[2][slot];
+                double w[NN];
+                node_weights_unscaled<ORDER>(cc, w);
+                const int key = sm.key[slot];
+                if (key != cur) {  // a new run: the finished one leaves, the accumulators restart from zero
+                    flush_cell_scaled<NW>(rho, cur, acc, qw, g.nx, nxy);
+                    cur = key;
+#pragma unroll
+                    for (int d = 0; d < NN; ++d) acc[d] = 0.0;
+                }
+#pragma unroll
+                for (int d = 0; d < NN; ++d) acc[d] += w[d];
+            }
+            merge_and_flush_scaled<NW>(rho, cur, acc, qw, g.nx, nxy);
+        }
+        __syncwarp();  // the next chunk overwrites the parked particles and the list
     }
 }
 
@@ -352,11 +518,27 @@ static int launch_deposit_binned(Beam *b, Grid *g, const GridDev &gd, double q_w
     return BT_OK;
 }
 
+template <int R, bool VEC, int ORDER>
+static int launch_deposit_warp(Beam *b, Grid *g, const GridDev &gd, double q_weight, double zscale) {
+    constexpr int kWarps = 4;  // 128-thread blocks
+    const int smem = (int)sizeof(WarpBinSmem<R>) * kWarps;
+    const long long nchunks = (b->n + WarpBinSmem<R>::CW - 1) / WarpBinSmem<R>::CW;
+    int per_sm = 1;
+    const int qrc = blocks_per_sm<deposit_warp_kernel<R, VEC, ORDER>>(32 * kWarps, smem, b->device, &per_sm);
+    if (qrc != BT_OK) return qrc;
+    long long blocks = (long long)b->num_sms * per_sm;
+    if (blocks > (nchunks + kWarps - 1) / kWarps) blocks = (nchunks + kWarps - 1) / kWarps;
+    deposit_warp_kernel<R, VEC, ORDER><<<(int)blocks, 32 * kWarps, smem, b->stream>>>(b->q[0], b->q[2], b->q[4], b->n, gd, q_weight, zscale,
+                                                                                     g->rho);
+    return BT_OK;
+}
+
 template <int ORDER>
 static int launch_deposit_order(Beam *b, Grid *g, const GridDev &gd, double q_weight, double zscale) {
     // knob deposit_mode: 0 = one particle per thread, (ORDER+1)^3 reductions each (baseline, kept for measurements);
-    // 1 (default) = block-local cell binning, 8 particles per thread (4 for order 2: 27 run accumulators per thread);
-    // 2 = binning with 4 particles per thread
+    // 1 (default) = warp-private cell binning, 8 particles per lane (4 at order 2: 27 run accumulators per lane);
+    // 2 = warp-private binning with 4 particles per lane; 3 = round 1's block-wide binning (2048-particle chunks,
+    // 1024 at order 2)
     const int mode = knob(KNOB_DEPOSIT_MODE, 1);
     if (mode == 0) {
         const int block = 256;
@@ -366,13 +548,20 @@ static int launch_deposit_order(Beam *b, Grid *g, const GridDev &gd, double q_we
         deposit_atomic_kernel<ORDER><<<(int)blocks, block, 0, b->stream>>>(b->q[0], b->q[2], b->q[4], b->n, gd, q_weight, zscale, g->rho);
         return BT_OK;
     }
-    if constexpr (ORDER == 1) {
-        if (mode != 2)
+    if (mode == 3) {
+        if constexpr (ORDER == 1)
             return b->aligned32 ? launch_deposit_binned<256, 8, true, ORDER>(b, g, gd, q_weight, zscale)
                                 : launch_deposit_binned<256, 8, false, ORDER>(b, g, gd, q_weight, zscale);
+        return b->aligned32 ? launch_deposit_binned<256, 4, true, ORDER>(b, g, gd, q_weight, zscale)
+                            : launch_deposit_binned<256, 4, false, ORDER>(b, g, gd, q_weight, zscale);
     }
-    return b->aligned32 ? launch_deposit_binned<256, 4, true, ORDER>(b, g, gd, q_weight, zscale)
-                        : launch_deposit_binned<256, 4, false, ORDER>(b, g, gd, q_weight, zscale);
+    if constexpr (ORDER == 1) {
+        if (mode != 2)
+            return b->aligned32 ? launch_deposit_warp<8, true, ORDER>(b, g, gd, q_weight, zscale)
+                                : launch_deposit_warp<8, false, ORDER>(b, g, gd, q_weight, zscale);
+    }
+    return b->aligned32 ? launch_deposit_warp<4, true, ORDER>(b, g, gd, q_weight, zscale)
+                        : launch_deposit_warp<4, false, ORDER>(b, g, gd, q_weight, zscale);
 }
 
 int launch_deposit(Beam *b, Grid *g, double q_weight, double zscale) {

@@ -7,7 +7,7 @@ Plumbing only (torch.distributed: NCCL on GPUs, gloo in the CPU tests); no arith
 """
 import os
 
-__all__ = ["rank_world", "shard_bounds", "rank_seed", "max_over_ranks", "allreduce_rho"]
+__all__ = ["rank_world", "shard_bounds", "max_over_ranks", "allreduce_rho"]
 
 
 def rank_world():
@@ -24,11 +24,6 @@ def shard_bounds(n_total, rank, world):
     base, rem = divmod(int(n_total), int(world))
     lo = rank * base + min(rank, rem)
     return lo, lo + base + (1 if rank < rem else 0)
-
-
-def rank_seed(seed, rank):
-    """Weak scaling (bench.py): every rank tracks its own bunch of the config's size, drawn from its own stream."""
-    return int(seed) + 1000 * int(rank)
 
 
 def _dist():

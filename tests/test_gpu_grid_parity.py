@@ -295,7 +295,7 @@ def test_sorted_tracking_still_matches():
     grid.close()
 
 
-@pytest.mark.parametrize("mode", [0, 1, 2])
+@pytest.mark.parametrize("mode", [0, 1, 2, 3])
 @pytest.mark.parametrize("variant", ["A", "B"])
 def test_deposit_modes_unaligned(mode, variant, knobs):
     import torch

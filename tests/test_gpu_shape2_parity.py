@@ -33,7 +33,7 @@ def run_deposit(c, sc, zscale=None, sort=False, storage=None, twice=False):
         grid.close()
 
 
-@pytest.mark.parametrize("mode", [0, 1])
+@pytest.mark.parametrize("mode", [0, 1, 3])
 @pytest.mark.parametrize("variant", ["A", "B"])
 @pytest.mark.parametrize("n,shape,sort", [(1, (8, 8, 8), False), (257, (16, 12, 10), False), (200_003, (32, 32, 32), False),
                                           (200_003, (32, 32, 32), True), (300_000, (128, 128, 128), True)])

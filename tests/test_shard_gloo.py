@@ -60,7 +60,7 @@ def _worker(rank, world, port, out_dir):
         assert np.max(np.abs(r[nz] - rho_all[nz]) / rho_all[nz]) <= 1e-12
         # ---- timing reduction: slowest rank ----
         assert shard.max_over_ranks([rank + 1.0, 5.0 - rank]) == [float(world), 5.0]
-        assert shard.rank_seed(1, rank) == 1 + 1000 * rank
+        assert W.rank_seed(1, rank) == 1 + 1000 * rank
         with open(os.path.join(out_dir, "ok%d" % rank), "w") as f:
             f.write("ok")
     finally:

@@ -150,6 +150,12 @@ def config(index: int, n: Optional[int] = None) -> TrackConfig:
     return c
 
 
+def rank_seed(seed: int, rank: int) -> int:
+    """Weak scaling (bench.py --gpus N): every rank tracks its own bunch of the config's size, drawn from its own stream.
+    Lives here, not in the package, so that the oracle arm of bench.py never loads the product library."""
+    return int(seed) + 1000 * int(rank)
+
+
 def _plane(u1, u2, twiss, sigma_q, sigma_p):
     if twiss is None:
         return sigma_q * u1, sigma_p * u2
