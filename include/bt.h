@@ -267,14 +267,19 @@ int bt_gather_kick(bt_beam *beam, const bt_grid *grid, const double coef[3], dou
 int bt_beam_moments(bt_beam *beam, double host_mean[6], double host_cov[36]);
 
 /*
- * Element-step diagnostics (mirrors sim.set_slice_step_diagnostics(True), P:l.61, at element granularity): the same walk
- * as bt_track(nturns) -- bit-identical final coordinates, reference energy, s and turn -- but one launch per element, each
- * followed by bt_beam_moments.  host_moments receives nturns * n_elems records of 42 doubles (mean[6], then cov[36] row-major)
- * in walk order: record (turn * n_elems + e) is the beam right after element e of that turn.  Costs 144 bytes of HBM
- * traffic per particle and element instead of 96 per call (two launches per element, no synchronisation until the end,
- * where the records are copied to the host): a diagnostics mode.
+ * Slice-step diagnostics (mirrors sim.set_slice_step_diagnostics(True), P:l.61; the statistics are P:l.43 "beam statistics"):
+ * the same walk as bt_track(nturns) -- bit-identical final coordinates, reference energy, s and turn -- with the beam
+ * statistics of bt_beam_moments taken INSIDE the walk, after every element (BT_DIAG_ELEMENT) or after every slice of every
+ * element (BT_DIAG_SLICE).  host_moments receives nturns * B records of 42 doubles (mean[6], then cov[36] row-major) in walk
+ * order, B = number of elements (resp. the sum of their nslice): record (turn * B + b) is the beam right after boundary b
+ * of that turn.  No extra pass over the particles (96 bytes per particle per launch, as bt_track): each warp writes one
+ * 216-byte row of partial sums per boundary and a second kernel combines them in a fixed order (bit-reproducible); O(1)
+ * launches per record table (<= 510 records) / per GiB of rows.  The sums are taken about the centre of the bunch as it
+ * is when the call starts, so a record loses about 2 log10(|mean - centre| / sigma) digits if the centroid runs away from
+ * there during the walk (none on any configuration whose centroid stays within a few sigma).  Synchronous.
  */
-int bt_track_diagnostics(bt_beam *beam, int32_t nturns, double *host_moments);
+enum { BT_DIAG_ELEMENT = 0, BT_DIAG_SLICE = 1 };
+int bt_track_diagnostics(bt_beam *beam, int32_t nturns, int32_t granularity, double *host_moments);
 
 /* ---- utilities ------------------------------------------------------------------------------ */
 int bt_sync(bt_beam *beam); /* cudaStreamSynchronize on the beam's stream */

@@ -61,7 +61,7 @@ EXPORTS = {
     "bt_deposit_cic": (C.c_int, [_vp, _vp, C.c_double, C.c_double, C.c_int]),
     "bt_gather_kick": (C.c_int, [_vp, _vp, _dp, C.c_double, C.c_double, C.c_double]),
     "bt_beam_moments": (C.c_int, [_vp, _dp, _dp]),
-    "bt_track_diagnostics": (C.c_int, [_vp, C.c_int32, _dp]),
+    "bt_track_diagnostics": (C.c_int, [_vp, C.c_int32, C.c_int32, _dp]),
     "bt_sync": (C.c_int, [_vp]),
     "bt_last_error": (C.c_char_p, []),
     "bt_version": (C.c_int, []),
@@ -252,12 +252,14 @@ class Beam:
         c = (C.c_double * 3)(*coef)
         _check(lib.bt_gather_kick(self._h, grid._h, c, zscale, half_drift_before, half_drift_after), "bt_gather_kick")
 
-    def track_diagnostics(self, nturns, n_elems):
-        """bt_track(nturns) with the beam statistics after every element: returns (mean[nturns, n_elems, 6],
-        cov[nturns, n_elems, 6, 6])."""
-        out = np.zeros((int(nturns), int(n_elems), 42))
-        _check(lib.bt_track_diagnostics(self._h, int(nturns), out.ctypes.data_as(_dp)), "bt_track_diagnostics")
-        return out[:, :, :6].copy(), out[:, :, 6:].reshape(int(nturns), int(n_elems), 6, 6).copy()
+    def track_diagnostics(self, nturns, n_boundaries, granularity="element"):
+        """bt_track(nturns) with the beam statistics taken inside the walk after every element ("element": n_boundaries =
+        number of elements) or every slice ("slice": n_boundaries = sum of nslice): returns
+        (mean[nturns, n_boundaries, 6], cov[nturns, n_boundaries, 6, 6])."""
+        gran = {"element": 0, "slice": 1}[granularity]
+        out = np.zeros((int(nturns), int(n_boundaries), 42))
+        _check(lib.bt_track_diagnostics(self._h, int(nturns), gran, out.ctypes.data_as(_dp)), "bt_track_diagnostics")
+        return out[:, :, :6].copy(), out[:, :, 6:].reshape(int(nturns), int(n_boundaries), 6, 6).copy()
 
     def moments(self):
         """(mean[6], cov[6, 6]) of x, px, y, py, t, pt -- computed on the device, returned as numpy arrays."""

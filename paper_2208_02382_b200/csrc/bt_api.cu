@@ -91,11 +91,15 @@ static void fuse_halfcell_runs(std::vector<DevOp> &out, size_t start) {
 }
 
 // ---- S1/S3: coefficients of one slice map per element, for one pass at reference gamma ----------
-double build_turn_table(const std::vector<bt_element> &lat, double gamma, std::vector<DevOp> &out, double *slots) {
+// diag != 0: tables of the diagnostics walk -- no record spans two elements (no fusion) and the last record of every element
+// is marked OP_MARK; diag == 2 (slice granularity): exactly one looped record per element (no five-slice groups either).
+// The coefficients are the same expressions, so the walk is bit-identical to bt_track's.
+double build_turn_table(const std::vector<bt_element> &lat, double gamma, std::vector<DevOp> &out, double *slots, int diag) {
     double nslots = 0.0;
-    const bool fuse = g_knob[KNOB_TRACK_FUSE].load() != 0;  // 0: one record per element (A/B measurements, bit-identity test)
+    const bool fuse = !diag && g_knob[KNOB_TRACK_FUSE].load() != 0;  // 0: one record per element (A/B measurements, bit-identity test)
     const size_t start = out.size();
     for (size_t i = 0; i < lat.size(); ++i) {
+        if (diag && i > 0) out.back().op |= OP_MARK;  // the previous element ended with the last record pushed so far
         const bt_element &e = lat[i];
         DevOp o;
         memset(&o, 0, sizeof(o));
@@ -115,7 +119,7 @@ double build_turn_table(const std::vector<bt_element> &lat, double gamma, std::v
                     out.back().c[4] = tc;
                     break;
                 }
-                o.op = e.nslice == 1 ? OP_DRIFT1 : OP_DRIFT;
+                o.op = (e.nslice == 1 && diag != 2) ? OP_DRIFT1 : OP_DRIFT;
                 o.c[0] = h;
                 o.c[1] = tc;
                 out.push_back(o);
@@ -123,7 +127,7 @@ double build_turn_table(const std::vector<bt_element> &lat, double gamma, std::v
             case BT_QUAD: {
                 const double k = e.p[0];
                 if (k == 0.0) {  // R5: k = 0 is a drift
-                    o.op = e.nslice == 1 ? OP_DRIFT1 : OP_DRIFT;
+                    o.op = (e.nslice == 1 && diag != 2) ? OP_DRIFT1 : OP_DRIFT;
                     o.c[0] = h;
                     o.c[1] = tc;
                     nslots += 3.0 * e.nslice;
@@ -143,6 +147,11 @@ double build_turn_table(const std::vector<bt_element> &lat, double gamma, std::v
                 o.c[5] = yb[2];
                 o.c[6] = tc;
                 nslots += 9.0 * e.nslice;
+                if (diag == 2) {
+                    o.op = OP_QUAD;
+                    out.push_back(o);
+                    break;
+                }
                 // nslice = 5a + b: a groups of five slices, then b single slices (same slice map, same order)
                 if (e.nslice / 5 > 0) {
                     o.op = OP_QUAD5;
@@ -261,6 +270,7 @@ double build_turn_table(const std::vector<bt_element> &lat, double gamma, std::v
         }
     }
     if (fuse) fuse_halfcell_runs(out, start);
+    if (diag && out.size() > start) out.back().op |= OP_MARK;
     if (slots) *slots = nslots;
     return gamma;
 }
@@ -440,6 +450,7 @@ void bt_beam_destroy(bt_beam *beam) {
     for (int *p : ibufs)
         if (p) cudaFree(p);
     if (b.mom_buf) cudaFree(b.mom_buf);
+    if (b.diag_rows) cudaFree(b.diag_rows);
     for (int i = 0; i < 3; ++i) {
         if (b.pipe_stream[i]) cudaStreamDestroy(b.pipe_stream[i]);
         if (b.pipe_event[i]) cudaEventDestroy(b.pipe_event[i]);
@@ -567,48 +578,90 @@ int bt_track(bt_beam *beam, int32_t nturns) {
     return BT_OK;
 }
 
-// Element-step diagnostics (P:l.61 set_slice_step_diagnostics; SURVEY 8(f) NEXT-1 "callable between elements"): the same walk,
-// one launch per element, with the beam statistics taken after every element.
-int bt_track_diagnostics(bt_beam *beam, int32_t nturns, double *host_moments) {
+// Slice-step / element-step diagnostics fused into the walk (P:l.61 set_slice_step_diagnostics): O(1)
+// launches per table -- the diagnostics walk writes one 216-byte row per (warp, boundary), a combine kernel turns the
+// rows of a launch into records.  Launches are cut where the record table (510 records) or the row buffer (1 GiB) is full.
+int bt_track_diagnostics(bt_beam *beam, int32_t nturns, int32_t granularity, double *host_moments) {
     if (!beam || !host_moments) return fail(BT_ERR_INVALID, "bt_track_diagnostics: NULL argument");
     if (nturns < 0) return fail(BT_ERR_INVALID, "bt_track_diagnostics: nturns < 0");
+    if (granularity != BT_DIAG_ELEMENT && granularity != BT_DIAG_SLICE) return fail(BT_ERR_INVALID, "bt_track_diagnostics: granularity must be BT_DIAG_ELEMENT or BT_DIAG_SLICE");
     Beam &b = beam->b;
     if (b.lattice.empty()) return fail(BT_ERR_STATE, "bt_track_diagnostics: bt_lattice_set not called");
     if (!b.has_ref) return fail(BT_ERR_STATE, "bt_track_diagnostics: bt_beam_set_ref not called");
-    std::vector<bt_element> one(1);
-    std::vector<DevOp> ops;
-    const size_t nrec = (size_t)nturns * b.lattice.size();
+    const bool slice = granularity == BT_DIAG_SLICE;
+    long long per_turn = 0;
+    for (const bt_element &e : b.lattice) per_turn += slice ? e.nslice : 1;
+    const long long nrec = per_turn * nturns;
     if (nrec == 0) return BT_OK;
-    double *dev = nullptr;  // all records stay on the device until the end: no synchronisation inside the walk
-    BT_CUDA_TRY(cudaMalloc(&dev, nrec * 42 * sizeof(double)));
-    double *out = dev;
-    int rc_all = BT_OK;
-    for (int32_t t = 0; t < nturns && rc_all == BT_OK; ++t) {
-        for (size_t e = 0; e < b.lattice.size(); ++e) {
-            one[0] = b.lattice[e];
-            ops.clear();
-            double slots = 0.0;
-            const double gamma_after = build_turn_table(one, b.gamma, ops, &slots);
-            for (size_t lo = 0; lo < ops.size(); lo += (size_t)kTableRecords) {
-                const size_t len = ops.size() - lo < (size_t)kTableRecords ? ops.size() - lo : (size_t)kTableRecords;
-                rc_all = launch_track(&b, ops.data() + lo, (int32_t)len, 1, slots / (double)ops.size());
-                if (rc_all != BT_OK) break;
-            }
-            if (rc_all != BT_OK) break;
-            b.gamma = gamma_after;
-            b.s += b.lattice[e].ds;
-            rc_all = launch_moments_async(&b, out);
-            if (rc_all != BT_OK) break;
-            out += 42;
+    int P = 1, block = 128;
+    const long long nwarps = diag_warps(&b, &P, &block);
+    const long long row_bytes = nwarps * 27 * (long long)sizeof(double);      // one boundary
+    const long long budget = 1LL << 30;
+    long long cap = budget / row_bytes;                                       // boundaries per launch
+    if (cap < 1) cap = 1;
+    if (cap > nrec) cap = nrec;
+    double *dev_out = nullptr, *centre = nullptr;
+    if (b.diag_rows_bytes < (size_t)(cap * row_bytes)) {  // the row buffer stays with the beam (up to 1 GiB)
+        if (b.diag_rows) {
+            BT_CUDA_TRY(cudaStreamSynchronize(b.stream));
+            BT_CUDA_TRY(cudaFree(b.diag_rows));
+            b.diag_rows = nullptr, b.diag_rows_bytes = 0;
         }
-        if (rc_all == BT_OK) b.turn += 1;
+        BT_CUDA_TRY(cudaMalloc(&b.diag_rows, (size_t)(cap * row_bytes)));
+        b.diag_rows_bytes = (size_t)(cap * row_bytes);
     }
-    b.table_valid = false;  // the constant bank no longer holds this beam's whole-lattice table
-    if (rc_all == BT_OK && cudaMemcpyAsync(host_moments, dev, nrec * 42 * sizeof(double), cudaMemcpyDeviceToHost, b.stream) != cudaSuccess)
-        rc_all = fail(BT_ERR_CUDA, "bt_track_diagnostics: copy of the records failed");
+    double *rows = b.diag_rows;
+    BT_CUDA_TRY(cudaMalloc(&dev_out, (size_t)nrec * 42 * sizeof(double) + 64));
+    centre = dev_out + nrec * 42;
+    int rc = launch_moments_centre(&b, centre);
+    std::vector<DevOp> ops, pend;
+    long long pend_b = 0, done_b = 0;
+    auto flush = [&]() -> int {
+        if (pend.empty()) return BT_OK;
+        const int r = launch_track_diag(&b, pend.data(), (int32_t)pend.size(), slice ? 1 : 0, (int)pend_b, centre, rows, dev_out + done_b * 42);
+        done_b += pend_b;
+        pend.clear();
+        pend_b = 0;
+        return r;
+    };
+    double gamma = b.gamma;
+    for (int32_t t = 0; t < nturns && rc == BT_OK; ++t) {
+        ops.clear();
+        gamma = build_turn_table(b.lattice, gamma, ops, nullptr, slice ? 2 : 1);
+        for (size_t i = 0; i < ops.size() && rc == BT_OK; ++i) {
+            DevOp o = ops[i];
+            const bool looped = (o.op & (OP_DRIFT | OP_QUAD | OP_SBEND | OP_DRIFTX | OP_QUADCHR)) != 0;
+            if (!(slice && looped)) {  // an indivisible record: a thin element, or any record at element granularity
+                const long long owes = slice ? 1 : ((o.op & OP_MARK) ? 1 : 0);
+                if (pend_b + owes > cap || (long long)pend.size() == kTableRecords) rc = flush();
+                if (rc != BT_OK) break;
+                pend.push_back(o);
+                pend_b += owes;
+                continue;
+            }
+            long long left = o.count;  // slice granularity: one row per slice; a long element may be cut between two launches
+            while (left > 0 && rc == BT_OK) {
+                if (pend_b == cap || (long long)pend.size() == kTableRecords) rc = flush();
+                if (rc != BT_OK) break;
+                const long long take = left < cap - pend_b ? left : cap - pend_b;
+                o.count = (int32_t)take;
+                pend.push_back(o);
+                pend_b += take;
+                left -= take;
+            }
+        }
+    }
+    if (rc == BT_OK) rc = flush();
+    if (rc == BT_OK) {
+        b.gamma = gamma;
+        b.s += b.lattice_length * (double)nturns;
+        b.turn += nturns;
+        if (cudaMemcpyAsync(host_moments, dev_out, (size_t)nrec * 42 * sizeof(double), cudaMemcpyDeviceToHost, b.stream) != cudaSuccess)
+            rc = fail(BT_ERR_CUDA, "bt_track_diagnostics: copy of the records failed");
+    }
     cudaStreamSynchronize(b.stream);
-    cudaFree(dev);
-    return rc_all;
+    cudaFree(dev_out);
+    return rc;
 }
 
 // Host-to-host walk: chunks of the bunch ride three streams, so that the H2D copy of chunk k+1, the walk of chunk k and

@@ -55,6 +55,7 @@ enum Op : int32_t {
     OP_RFSIN = 1 << 14,   // sinusoidal short RF (R18): px *= c0; py *= c0; pt = c0 pt + c1 (cos(c2 t + c3) - c4)
     OP_TAILDRIFT = 1 << 12,  // modifier of SEXT/OCT/SEXTOCT: the single-slice drift that follows the kick rides in the
                              // same record (c3 = h, c4 = h/(b0 g0)^2); same arithmetic, same order, one dispatch less
+    OP_MARK = 1 << 17,      // diagnostics tables only: an element ends with this record (a statistics row follows its last slice)
     OP_HALFCELL = 1 << 16   // head of a run of `count` half cells [QUAD1][SEXTOCT|TAILDRIFT]: this record holds the first quad's
                             // coefficients (c0..c6 as QUAD1), the next one the kicks' and the drift's (as SEXTOCT|TAILDRIFT), and so
                             // on for 2*count records, which the walk consumes in one dispatch
@@ -120,6 +121,8 @@ struct Beam {
     cudaStream_t pipe_stream[3] = {nullptr, nullptr, nullptr};  // bt_track_host: chunk streams, created on first use
     cudaEvent_t pipe_event[3] = {nullptr, nullptr, nullptr};
     double *mom_buf = nullptr;  // beam statistics: out[42], pad, per-block partials, ticket (moments.cu)
+    double *diag_rows = nullptr;  // bt_track_diagnostics: per-(boundary, warp) rows of partial sums, kept between calls
+    size_t diag_rows_bytes = 0;
 };
 
 struct Grid {
@@ -142,7 +145,7 @@ struct Grid {
 // Appends the records of one pass over the lattice starting at reference gamma; returns gamma after.
 // The number of records appended depends on the lattice only (not on gamma).  *slots (may be NULL) receives the
 // FP64 instruction slots one particle spends in this pass (minimal DFMA/DMUL sequences).
-double build_turn_table(const std::vector<bt_element> &lat, double gamma, std::vector<DevOp> &out, double *slots);
+double build_turn_table(const std::vector<bt_element> &lat, double gamma, std::vector<DevOp> &out, double *slots, int diag = 0);
 
 int grid_acquire(Grid *g, cudaStream_t s);  // make `s` wait for the last operation enqueued on the grid (no-op on the same stream)
 int grid_release(Grid *g, cudaStream_t s);  // record that the grid's latest operation was enqueued on `s`
@@ -151,6 +154,11 @@ int grid_release(Grid *g, cudaStream_t s);  // record that the grid's latest ope
 // One fused-walk launch: n_ops (<= kTableRecords) host records travel as kernel parameters and are walked nturns times.
 // slots_per_record (FP64 slots per particle per record, averaged) steers the particles-per-thread choice.
 int launch_track(Beam *b, const DevOp *h_table, int32_t n_ops, int32_t nturns, double slots_per_record);
+// Diagnostics walk (un-fused records, OP_MARK at element ends): one walk launch writing `nb` boundaries' rows + their combination
+// into out[nb][42].  diag_warps = rows per boundary for this beam (sizes the row buffer).
+int launch_track_diag(Beam *b, const DevOp *h_table, int32_t n_ops, int slice_gran, int nb, const double *centre, double *rows, double *out);
+int diag_warps(const Beam *b, int *particles_per_thread, int *block);
+int launch_moments_centre(Beam *b, double *dev_centre);  // provisional centre k[6] of the current bunch (moments.cu)
 int launch_deposit(Beam *b, Grid *g, double q_weight, double zscale);
 int launch_gather_kick(Beam *b, const Grid *g, const double coef[3], double zscale, double h_before,
                        double tc_before, double h_after, double tc_after);

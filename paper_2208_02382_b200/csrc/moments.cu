@@ -145,6 +145,34 @@ __global__ void __launch_bounds__(kMomBlock) moments_kernel(const __grid_constan
     if (threadIdx.x == 0) *a.ticket = 0u;  // ready for the next call
 }
 
+// k[6] = mean of min(n, 256) particles sampled at a stride of n/256: the provisional centre of the diagnostics walk, which
+// needs it BEFORE the walk overwrites the bunch (moments_kernel computes the same sample itself, per block).
+__global__ void __launch_bounds__(kMomBlock) moments_centre_kernel(const __grid_constant__ MomArgs a) {
+    __shared__ double scratch[kMomBlock / 32];
+    const long long m = a.n < kCentreSample ? a.n : kCentreSample;
+    const long long stride = a.n / m;
+#pragma unroll
+    for (int c = 0; c < 6; ++c) {
+        const double v = threadIdx.x < m ? a.q[c][threadIdx.x * stride] : 0.0;
+        const double k = block_sum(v, scratch) / (double)m;
+        if (threadIdx.x == 0) a.out[c] = k;
+    }
+}
+
+int launch_moments_centre(Beam *b, double *dev_centre) {
+    MomArgs a;
+    for (int c = 0; c < 6; ++c) a.q[c] = b->q[c];
+    a.n = b->n;
+    a.out = dev_centre;
+    a.partial = nullptr;
+    a.ticket = nullptr;
+    moments_centre_kernel<<<1, kMomBlock, 0, b->stream>>>(a);
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return fail(BT_ERR_CUDA, std::string("bt_track_diagnostics centre: ") + cudaGetErrorString(e));
+    g_launch_count.fetch_add(1);
+    return BT_OK;
+}
+
 // Enqueues the reduction; the 42 results (mean[6], cov[36]) land in dev_out (device memory) on the beam's stream.
 int launch_moments_async(Beam *b, double *dev_out) {
     const int max_blocks = b->num_sms * 4;

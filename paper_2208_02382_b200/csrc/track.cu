@@ -105,6 +105,74 @@ __device__ __forceinline__ void oct_kick(Ptc<P> &p, double c) {
     }
 }
 
+// R7 thin dipole edge: 2 slots
+template <int P>
+__device__ __forceinline__ void edge_kick(Ptc<P> &p, double c0, double c1) {
+    BT_FORP {
+        p.px[j] = fma(c0, p.x[j], p.px[j]);
+        p.py[j] = fma(c1, p.y[j], p.py[j]);
+    }
+}
+// R6 sector bend: 10 slots per slice (2 DMUL + 8 DFMA)
+template <int P>
+__device__ __forceinline__ void sbend_slice(Ptc<P> &p, double c0, double c1, double c2, double c3, double c4, double c5, double c6) {
+    BT_FORP {
+        const double x = p.x[j], px = p.px[j], pt = p.pt[j];
+        p.x[j] = fma(c3, pt, fma(c1, px, c0 * x));
+        p.px[j] = fma(c4, pt, fma(c0, px, c2 * x));
+        p.y[j] = fma(c6, p.py[j], p.y[j]);
+        // t += r51 x + r52 px + r56 pt with r51 = -r26 = -c4, r52 = -r16 = -c3
+        p.t[j] = fma(c5, pt, fma(-c3, px, fma(-c4, x, p.t[j])));
+    }
+}
+// R9 short RF, linearised: 4 slots
+template <int P>
+__device__ __forceinline__ void rf_kick(Ptc<P> &p, double c0, double c1) {
+    BT_FORP {
+        p.px[j] *= c0;
+        p.py[j] *= c0;
+        p.pt[j] = fma(c0, p.pt[j], c1 * p.t[j]);
+    }
+}
+// R17 exact drift: straight line with the exact time of flight; c0 = h, c1 = 1/beta0
+template <int P>
+__device__ __forceinline__ void driftx_slice(Ptc<P> &p, double c0, double c1) {
+    BT_FORP {
+        const double px = p.px[j], py = p.py[j], pt = p.pt[j];
+        const double a = fma(pt, pt, fma(-2.0 * pt, c1, 1.0)) - fma(px, px, py * py);
+        const double ips = 1.0 / sqrt(a);  // p0 / p_s
+        p.x[j] = fma(c0 * px, ips, p.x[j]);
+        p.y[j] = fma(c0 * py, ips, p.y[j]);
+        p.t[j] = fma(c0, fma(c1 - pt, ips, -c1), p.t[j]);
+    }
+}
+// R18 sinusoidal short RF: the energy kick qV cos(k t + phi) without the expansion in t
+template <int P>
+__device__ __forceinline__ void rfsin_kick(Ptc<P> &p, double c0, double c1, double c2, double c3, double c4) {
+    BT_FORP {
+        p.px[j] *= c0;
+        p.py[j] *= c0;
+        p.pt[j] = fma(c1, cos(fma(c2, p.t[j], c3)) - c4, c0 * p.pt[j]);
+    }
+}
+// R8 general order: repeated complex multiplication
+template <int P>
+__device__ __forceinline__ void mult_kick(Ptc<P> &p, double c0, double c1, int m) {
+    BT_FORP {
+        const double x = p.x[j], y = p.y[j];
+        double zr = 1.0, zi = 0.0;
+#pragma unroll 1
+        for (int k = 1; k < m; ++k) {
+            const double nr = fma(-zi, y, zr * x);
+            const double ni = fma(zi, x, zr * y);
+            zr = nr;
+            zi = ni;
+        }
+        p.px[j] -= fma(-c1, zi, c0 * zr);
+        p.py[j] += fma(c1, zr, c0 * zi);
+    }
+}
+
 // R20 chromatic quad for ONE particle: per-particle focusing strength k/(1+delta), closed-form flow of
 // H = -(1+d) + (px^2+py^2)/(2(1+d)) + k(x^2-y^2)/2 - pt/beta0.  Deliberately NOT inlined: two square roots, sincos, exp and
 // a reciprocal need ~100 registers of their own; as a real call they do not weigh on the register allocation of the
@@ -142,6 +210,15 @@ __device__ __noinline__ ChrOut quadchr_one(double x, double px, double y, double
     }
     o.t = t + (((ib - pt) / opd) * fma(integral, 0.5 / (opd * opd), h) - h * ib);
     return o;
+}
+
+// R20 chromatic quad, one slice: a call per particle (see quadchr_one)
+template <int P>
+__device__ __forceinline__ void quadchr_slice(Ptc<P> &p, double h, double ib, double ak, double sgn) {
+    BT_FORP {
+        const ChrOut o = quadchr_one(p.x[j], p.px[j], p.y[j], p.py[j], p.t[j], p.pt[j], h, ib, ak, sgn);
+        p.x[j] = o.x, p.px[j] = o.px, p.y[j] = o.y, p.py[j] = o.py, p.t[j] = o.t;
+    }
 }
 
 // ---- the record at tab[e] applied to the P particles of this thread; returns how many records it consumed ----------
@@ -200,81 +277,30 @@ __device__ __forceinline__ int apply(Ptc<P> &p, const DevOp *__restrict__ tab, c
         if (op & (OP_SEXTOCT | OP_OCT)) oct_kick<P>(p, r.c[2]);
         if (op & OP_TAILDRIFT) drift_slice<P>(p, r.c[3], r.c[4]);  // the single-slice drift that follows, same dispatch
     } else if (op & (OP_SBEND | OP_EDGE)) {
-        if (op & OP_EDGE) {  // R7: 2 slots
-            const double c0 = r.c[0], c1 = r.c[1];
-            BT_FORP {
-                p.px[j] = fma(c0, p.x[j], p.px[j]);
-                p.py[j] = fma(c1, p.y[j], p.py[j]);
-            }
-        } else {  // R6: 10 slots per slice (2 DMUL + 8 DFMA)
+        if (op & OP_EDGE) {
+            edge_kick<P>(p, r.c[0], r.c[1]);
+        } else {
             const double c0 = r.c[0], c1 = r.c[1], c2 = r.c[2], c3 = r.c[3], c4 = r.c[4], c5 = r.c[5], c6 = r.c[6];
             const int cnt = r.count;
 #pragma unroll 1
-            for (int s = 0; s < cnt; ++s) {
-                BT_FORP {
-                    const double x = p.x[j], px = p.px[j], pt = p.pt[j];
-                    p.x[j] = fma(c3, pt, fma(c1, px, c0 * x));
-                    p.px[j] = fma(c4, pt, fma(c0, px, c2 * x));
-                    p.y[j] = fma(c6, p.py[j], p.y[j]);
-                    // t += r51 x + r52 px + r56 pt with r51 = -r26 = -c4, r52 = -r16 = -c3
-                    p.t[j] = fma(c5, pt, fma(-c3, px, fma(-c4, x, p.t[j])));
-                }
-            }
+            for (int s = 0; s < cnt; ++s) sbend_slice<P>(p, c0, c1, c2, c3, c4, c5, c6);
         }
-    } else if (op & OP_RF) {  // R9: 4 slots
-        const double c0 = r.c[0], c1 = r.c[1];
-        BT_FORP {
-            p.px[j] *= c0;
-            p.py[j] *= c0;
-            p.pt[j] = fma(c0, p.pt[j], c1 * p.t[j]);
-        }
-    } else if (NL && (op & OP_DRIFTX)) {  // R17 exact drift: straight line with the exact time of flight; c0 = h, c1 = 1/beta0
+    } else if (op & OP_RF) {
+        rf_kick<P>(p, r.c[0], r.c[1]);
+    } else if (NL && (op & OP_DRIFTX)) {
         const double c0 = r.c[0], c1 = r.c[1];
         const int cnt = r.count;
 #pragma unroll 1
-        for (int s = 0; s < cnt; ++s) {
-            BT_FORP {
-                const double px = p.px[j], py = p.py[j], pt = p.pt[j];
-                const double a = fma(pt, pt, fma(-2.0 * pt, c1, 1.0)) - fma(px, px, py * py);
-                const double ips = 1.0 / sqrt(a);  // p0 / p_s
-                p.x[j] = fma(c0 * px, ips, p.x[j]);
-                p.y[j] = fma(c0 * py, ips, p.y[j]);
-                p.t[j] = fma(c0, fma(c1 - pt, ips, -c1), p.t[j]);
-            }
-        }
-    } else if (NL && (op & OP_QUADCHR)) {  // R20 chromatic quad: a call per particle (see quadchr_one)
+        for (int s = 0; s < cnt; ++s) driftx_slice<P>(p, c0, c1);
+    } else if (NL && (op & OP_QUADCHR)) {
         const double h = r.c[0], ib = r.c[1], ak = r.c[2], sgn = r.c[3];
         const int cnt = r.count;
 #pragma unroll 1
-        for (int s = 0; s < cnt; ++s) {
-            BT_FORP {
-                const ChrOut o = quadchr_one(p.x[j], p.px[j], p.y[j], p.py[j], p.t[j], p.pt[j], h, ib, ak, sgn);
-                p.x[j] = o.x, p.px[j] = o.px, p.y[j] = o.y, p.py[j] = o.py, p.t[j] = o.t;
-            }
-        }
-    } else if (NL && (op & OP_RFSIN)) {  // R18: the energy kick qV cos(k t + phi) without the expansion in t
-        const double c0 = r.c[0], c1 = r.c[1], c2 = r.c[2], c3 = r.c[3], c4 = r.c[4];
-        BT_FORP {
-            p.px[j] *= c0;
-            p.py[j] *= c0;
-            p.pt[j] = fma(c1, cos(fma(c2, p.t[j], c3)) - c4, c0 * p.pt[j]);
-        }
-    } else if (op & OP_MULT) {  // R8 general order: repeated complex multiplication; count = m
-        const double c0 = r.c[0], c1 = r.c[1];
-        const int m = r.count;
-        BT_FORP {
-            const double x = p.x[j], y = p.y[j];
-            double zr = 1.0, zi = 0.0;
-#pragma unroll 1
-            for (int k = 1; k < m; ++k) {
-                const double nr = fma(-zi, y, zr * x);
-                const double ni = fma(zi, x, zr * y);
-                zr = nr;
-                zi = ni;
-            }
-            p.px[j] -= fma(-c1, zi, c0 * zr);
-            p.py[j] += fma(c1, zr, c0 * zi);
-        }
+        for (int s = 0; s < cnt; ++s) quadchr_slice<P>(p, h, ib, ak, sgn);
+    } else if (NL && (op & OP_RFSIN)) {
+        rfsin_kick<P>(p, r.c[0], r.c[1], r.c[2], r.c[3], r.c[4]);
+    } else if (op & OP_MULT) {
+        mult_kick<P>(p, r.c[0], r.c[1], r.count);
     }
     return 1;
 }
@@ -379,6 +405,194 @@ __global__ void __launch_bounds__(kMaxBlock, kMinBlocks<P>) track_kernel(const _
     }
 }
 
+// ---- slice-step / element-step diagnostics INSIDE the walk (P:l.61 set_slice_step_diagnostics) ---------------
+// The same walk, on tables built WITHOUT record fusion (one record per element, `count` slices of one kind), and after every
+// slice (slice granularity) or after the last slice of every element (element granularity) each warp reduces the 27 sums
+//   S_i = sum (q_i - k_i),  P_ij = sum (q_i - k_i)(q_j - k_j)   (i <= j; k = a provisional centre, moments.cu)
+// of its 32*P particles and writes them as one 216-byte row: no extra pass over the particles, 96 B per particle per launch
+// as in bt_track.  The reduction across lanes is a transposing butterfly: 31 shuffles of doubles leave the total of value L
+// in lane L (27 separate butterflies would need 135).  diag_combine_kernel then adds the rows of one boundary in a fixed
+// order (bit-reproducible) and forms mean = k + S/n, cov = P/n - (S/n)(S/n)^T.
+constexpr int kDiagVals = 27;
+
+// one slice map of the record's kind; `count` is the diagnostics walk's business
+template <int P, bool NL>
+__device__ __forceinline__ void apply_one_slice(Ptc<P> &p, const DevOp &r) {
+    const int op = r.op;
+    if (op & OP_QUAD) {
+        quad_slice<P>(p, r.c[0], r.c[1], r.c[2], r.c[3], r.c[4], r.c[5], r.c[6]);
+    } else if (op & OP_DRIFT) {
+        drift_slice<P>(p, r.c[0], r.c[1]);
+    } else if (op & (OP_SEXT | OP_OCT)) {
+        if (op & OP_SEXT) sext_kick<P>(p, r.c[0], r.c[1]);
+        else oct_kick<P>(p, r.c[2]);
+    } else if (op & (OP_SBEND | OP_EDGE)) {
+        if (op & OP_EDGE) edge_kick<P>(p, r.c[0], r.c[1]);
+        else sbend_slice<P>(p, r.c[0], r.c[1], r.c[2], r.c[3], r.c[4], r.c[5], r.c[6]);
+    } else if (op & OP_RF) {
+        rf_kick<P>(p, r.c[0], r.c[1]);
+    } else if (NL && (op & OP_DRIFTX)) {
+        driftx_slice<P>(p, r.c[0], r.c[1]);
+    } else if (NL && (op & OP_QUADCHR)) {
+        quadchr_slice<P>(p, r.c[0], r.c[1], r.c[2], r.c[3]);
+    } else if (NL && (op & OP_RFSIN)) {
+        rfsin_kick<P>(p, r.c[0], r.c[1], r.c[2], r.c[3], r.c[4]);
+    } else if (op & OP_MULT) {
+        mult_kick<P>(p, r.c[0], r.c[1], r.count);
+    }
+}
+
+template <int NREC>
+struct DiagArgs {
+    double *q[6];
+    long long n;
+    const double *centre;  // k[6], device memory (moments_centre_kernel)
+    double *rows;          // [boundary][warp][27]
+    long long nwarps;      // warps of the launch = rows per boundary
+    int n_ops;
+    int slice_gran;        // 1: a row after every slice; 0: after every element
+    DevOp tab[NREC];
+};
+static_assert(sizeof(DiagArgs<kTableRecords>) <= 32764, "kernel parameter space is 32 764 bytes");
+
+template <int P>
+__device__ __forceinline__ void diag_emit(const Ptc<P> &p, const double (&k)[6], const bool (&valid)[P], double *__restrict__ row) {
+    double v[32];
+#pragma unroll
+    for (int i = 0; i < 32; ++i) v[i] = 0.0;
+    BT_FORP {
+        double d[6];
+        d[0] = p.x[j] - k[0], d[1] = p.px[j] - k[1], d[2] = p.y[j] - k[2];
+        d[3] = p.py[j] - k[3], d[4] = p.t[j] - k[4], d[5] = p.pt[j] - k[5];
+        if (!valid[j]) {
+#pragma unroll
+            for (int c = 0; c < 6; ++c) d[c] = 0.0;
+        }
+        int idx = 6;
+#pragma unroll
+        for (int a = 0; a < 6; ++a) {
+            v[a] += d[a];
+#pragma unroll
+            for (int b = a; b < 6; ++b) v[idx] = fma(d[a], d[b], v[idx]), ++idx;
+        }
+    }
+    // transposing butterfly: after the round with distance d a lane keeps the half of its values selected by its bit d
+    const int lane = threadIdx.x & 31;
+#pragma unroll
+    for (int d = 16; d >= 1; d >>= 1) {
+        const bool up = (lane & d) != 0;
+#pragma unroll
+        for (int i = 0; i < d; ++i) {
+            const double send = up ? v[i] : v[i + d];
+            const double keep = up ? v[i + d] : v[i];
+            v[i] = keep + __shfl_xor_sync(0xffffffffu, send, d);
+        }
+    }
+    if (lane < kDiagVals) row[lane] = v[0];  // lane L holds the warp's total of value L
+}
+
+// SLICE = false (element granularity): records are applied by the regular apply() -- whole elements, five-slice quad groups
+// included -- and a row follows every record marked OP_MARK (the last record of an element); SLICE = true: one slice at a
+// time, a row after each.
+template <int P, bool NL, int NREC, bool SLICE>
+__global__ void __launch_bounds__(128, P == 4 ? 3 : 4) track_diag_kernel(const __grid_constant__ DiagArgs<NREC> a) {
+    const int tid = threadIdx.x, B = blockDim.x;
+    const long long gw = (long long)blockIdx.x * (B >> 5) + (tid >> 5);
+    const long long base = (long long)blockIdx.x * (P * B);
+    // particle j of this thread (same assignment as track_kernel: pairs 2 tid, 2 tid + 1 of every 2B-particle group)
+    long long idx[P];
+    bool valid[P];
+    BT_FORP {
+        idx[j] = P >= 2 ? base + (long long)(j / 2) * 2 * B + 2 * tid + (j & 1) : base + tid;
+        valid[j] = idx[j] < a.n;
+    }
+    Ptc<P> p;
+    const bool full = base + (long long)P * B <= a.n;  // block-uniform
+    if (full) {
+        double *q[6];
+#pragma unroll
+        for (int c = 0; c < 6; ++c) q[c] = a.q[c] + base + (P >= 2 ? 2 * tid : tid);
+        load_ptc<P>(p, q, B);
+    } else {
+        BT_FORP {
+            p.x[j] = valid[j] ? a.q[0][idx[j]] : 0.0, p.px[j] = valid[j] ? a.q[1][idx[j]] : 0.0;
+            p.y[j] = valid[j] ? a.q[2][idx[j]] : 0.0, p.py[j] = valid[j] ? a.q[3][idx[j]] : 0.0;
+            p.t[j] = valid[j] ? a.q[4][idx[j]] : 0.0, p.pt[j] = valid[j] ? a.q[5][idx[j]] : 0.0;
+        }
+    }
+    double k[6];
+#pragma unroll
+    for (int c = 0; c < 6; ++c) k[c] = a.centre[c];
+    double *row = a.rows + gw * kDiagVals;
+    const long long row_stride = a.nwarps * kDiagVals;
+    if constexpr (SLICE) {
+#pragma unroll 1
+        for (int e = 0; e < a.n_ops; ++e) {
+            const DevOp &r = a.tab[e];
+            const int cnt = (r.op & (OP_DRIFT | OP_QUAD | OP_SBEND | OP_DRIFTX | OP_QUADCHR)) ? r.count : 1;
+#pragma unroll 1
+            for (int sl = 0; sl < cnt; ++sl) {
+                apply_one_slice<P, NL>(p, r);
+                diag_emit<P>(p, k, valid, row);
+                row += row_stride;
+            }
+        }
+    } else {
+#pragma unroll 1
+        for (int e = 0; e < a.n_ops;) {
+            const int mark = a.tab[e].op & OP_MARK;
+            e += apply<P, NL>(p, a.tab, e);
+            if (mark) {
+                diag_emit<P>(p, k, valid, row);
+                row += row_stride;
+            }
+        }
+    }
+    if (full) {
+        double *q[6];
+#pragma unroll
+        for (int c = 0; c < 6; ++c) q[c] = a.q[c] + base + (P >= 2 ? 2 * tid : tid);
+        store_ptc<P>(p, q, B);
+    } else {
+        BT_FORP {
+            if (valid[j]) {
+                a.q[0][idx[j]] = p.x[j], a.q[1][idx[j]] = p.px[j], a.q[2][idx[j]] = p.y[j];
+                a.q[3][idx[j]] = p.py[j], a.q[4][idx[j]] = p.t[j], a.q[5][idx[j]] = p.pt[j];
+            }
+        }
+    }
+}
+
+// rows of one boundary -> mean[6], cov[36]; one block per boundary, fixed summation order
+__global__ void __launch_bounds__(256) diag_combine_kernel(const double *__restrict__ rows, long long nwarps, const double *__restrict__ centre,
+                                                           long long n, double *__restrict__ out) {
+    __shared__ double part[8][32];
+    __shared__ double total[32];
+    const int lane = threadIdx.x & 31, grp = threadIdx.x >> 5;
+    const double *r = rows + (long long)blockIdx.x * nwarps * kDiagVals;
+    double s = 0.0;
+    if (lane < kDiagVals)
+        for (long long w = grp; w < nwarps; w += 8) s += r[w * kDiagVals + lane];
+    part[grp][lane] = s;
+    __syncthreads();
+    if (threadIdx.x < 32) {
+        double t = 0.0;
+#pragma unroll
+        for (int g = 0; g < 8; ++g) t += part[g][threadIdx.x];
+        total[threadIdx.x] = t;
+    }
+    __syncthreads();
+    const double inv_n = 1.0 / (double)n;
+    double *o = out + (long long)blockIdx.x * 42;
+    if (threadIdx.x < 6) o[threadIdx.x] = centre[threadIdx.x] + total[threadIdx.x] * inv_n;
+    if (threadIdx.x < 36) {
+        const int i = threadIdx.x / 6, j = threadIdx.x % 6;
+        const int lo = i < j ? i : j, hi = i < j ? j : i;
+        const int idx = 6 + lo * 6 - lo * (lo - 1) / 2 + (hi - lo);  // position of (lo, hi) in the packed upper triangle
+        o[6 + threadIdx.x] = total[idx] * inv_n - (total[lo] * inv_n) * (total[hi] * inv_n);
+    }
+}
+
 template <int P, bool NL, int NREC>
 static cudaError_t launch_one(const TrackArgs<NREC> &a, int grid, int block, cudaStream_t stream) {
     track_kernel<P, NL, NREC><<<grid, block, 0, stream>>>(a);
@@ -459,6 +673,76 @@ int launch_track(Beam *b, const DevOp *h_table, int32_t n_ops, int32_t nturns, d
     b->last_launch.block = block;
     b->last_launch.ppt = P;
     b->last_launch.smem = 0;
+    b->last_launch.launches += 1;
+    return BT_OK;
+}
+
+// ---- diagnostics walk: one launch over `n_ops` un-fused records, rows for `nb` boundaries, then their combination ----------
+int diag_warps(const Beam *b, int *P_out, int *block_out) {
+    int P = (b->aligned16 && b->n >= 65536) ? 4 : 1;
+    P = knob(KNOB_TRACK_PPT, P);
+    if (P != 1 && !(b->aligned16 && (P == 2 || P == 4))) P = 1;
+    const int block = 128;
+    *P_out = P;
+    *block_out = block;
+    const long long per_block = (long long)P * block;
+    return (int)((b->n + per_block - 1) / per_block) * (block / 32);
+}
+
+template <int P, int NREC>
+static cudaError_t launch_diag_p(const DiagArgs<NREC> &a, bool nl, bool slice, int grid, int block, cudaStream_t s) {
+    if (slice) {
+        if (nl) track_diag_kernel<P, true, NREC, true><<<grid, block, 0, s>>>(a);
+        else track_diag_kernel<P, false, NREC, true><<<grid, block, 0, s>>>(a);
+    } else {
+        if (nl) track_diag_kernel<P, true, NREC, false><<<grid, block, 0, s>>>(a);
+        else track_diag_kernel<P, false, NREC, false><<<grid, block, 0, s>>>(a);
+    }
+    return cudaGetLastError();
+}
+
+template <int NREC>
+static cudaError_t launch_diag_sized(DiagArgs<NREC> &a, const DevOp *h_table, int n_ops, int P, bool nl, int grid, int block, cudaStream_t s) {
+    memcpy(a.tab, h_table, (size_t)n_ops * sizeof(DevOp));
+    return P == 4 ? launch_diag_p<4, NREC>(a, nl, a.slice_gran != 0, grid, block, s)
+         : P == 2 ? launch_diag_p<2, NREC>(a, nl, a.slice_gran != 0, grid, block, s)
+                  : launch_diag_p<1, NREC>(a, nl, a.slice_gran != 0, grid, block, s);
+}
+
+int launch_track_diag(Beam *b, const DevOp *h_table, int32_t n_ops, int slice_gran, int nb, const double *centre, double *rows, double *out) {
+    if (n_ops < 1 || n_ops > kTableRecords) return fail(BT_ERR_INVALID, "launch_track_diag: table size");
+    int P, block;
+    const long long nwarps = diag_warps(b, &P, &block);
+    const int grid = (int)(nwarps / (block / 32));
+    bool nl = false;
+    for (int32_t e = 0; e < n_ops; ++e) nl = nl || (h_table[e].op & (OP_DRIFTX | OP_RFSIN | OP_QUADCHR));
+    auto fill = [&](auto &a) {
+        for (int c = 0; c < 6; ++c) a.q[c] = b->q[c];
+        a.n = b->n;
+        a.centre = centre;
+        a.rows = rows;
+        a.nwarps = nwarps;
+        a.n_ops = n_ops;
+        a.slice_gran = slice_gran;
+    };
+    cudaError_t e;
+    if (n_ops <= kTableRecordsSmall) {
+        DiagArgs<kTableRecordsSmall> a;
+        fill(a);
+        e = launch_diag_sized(a, h_table, n_ops, P, nl, grid, block, b->stream);
+    } else {
+        DiagArgs<kTableRecords> a;
+        fill(a);
+        e = launch_diag_sized(a, h_table, n_ops, P, nl, grid, block, b->stream);
+    }
+    if (e != cudaSuccess) return fail(BT_ERR_CUDA, std::string("bt_track_diagnostics launch: ") + cudaGetErrorString(e));
+    if (nb > 0) diag_combine_kernel<<<nb, 256, 0, b->stream>>>(rows, nwarps, centre, b->n, out);
+    e = cudaGetLastError();
+    if (e != cudaSuccess) return fail(BT_ERR_CUDA, std::string("bt_track_diagnostics combine: ") + cudaGetErrorString(e));
+    g_launch_count.fetch_add(2);
+    b->last_launch.grid = grid;
+    b->last_launch.block = block;
+    b->last_launch.ppt = P;
     b->last_launch.launches += 1;
     return BT_OK;
 }

@@ -105,12 +105,26 @@ def test_moments_argument_errors():
     beam.close()
 
 
-@pytest.mark.parametrize("idx", [0, 3])
-def test_track_diagnostics_moments_after_every_element(idx):
-    """bt_track_diagnostics: final state bit-identical to bt_track; every per-element record equals the oracle's moments of
-    the oracle's bunch at that point of the walk (config 0: FODO cell; config 3: ring with kicks and an RF cavity)."""
-    cfg = W.config(idx, n=20_000)
-    lat = cfg.lattice if idx == 0 else cfg.lattice[:16] + cfg.lattice[-1:]
+def _slice_lattice(lat):
+    """Every element cut into its slices as separate single-slice elements of length ds/nslice (the oracle then stops after
+    every slice; h = ds/nslice is the same rounded division on both sides)."""
+    out = []
+    for el in lat:
+        kind, ds, ns = el[0], el[1], el[2]
+        out += [(kind, ds / ns, 1) + tuple(el[3:])] * ns
+    return out
+
+
+@pytest.mark.parametrize("idx,n,granularity", [(0, 20_000, "element"), (0, 20_000, "slice"), (3, 20_000, "element"),
+                                               (3, 70_001, "element"), (1, 70_001, "slice")])
+def test_track_diagnostics_inside_the_walk(idx, n, granularity):
+    """bt_track_diagnostics (statistics taken inside the fused walk): final state bit-identical to bt_track; every record
+    equals the oracle's moments of the oracle's bunch at that boundary of the walk -- after every element or after every
+    slice (config 0: FODO cell with 10-slice quads; config 3: ring with kicks and an RF cavity that moves the reference
+    energy; config 1's cell with 25-slice quads; 70 001 particles = four particles per thread + a ragged last block); and
+    the whole table costs O(1) launches."""
+    cfg = W.config(idx, n=n)
+    lat = {0: cfg.lattice, 1: cfg.lattice[:5], 3: cfg.lattice[:16] + cfg.lattice[-1:]}[idx]
     nturns = 2
     c = W.make_bunch(cfg)
     beam = bt.Beam(cfg.n)
@@ -121,7 +135,11 @@ def test_track_diagnostics_moments_after_every_element(idx):
     plain, ref_state = beam.download(), beam.get_ref()
     beam.set_ref(cfg.kin_energy_MeV, cfg.mass_MeV, cfg.charge_qe)
     beam.upload(c)
-    mean, cov = beam.track_diagnostics(nturns, len(lat))
+    steps = _slice_lattice(lat) if granularity == "slice" else lat
+    n0 = bt.launch_count()
+    mean, cov = beam.track_diagnostics(nturns, len(steps), granularity)
+    launches = bt.launch_count() - n0
+    assert launches <= 1 + 2 * 2, launches             # centre + (walk, combine) per record table; RF lattices: one table per turn here
     got = beam.download()
     for a, b in zip(got, plain):
         assert np.array_equal(a, b)
@@ -129,10 +147,38 @@ def test_track_diagnostics_moments_after_every_element(idx):
     ref = [a.copy() for a in c]
     g = O.ref_from_kinetic(cfg.kin_energy_MeV, cfg.mass_MeV)[0]
     for t in range(nturns):
-        for e, el in enumerate(lat):
+        for e, el in enumerate(steps):
             g, _ = O.track(ref, [el], 1, g)
             rm, rc = O.moments(ref)
             sig = np.sqrt(np.diag(rc))
             assert np.max(np.abs(cov[t, e] - rc) / np.outer(sig, sig)) <= 1e-11, (t, e)
             assert np.all(np.abs(mean[t, e] - rm) <= 1e-11 * sig + 1e-15 * np.abs(rm)), (t, e)
+    beam.close()
+
+
+def test_track_diagnostics_many_boundaries_are_cut_into_launches():
+    """More boundaries than one row buffer / one record table holds (config 1's channel, slice granularity: 10 600 rows per
+    warp over 2 turns, 1000 records): the launches are cut, elements split between launches, and the records still line up."""
+    cfg = W.config(1, n=20_000)
+    c = W.make_bunch(cfg)
+    beam = bt.Beam(cfg.n)
+    beam.set_ref(cfg.kin_energy_MeV, cfg.mass_MeV, cfg.charge_qe)
+    beam.lattice_set(cfg.lattice)
+    beam.upload(c)
+    nb = cfg.slice_maps_per_turn
+    mean, cov = beam.track_diagnostics(2, nb, "slice")
+    got = beam.download()
+    final = [a.copy() for a in c]
+    O.track(final, cfg.lattice, 2, O.ref_from_kinetic(cfg.kin_energy_MeV, cfg.mass_MeV)[0])
+    rm, rc = O.moments(final)
+    sig = np.sqrt(np.diag(rc))
+    assert np.max(np.abs(cov[1, nb - 1] - rc) / np.outer(sig, sig)) <= 1e-11          # the last record = the final bunch
+    gm, gc = O.moments(got)
+    assert np.max(np.abs(cov[1, nb - 1] - gc) / np.outer(sig, sig)) <= 1e-12
+    # a matched beam in a periodic channel: the records at the cell ends repeat (P:l.112 "second moments remain matched")
+    per_cell = nb // 100
+    ends = cov[0, per_cell - 1::per_cell, 0, 0]
+    assert ends.shape == (100,) and np.max(np.abs(ends / ends[0] - 1.0)) < 2e-2
+    assert np.all(np.isfinite(cov)) and np.all(np.isfinite(mean))
+    assert bt.lib.bt_track_diagnostics(beam._h, 1, 7, np.zeros(42).ctypes.data_as(bt._dp)) == bt.BT_ERR_INVALID
     beam.close()
