@@ -342,6 +342,13 @@ def bench_other_configs(bt, torch, flush, peaks, nominal_peak, traffic):
             entry["moments"] = {"ms": tm * 1e3, "roofline": {"bound": "hbm", "achieved": 48.0 * n / tm / 1e9, "peak": hbm / 1e9,
                                                               "unit": "GB/s", "frac": 48.0 * n / tm / hbm,
                                                               "traffic": traffic_of(traffic, "moments:%d" % n)}}
+        if idx == 1:
+            # slice-step diagnostics inside the walk (P:l.61): the same walk + the beam statistics after
+            # every element / every slice, O(1) launches; the call is synchronous and returns the records on the host
+            for gran, nbound in (("element", cfg.n_elements), ("slice", cfg.slice_maps_per_turn)):
+                beam.track_diagnostics(1, nbound, gran)
+                td = statistics.mean(_event_ms(torch, lambda: beam.track_diagnostics(1, nbound, gran), 3, flush, restore))
+                entry["diagnostics_" + gran] = {"ms_per_call": td, "records": nbound, "vs_plain_track": td / (t * 1e3)}
         entry["cpu_baseline"] = oracle_track_baseline(cfg, budget_s=6.0, single_budget_s=3.0)
         out.append(entry)
         beam.close()

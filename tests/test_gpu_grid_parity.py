@@ -134,26 +134,36 @@ def test_gather_requires_field_and_ref():
     grid.close()
 
 
+@pytest.mark.parametrize("resort", [0, 3])
 @pytest.mark.parametrize("variant", ["A", "B"])
-def test_config4_in_run_reduced(variant):
-    """The BASELINE configs[4] step sequence (SURVEY 8d): oracle = 10 x [D(.005); deposit; gather+kick(.01); D(.005)];
-    library = bt_track(D(.005)) once, then per step deposit + gather_kick(0, .01 or .005 on the last)."""
+def test_config4_in_run_reduced(variant, resort):
+    """The BASELINE configs[4] step sequence at 4e5 particles / 64^3 nodes, in the caller's order and with the
+    library re-sorting by cell every third deposit."""
     sc = W.spacecharge_config(variant, n=400_000, shape=(64, 64, 64))
-    run_config4(sc)
+    run_config4(sc, resort)
 
 
-def run_config4(sc):
+def run_config4(sc, resort_interval=0):
+    """oracle = 10 x [D(.005); deposit; gather+kick(.01); D(.005)]; library = bt_track(D(.005)) once, then per step
+    bt_deposit_cic + bt_gather_kick(0, .01 -- .005 on the last step): deposit and gather see the same positions.
+    Checked: R15 (ii) (in-run: |rho - rho_ref| <= 1e-12 max(rho_ref, q_weight)) and the total charge at the first and at the
+    last step -- the library's positions there differ from the oracle's by rounding (its drifts are FMAs, the oracle's are a
+    rounded product and a rounded sum), which is exactly the case R15 (ii) is for; R15 (i) (isolated: strict 1e-12 on every
+    non-zero node, identical zero set) on the ORACLE's positions of the first and of the last step, deposited by a second
+    beam with the same storage handling; R14 on the final coordinates; s."""
     c = W.make_spacecharge_bunch(sc)
     E = W.gaussian_bunch_field(sc)
     g0 = O.ref_from_kinetic(sc.kin_energy_MeV, sc.mass_MeV)[0]
     half = [("drift", sc.ds / 2, 1)]
+    check_steps = (0, sc.nsteps - 1)
     # oracle
     ref = [a.copy() for a in c]
-    rho_ref = []
+    rho_ref, pos_ref = {}, {}
     for step in range(sc.nsteps):
         O.track(ref, half, 1, g0)
-        r, n_in = O.deposit_cic(ref[0], ref[2], ref[4], sc.shape, sc.lo, sc.d, sc.q_weight, sc.zscale)
-        rho_ref.append((r, n_in))
+        if step in check_steps:
+            rho_ref[step] = O.deposit_cic(ref[0], ref[2], ref[4], sc.shape, sc.lo, sc.d, sc.q_weight, sc.zscale)
+            pos_ref[step] = [a.copy() for a in ref]
         O.gather_kick(ref, sc.shape, sc.lo, sc.d, E, sc.kick_coef, sc.zscale)
         O.track(ref, half, 1, g0)
     # library
@@ -164,50 +174,38 @@ def run_config4(sc):
     beam.upload(c)
     beam.lattice_set(half)
     beam.track(1)
+    beam.set_resort_interval(resort_interval)
     for step in range(sc.nsteps):
         beam.deposit_cic(grid, sc.q_weight, sc.zscale, zero_first=True)
-        if step in (0, sc.nsteps - 1):
+        if step in check_steps:
             rho = grid.download_rho()
             r, n_in = rho_ref[step]
-            tol = 1e-12 * np.maximum(r, sc.q_weight)          # R15 (ii) in-run criterion
-            if step == 0:
-                assert r15_isolated(rho, r) <= 1e-12           # positions still bit-identical after one exact drift? (not guaranteed)  # noqa
-            assert np.all(np.abs(rho - r) <= tol)
+            assert np.all(np.abs(rho - r) <= 1e-12 * np.maximum(r, sc.q_weight)), step          # R15 (ii)
             assert abs(math.fsum(rho.ravel()) - sc.q_weight * n_in) <= 1e-13 * sc.q_weight * n_in
         beam.gather_kick(grid, sc.kick_coef, sc.zscale, 0.0, sc.ds if step < sc.nsteps - 1 else sc.ds / 2)
     got = beam.download()
     assert max(r14_error(got, ref)) <= 1e-11
     assert abs(beam.get_ref()[1] - sc.nsteps * sc.ds) < 1e-12
     beam.close()
+    # R15 (i): the oracle's own positions (bit-identical input), same storage handling
+    iso = bt.Beam(sc.n)
+    iso.set_ref(sc.kin_energy_MeV, sc.mass_MeV, sc.charge_qe)
+    for step in check_steps:
+        iso.upload(pos_ref[step])
+        if resort_interval:
+            iso.sort_by_cell(grid, sc.zscale)
+        iso.deposit_cic(grid, sc.q_weight, sc.zscale, zero_first=True)
+        assert r15_isolated(grid.download_rho(), rho_ref[step][0]) <= 1e-12, step
+    iso.close()
     grid.close()
 
 
+@pytest.mark.parametrize("resort", [0, 10])
 @pytest.mark.parametrize("variant", ["A", "B"])
-def test_config4_full_size(variant):
-    """8M particles, 128^3 nodes, as bench/BASELINE: isolated deposit on every node, gather+kick with drifts on every
-    particle (one step), total charge."""
-    sc = W.spacecharge_config(variant)
-    c = W.make_spacecharge_bunch(sc)
-    E = W.gaussian_bunch_field(sc)
-    beam = bt.Beam(sc.n)
-    grid = bt.Grid(sc.shape, sc.lo, sc.d)
-    beam.set_ref(sc.kin_energy_MeV, sc.mass_MeV, sc.charge_qe)
-    grid.set_field(*E)
-    beam.upload(c)
-    beam.deposit_cic(grid, sc.q_weight, sc.zscale, zero_first=True)
-    rho = grid.download_rho()
-    ref_rho, n_in = O.deposit_cic(c[0], c[2], c[4], sc.shape, sc.lo, sc.d, sc.q_weight, sc.zscale)
-    assert r15_isolated(rho, ref_rho) <= 1e-12
-    assert abs(math.fsum(rho.ravel()) - sc.q_weight * n_in) <= 1e-13 * sc.q_weight * n_in
-    beam.gather_kick(grid, sc.kick_coef, sc.zscale, 0.0, sc.ds)
-    got = beam.download()
-    ref = [a.copy() for a in c]
-    g0 = O.ref_from_kinetic(sc.kin_energy_MeV, sc.mass_MeV)[0]
-    O.gather_kick(ref, sc.shape, sc.lo, sc.d, E, sc.kick_coef, sc.zscale)
-    O.track(ref, [("drift", sc.ds, 1)], 1, g0)
-    assert max(r14_error(got, ref)) <= 1e-11
-    beam.close()
-    grid.close()
+def test_config4_full_size(variant, resort):
+    """configs[4] as BASELINE states it -- 8e6 particles, 128^3 nodes, all 10 steps -- in the caller's order and with
+    bt_beam_set_resort_interval(10); criteria in run_config4."""
+    run_config4(W.spacecharge_config(variant), resort)
 
 
 # ---- S4 cell binning ---------------------------------------------------------------------------------

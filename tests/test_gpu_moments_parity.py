@@ -33,7 +33,7 @@ def check(c, beam=None):
     return mean, cov
 
 
-@pytest.mark.parametrize("n", [1, 2, 3, 255, 4097, 100_003, 1_000_000])
+@pytest.mark.parametrize("n", [1, 2, 3, 255, 4097, 100_003, 1_000_000, 64_000_000])
 def test_moments_gaussian_sizes(n):
     cfg = W.config(0, n=n)
     check(W.make_bunch(cfg))
@@ -47,6 +47,22 @@ def test_moments_offset_and_correlated_bunch():
     c[4] -= 3.0
     c[1] += 0.7 * c[0]
     check(c)
+
+
+def test_moments_on_a_cell_sorted_offset_bunch_at_bench_size():
+    """configs[4]'s 8e6-particle bunch, shifted by five sigma and cell-sorted: the first particles of the storage then all sit
+    in one corner of the grid, so the provisional centre must come from a sample spread over the whole storage."""
+    sc = W.spacecharge_config("A")
+    c = W.make_spacecharge_bunch(sc)
+    c[0] += 5e-3
+    c[3] -= 2e-3
+    beam = bt.Beam(sc.n)
+    grid = bt.Grid(sc.shape, [l + (5e-3 if a == 0 else 0.0) for a, l in enumerate(sc.lo)], sc.d)
+    beam.upload(c)
+    beam.sort_by_cell(grid, sc.zscale)
+    check(c, beam)
+    beam.close()
+    grid.close()
 
 
 def test_moments_unaligned_storage_and_odd_count():
