@@ -302,7 +302,7 @@ def walk_roofline(n, lattice, nturns, launches, t_s, peaks, nominal_peak):
             "roofline_time_ms": t_hbm * 1e3}
 
 
-def bench_other_configs(bt, torch, flush, peaks, nominal_peak, traffic):
+def bench_other_configs(bt, torch, flush, peaks, nominal_peak, traffic, with_cpu=True):
     """bt_track on configs[0], [1], [2] at full size (one call = the config's nturns), each with the oracle timed beside it."""
     out = []
     hbm = float(peaks["hbm_gbs"]) * 1e9
@@ -349,7 +349,8 @@ def bench_other_configs(bt, torch, flush, peaks, nominal_peak, traffic):
                 beam.track_diagnostics(1, nbound, gran)
                 td = statistics.mean(_event_ms(torch, lambda: beam.track_diagnostics(1, nbound, gran), 3, flush, restore))
                 entry["diagnostics_" + gran] = {"ms_per_call": td, "records": nbound, "vs_plain_track": td / (t * 1e3)}
-        entry["cpu_baseline"] = oracle_track_baseline(cfg, budget_s=6.0, single_budget_s=3.0)
+        if with_cpu:
+            entry["cpu_baseline"] = oracle_track_baseline(cfg, budget_s=6.0, single_budget_s=3.0)
         out.append(entry)
         beam.close()
         del pristine, beam
@@ -357,7 +358,7 @@ def bench_other_configs(bt, torch, flush, peaks, nominal_peak, traffic):
     return out
 
 
-def bench_spacecharge(bt, torch, flush, peaks, traffic, interval):
+def bench_spacecharge(bt, torch, flush, peaks, traffic, interval, with_cpu=True):
     """configs[4] A and B at full size (8e6 particles, 128^3 nodes): 10 steps of bt_deposit_cic + bt_gather_kick(0, ds)
     (SURVEY 8d call sequence) with the library's own re-sort cadence (bt_beam_set_resort_interval: every sort the run
     needs is inside the timed deposit calls), every call timed with CUDA events, L2 flushed before each.
@@ -441,7 +442,7 @@ def bench_spacecharge(bt, torch, flush, peaks, traffic, interval):
         }
         if poisson:
             out[key]["poisson_solve"] = poisson
-        if order == 1:
+        if order == 1 and with_cpu:
             out[key]["cpu_baseline"] = oracle_grid_baseline(sc, c, E)
         beam.close()
         grid.close()
@@ -473,6 +474,20 @@ def run_ours(args):
         if world > 1:
             dist.barrier()
         torch.cuda.synchronize()
+
+    if args.section in ("tracking", "spacecharge"):
+        # one part of the N=1 extras on its own (used for the ncu captures under profiles/): same code, same numbers
+        peaks, _kind = load_peaks()
+        traffic = load_traffic()
+        nominal_peak = 148 * 64 * float(peaks.get("sm_max_mhz", 1965.0)) * 1e6
+        flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
+        if args.section == "tracking":
+            part = {"other_configs": bench_other_configs(bt, torch, flush, peaks, nominal_peak, traffic, not args.no_cpu)}
+        else:
+            part = {"spacecharge": bench_spacecharge(bt, torch, flush, peaks, traffic, args.resort_interval, not args.no_cpu)}
+        part["section"] = args.section
+        print(json.dumps(part), flush=True)
+        return 0
 
     cfg = get_workload(args.workload, rank)
     n = cfg.n
@@ -571,13 +586,13 @@ def run_ours(args):
         else:
             roof["peak_kind"] = peaks_kind + " copy bandwidth"
         # CPU baseline: the oracle as it stands, bounded sample, host cores (all cores, and one thread)
-        cpu_baseline = oracle_track_baseline(get_workload(args.workload, 0), budget_s=15.0, single_budget_s=5.0)
+        cpu_baseline = None if args.no_cpu else oracle_track_baseline(get_workload(args.workload, 0), budget_s=15.0, single_budget_s=5.0)
         extras = {}
-        if world == 1 and not args.no_extras:
+        if world == 1 and not args.no_extras and args.section == "all":
             del pinned_out, pristine
             torch.cuda.empty_cache()
-            extras["other_configs"] = bench_other_configs(bt, torch, flush, peaks, nominal_peak, traffic)
-            extras["spacecharge"] = bench_spacecharge(bt, torch, flush, peaks, traffic, args.resort_interval)
+            extras["other_configs"] = bench_other_configs(bt, torch, flush, peaks, nominal_peak, traffic, not args.no_cpu)
+            extras["spacecharge"] = bench_spacecharge(bt, torch, flush, peaks, traffic, args.resort_interval, not args.no_cpu)
         cfgd = config_dict(cfg, world)
         result = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
@@ -615,6 +630,10 @@ def main():
     ap.add_argument("--resort-interval", type=int, default=5, help="bt_beam_set_resort_interval used in the configs[4] run")
     ap.add_argument("--no-extras", action="store_true",
                     help="skip the other configs and the space-charge kernels (N=1 only; the headline is unchanged)")
+    ap.add_argument("--section", default="all", choices=["all", "headline", "tracking", "spacecharge"],
+                    help="N=1: all = the contract line with other_configs and spacecharge; headline = the contract line alone; "
+                         "tracking / spacecharge = that part of the extras alone (for the ncu captures under profiles/)")
+    ap.add_argument("--no-cpu", action="store_true", help="skip the oracle timings (profiling runs only)")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
