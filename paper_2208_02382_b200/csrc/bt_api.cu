@@ -451,6 +451,7 @@ void bt_beam_destroy(bt_beam *beam) {
         if (p) cudaFree(p);
     if (b.mom_buf) cudaFree(b.mom_buf);
     if (b.diag_rows) cudaFree(b.diag_rows);
+    if (b.diag_out) cudaFree(b.diag_out);
     for (int i = 0; i < 3; ++i) {
         if (b.pipe_stream[i]) cudaStreamDestroy(b.pipe_stream[i]);
         if (b.pipe_event[i]) cudaEventDestroy(b.pipe_event[i]);
@@ -611,7 +612,17 @@ int bt_track_diagnostics(bt_beam *beam, int32_t nturns, int32_t granularity, dou
         b.diag_rows_bytes = (size_t)(cap * row_bytes);
     }
     double *rows = b.diag_rows;
-    BT_CUDA_TRY(cudaMalloc(&dev_out, (size_t)nrec * 42 * sizeof(double) + 64));
+    const size_t out_bytes = (size_t)nrec * 42 * sizeof(double) + 64;
+    if (b.diag_out_bytes < out_bytes) {  // the record buffer stays with the beam as well (no allocation on repeated calls)
+        if (b.diag_out) {
+            BT_CUDA_TRY(cudaStreamSynchronize(b.stream));
+            BT_CUDA_TRY(cudaFree(b.diag_out));
+            b.diag_out = nullptr, b.diag_out_bytes = 0;
+        }
+        BT_CUDA_TRY(cudaMalloc(&b.diag_out, out_bytes));
+        b.diag_out_bytes = out_bytes;
+    }
+    dev_out = b.diag_out;
     centre = dev_out + nrec * 42;
     int rc = launch_moments_centre(&b, centre);
     std::vector<DevOp> ops, pend;
@@ -659,8 +670,7 @@ int bt_track_diagnostics(bt_beam *beam, int32_t nturns, int32_t granularity, dou
         if (cudaMemcpyAsync(host_moments, dev_out, (size_t)nrec * 42 * sizeof(double), cudaMemcpyDeviceToHost, b.stream) != cudaSuccess)
             rc = fail(BT_ERR_CUDA, "bt_track_diagnostics: copy of the records failed");
     }
-    cudaStreamSynchronize(b.stream);
-    cudaFree(dev_out);
+    if (cudaStreamSynchronize(b.stream) != cudaSuccess && rc == BT_OK) rc = fail(BT_ERR_CUDA, "bt_track_diagnostics: stream synchronisation failed");
     return rc;
 }
 

@@ -123,6 +123,8 @@ struct Beam {
     double *mom_buf = nullptr;  // beam statistics: out[42], pad, per-block partials, ticket (moments.cu)
     double *diag_rows = nullptr;  // bt_track_diagnostics: per-(boundary, warp) rows of partial sums, kept between calls
     size_t diag_rows_bytes = 0;
+    double *diag_out = nullptr;   // bt_track_diagnostics: records (42 doubles per boundary) + the provisional centre, kept between calls
+    size_t diag_out_bytes = 0;
 };
 
 struct Grid {

@@ -410,8 +410,8 @@ __global__ void __launch_bounds__(kMaxBlock, kMinBlocks<P>) track_kernel(const _
 // slice (slice granularity) or after the last slice of every element (element granularity) each warp reduces the 27 sums
 //   S_i = sum (q_i - k_i),  P_ij = sum (q_i - k_i)(q_j - k_j)   (i <= j; k = a provisional centre, moments.cu)
 // of its 32*P particles and writes them as one 216-byte row: no extra pass over the particles, 96 B per particle per launch
-// as in bt_track.  The reduction across lanes is a transposing butterfly: 31 shuffles of doubles leave the total of value L
-// in lane L (27 separate butterflies would need 135).  diag_combine_kernel then adds the rows of one boundary in a fixed
+// as in bt_track.  The reduction across lanes is a transposition through shared memory: lane L adds the 32 lanes' copies of
+// value L.  diag_combine_kernel then adds the rows of one boundary in a fixed
 // order (bit-reproducible) and forms mean = k + S/n, cov = P/n - (S/n)(S/n)^T.
 constexpr int kDiagVals = 27;
 
@@ -455,11 +455,14 @@ struct DiagArgs {
 };
 static_assert(sizeof(DiagArgs<kTableRecords>) <= 32764, "kernel parameter space is 32 764 bytes");
 
+constexpr int kDiagPitch = 33;  // doubles per value row of a warp's transposition buffer (32 lanes + 1 pad)
+
 template <int P>
-__device__ __forceinline__ void diag_emit(const Ptc<P> &p, const double (&k)[6], const bool (&valid)[P], double *__restrict__ row) {
-    double v[32];
+__device__ __forceinline__ void diag_emit(const Ptc<P> &p, const double (&k)[6], const bool (&valid)[P], double *__restrict__ row,
+                                          double *__restrict__ tr) {
+    double v[kDiagVals];
 #pragma unroll
-    for (int i = 0; i < 32; ++i) v[i] = 0.0;
+    for (int i = 0; i < kDiagVals; ++i) v[i] = 0.0;
     BT_FORP {
         double d[6];
         d[0] = p.x[j] - k[0], d[1] = p.px[j] - k[1], d[2] = p.y[j] - k[2];
@@ -476,19 +479,21 @@ __device__ __forceinline__ void diag_emit(const Ptc<P> &p, const double (&k)[6],
             for (int b = a; b < 6; ++b) v[idx] = fma(d[a], d[b], v[idx]), ++idx;
         }
     }
-    // transposing butterfly: after the round with distance d a lane keeps the half of its values selected by its bit d
+    // transposition through the warp's shared buffer: every lane parks its 27 sums (conflict-free: consecutive lanes,
+    // consecutive words), then lane L adds the 32 lanes' copies of value L in a fixed order (four chains for ILP) --
+    // 27 STS + 32 LDS + 31 DADD per lane and boundary (a shuffle butterfly needs 62 SHFL + 124 SEL + 31 DADD)
     const int lane = threadIdx.x & 31;
 #pragma unroll
-    for (int d = 16; d >= 1; d >>= 1) {
-        const bool up = (lane & d) != 0;
+    for (int i = 0; i < kDiagVals; ++i) tr[i * kDiagPitch + lane] = v[i];
+    __syncwarp();
+    if (lane < kDiagVals) {
+        const double *src = tr + lane * kDiagPitch;
+        double s0 = 0.0, s1 = 0.0, s2 = 0.0, s3 = 0.0;
 #pragma unroll
-        for (int i = 0; i < d; ++i) {
-            const double send = up ? v[i] : v[i + d];
-            const double keep = up ? v[i + d] : v[i];
-            v[i] = keep + __shfl_xor_sync(0xffffffffu, send, d);
-        }
+        for (int j = 0; j < 32; j += 4) s0 += src[j], s1 += src[j + 1], s2 += src[j + 2], s3 += src[j + 3];
+        row[lane] = (s0 + s1) + (s2 + s3);
     }
-    if (lane < kDiagVals) row[lane] = v[0];  // lane L holds the warp's total of value L
+    __syncwarp();
 }
 
 // SLICE = false (element granularity): records are applied by the regular apply() -- whole elements, five-slice quad groups
@@ -525,6 +530,8 @@ __global__ void __launch_bounds__(128, P == 4 ? 3 : 4) track_diag_kernel(const _
     for (int c = 0; c < 6; ++c) k[c] = a.centre[c];
     double *row = a.rows + gw * kDiagVals;
     const long long row_stride = a.nwarps * kDiagVals;
+    __shared__ double tr_all[4][kDiagVals * kDiagPitch];  // blocks of 128 threads: one buffer per warp
+    double *tr = tr_all[tid >> 5];
     if constexpr (SLICE) {
 #pragma unroll 1
         for (int e = 0; e < a.n_ops; ++e) {
@@ -533,7 +540,7 @@ __global__ void __launch_bounds__(128, P == 4 ? 3 : 4) track_diag_kernel(const _
 #pragma unroll 1
             for (int sl = 0; sl < cnt; ++sl) {
                 apply_one_slice<P, NL>(p, r);
-                diag_emit<P>(p, k, valid, row);
+                diag_emit<P>(p, k, valid, row, tr);
                 row += row_stride;
             }
         }
@@ -543,7 +550,7 @@ __global__ void __launch_bounds__(128, P == 4 ? 3 : 4) track_diag_kernel(const _
             const int mark = a.tab[e].op & OP_MARK;
             e += apply<P, NL>(p, a.tab, e);
             if (mark) {
-                diag_emit<P>(p, k, valid, row);
+                diag_emit<P>(p, k, valid, row, tr);
                 row += row_stride;
             }
         }
