@@ -179,7 +179,7 @@ class Beam:
         _check(lib.bt_beam_create(C.byref(self._h), self.n, dev, _vp(self.stream)), "bt_beam_create")
 
     def close(self):
-        if getattr(self, "_h", None) is not None and self._h:
+        if getattr(self, "_h", None) is not None and self._h and lib is not None:   # lib is None at interpreter shutdown
             lib.bt_beam_destroy(self._h)
             self._h = None
 
@@ -290,7 +290,7 @@ class Grid:
         _check(lib.bt_grid_create(C.byref(self._h), self.shape[0], self.shape[1], self.shape[2], lo_a, d_a), "bt_grid_create")
 
     def close(self):
-        if getattr(self, "_h", None) is not None and self._h:
+        if getattr(self, "_h", None) is not None and self._h and lib is not None:
             lib.bt_grid_destroy(self._h)
             self._h = None
 

@@ -450,6 +450,7 @@ void bt_beam_destroy(bt_beam *beam) {
     for (int *p : ibufs)
         if (p) cudaFree(p);
     if (b.mom_buf) cudaFree(b.mom_buf);
+    if (b.mom_host) cudaFreeHost(b.mom_host);
     if (b.diag_rows) cudaFree(b.diag_rows);
     if (b.diag_out) cudaFree(b.diag_out);
     for (int i = 0; i < 3; ++i) {

@@ -121,6 +121,9 @@ struct Beam {
     cudaStream_t pipe_stream[3] = {nullptr, nullptr, nullptr};  // bt_track_host: chunk streams, created on first use
     cudaEvent_t pipe_event[3] = {nullptr, nullptr, nullptr};
     double *mom_buf = nullptr;  // beam statistics: out[42], pad, per-block partials, ticket (moments.cu)
+    double *mom_host = nullptr; // 42 doubles of mapped pinned host memory: bt_beam_moments' result lands there without a copy
+    double *mom_host_dev = nullptr;  // device address of mom_host
+    int mom_blocks = 0;         // resident blocks of moments_kernel on this device (occupancy query, once)
     double *diag_rows = nullptr;  // bt_track_diagnostics: per-(boundary, warp) rows of partial sums, kept between calls
     size_t diag_rows_bytes = 0;
     double *diag_out = nullptr;   // bt_track_diagnostics: records (42 doubles per boundary) + the provisional centre, kept between calls

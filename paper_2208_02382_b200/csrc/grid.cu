@@ -127,6 +127,55 @@ __device__ __forceinline__ void merge_and_flush_scaled(double *__restrict__ rho,
     if (head) flush_cell_scaled<NW>(rho, cur, acc, qw, nx, nxy);
 }
 
+// The same merge for lanes that also carry a HEAD run: the first run of a lane's entries, which may be the continuation of
+// the run the previous lanes ended with (a lane's first key change used to flush that part on its own: with runs of ~10
+// particles and 8 entries per lane nearly every lane has such a seam, and the flushed runs were half as long as the cells'
+// populations allow -- profiles/r02_summary.md).  nrun = runs seen by the lane; nrun >= 2: (head_key, head) is the first,
+// (cur, acc) the last; nrun == 1: the single run is (cur, acc); nrun == 0: cur = -1.  Tails are merged over contiguous
+// equal keys as before; the head lane of each merged block additionally takes the head run of the lane that follows the
+// block when its key matches, so every run of the chunk's cell-ordered list reaches rho exactly once.
+template <int NW>
+__device__ __forceinline__ void merge_heads_and_flush_scaled(double *__restrict__ rho, int cur, double (&acc)[NW * NW * NW], int nrun, int head_key,
+                                                             const double (&head)[NW * NW * NW], double qw, int nx, long long nxy) {
+    constexpr unsigned kFull = 0xffffffffu;
+    const int lane = threadIdx.x & 31;
+    const int prev = __shfl_up_sync(kFull, cur, 1);
+    const bool first = (lane == 0) || (prev != cur);
+    const unsigned firsts = __ballot_sync(kFull, first);
+    const unsigned above = (lane == 31) ? 0u : (firsts >> (lane + 1));
+    const int end = above ? lane + __ffs(above) - 1 : 31;  // last lane of the block of equal tail keys this lane is in
+    if (firsts != kFull) {                                  // warp-uniform: some block spans lanes
+        const int span = __reduce_max_sync(kFull, end - lane);
+#pragma unroll
+        for (int d = 1; d < 32; d <<= 1) {
+            if (d > span) break;  // warp-uniform
+            const bool take = lane + d <= end;
+#pragma unroll
+            for (int k = 0; k < NW * NW * NW; ++k) {
+                const double o = __shfl_down_sync(kFull, acc[k], d);
+                if (take) acc[k] += o;
+            }
+        }
+    }
+    // head runs: donated to the block that ends in the previous lane when the keys match, else flushed by their own lane
+    const int hk = nrun >= 2 ? head_key : -2;
+    // (only a lane that STARTS a block can donate: the block before it then ends at lane - 1 and looks at this lane; a lane
+    // inside a block whose head happens to carry the block's key -- aliased bins: runs X Y X -- flushes the head itself)
+    const bool donated = lane > 0 && first && hk == prev;   // prev = tail key of lane - 1 = key of the block ending there
+    const int donor = (end + 1) & 31;
+    const int donor_hk = __shfl_sync(kFull, hk, donor);
+    const bool take_head = first && end < 31 && donor_hk == cur && cur >= 0;
+    if (__any_sync(kFull, take_head)) {
+#pragma unroll
+        for (int k = 0; k < NW * NW * NW; ++k) {
+            const double o = __shfl_sync(kFull, head[k], donor);
+            if (take_head) acc[k] += o;
+        }
+    }
+    if (first) flush_cell_scaled<NW>(rho, cur, acc, qw, nx, nxy);
+    if (nrun >= 2 && !donated) flush_cell_scaled<NW>(rho, head_key, head, qw, nx, nxy);
+}
+
 template <int NT, int R>
 struct BinSmem {
     static constexpr int CH = NT * R;
@@ -359,7 +408,7 @@ struct WarpBinSmem {
 };
 
 template <int R, int ORDER>
-constexpr int kWarpDepBlocks = ORDER == 1 ? (R >= 8 ? 5 : 8) : 4;  // 128-thread blocks per SM (shared memory and registers)
+constexpr int kWarpDepBlocks = ORDER == 1 ? (R >= 8 ? 5 : 6) : 4;  // 128-thread blocks per SM (shared memory and registers)
 
 template <int R, bool VEC, int ORDER>
 __global__ void __launch_bounds__(128, kWarpDepBlocks<R, ORDER>) deposit_warp_kernel(const double *__restrict__ x, const double *__restrict__ y,
@@ -382,21 +431,26 @@ __global__ void __launch_bounds__(128, kWarpDepBlocks<R, ORDER>) deposit_warp_ke
         // ---- phase 1: load, locate, park in shared memory, count per bin (one atomic per run of equal bins) ----
         int bin[R], rank[R];
         {
-            const long long p0 = ch * CW + (long long)lane * R;
-            double qx[R], qy[R], qt[R];
-            load_run<R, VEC>(x, p0, n, CUDART_NAN, qx);  // NaN => outside => contributes nothing
-            load_run<R, VEC>(y, p0, n, 0.0, qy);
-            load_run<R, VEC>(t, p0, n, 0.0, qt);
+            // sub-batches of 8 particles per lane keep the loaded coordinates at 24 doubles whatever R is
+            constexpr int SB = R < 8 ? R : 8;
 #pragma unroll
-            for (int r = 0; r < R; ++r) {
-                Cic c;
-                const bool in = shape_locate<ORDER>(g, qx[r], qy[r], qt[r], zscale, c);
-                const int slot = lane * (R + 1) + r;
-                sm.key[slot] = (c.k * g.ny + c.j) * g.nx + c.i;
-                sm.w1[0][slot] = c.wx1;
-                sm.w1[1][slot] = c.wy1;
-                sm.w1[2][slot] = c.wz1;
-                bin[r] = in ? (((c.k & 7) << 6) | ((c.j & 7) << 3) | (c.i & 7)) : -1;
+            for (int h = 0; h < R / SB; ++h) {
+                const long long p0 = ch * CW + (long long)lane * R + h * SB;
+                double qx[SB], qy[SB], qt[SB];
+                load_run<SB, VEC>(x, p0, n, CUDART_NAN, qx);  // NaN => outside => contributes nothing
+                load_run<SB, VEC>(y, p0, n, 0.0, qy);
+                load_run<SB, VEC>(t, p0, n, 0.0, qt);
+#pragma unroll
+                for (int r = 0; r < SB; ++r) {
+                    Cic c;
+                    const bool in = shape_locate<ORDER>(g, qx[r], qy[r], qt[r], zscale, c);
+                    const int slot = lane * (R + 1) + h * SB + r;
+                    sm.key[slot] = (c.k * g.ny + c.j) * g.nx + c.i;
+                    sm.w1[0][slot] = c.wx1;
+                    sm.w1[1][slot] = c.wy1;
+                    sm.w1[2][slot] = c.wz1;
+                    bin[h * SB + r] = in ? (((c.k & 7) << 6) | ((c.j & 7) << 3) | (c.i & 7)) : -1;
+                }
             }
             int len[R];
             len[R - 1] = 1;
@@ -459,10 +513,15 @@ __global__ void __launch_bounds__(128, kWarpDepBlocks<R, ORDER>) deposit_warp_ke
                 const uint2 u = *reinterpret_cast<const uint2 *>(&sm.idx[lane * R]);
                 my[0] = u.x & 0xffff, my[1] = u.x >> 16, my[2] = u.y & 0xffff, my[3] = u.y >> 16;
             }
-            int cur = -1;
-            double acc[NN];
+            // HEADS: the lane's first run is kept and merged across lanes too (order 1: 8 more accumulators; at order 2 the 27
+            // would not fit the register file, there a lane's first key change flushes as in round 1)
+            constexpr bool HEADS = ORDER == 1;
+            int cur = -1, nrun = 0, head_key = -1;
+            double acc[NN], head[HEADS ? NN : 1];
 #pragma unroll
             for (int d = 0; d < NN; ++d) acc[d] = 0.0;
+#pragma unroll
+            for (int d = 0; d < (HEADS ? NN : 1); ++d) head[d] = 0.0;
 #pragma unroll
             for (int r = 0; r < R; ++r) {
                 if (lane * R + r >= total) break;
@@ -473,8 +532,15 @@ __global__ void __launch_bounds__(128, kWarpDepBlocks<R, ORDER>) deposit_warp_ke
                 double w[NN];
                 node_weights_unscaled<ORDER>(cc, w);
                 const int key = sm.key[slot];
-                if (key != cur) {  // a new run: the finished one leaves, the accumulators restart from zero
-                    flush_cell_scaled<NW>(rho, cur, acc, qw, g.nx, nxy);
+                if (key != cur) {  // a new run starts
+                    if (HEADS && nrun == 1) {  // the lane's first run ends: kept as the head run (merged across lanes below)
+                        head_key = cur;
+#pragma unroll
+                        for (int d = 0; d < (HEADS ? NN : 1); ++d) head[d] = acc[d];
+                    } else {                   // a run that began and ended inside this lane's entries (no-op for cur = -1)
+                        flush_cell_scaled<NW>(rho, cur, acc, qw, g.nx, nxy);
+                    }
+                    ++nrun;
                     cur = key;
 #pragma unroll
                     for (int d = 0; d < NN; ++d) acc[d] = 0.0;
@@ -482,7 +548,8 @@ __global__ void __launch_bounds__(128, kWarpDepBlocks<R, ORDER>) deposit_warp_ke
 #pragma unroll
                 for (int d = 0; d < NN; ++d) acc[d] += w[d];
             }
-            merge_and_flush_scaled<NW>(rho, cur, acc, qw, g.nx, nxy);
+            if constexpr (HEADS) merge_heads_and_flush_scaled<NW>(rho, cur, acc, nrun, head_key, head, qw, g.nx, nxy);
+            else merge_and_flush_scaled<NW>(rho, cur, acc, qw, g.nx, nxy);
         }
         __syncwarp();  // the next chunk overwrites the parked particles and the list
     }

@@ -9,7 +9,10 @@
 // size: k is the mean of min(n, 256) particles sampled at a stride of n/256 through the storage (every block recomputes
 // it), so the subtracted term is ~ cov/256 in any storage order, cell-sorted included.
 // HBM-bound: 48 bytes and 33 FP64 issue slots per particle.  Deterministic: fixed partition, fixed reduction trees,
-// the per-block partials are combined in block order by the last block to finish.
+// the per-block partials are combined in block order by the last block to finish.  Fixed costs are kept small because a
+// 16e6-particle bunch is only 119 us of HBM time: the grid is exactly the resident blocks (one wave), the centre and the 27
+// block totals each take ONE barrier pair (all values shuffled first, then exchanged through shared memory at once), and
+// bt_beam_moments' 42 results are written straight into mapped pinned host memory (no copy, one stream synchronisation).
 #include "bt_internal.h"
 
 namespace bt {
@@ -39,6 +42,32 @@ __device__ __forceinline__ double block_sum(double v, double *scratch /*[kMomBlo
     return tot;
 }
 
+// block totals of NV values at once: warp shuffles, one exchange through shared memory ([NV][warps]), one barrier pair;
+// every thread returns with all NV totals (same summation order everywhere)
+template <int NV>
+__device__ __forceinline__ void block_sum_all(double (&v)[NV], double *scratch /*[NV * kMomBlock/32]*/) {
+    constexpr int NWARP = kMomBlock / 32;
+#pragma unroll
+    for (int i = 0; i < NV; ++i) {
+#pragma unroll
+        for (int d = 16; d > 0; d >>= 1) v[i] += __shfl_xor_sync(0xffffffffu, v[i], d);
+    }
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    __syncthreads();  // scratch free
+    if (lane == 0) {
+#pragma unroll
+        for (int i = 0; i < NV; ++i) scratch[i * NWARP + wid] = v[i];
+    }
+    __syncthreads();
+#pragma unroll
+    for (int i = 0; i < NV; ++i) {
+        double tot = 0.0;
+#pragma unroll
+        for (int w = 0; w < NWARP; ++w) tot += scratch[i * NWARP + w];
+        v[i] = tot;
+    }
+}
+
 __device__ __forceinline__ void accumulate(const double (&d)[6], double (&s)[6], double (&pr)[21]) {
     int k = 0;
 #pragma unroll
@@ -50,8 +79,8 @@ __device__ __forceinline__ void accumulate(const double (&d)[6], double (&s)[6],
 }
 
 template <bool VEC2>
-__global__ void __launch_bounds__(kMomBlock) moments_kernel(const __grid_constant__ MomArgs a) {
-    __shared__ double scratch[kMomBlock / 32];
+__global__ void __launch_bounds__(kMomBlock, 2) moments_kernel(const __grid_constant__ MomArgs a) {
+    __shared__ double scratch[kMomVals * (kMomBlock / 32)];
     __shared__ bool is_last;
     // provisional centre: mean of min(n, 256) particles taken at a stride of n/256 through the storage -- representative in
     // any storage order (after bt_beam_sort_by_cell the FIRST 256 particles all sit in one corner of the grid, several
@@ -64,8 +93,9 @@ __global__ void __launch_bounds__(kMomBlock) moments_kernel(const __grid_constan
         double v[6];
 #pragma unroll
         for (int c = 0; c < 6; ++c) v[c] = threadIdx.x < m ? a.q[c][threadIdx.x * stride] : 0.0;
+        block_sum_all<6>(v, scratch);
 #pragma unroll
-        for (int c = 0; c < 6; ++c) k[c] = block_sum(v[c], scratch) / (double)m;
+        for (int c = 0; c < 6; ++c) k[c] = v[c] / (double)m;
     }
     double s[6], pr[21];
 #pragma unroll
@@ -100,17 +130,19 @@ __global__ void __launch_bounds__(kMomBlock) moments_kernel(const __grid_constan
             accumulate(d, s, pr);
         }
     }
-    // block reduction, one value at a time (27 x (5 shuffles + 8 shared reads)): once per block, negligible
-    double *mine = a.partial + (long long)blockIdx.x * kMomVals;
+    // block reduction of the 27 sums at once
+    {
+        double all[kMomVals];
 #pragma unroll
-    for (int c = 0; c < 6; ++c) {
-        const double tot = block_sum(s[c], scratch);
-        if (threadIdx.x == 0) mine[c] = tot;
-    }
+        for (int c = 0; c < 6; ++c) all[c] = s[c];
 #pragma unroll
-    for (int c = 0; c < 21; ++c) {
-        const double tot = block_sum(pr[c], scratch);
-        if (threadIdx.x == 0) mine[6 + c] = tot;
+        for (int c = 0; c < 21; ++c) all[6 + c] = pr[c];
+        block_sum_all<kMomVals>(all, scratch);
+        double *mine = a.partial + (long long)blockIdx.x * kMomVals;
+        if (threadIdx.x == 0) {
+#pragma unroll
+            for (int c = 0; c < kMomVals; ++c) mine[c] = all[c];
+        }
     }
     // the last block to finish combines the partials in block order
     if (threadIdx.x == 0) {
@@ -121,11 +153,23 @@ __global__ void __launch_bounds__(kMomBlock) moments_kernel(const __grid_constan
     __syncthreads();
     if (!is_last) return;
     __threadfence();
+    // warp w adds the partials of blocks w, w + 8, ... (lane = value), then the eight sums are added in warp order: a fixed
+    // order for a given grid, with 8 x 27 independent load streams instead of 27 serial ones
     __shared__ double total[kMomVals];
-    if (threadIdx.x < kMomVals) {
+    {
+        const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
         double tot = 0.0;
-        for (unsigned int b = 0; b < gridDim.x; ++b) tot += __ldcg(a.partial + (long long)b * kMomVals + threadIdx.x);
-        total[threadIdx.x] = tot;
+        if (lane < kMomVals)
+            for (unsigned int b = wid; b < gridDim.x; b += kMomBlock / 32) tot += __ldcg(a.partial + (long long)b * kMomVals + lane);
+        __syncthreads();  // scratch free
+        if (lane < kMomVals) scratch[lane * (kMomBlock / 32) + wid] = tot;
+        __syncthreads();
+        if (threadIdx.x < kMomVals) {
+            double t = 0.0;
+#pragma unroll
+            for (int w = 0; w < kMomBlock / 32; ++w) t += scratch[threadIdx.x * (kMomBlock / 32) + w];
+            total[threadIdx.x] = t;
+        }
     }
     __syncthreads();
     const double inv_n = 1.0 / (double)a.n;
@@ -173,9 +217,17 @@ int launch_moments_centre(Beam *b, double *dev_centre) {
     return BT_OK;
 }
 
-// Enqueues the reduction; the 42 results (mean[6], cov[36]) land in dev_out (device memory) on the beam's stream.
+// Enqueues the reduction; the 42 results (mean[6], cov[36]) land in dev_out on the beam's stream (device memory, or the
+// device address of mapped host memory).
 int launch_moments_async(Beam *b, double *dev_out) {
-    const int max_blocks = b->num_sms * 4;
+    if (b->mom_blocks == 0) {  // one wave: the grid is what is resident at once
+        int per_sm_v = 1, per_sm_s = 1;
+        BT_CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm_v, moments_kernel<true>, kMomBlock, 0));
+        BT_CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm_s, moments_kernel<false>, kMomBlock, 0));
+        const int per_sm = per_sm_v < per_sm_s ? per_sm_v : per_sm_s;
+        b->mom_blocks = b->num_sms * (per_sm > 0 ? per_sm : 1);
+    }
+    const int max_blocks = b->mom_blocks;
     if (!b->mom_buf) {
         const size_t bytes = (size_t)(6 + 42 + (size_t)max_blocks * kMomVals) * sizeof(double) + 16;
         BT_CUDA_TRY(cudaMalloc(&b->mom_buf, bytes));
@@ -201,13 +253,15 @@ int launch_moments_async(Beam *b, double *dev_out) {
 }
 
 int launch_moments(Beam *b, double host_mean[6], double host_cov[36]) {
-    const int rc = launch_moments_async(b, nullptr);
+    if (!b->mom_host) {
+        BT_CUDA_TRY(cudaHostAlloc(&b->mom_host, 42 * sizeof(double), cudaHostAllocMapped));
+        BT_CUDA_TRY(cudaHostGetDevicePointer(&b->mom_host_dev, b->mom_host, 0));
+    }
+    const int rc = launch_moments_async(b, b->mom_host_dev);
     if (rc != BT_OK) return rc;
-    double h[42];
-    BT_CUDA_TRY(cudaMemcpyAsync(h, b->mom_buf, sizeof(h), cudaMemcpyDeviceToHost, b->stream));
-    BT_CUDA_TRY(cudaStreamSynchronize(b->stream));
-    for (int i = 0; i < 6; ++i) host_mean[i] = h[i];
-    for (int i = 0; i < 36; ++i) host_cov[i] = h[6 + i];
+    BT_CUDA_TRY(cudaStreamSynchronize(b->stream));  // the kernel's writes to mapped host memory are complete
+    for (int i = 0; i < 6; ++i) host_mean[i] = b->mom_host[i];
+    for (int i = 0; i < 36; ++i) host_cov[i] = b->mom_host[6 + i];
     return BT_OK;
 }
 

@@ -496,6 +496,45 @@ __device__ __forceinline__ void diag_emit(const Ptc<P> &p, const double (&k)[6],
     __syncwarp();
 }
 
+// The same emission with the lane reduction done by a transposing shuffle butterfly (31 exchanges of doubles leave the total of
+// value L in lane L).  Used at SLICE granularity, where an emission follows every slice map and the L1 data pipe, not the
+// FP64 pipe, is what the emissions load: 62 SHFL cost it less than 27 STS.64 + 32 LDS.64 (measured on configs[1], 5 300
+// boundaries: 34.5 ms against 44.0 ms); at element granularity the shared-memory transposition wins (4.64 against 5.59 ms).
+template <int P>
+__device__ __forceinline__ void diag_emit_shfl(const Ptc<P> &p, const double (&k)[6], const bool (&valid)[P], double *__restrict__ row) {
+    double v[32];
+#pragma unroll
+    for (int i = 0; i < 32; ++i) v[i] = 0.0;
+    BT_FORP {
+        double d[6];
+        d[0] = p.x[j] - k[0], d[1] = p.px[j] - k[1], d[2] = p.y[j] - k[2];
+        d[3] = p.py[j] - k[3], d[4] = p.t[j] - k[4], d[5] = p.pt[j] - k[5];
+        if (!valid[j]) {
+#pragma unroll
+            for (int c = 0; c < 6; ++c) d[c] = 0.0;
+        }
+        int idx = 6;
+#pragma unroll
+        for (int a = 0; a < 6; ++a) {
+            v[a] += d[a];
+#pragma unroll
+            for (int b = a; b < 6; ++b) v[idx] = fma(d[a], d[b], v[idx]), ++idx;
+        }
+    }
+    const int lane = threadIdx.x & 31;
+#pragma unroll
+    for (int d = 16; d >= 1; d >>= 1) {  // after the round with distance d a lane keeps the half of its values selected by its bit d
+        const bool up = (lane & d) != 0;
+#pragma unroll
+        for (int i = 0; i < d; ++i) {
+            const double send = up ? v[i] : v[i + d];
+            const double keep = up ? v[i + d] : v[i];
+            v[i] = keep + __shfl_xor_sync(0xffffffffu, send, d);
+        }
+    }
+    if (lane < kDiagVals) row[lane] = v[0];  // lane L holds the warp's total of value L
+}
+
 // SLICE = false (element granularity): records are applied by the regular apply() -- whole elements, five-slice quad groups
 // included -- and a row follows every record marked OP_MARK (the last record of an element); SLICE = true: one slice at a
 // time, a row after each.
@@ -530,8 +569,9 @@ __global__ void __launch_bounds__(128, P == 4 ? 3 : 4) track_diag_kernel(const _
     for (int c = 0; c < 6; ++c) k[c] = a.centre[c];
     double *row = a.rows + gw * kDiagVals;
     const long long row_stride = a.nwarps * kDiagVals;
-    __shared__ double tr_all[4][kDiagVals * kDiagPitch];  // blocks of 128 threads: one buffer per warp
-    double *tr = tr_all[tid >> 5];
+    __shared__ double tr_all[SLICE ? 1 : 4][SLICE ? 1 : kDiagVals * kDiagPitch];  // blocks of 128 threads: one buffer per warp
+    double *tr = SLICE ? tr_all[0] : tr_all[tid >> 5];
+    (void)tr;
     if constexpr (SLICE) {
 #pragma unroll 1
         for (int e = 0; e < a.n_ops; ++e) {
@@ -540,7 +580,7 @@ __global__ void __launch_bounds__(128, P == 4 ? 3 : 4) track_diag_kernel(const _
 #pragma unroll 1
             for (int sl = 0; sl < cnt; ++sl) {
                 apply_one_slice<P, NL>(p, r);
-                diag_emit<P>(p, k, valid, row, tr);
+                diag_emit_shfl<P>(p, k, valid, row);
                 row += row_stride;
             }
         }

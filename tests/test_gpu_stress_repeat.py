@@ -52,6 +52,7 @@ def test_no_kernel_writes_outside_the_particle_arrays(n, lead, knobs):
     c = W.make_spacecharge_bunch(sc)
     E = W.gaussian_bunch_field(sc)
     views, check = banded_storage(n, band=1024, lead=lead)
+    aligned16 = all(v.data_ptr() % 16 == 0 for v in views)   # odd n or lead: every other array starts 8 bytes off
     beam = bt.Beam(n, storage=views)
     grid = bt.Grid(sc.shape, sc.lo, sc.d)
     try:
@@ -63,7 +64,7 @@ def test_no_kernel_writes_outside_the_particle_arrays(n, lead, knobs):
         for lattice in (W.fodo_cell(7), W.nonlinear_ring()[:40] + [W.nonlinear_ring()[-1]]):
             beam.lattice_set(lattice)
             for ppt in (1, 2, 4):
-                if ppt > 1 and lead:
+                if ppt > 1 and not aligned16:
                     continue  # vector variants need 16-byte aligned arrays (rejected by the library otherwise)
                 knobs("track_ppt", ppt)
                 beam.track(2)
