@@ -439,6 +439,10 @@ def bench_spacecharge(bt, torch, flush, peaks, traffic, interval, with_cpu=True)
                                                "frac": gat_bytes / mg / 1e9 / hbm,
                                                "traffic": traffic_of(traffic, "gather:%s:%d" % (variant, order))}},
             "ms_per_step_incl_sort_amortised": (md_all + mg) * 1e3,
+            "ms_per_step_steady_state": (md + mg) * 1e3 + min(t_resort) / interval,
+            "steady_state_note": "deposit (no sort) + gather + one re-sort of the sorted beam per %d steps; "
+                                 "ms_per_step_incl_sort_amortised instead charges the window's ONE sort from the caller's order "
+                                 "(a once-per-run cost) to its 10 steps" % interval,
         }
         if poisson:
             out[key]["poisson_solve"] = poisson
