@@ -844,22 +844,33 @@ static int launch_gather_pipe(Beam *b, const GatherArgs &a0) {
 // broadcast wavefront.  A chunk whose box exceeds kTileCap nodes (unsorted input, thin tails) reads through L1 as before.
 constexpr int kTileCap = 1280;  // nodes: 30 KiB of shared memory; a drifted 256-particle chunk of configs[4] needs ~1200 at order 2
 
+constexpr int kGtBins = 512;  // regrouping bins: the low three bits of each index of the stencil's base node
+
 template <int CH>
 struct GtSmem {
     alignas(128) double q[kGpStages][6][CH];
     alignas(16) double tile[3][kTileCap];
+    alignas(16) int hist[kGtBins + 8];  // [kGtBins] = particles outside the grid
+    unsigned short idx[CH];             // REGROUP: slot of the particle a thread works on (cell order)
+    int warp_tot[8];
     int box[2][8];
     alignas(8) uint64_t full[kGpStages];
 };
 
-template <int ORDER>
+// REGROUP (default at order 2): the threads of a block work on the chunk's particles in CELL order instead of storage
+// order -- a counting sort of the 256 slots by the stencil's base cell (shared histogram, block scan, 2-byte slot list),
+// results written back IN PLACE, so nothing moves in HBM and no id travels.  Why: the 27 x 3 LDS.64 per particle are what
+// loads the L1 data pipe (76 % of peak, 3.4 wavefronts per LDS.64 with the lanes of a warp spread over ~12 cells after a few
+// steps of wandering); lanes that sit in the same cell read the same words (one broadcast wavefront), lanes in x-adjacent
+// cells read adjacent words (no bank conflict), so a warp of cell-ordered particles needs 1-2 wavefronts per load.
+template <int ORDER, bool REGROUP>
 __global__ void __launch_bounds__(256, 3) gather_kick_tile_kernel(const __grid_constant__ GatherArgs a, long long nchunks, int store_positions) {
     constexpr int NT = 256, CH = 256, NW = ORDER + 1;
     constexpr uint32_t kArrBytes = CH * sizeof(double);
     constexpr int kBig = 0x7fffffff;
     extern __shared__ __align__(128) unsigned char gt_smem_raw[];
     GtSmem<CH> &sm = *reinterpret_cast<GtSmem<CH> *>(gt_smem_raw);
-    const int tid = threadIdx.x, lane = tid & 31;
+    const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
     const auto issue_load = [&](long long ch, int s) {
         mbar_expect_tx(&sm.full[s], 6 * kArrBytes);
 #pragma unroll
@@ -873,6 +884,10 @@ __global__ void __launch_bounds__(256, 3) gather_kick_tile_kernel(const __grid_c
         if ((long long)blockIdx.x + gridDim.x < nchunks) issue_load((long long)blockIdx.x + gridDim.x, 1);
     }
     if (tid < 8) sm.box[0][tid] = (tid >= 3 && tid < 6) ? -1 : kBig;
+    if (REGROUP) {
+        sm.hist[2 * tid] = 0, sm.hist[2 * tid + 1] = 0;
+        if (tid < 8) sm.hist[kGtBins + tid] = 0;
+    }
     __syncthreads();
     int s = 0, bpar = 0;
     uint32_t parity = 0;
@@ -888,7 +903,7 @@ __global__ void __launch_bounds__(256, 3) gather_kick_tile_kernel(const __grid_c
             t = fma(a.tcb, pt, t);
         }
         Cic c;
-        const bool in = shape_locate<ORDER>(a.g, x, y, t, a.zscale, c);
+        bool in = shape_locate<ORDER>(a.g, x, y, t, a.zscale, c);
         {   // bounding box of the chunk's stencil bases
             int lo_i = in ? c.i : kBig, lo_j = in ? c.j : kBig, lo_k = in ? c.k : kBig;
             int hi_i = in ? c.i : -1, hi_j = in ? c.j : -1, hi_k = in ? c.k : -1;
@@ -900,7 +915,12 @@ __global__ void __launch_bounds__(256, 3) gather_kick_tile_kernel(const __grid_c
                 atomicMax(&box[3], hi_i), atomicMax(&box[4], hi_j), atomicMax(&box[5], hi_k);
             }
         }
-        __syncthreads();  // (1) box complete
+        int bin = 0, rank = 0;
+        if (REGROUP) {
+            bin = in ? (((c.k & 7) << 6) | ((c.j & 7) << 3) | (c.i & 7)) : kGtBins;
+            rank = atomicAdd(&sm.hist[bin], 1);
+        }
+        __syncthreads();  // (1) box (and histogram) complete
         if (tid < 8) sm.box[bpar ^ 1][tid] = (tid >= 3 && tid < 6) ? -1 : kBig;  // next chunk's box
         const int i0 = box[0], j0 = box[1], k0 = box[2];
         const int tx = box[3] - i0 + NW, ty = box[4] - j0 + NW, tz = box[5] - k0 + NW;  // nodes per axis of the tile
@@ -919,7 +939,45 @@ __global__ void __launch_bounds__(256, 3) gather_kick_tile_kernel(const __grid_c
                 }
             }
         }
-        __syncthreads();  // (2) tile staged
+        int slot = tid;  // the particle this thread works on
+        if (REGROUP) {
+            // exclusive scan of the 512 counters (two per thread), the slot list, then every thread picks up the particle
+            // at ITS position of the cell order and locates it again (cheaper than parking the located particles)
+            const int v0 = sm.hist[2 * tid], v1 = sm.hist[2 * tid + 1];
+            const int sum = v0 + v1;
+            int incl = sum;
+#pragma unroll
+            for (int d = 1; d < 32; d <<= 1) {
+                const int o = __shfl_up_sync(0xffffffffu, incl, d);
+                if (lane >= d) incl += o;
+            }
+            if (lane == 31) sm.warp_tot[wid] = incl;
+            __syncthreads();  // (2) warp totals (and every thread has read its two counters)
+            int off = incl - sum, inside = 0;
+#pragma unroll
+            for (int w = 0; w < NT / 32; ++w) {
+                const int wt = sm.warp_tot[w];
+                off += (w < wid) ? wt : 0;
+                inside += wt;
+            }
+            sm.hist[2 * tid] = off, sm.hist[2 * tid + 1] = off + v0;
+            __syncthreads();  // (3) offsets ready
+            const int pos = (bin < kGtBins ? sm.hist[bin] : inside) + rank;
+            sm.idx[pos] = (unsigned short)tid;
+            __syncthreads();  // (4) slot list complete (and the tile is staged)
+            sm.hist[2 * tid] = 0, sm.hist[2 * tid + 1] = 0;  // for the next chunk (its first atomic follows barrier (5))
+            if (tid == 0) sm.hist[kGtBins] = 0;
+            slot = sm.idx[tid];
+            x = q[0][slot], px = q[1][slot], y = q[2][slot], py = q[3][slot], t = q[4][slot], pt = q[5][slot];
+            if (a.hb != 0.0 || a.tcb != 0.0) {
+                x = fma(a.hb, px, x);
+                y = fma(a.hb, py, y);
+                t = fma(a.tcb, pt, t);
+            }
+            in = shape_locate<ORDER>(a.g, x, y, t, a.zscale, c);
+        } else {
+            __syncthreads();  // (2) tile staged
+        }
         if (in) {
             double wx[NW], wy[NW], wz[NW];
             axis_weights<ORDER>(c.wx1, wx);
@@ -966,9 +1024,9 @@ __global__ void __launch_bounds__(256, 3) gather_kick_tile_kernel(const __grid_c
             y = fma(a.ha, py, y);
             t = fma(a.tca, pt, t);
         }
-        q[0][tid] = x, q[1][tid] = px, q[2][tid] = y, q[3][tid] = py, q[4][tid] = t, q[5][tid] = pt;
+        q[0][slot] = x, q[1][slot] = px, q[2][slot] = y, q[3][slot] = py, q[4][slot] = t, q[5][slot] = pt;
         fence_proxy_async_smem();  // this thread's shared-memory writes -> visible to the copy engine
-        __syncthreads();           // (3) stage complete; everyone is done with the tile
+        __syncthreads();           // (last) stage complete; everyone is done with the tile
         if (tid == 0) {
 #pragma unroll
             for (int cc = 0; cc < 6; ++cc)
@@ -985,19 +1043,19 @@ __global__ void __launch_bounds__(256, 3) gather_kick_tile_kernel(const __grid_c
     if (tid == 0) bulk_wait_all<0>();  // shared memory must outlive the last stores
 }
 
-template <int ORDER>
+template <int ORDER, bool REGROUP>
 static int launch_gather_tile(Beam *b, const GatherArgs &a0) {
     constexpr int CH = 256;
     const int smem = (int)sizeof(GtSmem<CH>);
     const long long nchunks = b->n / CH;
     if (nchunks > 0) {
         int per_sm = 1;
-        const int qrc = blocks_per_sm<gather_kick_tile_kernel<ORDER>>(256, smem, b->device, &per_sm);
+        const int qrc = blocks_per_sm<gather_kick_tile_kernel<ORDER, REGROUP>>(256, smem, b->device, &per_sm);
         if (qrc != BT_OK) return qrc;
         long long blocks = (long long)b->num_sms * (per_sm > 0 ? per_sm : 1);
         if (blocks > nchunks) blocks = nchunks;
         const int store_positions = (a0.hb != 0.0 || a0.ha != 0.0 || a0.tcb != 0.0 || a0.tca != 0.0) ? 1 : 0;
-        gather_kick_tile_kernel<ORDER><<<(int)blocks, 256, smem, b->stream>>>(a0, nchunks, store_positions);
+        gather_kick_tile_kernel<ORDER, REGROUP><<<(int)blocks, 256, smem, b->stream>>>(a0, nchunks, store_positions);
     }
     const long long done = nchunks * CH;
     if (done < b->n) {  // ragged tail: one particle per thread
@@ -1013,13 +1071,15 @@ template <int ORDER>
 static int launch_gather_order(Beam *b, const GatherArgs &a) {
     // knob gather_mode: 0 = one particle per thread, everything through registers (also the path for arrays that are not
     // 16-byte aligned); 1 (default) = streaming pipeline, 256-particle chunks, field through L1 (order 1) or staged in shared
-    // memory (order 2); 2 / 3 = L1 pipeline with 512 / 128-particle chunks; 4 = shared-memory tile at any order
+    // memory (order 2); 2 / 3 = L1 pipeline with 512 / 128-particle chunks; 4 = shared-memory tile at any order (threads work in cell order at
+    // order 2); 5 = the tile with the other regrouping choice
     const int mode = knob(KNOB_GATHER_MODE, 1);
     // field tile staged in shared memory: the default at order 2 (measured 4A 10-step mean 547 -> 477 us, 4B 529 -> 430 us),
     // selectable at order 1 (knob gather_mode = 4), where the L1 path is faster (181 against 216 us)
     // only on cell-sorted beams: in the caller's order no chunk's box fits the tile and the pass through L1 is faster from
     // the plain pipeline (order 2, unsorted kick: 0.79 against 1.51 ms)
-    if ((mode == 4 || (mode == 1 && ORDER == 2 && b->permuted)) && b->aligned16) return launch_gather_tile<ORDER>(b, a);
+    if ((mode == 4 || (mode == 1 && ORDER == 2 && b->permuted)) && b->aligned16) return launch_gather_tile<ORDER, ORDER == 2>(b, a);
+    if (mode == 5 && b->aligned16) return launch_gather_tile<ORDER, ORDER != 2>(b, a);  // the other regrouping choice, for A/B runs
     if (mode >= 1 && b->aligned16)
         return mode == 2 ? launch_gather_pipe<512, 1, ORDER>(b, a) : mode == 3 ? launch_gather_pipe<128, 1, ORDER>(b, a) : launch_gather_pipe<256, 1, ORDER>(b, a);
     const int block = 256;
