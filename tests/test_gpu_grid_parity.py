@@ -312,7 +312,7 @@ def test_deposit_modes_unaligned(mode, variant, knobs):
     grid.close()
 
 
-@pytest.mark.parametrize("mode", [0, 1, 2, 3, 4])
+@pytest.mark.parametrize("mode", [0, 1, 2, 3, 4, 5])
 @pytest.mark.parametrize("offset", [0, 1])
 def test_gather_modes(mode, offset, knobs):
     """Every gather path (registers / streaming pipeline with 256-, 512-, 128-particle chunks), on aligned and on

@@ -67,7 +67,7 @@ def test_deposit_order2_boundaries_zscale_unaligned_accumulate():
     assert r15_isolated(twice, ref2) <= 1e-12
 
 
-@pytest.mark.parametrize("mode", [0, 1, 2, 3, 4])
+@pytest.mark.parametrize("mode", [0, 1, 2, 3, 4, 5])
 @pytest.mark.parametrize("offset", [0, 1])
 def test_gather_order2(mode, offset, knobs):
     import torch

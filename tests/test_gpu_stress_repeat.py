@@ -86,7 +86,7 @@ def test_no_kernel_writes_outside_the_particle_arrays(n, lead, knobs):
                 beam.deposit_cic(grid, sc.q_weight, sc.zscale, True)
                 check("bt_deposit_cic order %d mode %d" % (order, mode))
             knobs("deposit_mode", -1)
-            for mode in (0, 1, 2, 3, 4):
+            for mode in (0, 1, 2, 3, 4, 5):
                 knobs("gather_mode", mode)
                 beam.gather_kick(grid, sc.kick_coef, sc.zscale, sc.ds / 2, sc.ds / 2)
                 check("bt_gather_kick order %d mode %d" % (order, mode))
@@ -123,7 +123,7 @@ def test_gather_sort_and_deposit_repeat_identically(variant, order, knobs):
         ref_rho, _ = O.deposit_cic(c[0], c[2], c[4], sc.shape, sc.lo, sc.d, sc.q_weight, sc.zscale, order=order)
         first = None
         for sorted_storage in (False, True):
-            for mode in (0, 1, 2, 3, 4):
+            for mode in (0, 1, 2, 3, 4, 5):
                 knobs("gather_mode", mode)
                 for rep in range(4):
                     beam.upload(c)
