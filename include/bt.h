@@ -146,8 +146,8 @@ int bt_beam_sort_by_cell(bt_beam *beam, const bt_grid *grid, double zscale);
  * Cadence of the cell binning: with every_n_deposits = n > 0, bt_deposit_cic calls bt_beam_sort_by_cell(beam, grid, zscale)
  * itself before its 1st, (n+1)th, (2n+1)th ... call since the last bt_beam_upload; 0 (default) = never, the caller sorts.
  * Particles wander away from where a sort left them and chunk membership is fixed, so deposit and gather slow down from
- * one sort to the next (measured on configs[4]: deposit 126 -> 140 us after 10 steps, 290 after 20; gather 140 -> 203 ->
- * 237 us; one re-sort of a nearly sorted beam 0.57 ms): n = 10 is the measured optimum there.  Results never depend on it.
+ * one sort to the next (measured on configs[4]: deposit 101 -> 116 us over 5 steps, gather 141 -> 188 us; one re-sort of a
+ * nearly sorted beam 0.27 ms): n = 5..6 is the measured optimum there.  Results never depend on it.
  */
 int bt_beam_set_resort_interval(bt_beam *beam, int32_t every_n_deposits);
 /* Device array of n int32: ids[j] = original index of storage slot j; NULL while storage order == original order. */
