@@ -364,9 +364,14 @@ def bench_other_configs(bt, torch, flush, peaks, nominal_peak, traffic, with_cpu
             # beam statistics: bt_beam_moments = 1 launch + a 336-byte read-back, 48 B/particle
             beam.moments()
             tm = statistics.mean(_event_ms(torch, beam.moments, 5, flush)) * 1e-3
+            dev_out = torch.empty(42, dtype=torch.float64, device="cuda")
+            beam.moments_device(dev_out)
+            ta = statistics.mean(_event_ms(torch, lambda: beam.moments_device(dev_out), 5, flush)) * 1e-3
             entry["moments"] = {"ms": tm * 1e3, "roofline": {"bound": "hbm", "achieved": 48.0 * n / tm / 1e9, "peak": hbm / 1e9,
                                                               "unit": "GB/s", "frac": 48.0 * n / tm / hbm,
-                                                              "traffic": traffic_of(traffic, "moments:%d" % n)}}
+                                                              "traffic": traffic_of(traffic, "moments:%d" % n)},
+                                "device_variant": {"call": "bt_beam_moments_device (result stays on the device, no synchronisation)",
+                                                   "ms": ta * 1e3, "frac": 48.0 * n / ta / hbm}}
         if idx == 1:
             # slice-step diagnostics inside the walk (P:l.61): the same walk + the beam statistics after
             # every element / every slice, O(1) launches; the call is synchronous and returns the records on the host

@@ -265,6 +265,13 @@ int bt_gather_kick(bt_beam *beam, const bt_grid *grid, const double coef[3], dou
  * unnormalised rms emittance of a plane is sqrt(cov_qq*cov_pp - cov_qp^2).  NaN/Inf coordinates propagate.
  */
 int bt_beam_moments(bt_beam *beam, double host_mean[6], double host_cov[36]);
+/*
+ * The same statistics (P:l.43, l.61), left on the DEVICE: dev_out receives 42 doubles (mean[6], then cov[36] row-major) in
+ * device memory owned by the caller, written by the beam's stream; the call only enqueues the kernel and returns -- no
+ * synchronisation, no copy -- so a step loop can take the statistics every step and read them back whenever it likes.
+ * Bit-identical to bt_beam_moments.
+ */
+int bt_beam_moments_device(bt_beam *beam, double *dev_out);
 
 /*
  * Slice-step diagnostics (mirrors sim.set_slice_step_diagnostics(True), P:l.61; the statistics are P:l.43 "beam statistics"):

@@ -61,6 +61,7 @@ EXPORTS = {
     "bt_deposit_cic": (C.c_int, [_vp, _vp, C.c_double, C.c_double, C.c_int]),
     "bt_gather_kick": (C.c_int, [_vp, _vp, _dp, C.c_double, C.c_double, C.c_double]),
     "bt_beam_moments": (C.c_int, [_vp, _dp, _dp]),
+    "bt_beam_moments_device": (C.c_int, [_vp, _vp]),
     "bt_track_diagnostics": (C.c_int, [_vp, C.c_int32, C.c_int32, _dp]),
     "bt_sync": (C.c_int, [_vp]),
     "bt_last_error": (C.c_char_p, []),
@@ -266,6 +267,13 @@ class Beam:
         mean, cov = np.zeros(6), np.zeros(36)
         _check(lib.bt_beam_moments(self._h, mean.ctypes.data_as(_dp), cov.ctypes.data_as(_dp)), "bt_beam_moments")
         return mean, cov.reshape(6, 6)
+
+    def moments_device(self, out):
+        """bt_beam_moments_device: the 42 statistics (mean[6], cov[36]) into a CUDA float64 tensor of >= 42 elements, enqueued
+        on the beam's stream without synchronisation."""
+        assert out.is_cuda and out.is_contiguous() and out.element_size() == 8 and out.numel() >= 42
+        _check(lib.bt_beam_moments_device(self._h, _vp(out.data_ptr())), "bt_beam_moments_device")
+        return out
 
     def set_resort_interval(self, every_n_deposits):
         _check(lib.bt_beam_set_resort_interval(self._h, int(every_n_deposits)), "bt_beam_set_resort_interval")

@@ -910,6 +910,11 @@ int bt_beam_moments(bt_beam *beam, double host_mean[6], double host_cov[36]) {
     return launch_moments(&beam->b, host_mean, host_cov);
 }
 
+int bt_beam_moments_device(bt_beam *beam, double *dev_out) {
+    if (!beam || !dev_out) return fail(BT_ERR_INVALID, "bt_beam_moments_device: NULL argument");
+    return launch_moments_async(&beam->b, dev_out);
+}
+
 int bt_gather_kick(bt_beam *beam, const bt_grid *grid, const double coef[3], double zscale, double half_drift_before,
                    double half_drift_after) {
     if (!beam || !grid || !coef) return fail(BT_ERR_INVALID, "bt_gather_kick: NULL argument");

@@ -198,3 +198,22 @@ def test_track_diagnostics_many_boundaries_are_cut_into_launches():
     assert np.all(np.isfinite(cov)) and np.all(np.isfinite(mean))
     assert bt.lib.bt_track_diagnostics(beam._h, 1, 7, np.zeros(42).ctypes.data_as(bt._dp)) == bt.BT_ERR_INVALID
     beam.close()
+
+
+def test_moments_device_variant_is_bit_identical_and_asynchronous():
+    """bt_beam_moments_device leaves the 42 numbers in device memory (no synchronisation): same bits as bt_beam_moments."""
+    import torch
+    cfg = W.config(1, n=300_001)
+    c = W.make_bunch(cfg)
+    beam = bt.Beam(cfg.n)
+    beam.upload(c)
+    mean, cov = beam.moments()
+    out = torch.full((3, 42), float("nan"), dtype=torch.float64, device="cuda")
+    for k in range(3):                       # three calls back to back on the stream, read once at the end
+        beam.moments_device(out[k])
+    torch.cuda.synchronize()
+    got = out.cpu().numpy()
+    for k in range(3):
+        assert np.array_equal(got[k, :6], mean) and np.array_equal(got[k, 6:].reshape(6, 6), cov)
+    assert bt.lib.bt_beam_moments_device(beam._h, None) == bt.BT_ERR_INVALID
+    beam.close()
