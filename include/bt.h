@@ -131,8 +131,9 @@ int64_t bt_beam_size(const bt_beam *beam);
 
 /*
  * Cell binning (S4; B:north_star "bins particles by cell").  Physically reorders the beam's six arrays by
- * the linear index (k*ny + j)*nx + i of each particle's lower-corner node on `grid` (R11 canonical index,
- * third axis zscale*t; particles outside the grid go last), by a counting sort on the beam's stream.
+ * the linear index (k*ny + j)*nx + i of the lowest node of each particle's stencil on `grid` for the grid's particle shape
+ * (order 1: the cell's lower-corner node, R11 canonical index; order 2: nearest node - 1, R16; third axis zscale*t;
+ * particles outside the grid go last), by a counting sort on the beam's stream.
  * Opt-in and purely a performance hint: it makes every chunk of consecutive particles spatially compact, which is
  * what bt_deposit_cic needs to bin a chunk by cell in shared memory and sum same-cell particles in registers before
  * touching rho, and what lets bt_gather_kick find its nodes in L1; both remain correct for any order and stay fast

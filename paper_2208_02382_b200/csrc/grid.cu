@@ -603,7 +603,8 @@ static int launch_deposit_warp(Beam *b, Grid *g, const GridDev &gd, double q_wei
 template <int ORDER>
 static int launch_deposit_order(Beam *b, Grid *g, const GridDev &gd, double q_weight, double zscale) {
     // knob deposit_mode: 0 = one particle per thread, (ORDER+1)^3 reductions each (baseline, kept for measurements);
-    // 1 (default) = warp-private cell binning, 8 particles per lane (4 at order 2: 27 run accumulators per lane);
+    // 1 (default) = warp-private cell binning, 8 particles per lane (at order 2 as well: longer lane segments mean fewer
+    // separately flushed head runs of 27 reductions each -- 4A 322 -> 284 us, 4B 298 -> 196 us against 4 per lane);
     // 2 = warp-private binning with 4 particles per lane; 3 = round 1's block-wide binning (2048-particle chunks,
     // 1024 at order 2)
     const int mode = knob(KNOB_DEPOSIT_MODE, 1);
@@ -622,11 +623,9 @@ static int launch_deposit_order(Beam *b, Grid *g, const GridDev &gd, double q_we
         return b->aligned32 ? launch_deposit_binned<256, 4, true, ORDER>(b, g, gd, q_weight, zscale)
                             : launch_deposit_binned<256, 4, false, ORDER>(b, g, gd, q_weight, zscale);
     }
-    if constexpr (ORDER == 1) {
-        if (mode != 2)
-            return b->aligned32 ? launch_deposit_warp<8, true, ORDER>(b, g, gd, q_weight, zscale)
-                                : launch_deposit_warp<8, false, ORDER>(b, g, gd, q_weight, zscale);
-    }
+    if (mode != 2)
+        return b->aligned32 ? launch_deposit_warp<8, true, ORDER>(b, g, gd, q_weight, zscale)
+                            : launch_deposit_warp<8, false, ORDER>(b, g, gd, q_weight, zscale);
     return b->aligned32 ? launch_deposit_warp<4, true, ORDER>(b, g, gd, q_weight, zscale)
                         : launch_deposit_warp<4, false, ORDER>(b, g, gd, q_weight, zscale);
 }

@@ -45,14 +45,17 @@ struct SortTable {          // per warp
 
 __device__ __forceinline__ int sort_bin(const Cic &c) { return ((c.k & 7) << 6) | ((c.j & 7) << 3) | (c.i & 7); }
 
-// keys and table bins of a lane's 8 particles; key = -1 for slots beyond n
-template <int R>
+// keys and table bins of a lane's particles; key = -1 for slots beyond n.  ORDER: the grid's particle shape -- the key is the
+// lowest node of THAT shape's stencil (order 1: the cell's lower corner; order 2: nearest node - 1), so that what the sort
+// brings together is what the deposit of that shape accumulates in one run (sorted by the order-1 cell, the particles of a
+// cell split over up to 8 order-2 stencils)
+template <int R, int ORDER>
 __device__ __forceinline__ void sort_keys(long long p0, long long n, const GridDev &g, double zscale, int nn, const double (&qx)[R],
                                           const double (&qy)[R], const double (&qt)[R], int (&key)[R], int (&bin)[R]) {
 #pragma unroll
     for (int r = 0; r < R; ++r) {
         Cic c;
-        const bool in = cic_locate(g, qx[r], qy[r], qt[r], zscale, c);
+        const bool in = shape_locate<ORDER>(g, qx[r], qy[r], qt[r], zscale, c);
         key[r] = (p0 + r < n) ? (in ? (c.k * g.ny + c.j) * g.nx + c.i : nn) : -1;
         bin[r] = in ? sort_bin(c) : kSortBins - 1;   // outside particles share the last bin (tagged nn)
     }
@@ -84,7 +87,7 @@ __device__ __forceinline__ void sort_claim(SortTable &tb, const int (&key)[R], c
     }
 }
 
-template <int R, bool VEC>
+template <int R, bool VEC, int ORDER>
 __global__ void __launch_bounds__(32 * kSortWarps) sort_count_kernel(const double *__restrict__ x, const double *__restrict__ y,
                                                                       const double *__restrict__ t, long long n, GridDev g, double zscale,
                                                                       int *__restrict__ count) {
@@ -110,7 +113,7 @@ __global__ void __launch_bounds__(32 * kSortWarps) sort_count_kernel(const doubl
         load_lane<R, VEC>(x, p0, n, 0.0, qx);
         load_lane<R, VEC>(y, p0, n, 0.0, qy);
         load_lane<R, VEC>(t, p0, n, 0.0, qt);
-        sort_keys<R>(p0, n, g, zscale, nn, qx, qy, qt, key, bin);
+        sort_keys<R, ORDER>(p0, n, g, zscale, nn, qx, qy, qt, key, bin);
         sort_claim<R>(tb, key, bin, rank, ok, len);
 #pragma unroll
         for (int r = 0; r < R; ++r) {
@@ -160,7 +163,7 @@ struct SortMoveSmem {       // per warp
 
 // R = 4: every coordinate of the lane's particles is loaded up front (7 independent streams in flight per lane), so the
 // only global latencies on a chunk's critical path are that load and the cursor atomics; 96 registers, 20 warps per SM.
-template <int R, bool VEC>
+template <int R, bool VEC, int ORDER>
 __global__ void __launch_bounds__(32 * kSortWarps, R == 4 ? 5 : 3) sort_move_kernel(const __grid_constant__ SortMoveArgs a) {
     extern __shared__ __align__(16) unsigned char sort_smem_raw[];
     constexpr int CW = 32 * R;
@@ -187,7 +190,7 @@ __global__ void __launch_bounds__(32 * kSortWarps, R == 4 ? 5 : 3) sort_move_ker
         for (int r = 0; r < R; ++r) id[r] = (p0 + r < a.n) ? (a.ids_in ? a.ids_in[p0 + r] : (int)(p0 + r)) : 0;
         int key[R], bin[R], rank[R], len[R];
         bool ok[R];
-        sort_keys<R>(p0, a.n, a.g, a.zscale, nn, v[0], v[2], v[4], key, bin);
+        sort_keys<R, ORDER>(p0, a.n, a.g, a.zscale, nn, v[0], v[2], v[4], key, bin);
         sort_claim<R>(sm.tb, key, bin, rank, ok, len);
         const int present = (int)(a.n - ch * CW < CW ? a.n - ch * CW : CW);  // particles of this chunk
         // table collisions: the run takes its destination from the global cursor right away and places at the END of the
@@ -431,7 +434,8 @@ void set_current_storage(Beam *b, bool use_alt) {
     }
 }
 
-int sort_by_cell(Beam *b, const Grid *g, double zscale) {
+template <int ORDER>
+static int sort_by_cell_order(Beam *b, const Grid *g, double zscale) {
     if (b->n > 0x7fffffffLL) return fail(BT_ERR_UNSUPPORTED, "bt_beam_sort_by_cell: n exceeds int32");
     const long long nn = g->nn;
     int rc = ensure_sort_buffers(b, nn);
@@ -448,9 +452,9 @@ int sort_by_cell(Beam *b, const Grid *g, double zscale) {
 
     BT_CUDA_TRY(cudaMemsetAsync(b->sort_count, 0, (size_t)m * sizeof(int), s));
     if (b->aligned32)
-        sort_count_kernel<R, true><<<(int)blocks, 32 * kSortWarps, 0, s>>>(b->q[0], b->q[2], b->q[4], n, gd, zscale, b->sort_count);
+        sort_count_kernel<R, true, ORDER><<<(int)blocks, 32 * kSortWarps, 0, s>>>(b->q[0], b->q[2], b->q[4], n, gd, zscale, b->sort_count);
     else
-        sort_count_kernel<R, false><<<(int)blocks, 32 * kSortWarps, 0, s>>>(b->q[0], b->q[2], b->q[4], n, gd, zscale, b->sort_count);
+        sort_count_kernel<R, false, ORDER><<<(int)blocks, 32 * kSortWarps, 0, s>>>(b->q[0], b->q[2], b->q[4], n, gd, zscale, b->sort_count);
     BT_LAUNCH_CHECK("sort_count_kernel");
     scan_reduce_kernel<<<nb, kScanBlock, 0, s>>>(b->sort_count, m, b->sort_block_sum);
     BT_LAUNCH_CHECK("scan_reduce_kernel");
@@ -474,16 +478,16 @@ int sort_by_cell(Beam *b, const Grid *g, double zscale) {
     const int smem = (int)sizeof(SortMoveSmem<R>) * kSortWarps;
     static std::atomic<int> attr_set[kMaxDevices];
     if (b->device >= 0 && b->device < kMaxDevices && !attr_set[b->device].load()) {
-        BT_CUDA_TRY(cudaFuncSetAttribute(sort_move_kernel<R, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
-        BT_CUDA_TRY(cudaFuncSetAttribute(sort_move_kernel<R, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+        BT_CUDA_TRY(cudaFuncSetAttribute(sort_move_kernel<R, true, ORDER>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+        BT_CUDA_TRY(cudaFuncSetAttribute(sort_move_kernel<R, false, ORDER>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
         attr_set[b->device].store(1);
     }
     long long mblocks = (long long)b->num_sms * 5;
     if (mblocks > (nchunks + kSortWarps - 1) / kSortWarps) mblocks = (nchunks + kSortWarps - 1) / kSortWarps;
     if (b->aligned32)
-        sort_move_kernel<R, true><<<(int)mblocks, 32 * kSortWarps, smem, s>>>(a);
+        sort_move_kernel<R, true, ORDER><<<(int)mblocks, 32 * kSortWarps, smem, s>>>(a);
     else
-        sort_move_kernel<R, false><<<(int)mblocks, 32 * kSortWarps, smem, s>>>(a);
+        sort_move_kernel<R, false, ORDER><<<(int)mblocks, 32 * kSortWarps, smem, s>>>(a);
     BT_LAUNCH_CHECK("sort_move_kernel");
     set_current_storage(b, to_alt);
     int *tmp = b->ids;
@@ -491,6 +495,10 @@ int sort_by_cell(Beam *b, const Grid *g, double zscale) {
     b->ids_tmp = tmp;
     b->permuted = true;
     return BT_OK;
+}
+
+int sort_by_cell(Beam *b, const Grid *g, double zscale) {
+    return g->order == 2 ? sort_by_cell_order<2>(b, g, zscale) : sort_by_cell_order<1>(b, g, zscale);
 }
 
 // storage order -> original order for one coordinate: out[ids[j]] = q[j]
