@@ -275,6 +275,43 @@ int bt_beam_moments(bt_beam *beam, double host_mean[6], double host_cov[36]);
 int bt_beam_moments_device(bt_beam *beam, double *dev_out);
 
 /*
+ * The same statistics (P:l.43 "beam statistics", P:l.112 second moments) for a caller that is not allowed to allocate
+ * device memory: no bt_beam is needed and the call makes no cudaMalloc / cudaFree / cudaHostAlloc or any other
+ * allocating call, now or later.
+ *
+ * Who that is: a host application whose own memory arena took (almost) all of HBM at start-up, as the mesh frameworks
+ * underneath the paper's code do, so that an allocation made behind its back fails or eats into what the arena counts
+ * on; a step loop with several busy streams, which a cudaMalloc would stall because it synchronises the whole device;
+ * a process run under an allocation checker that treats any device allocation by a library as an error.  Every other
+ * statistics call of this library allocates on first use (bt_beam_create, the partial-sum buffer of bt_beam_moments).
+ *
+ *   dev_q       six DEVICE arrays of n doubles, order x, px, y, py, t, pt, owned by the caller, read only; 8-byte
+ *               aligned (all six 16-byte aligned: the vectorised kernel).  They must belong to the CURRENT device.
+ *   n           1 <= n <= BT_MOMENTS_STATIC_MAX_PARTICLES.  Anything larger returns BT_ERR_INVALID and launches
+ *               nothing: the partial sums go into a fixed array inside the library (one 216-byte row per 32 768
+ *               particles, 2 048 rows), and that array cannot grow.
+ *   dev_out     DEVICE array of 42 doubles owned by the caller: mean[6], then cov[36] row-major, as bt_beam_moments_device.
+ *   cuda_stream cudaStream_t cast to void* (0 = legacy default stream).  The call enqueues one 4-byte memset and one
+ *               kernel there and returns; nothing is synchronised.
+ *
+ * Same definition and same kernel as bt_beam_moments; the grid depends on n only (not on the GPU model), so the fp64
+ * sums are associated differently and the results agree with bt_beam_moments to rounding (|d cov_ij| <= 1e-12
+ * sqrt(cov_ii cov_jj)), not bit for bit.  Deterministic run to run.
+ *
+ * What the fixed array costs -- read before use:
+ *  - 432.25 KiB of device memory on EVERY GPU that loads libbt.so, from load until the process exits, used or not.
+ *  - One array per GPU, shared by all calls from all threads.  Two calls whose kernels can run at the same time on one GPU
+ *    (different streams without an event between them, different host threads) corrupt each other's sums.  Issue them
+ *    on one stream, or order the streams yourself.
+ *  - The array still holds the previous call's rows.  Nothing depends on that (rows are written before they are read;
+ *    the completion counter is cleared on cuda_stream before every launch), so a failed earlier call does no harm.
+ *  - The first call on each GPU looks up the array's device address (cudaGetSymbolAddress, with that GPU current) and
+ *    caches it.  Make that first call during set-up, outside any stream capture.
+ */
+#define BT_MOMENTS_STATIC_MAX_PARTICLES 67108864LL /* 2048 rows x 32768 particles */
+int bt_moments_static(const double *const dev_q[6], int64_t n, double *dev_out, void *cuda_stream);
+
+/*
  * Slice-step diagnostics (mirrors sim.set_slice_step_diagnostics(True), P:l.61; the statistics are P:l.43 "beam statistics"):
  * the same walk as bt_track(nturns) -- bit-identical final coordinates, reference energy, s and turn -- with the beam
  * statistics of bt_beam_moments taken INSIDE the walk, after every element (BT_DIAG_ELEMENT) or after every slice of every

@@ -16,7 +16,8 @@ import numpy as np
 from . import _build
 
 __all__ = ["lib", "BtError", "Beam", "Grid", "pack_lattice", "ELEMENT_DTYPE", "EXPORTS",
-           "calib_fp64", "calib_rw6", "launch_count", "debug_knob", "version"]
+           "calib_fp64", "calib_rw6", "launch_count", "debug_knob", "version", "moments_static",
+           "MOMENTS_STATIC_MAX_PARTICLES"]
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libbt.so")
@@ -62,6 +63,7 @@ EXPORTS = {
     "bt_gather_kick": (C.c_int, [_vp, _vp, _dp, C.c_double, C.c_double, C.c_double]),
     "bt_beam_moments": (C.c_int, [_vp, _dp, _dp]),
     "bt_beam_moments_device": (C.c_int, [_vp, _vp]),
+    "bt_moments_static": (C.c_int, [C.POINTER(_vp), C.c_int64, _vp, _vp]),
     "bt_track_diagnostics": (C.c_int, [_vp, C.c_int32, C.c_int32, _dp]),
     "bt_sync": (C.c_int, [_vp]),
     "bt_last_error": (C.c_char_p, []),
@@ -118,6 +120,20 @@ def launch_count():
 def debug_knob(name, value):
     """bt_debug_knob: force a kernel variant (tests, A/B measurements); value -1 restores the measured default."""
     _check(lib.bt_debug_knob(name.encode(), int(value)), "bt_debug_knob")
+
+
+MOMENTS_STATIC_MAX_PARTICLES = 67108864   # BT_MOMENTS_STATIC_MAX_PARTICLES of include/bt.h
+
+
+def moments_static(dev_ptrs, n, out_ptr, stream=0):
+    """bt_moments_static: beam statistics of six caller-owned device arrays without any device allocation by the
+    library, for hosts that cannot let a library call cudaMalloc: an application whose arena already holds all of HBM,
+    a multi-stream step loop that an allocation would stall (cudaMalloc synchronises the device), a process under an
+    allocation checker.  dev_ptrs: six device addresses (x, px, y, py, t, pt; n doubles each, on the current device);
+    out_ptr: device address of 42 doubles (mean[6], cov[36]); stream: a cudaStream_t handle (0 = default stream).
+    Only enqueues work.  n above MOMENTS_STATIC_MAX_PARTICLES raises BtError(BT_ERR_INVALID).  All calls on one GPU share
+    one fixed scratch array inside libbt.so: never let two of them overlap on the GPU (see include/bt.h)."""
+    _check(lib.bt_moments_static(_ptr6(dev_ptrs), int(n), _vp(int(out_ptr)), _vp(int(stream))), "bt_moments_static")
 
 
 def pack_lattice(lattice):

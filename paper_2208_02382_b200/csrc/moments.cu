@@ -13,6 +13,8 @@
 // 16e6-particle bunch is only 119 us of HBM time: the grid is exactly the resident blocks (one wave), the centre and the 27
 // block totals each take ONE barrier pair (all values shuffled first, then exchanged through shared memory at once), and
 // bt_beam_moments' 42 results are written straight into mapped pinned host memory (no copy, one stream synchronisation).
+#include <mutex>
+
 #include "bt_internal.h"
 
 namespace bt {
@@ -265,4 +267,97 @@ int launch_moments(Beam *b, double host_mean[6], double host_cov[36]) {
     return BT_OK;
 }
 
+// ---- bt_moments_static: the same statistics for callers that must not allocate device memory -------------------------------
+//
+// Who needs this.  bt_beam_moments / bt_beam_moments_device cudaMalloc their partial-sum buffer on a beam's first call, and
+// bt_beam_create itself creates library state.  Some hosts of this library cannot afford that:
+//   - an application whose own arena has already claimed (nearly) all of HBM at start-up -- the block-structured mesh
+//     frameworks the paper builds on work this way -- so that a cudaMalloc from a plug-in library fails, or succeeds only
+//     by taking memory the arena expected to grow into;
+//   - a time-critical step loop that keeps several streams busy: cudaMalloc and cudaFree synchronise the whole device, so
+//     one stray allocation stalls every stream;
+//   - code running under a memory checker / allocator hook that counts every device allocation as a leak or an error.
+// Such a caller already owns the six coordinate arrays and a 42-double result buffer.  The only other memory the reduction
+// needs is the table of per-block partial sums and a completion counter; here that lives in a fixed array in the library's
+// own device data segment, so this entry point makes no cudaMalloc, cudaFree, cudaHostAlloc or other allocating call.
+//
+// The price, all of which the header repeats:
+//   - the array has a fixed capacity (kStaticRows rows of 27 doubles).  The launch uses one block, and so one row, per
+//     kStaticSlab particles (a grid that depends on n only, not on the GPU model), hence the limit
+//     n <= BT_MOMENTS_STATIC_MAX_PARTICLES; larger n is refused;
+//   - every GPU that loads libbt.so carries the array (432.25 KiB) until the process exits, whether or not it is used;
+//   - there is ONE array per device, shared by all calls: two calls whose kernels may overlap on the same GPU (different
+//     streams, different host threads) race on it.  Order them on one stream or with events;
+//   - the array keeps whatever the previous call left.  Rows are always written before they are read, and the completion
+//     counter is cleared on the caller's stream before every launch, so a call that died half-way cannot poison the next.
+//
+// In host code the name g_static_scratch is only a handle to the symbol, not an address the GPU can use.  The device
+// address is fetched with cudaGetSymbolAddress, once per device with that device current, and cached; that happens in the
+// first call on each device (so make that first call outside any stream capture).
+constexpr long long kStaticSlab = 32768;  // particles reduced by one block = one row of partial sums
+constexpr long long kStaticRows = BT_MOMENTS_STATIC_MAX_PARTICLES / kStaticSlab;  // 2048
+static_assert(kStaticRows * kStaticSlab == BT_MOMENTS_STATIC_MAX_PARTICLES, "the limit must be a whole number of slabs");
+constexpr long long kStaticDoubles = kStaticRows * kMomVals + 32;  // rows, then 256 bytes holding the completion counter
+
+static __device__ __align__(256) double g_static_scratch[kStaticDoubles];
+
+static std::mutex g_static_mutex;
+static double *g_static_addr[kMaxDevices];  // device address of g_static_scratch per device ordinal, nullptr = not asked yet
+
+// device address of this device's copy of the array (the current device's); no allocation
+static int static_scratch_address(double **out) {
+    int dev = -1;
+    BT_CUDA_TRY(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= kMaxDevices) return fail(BT_ERR_UNSUPPORTED, "bt_moments_static: device ordinal beyond the library's table");
+    std::lock_guard<std::mutex> lock(g_static_mutex);
+    if (!g_static_addr[dev]) {
+        double *p = nullptr;
+        cudaError_t e = cudaGetSymbolAddress(reinterpret_cast<void **>(&p), g_static_scratch);
+        if (e != cudaSuccess || !p)
+            return fail(BT_ERR_CUDA, std::string("bt_moments_static: cudaGetSymbolAddress: ") + cudaGetErrorString(e));
+        g_static_addr[dev] = p;
+    }
+    *out = g_static_addr[dev];
+    return BT_OK;
+}
+
 }  // namespace bt
+
+extern "C" int bt_moments_static(const double *const dev_q[6], int64_t n, double *dev_out, void *cuda_stream) {
+    using namespace bt;
+    if (!dev_q || !dev_out) return fail(BT_ERR_INVALID, "bt_moments_static: NULL argument");
+    if (n < 1) return fail(BT_ERR_INVALID, "bt_moments_static: n must be >= 1");
+    if (n > BT_MOMENTS_STATIC_MAX_PARTICLES)
+        return fail(BT_ERR_INVALID, "bt_moments_static: n = " + std::to_string((long long)n) + " exceeds BT_MOMENTS_STATIC_MAX_PARTICLES = " +
+                                        std::to_string((long long)BT_MOMENTS_STATIC_MAX_PARTICLES) +
+                                        " (the fixed scratch array has one row per 32768 particles and 2048 rows); "
+                                        "use bt_beam_moments_device, which allocates, for larger bunches");
+    bool vec = true;
+    for (int c = 0; c < 6; ++c) {
+        if (!dev_q[c]) return fail(BT_ERR_INVALID, "bt_moments_static: NULL coordinate array");
+        if (reinterpret_cast<uintptr_t>(dev_q[c]) & 7) return fail(BT_ERR_INVALID, "bt_moments_static: coordinate arrays must be 8-byte aligned");
+        vec = vec && !(reinterpret_cast<uintptr_t>(dev_q[c]) & 15);
+    }
+    if (reinterpret_cast<uintptr_t>(dev_out) & 7) return fail(BT_ERR_INVALID, "bt_moments_static: dev_out must be 8-byte aligned");
+    double *scratch = nullptr;
+    const int rc = static_scratch_address(&scratch);
+    if (rc != BT_OK) return rc;
+    cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
+    MomArgs a;
+    for (int c = 0; c < 6; ++c) a.q[c] = dev_q[c];
+    a.n = n;
+    a.out = dev_out;
+    a.partial = scratch;
+    a.ticket = reinterpret_cast<unsigned int *>(scratch + kStaticRows * kMomVals);
+    // the counter must read zero when the first block arrives, whatever an earlier (possibly failed) launch left there
+    BT_CUDA_TRY(cudaMemsetAsync(a.ticket, 0, sizeof(unsigned int), stream));
+    const int blocks = (int)((n + kStaticSlab - 1) / kStaticSlab);  // <= kStaticRows: every block owns one row
+    if (vec)
+        moments_kernel<true><<<blocks, kMomBlock, 0, stream>>>(a);
+    else
+        moments_kernel<false><<<blocks, kMomBlock, 0, stream>>>(a);
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return fail(BT_ERR_CUDA, std::string("bt_moments_static launch: ") + cudaGetErrorString(e));
+    g_launch_count.fetch_add(1);
+    return BT_OK;
+}
