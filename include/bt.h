@@ -25,7 +25,8 @@
  *    fails with BT_ERR_CUDA.
  *  - Particle order seen through bt_beam_upload / bt_beam_download never changes.  bt_beam_ptrs exposes the
  *    STORAGE order, which equals the caller's order unless the caller has asked for bt_beam_sort_by_cell
- *    (then bt_beam_ids maps storage slots to original indices).
+ *    (then bt_beam_ids maps storage slots to original indices).  Arrays lent to bt_beam_create hold the bunch at all
+ *    times unless the caller opts in to bt_beam_set_sort_pingpong.
  *  - NaN/Inf coordinates are not checked on the hot path; in deposit/gather they count as
  *    "outside the grid" (R13).
  */
@@ -121,12 +122,28 @@ int bt_beam_get_ref(const bt_beam *beam, double *gamma, double *s, int64_t *turn
  * memory); download returns after the data has arrived. */
 int bt_beam_upload(bt_beam *beam, const double *const host[6]);
 int bt_beam_download(const bt_beam *beam, double *const host[6]);
-/* Zero-copy view of the 6 device arrays the particles live in (P:l.102 "zero-copy access"), in STORAGE order.  These are
- * the arrays given to / allocated by bt_beam_create until bt_beam_sort_by_cell is used: a sort moves the bunch into a
- * library-owned partner set of arrays and the next sort moves it back (ping-pong: a particle's data crosses memory once
- * per sort, no copy back), so ask again after any sort.  bt_beam_upload and bt_track_host return the bunch to the original
- * arrays. */
+/* Zero-copy view of the 6 device arrays the particles live in (P:l.102 "zero-copy access"), in STORAGE order.
+ * Arrays LENT to bt_beam_create always hold the bunch: these are the caller's own pointers, whatever was called in between,
+ * and the library never writes them except to update the bunch (external code holding the same pointers -- torch, cupy,
+ * numba -- keeps seeing the particles).  A sort works out of place, into a library-owned partner set, and copies the result
+ * back (one device copy, 96 bytes of traffic per particle and sort).
+ * Ping-pong mode skips that copy: a sort leaves the bunch in the partner set and the next one moves it back (a particle's
+ * data crosses memory once per sort).  It is the default for arrays the LIBRARY allocated (dev_ptrs == NULL) and opt-in for
+ * lent arrays (bt_beam_set_sort_pingpong): then the lent arrays are stale after every other sort -- including the sorts
+ * bt_deposit_cic triggers under bt_beam_set_resort_interval -- so ask bt_beam_ptrs again after anything that may sort, or
+ * compare bt_beam_storage's epoch, or call bt_beam_rehome before handing the arrays to other code.
+ * bt_beam_upload and bt_track_host always return the bunch to the original arrays. */
 int bt_beam_ptrs(bt_beam *beam, double *dev_ptrs_out[6]);
+/* enable != 0: sorts may leave the bunch in the partner arrays (see bt_beam_ptrs); 0: every sort ends in the arrays of
+ * bt_beam_create, and a bunch that is in the partner set now is copied back. */
+int bt_beam_set_sort_pingpong(bt_beam *beam, int enable);
+/* Bring the bunch back into the arrays of bt_beam_create if a ping-pong sort left it elsewhere (device copy on the beam's
+ * stream, storage order and bt_beam_ids unchanged); no-op otherwise. */
+int bt_beam_rehome(bt_beam *beam);
+/* Where the bunch is: *in_home = 1 iff bt_beam_ptrs currently returns the arrays of bt_beam_create; *epoch counts the
+ * events that changed the arrays or the storage order (sort, re-home, upload, bt_track_host) since creation -- a caller
+ * caching pointers or ids re-reads them when it moves.  Either out may be NULL. */
+int bt_beam_storage(const bt_beam *beam, int32_t *in_home, int64_t *epoch);
 int64_t bt_beam_size(const bt_beam *beam);
 
 /*
@@ -140,7 +157,7 @@ int64_t bt_beam_size(const bt_beam *beam);
  * while particles wander a few cells from where the sort left them, so one sort serves many steps.
  * bt_beam_download still returns the original order; bt_beam_upload resets storage to the caller's order.
  * The order of particles within one cell is not deterministic.  Needs n < 2^31; allocates 56 bytes per
- * particle on first use (the partner set of six arrays the bunch is moved into -- see bt_beam_ptrs -- and two id arrays).
+ * particle on first use (the partner set of six arrays the sort writes into -- see bt_beam_ptrs -- and two id arrays).
  */
 int bt_beam_sort_by_cell(bt_beam *beam, const bt_grid *grid, double zscale);
 /*
@@ -347,6 +364,9 @@ int bt_track_last_launch(const bt_beam *beam, int32_t *grid_dim, int32_t *block_
  *   "track_fuse"    0: one record per lattice element (no peephole fusion of records)
  *   "deposit_mode"  0: one particle per thread, plain reductions; 1: default; 2: 4 particles per thread
  *   "gather_mode"   0: registers; 1: default; 2 / 3: 512- / 128-particle chunks; 4: field tile in shared memory
+ *   "plan_window"   records of per-turn coefficient tables the host builds ahead of the launches (default 65 280 = 4 MiB;
+ *                   whole turns, at least one): bt_track / bt_track_host of many turns through a lattice whose RF changes
+ *                   the reference energy build and enqueue one such window at a time
  */
 int bt_debug_knob(const char *name, int32_t value);
 

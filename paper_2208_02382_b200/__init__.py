@@ -46,6 +46,9 @@ EXPORTS = {
     "bt_beam_size": (C.c_int64, [_vp]),
     "bt_beam_sort_by_cell": (C.c_int, [_vp, _vp, C.c_double]),
     "bt_beam_ids": (C.c_int, [_vp, C.POINTER(_vp)]),
+    "bt_beam_set_sort_pingpong": (C.c_int, [_vp, C.c_int]),
+    "bt_beam_rehome": (C.c_int, [_vp]),
+    "bt_beam_storage": (C.c_int, [_vp, C.POINTER(C.c_int32), C.POINTER(C.c_int64)]),
     "bt_beam_set_resort_interval": (C.c_int, [_vp, C.c_int32]),
     "bt_lattice_set": (C.c_int, [_vp, _vp, C.c_int32]),
     "bt_track": (C.c_int, [_vp, C.c_int32]),
@@ -177,16 +180,20 @@ def _current_stream_ptr():
 class Beam:
     """bt_beam handle.  `storage`: None -> six torch.float64 CUDA tensors are allocated here and lent to
     the library (PyTorch owns device memory); "library" -> bt_beam_create allocates; or a list of six
-    CUDA tensors to borrow."""
+    CUDA tensors to borrow.  `pingpong` (bt_beam_set_sort_pingpong): None = the safe default -- tensors passed in by the
+    caller always hold the bunch (a sort copies its result back into them); tensors allocated here and library storage
+    ping-pong (use .tensors / ptrs() after anything that may sort)."""
 
-    def __init__(self, n, storage=None, stream=None):
+    def __init__(self, n, storage=None, stream=None, pingpong=None):
         self._h = _vp()
         self.n = int(n)
         self._tensors = None
+        storage_was_none = False
         if storage == "library":
             dev = None
         else:
             import torch
+            storage_was_none = storage is None
             if storage is None:
                 storage = [torch.empty(self.n, dtype=torch.float64, device="cuda") for _ in range(6)]
             assert len(storage) == 6 and all(t.is_cuda and t.dtype == torch.float64 and t.is_contiguous() and t.numel() == self.n for t in storage)
@@ -194,6 +201,12 @@ class Beam:
             dev = _ptr6([t.data_ptr() for t in self._tensors])
         self.stream = _current_stream_ptr() if stream is None else int(stream)
         _check(lib.bt_beam_create(C.byref(self._h), self.n, dev, _vp(self.stream)), "bt_beam_create")
+        # Tensors this object allocated itself are reachable only through .tensors, which follows the bunch: ping-pong sorts
+        # (no copy back) are safe.  Tensors the caller passed in keep holding the bunch unless the caller says pingpong=True.
+        if pingpong is None and storage_was_none:
+            pingpong = True
+        if pingpong is not None:
+            self.set_sort_pingpong(pingpong)
 
     def close(self):
         if getattr(self, "_h", None) is not None and self._h and lib is not None:   # lib is None at interpreter shutdown
@@ -290,6 +303,18 @@ class Beam:
         assert out.is_cuda and out.is_contiguous() and out.element_size() == 8 and out.numel() >= 42
         _check(lib.bt_beam_moments_device(self._h, _vp(out.data_ptr())), "bt_beam_moments_device")
         return out
+
+    def set_sort_pingpong(self, enable):
+        _check(lib.bt_beam_set_sort_pingpong(self._h, int(bool(enable))), "bt_beam_set_sort_pingpong")
+
+    def rehome(self):
+        _check(lib.bt_beam_rehome(self._h), "bt_beam_rehome")
+
+    def storage(self):
+        """(in_home, epoch): whether the bunch is in the arrays of bt_beam_create, and the count of storage changes so far."""
+        h, e = C.c_int32(), C.c_int64()
+        _check(lib.bt_beam_storage(self._h, C.byref(h), C.byref(e)), "bt_beam_storage")
+        return bool(h.value), int(e.value)
 
     def set_resort_interval(self, every_n_deposits):
         _check(lib.bt_beam_set_resort_interval(self._h, int(every_n_deposits)), "bt_beam_set_resort_interval")

@@ -64,8 +64,8 @@ static int validate_element(const bt_element &e, int idx) {
 }
 
 // ---- debug knobs (bt_debug_knob): process-wide, typed, default -1 = "the measured default" ---------------------------
-std::atomic<int32_t> g_knob[KNOB_COUNT] = {{-1}, {-1}, {-1}, {-1}, {-1}};
-static const char *const kKnobNames[KNOB_COUNT] = {"track_ppt", "track_block", "track_fuse", "deposit_mode", "gather_mode"};
+std::atomic<int32_t> g_knob[KNOB_COUNT] = {{-1}, {-1}, {-1}, {-1}, {-1}, {-1}};
+static const char *const kKnobNames[KNOB_COUNT] = {"track_ppt", "track_block", "track_fuse", "deposit_mode", "gather_mode", "plan_window"};
 
 // Runs of half cells [QUAD1][SEXTOCT|TAILDRIFT] among the records appended since `start` become one dispatch: the first
 // record of a run is relabelled OP_HALFCELL with count = pairs in the run; the coefficients stay where they are, so the
@@ -292,7 +292,12 @@ int grid_release(Grid *g, cudaStream_t s) {
 // A plan is a list of (records, passes) launches over record storage it owns or borrows.  Static lattices: one table,
 // walked nturns times by one launch (or, when a turn needs more than kTableRecords records, its segments turn after turn).
 // Lattices whose RF changes the reference energy (S3): every turn has its own coefficients; as many whole turns as fit
-// one launch's table go into it.  The same plan serves every chunk of bt_track_host.
+// one launch's table go into it.
+// A plan covers a WINDOW of turns, not necessarily the whole call: per-turn tables cost 64 bytes per record and turn
+// (bt_track(10^6 turns) of a 200-record ring would be 12.8 GB of host memory if built at once), so plan_walk stops after
+// kPlanWindowRecords records (whole turns, at least one) and the caller asks again from the reference energy the window
+// ends at.  The records of a launch are copied into its parameters when it is enqueued, so a window's storage is reused at
+// once, and the host builds window k+1 (cos/sinh per turn) while the GPU walks window k.
 struct WalkPlan {
     struct Launch {
         size_t lo;
@@ -305,19 +310,26 @@ struct WalkPlan {
     double gamma_after = 0.0;
 };
 
-static void plan_walk(Beam &b, int32_t nturns, WalkPlan &plan) {
+constexpr int kPlanWindowRecords = 128 * kTableRecords;  // 65 280 records = 4 MiB of host memory per window
+
+// Plans the next window of a walk of `nturns` turns that starts at reference energy `gamma`; returns the turns it covers
+// (1..nturns) and leaves the energy after them in plan.gamma_after.
+static int32_t plan_walk(Beam &b, double gamma, int32_t nturns, WalkPlan &plan) {
     const size_t K = (size_t)kTableRecords;
+    const size_t window = (size_t)knob(KNOB_PLAN_WINDOW, kPlanWindowRecords);
+    plan.own.clear();
+    plan.launches.clear();
     auto add_segments = [&](size_t lo, size_t len, double spr) {
         for (size_t o = 0; o < len; o += K) plan.launches.push_back({lo + o, (int32_t)(len - o < K ? len - o : K), 1, spr});
     };
     if (!b.energy_changes) {
         if (!b.table_valid) {
             b.h_table.clear();
-            build_turn_table(b.lattice, b.gamma, b.h_table, &b.table_slots);
+            build_turn_table(b.lattice, gamma, b.h_table, &b.table_slots);
             b.table_valid = true;
         }
         plan.ops = &b.h_table;
-        plan.gamma_after = b.gamma;
+        plan.gamma_after = gamma;
         const double spr = b.table_slots / (double)b.h_table.size();
         // A periodic channel (configs[1]: one FODO cell x 100) is one period walked repeats x nturns times: the same
         // records in the same order, a table of 5 instead of 500 records in the launch's parameters.
@@ -332,21 +344,28 @@ static void plan_walk(Beam &b, int32_t nturns, WalkPlan &plan) {
         const long long passes = (long long)nturns * (long long)(b.h_table.size() / period);
         if (period <= K && passes <= 0x7fffffffLL) {
             plan.launches.push_back({0, (int32_t)period, (int32_t)passes, spr});
-        } else if (b.h_table.size() <= K) {
-            plan.launches.push_back({0, (int32_t)b.h_table.size(), nturns, spr});
-        } else {
-            for (int32_t t = 0; t < nturns; ++t) add_segments(0, b.h_table.size(), spr);
+            return nturns;
         }
-        return;
+        if (b.h_table.size() <= K) {
+            plan.launches.push_back({0, (int32_t)b.h_table.size(), nturns, spr});
+            return nturns;
+        }
+        // a turn longer than one table: its segments turn after turn, a window's worth of records at a time
+        long long turns = (long long)(window / b.h_table.size());
+        if (turns < 1) turns = 1;
+        if (turns > nturns) turns = nturns;
+        for (long long t = 0; t < turns; ++t) add_segments(0, b.h_table.size(), spr);
+        return (int32_t)turns;
     }
     plan.ops = &plan.own;
-    double gamma = b.gamma;
     size_t pend_lo = 0;  // records [pend_lo, own.size()) = whole turns not yet assigned to a launch
     double pend_spr = 0.0;
-    for (int32_t t = 0; t < nturns; ++t) {
+    int32_t t = 0;
+    while (t < nturns && (t == 0 || plan.own.size() < window)) {
         const size_t turn_lo = plan.own.size();
         double slots = 0.0;
         gamma = build_turn_table(b.lattice, gamma, plan.own, &slots);
+        ++t;
         const size_t turn_len = plan.own.size() - turn_lo;
         const double spr = slots / (double)turn_len;
         if (turn_len > K) {  // a single turn exceeds one table: flush what is pending, then its segments
@@ -363,6 +382,7 @@ static void plan_walk(Beam &b, int32_t nturns, WalkPlan &plan) {
     }
     if (plan.own.size() > pend_lo) plan.launches.push_back({pend_lo, (int32_t)(plan.own.size() - pend_lo), 1, pend_spr});
     plan.gamma_after = gamma;
+    return t;
 }
 
 static int run_plan(Beam &b, const WalkPlan &plan) {  // on b.range's stream when set, else on the beam's
@@ -370,6 +390,21 @@ static int run_plan(Beam &b, const WalkPlan &plan) {  // on b.range's stream whe
         const int rc = launch_track(&b, plan.ops->data() + l.lo, l.len, l.nturns, l.spr);
         if (rc != BT_OK) return rc;
     }
+    return BT_OK;
+}
+
+// All windows of a walk of nturns turns from the beam's current reference energy, on b.range's stream when set, else on
+// the beam's; *gamma_after = the reference energy at the end.  `plan` is working storage (reused window after window).
+static int run_walk(Beam &b, int32_t nturns, WalkPlan &plan, double *gamma_after) {
+    double gamma = b.gamma;
+    for (int32_t left = nturns; left > 0;) {
+        const int32_t did = plan_walk(b, gamma, left, plan);
+        const int rc = run_plan(b, plan);
+        if (rc != BT_OK) return rc;
+        gamma = plan.gamma_after;
+        left -= did;
+    }
+    *gamma_after = gamma;
     return BT_OK;
 }
 
@@ -418,6 +453,7 @@ int bt_beam_create(bt_beam **out, int64_t n, double *const dev_ptrs[6], void *cu
     if (dev_ptrs) {
         for (int i = 0; i < 6; ++i) b.q[i] = b.home[i] = dev_ptrs[i];
         b.owns = false;
+        b.pingpong = false;  // lent arrays always hold the bunch unless bt_beam_set_sort_pingpong says otherwise
     } else {
         // one allocation, 6 slices, each 256-byte aligned (S0)
         const size_t stride = (((size_t)n * sizeof(double)) + 255u) & ~(size_t)255u;
@@ -430,6 +466,7 @@ int bt_beam_create(bt_beam **out, int64_t n, double *const dev_ptrs[6], void *cu
         }
         for (int i = 0; i < 6; ++i) b.q[i] = b.home[i] = (double *)((char *)base + stride * i);
         b.owns = true;
+        b.pingpong = true;
     }
     b.aligned16 = b.aligned32 = true;
     for (int i = 0; i < 6; ++i) {
@@ -449,6 +486,7 @@ void bt_beam_destroy(bt_beam *beam) {
     int *ibufs[] = {b.ids, b.ids_tmp, b.sort_count, b.sort_block_sum};
     for (int *p : ibufs)
         if (p) cudaFree(p);
+    if (b.dl_tmp) cudaFree(b.dl_tmp);
     if (b.mom_buf) cudaFree(b.mom_buf);
     if (b.mom_host) cudaFreeHost(b.mom_host);
     if (b.diag_rows) cudaFree(b.diag_rows);
@@ -497,6 +535,7 @@ int bt_beam_upload(bt_beam *beam, const double *const host[6]) {
         BT_CUDA_TRY(cudaMemcpyAsync(b.q[i], host[i], (size_t)b.n * sizeof(double), cudaMemcpyHostToDevice, b.stream));
     b.permuted = false;
     b.deposits_since_sort = 0;
+    ++b.storage_epoch;
     return BT_OK;
 }
 
@@ -507,8 +546,13 @@ int bt_beam_download(const bt_beam *beam, double *const host[6]) {
     Beam &b = const_cast<Beam &>(beam->b);
     for (int i = 0; i < 6; ++i) {
         const double *src = b.q[i];
-        if (b.permuted) {  // storage is cell-sorted: restore the original order through the idle partner array
+        if (b.permuted) {  // storage is cell-sorted: restore the original order through the idle partner array --
+            // never through arrays the caller lent (their owner may be reading them): those get a scratch of the library's
             double *tmp = b.in_alt ? b.home[i] : b.alt[i];
+            if (b.in_alt && !b.owns) {
+                if (!b.dl_tmp) BT_CUDA_TRY(cudaMalloc(&b.dl_tmp, (size_t)b.n * sizeof(double)));
+                tmp = b.dl_tmp;
+            }
             int rc = unpermute_to(&b, i, tmp);
             if (rc != BT_OK) return rc;
             src = tmp;
@@ -529,6 +573,24 @@ int bt_beam_sort_by_cell(bt_beam *beam, const bt_grid *grid, double zscale) {
     if (!beam || !grid) return fail(BT_ERR_INVALID, "bt_beam_sort_by_cell: NULL argument");
     if (!isfinite(zscale)) return fail(BT_ERR_INVALID, "bt_beam_sort_by_cell: zscale not finite");
     return sort_by_cell(&beam->b, &grid->g, zscale);
+}
+
+int bt_beam_set_sort_pingpong(bt_beam *beam, int enable) {
+    if (!beam) return fail(BT_ERR_INVALID, "bt_beam_set_sort_pingpong: beam is NULL");
+    beam->b.pingpong = enable != 0;
+    return enable ? BT_OK : rehome(&beam->b);
+}
+
+int bt_beam_rehome(bt_beam *beam) {
+    if (!beam) return fail(BT_ERR_INVALID, "bt_beam_rehome: beam is NULL");
+    return rehome(&beam->b);
+}
+
+int bt_beam_storage(const bt_beam *beam, int32_t *in_home, int64_t *epoch) {
+    if (!beam) return fail(BT_ERR_INVALID, "bt_beam_storage: beam is NULL");
+    if (in_home) *in_home = beam->b.in_alt ? 0 : 1;
+    if (epoch) *epoch = beam->b.storage_epoch;
+    return BT_OK;
 }
 
 int bt_beam_ids(bt_beam *beam, int32_t **dev_ids_out) {
@@ -571,10 +633,10 @@ int bt_track(bt_beam *beam, int32_t nturns) {
     if (!b.has_ref) return fail(BT_ERR_STATE, "bt_track: bt_beam_set_ref not called");
     if (nturns == 0) return BT_OK;
     WalkPlan plan;
-    plan_walk(b, nturns, plan);
-    const int rc = run_plan(b, plan);
+    double gamma_after = b.gamma;
+    const int rc = run_walk(b, nturns, plan, &gamma_after);
     if (rc != BT_OK) return rc;
-    b.gamma = plan.gamma_after;  // S3
+    b.gamma = gamma_after;  // S3
     b.s += b.lattice_length * (double)nturns;
     b.turn += nturns;
     return BT_OK;
@@ -698,8 +760,11 @@ int bt_track_host(bt_beam *beam, const double *const host_in[6], double *const h
         if (!b.pipe_stream[i]) BT_CUDA_TRY(cudaStreamCreateWithFlags(&b.pipe_stream[i], cudaStreamNonBlocking));
         if (!b.pipe_event[i]) BT_CUDA_TRY(cudaEventCreateWithFlags(&b.pipe_event[i], cudaEventDisableTiming));
     }
+    // One plan serves every chunk when the whole call fits one window (the usual case).  Otherwise each chunk walks the
+    // windows on its own, rebuilding them (bounded host memory; the tables are cheap next to a chunk's copies).
     WalkPlan plan;
-    plan_walk(b, nturns, plan);
+    const bool whole = plan_walk(b, b.gamma, nturns, plan) == nturns;
+    double gamma_after = plan.gamma_after;
     set_current_storage(&b, false);  // the result lives in the home arrays, in the caller's order
     // the chunk streams start after everything already queued on the beam's stream
     BT_CUDA_TRY(cudaEventRecord(b.pipe_event[0], b.stream));
@@ -718,7 +783,7 @@ int bt_track_host(bt_beam *beam, const double *const host_in[6], double *const h
         TrackRange r;
         r.off = off, r.n = m, r.geom_n = b.n, r.stream = st;
         b.range = &r;
-        rc = run_plan(b, plan);
+        rc = whole ? run_plan(b, plan) : run_walk(b, nturns, plan, &gamma_after);
         b.range = nullptr;
         for (int i = 0; i < 6 && rc == BT_OK && ce == cudaSuccess; ++i)
             ce = cudaMemcpyAsync(host_out[i] + off, b.q[i] + off, (size_t)m * sizeof(double), cudaMemcpyDeviceToHost, st);
@@ -730,10 +795,11 @@ int bt_track_host(bt_beam *beam, const double *const host_in[6], double *const h
     const cudaError_t se = cudaStreamSynchronize(b.stream);
     b.permuted = false;  // storage order = the caller's order
     b.deposits_since_sort = 0;
+    ++b.storage_epoch;
     if (rc != BT_OK) return rc;
     if (ce != cudaSuccess) return fail(BT_ERR_CUDA, std::string("bt_track_host: copy: ") + cudaGetErrorString(ce));
     if (se != cudaSuccess) return fail(BT_ERR_CUDA, std::string("bt_track_host: ") + cudaGetErrorString(se));
-    b.gamma = plan.gamma_after;
+    b.gamma = gamma_after;
     b.s += b.lattice_length * (double)nturns;
     b.turn += nturns;
     return BT_OK;

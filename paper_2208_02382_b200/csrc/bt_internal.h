@@ -18,7 +18,7 @@ int fail(int code, const std::string &msg);
 extern std::atomic<int64_t> g_launch_count;
 
 // Debug knobs (bt_debug_knob): A/B measurements and the tests that exercise every kernel variant.  -1 = measured default.
-enum Knob { KNOB_TRACK_PPT = 0, KNOB_TRACK_BLOCK, KNOB_TRACK_FUSE, KNOB_DEPOSIT_MODE, KNOB_GATHER_MODE, KNOB_COUNT };
+enum Knob { KNOB_TRACK_PPT = 0, KNOB_TRACK_BLOCK, KNOB_TRACK_FUSE, KNOB_DEPOSIT_MODE, KNOB_GATHER_MODE, KNOB_PLAN_WINDOW, KNOB_COUNT };
 extern std::atomic<int32_t> g_knob[KNOB_COUNT];
 static inline int knob(Knob k, int dflt) {
     const int v = g_knob[k].load(std::memory_order_relaxed);
@@ -91,6 +91,9 @@ struct Beam {
     double *home[6] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};  // the caller's arrays (borrowed) or the library's
     double *alt[6] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};   // library-owned partner set (bt_beam_sort_by_cell ping-pong)
     bool in_alt = false;
+    bool pingpong = false;       // a sort may leave the bunch in alt (set at creation: library-owned storage yes, lent arrays no)
+    int64_t storage_epoch = 0;   // bumped whenever the bunch changes arrays or storage order (bt_beam_storage)
+    double *dl_tmp = nullptr;    // n doubles: bt_beam_download's un-permute scratch when the idle set is the caller's (lent) arrays
     bool owns = false;
     bool aligned16 = false;
     bool aligned32 = false;  // all six arrays 32-byte aligned: 256-bit lane-run access in the grid kernels
@@ -171,6 +174,7 @@ int sort_by_cell(Beam *b, const Grid *g, double zscale);
 int unpermute_to(Beam *b, int c, double *out);  // out[ids[j]] = q[c][j] on the beam's stream
 int ensure_alt_storage(Beam *b);                 // allocates the partner arrays and the id arrays on first use
 void set_current_storage(Beam *b, bool use_alt); // q = alt or home; refreshes the alignment flags
+int rehome(Beam *b);                             // bunch in alt -> device copy back into home (storage order kept); no-op in home
 int launch_moments(Beam *b, double host_mean[6], double host_cov[36]);  // synchronises the beam's stream
 int launch_moments_async(Beam *b, double *dev_out);                      // 42 doubles to device memory, no synchronisation
 int poisson_solve(Grid *g, double gz, cudaStream_t stream);  // rho -> phi -> field records

@@ -434,6 +434,15 @@ void set_current_storage(Beam *b, bool use_alt) {
     }
 }
 
+int rehome(Beam *b) {
+    if (!b->in_alt) return BT_OK;
+    for (int c = 0; c < 6; ++c)
+        BT_CUDA_TRY(cudaMemcpyAsync(b->home[c], b->alt[c], (size_t)b->n * sizeof(double), cudaMemcpyDeviceToDevice, b->stream));
+    set_current_storage(b, false);
+    ++b->storage_epoch;
+    return BT_OK;
+}
+
 template <int ORDER>
 static int sort_by_cell_order(Beam *b, const Grid *g, double zscale) {
     if (b->n > 0x7fffffffLL) return fail(BT_ERR_UNSUPPORTED, "bt_beam_sort_by_cell: n exceeds int32");
@@ -494,6 +503,10 @@ static int sort_by_cell_order(Beam *b, const Grid *g, double zscale) {
     b->ids = b->ids_tmp;
     b->ids_tmp = tmp;
     b->permuted = true;
+    ++b->storage_epoch;
+    // Lent arrays (the zero-copy contract, P:l.102): whoever lent them may read them at any time, so the bunch does not stay
+    // in the partner set unless the caller asked for ping-pong; one device copy (96 B per particle) brings it back.
+    if (b->in_alt && !b->pingpong) return rehome(b);
     return BT_OK;
 }
 

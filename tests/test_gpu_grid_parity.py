@@ -430,3 +430,71 @@ def test_resort_interval_sorts_inside_deposit_and_keeps_results():
     assert beam.ids_ptr() == 0                           # interval 0: the deposit never sorts
     beam.close()
     grid.close()
+
+
+@pytest.mark.parametrize("pingpong", [False, True])
+def test_lent_tensors_keep_holding_the_bunch_across_library_triggered_sorts(pingpong):
+    """The zero-copy contract (P:l.102) for arrays the caller lent: external code keeps the tensors it passed in, so after
+    any number of sorts -- the ones bt_deposit_cic triggers under a re-sort interval included -- those tensors ARE the bunch
+    (storage order, ids map back), and bt_beam_download never scribbles on them.  With ping-pong switched on explicitly the
+    bunch may sit in the library's partner arrays; bt_beam_storage says so, bt_beam_rehome brings it back, and the lent
+    tensors are left untouched meanwhile."""
+    import ctypes
+    import torch
+    sc = W.spacecharge_config("A", n=150_001, shape=(32, 32, 32))
+    c = W.make_spacecharge_bunch(sc)
+    E = W.gaussian_bunch_field(sc)
+    lent = [torch.empty(sc.n, dtype=torch.float64, device="cuda") for _ in range(6)]
+    lent_ptrs = [t.data_ptr() for t in lent]
+    beam = bt.Beam(sc.n, storage=lent, pingpong=pingpong if pingpong else None)
+    grid = bt.Grid(sc.shape, sc.lo, sc.d)
+    beam.set_ref(sc.kin_energy_MeV, sc.mass_MeV, 1.0)
+    grid.set_field(*E)
+    beam.set_resort_interval(2)
+    beam.upload(c)
+    assert beam.storage()[0] and beam.ptrs() == lent_ptrs
+    cudart = ctypes.cdll.LoadLibrary("libcudart.so")
+
+    def ids():
+        t = torch.empty(sc.n, dtype=torch.int32, device="cuda")
+        torch.cuda.synchronize()
+        cudart.cudaMemcpy(ctypes.c_void_p(t.data_ptr()), ctypes.c_void_p(beam.ids_ptr()), ctypes.c_size_t(4 * sc.n), 3)
+        return t.cpu().numpy()
+
+    seen_away = False
+    epochs = [beam.storage()[1]]
+    for step in range(5):                               # sorts before deposits 1, 3, 5
+        beam.deposit_cic(grid, sc.q_weight, sc.zscale, True)
+        beam.gather_kick(grid, sc.kick_coef, sc.zscale, 0.0, sc.ds)
+        in_home, epoch = beam.storage()
+        api = beam.download()                           # API order; must not disturb the lent tensors
+        if in_home:
+            assert beam.ptrs() == lent_ptrs
+            stored = [t.cpu().numpy() for t in lent]
+            perm = ids()
+            for a, b in zip(stored, api):               # the lent tensors hold the bunch: storage slot j = original particle ids[j]
+                assert np.array_equal(a, b[perm])
+        else:
+            assert pingpong
+            seen_away = True
+            assert beam.ptrs() != lent_ptrs
+            before = [t.clone() for t in lent]
+            beam.download()
+            for a, b in zip(before, lent):              # stale, but the caller's: not used as scratch
+                assert torch.equal(a, b)
+            beam.rehome()
+            assert beam.storage() == (True, epoch + 1) and beam.ptrs() == lent_ptrs
+            perm = ids()
+            for a, b in zip([t.cpu().numpy() for t in lent], api):
+                assert np.array_equal(a, b[perm])
+        epochs.append(beam.storage()[1])
+    assert seen_away == pingpong
+    assert epochs[1] > epochs[0] and epochs[2] == epochs[1] and epochs[3] > epochs[2]   # moved by deposits 1 and 3, not by 2
+    ref = [a.copy() for a in c]
+    g0 = O.ref_from_kinetic(sc.kin_energy_MeV, sc.mass_MeV)[0]
+    for step in range(5):
+        O.gather_kick(ref, sc.shape, sc.lo, sc.d, E, sc.kick_coef, sc.zscale)
+        O.track(ref, [("drift", sc.ds, 1)], 1, g0)
+    assert max(r14_error(beam.download(), ref)) <= 1e-11
+    beam.close()
+    grid.close()

@@ -94,6 +94,43 @@ def test_lattice_longer_than_one_launch_table():
     assert abs(g - g_ref) <= 1e-15 * g_ref
 
 
+@pytest.mark.parametrize("window", [1, 700, 3000])
+def test_walk_planned_in_windows_is_bit_identical(window, knobs):
+    """bt_track / bt_track_host build the per-turn coefficient tables one window of records at a time (bounded host memory for
+    any nturns) and carry the reference energy from window to window.  Forced here to windows of one turn, of a few turns and
+    of about a turn (lattice longer than one launch table): the same bits and the same final gamma as the whole-call plan."""
+    import torch
+    import paper_2208_02382_b200 as bt
+    cfg = W.config(3, n=20_003)
+    c = W.make_bunch(cfg)
+    cell = [("quad", 0.2, 1, 1.3), ("multipole", 0.0, 1, 3, 0.2, 0.0), ("drift", 0.1, 1), ("quad", 0.2, 7, -1.3),
+            ("multipole", 0.0, 1, 4, 2.0, 0.0), ("multipole", 0.0, 1, 3, -0.2, 0.0), ("multipole", 0.0, 1, 4, 0.9, 0.0), ("drift", 0.1, 2)]
+    long_static = cell * 300                                                   # 2400 records per turn, no RF
+    long_rf = long_static + [("shortrf", 0.0, 1, 1e-3, 1e7, -20.0)]
+    for lat, nturns in ((cfg.lattice, 7), (long_static, 3), (long_rf, 3)):    # cfg 3: RF ring, 7 turns = 2 launches unwindowed
+        results = []
+        for w in (-1, window):
+            knobs("plan_window", w)
+            beam = bt.Beam(cfg.n)
+            beam.set_ref(cfg.kin_energy_MeV, cfg.mass_MeV, cfg.charge_qe)
+            beam.lattice_set(lat)
+            beam.upload(c)
+            beam.track(nturns)
+            plain, ref = beam.download(), beam.get_ref()
+            beam.set_ref(cfg.kin_energy_MeV, cfg.mass_MeV, cfg.charge_qe)
+            pinned = [torch.from_numpy(a.copy()).pin_memory() for a in c]
+            out = [torch.empty(cfg.n, dtype=torch.float64).pin_memory() for _ in range(6)]
+            beam.track_host(pinned, out, nturns=nturns, nchunks=3)
+            assert beam.get_ref() == ref
+            for a, b in zip(out, plain):
+                assert np.array_equal(a.numpy(), b)
+            results.append((plain, ref))
+            beam.close()
+        for a, b in zip(results[0][0], results[1][0]):
+            assert np.array_equal(a, b)
+        assert results[0][1] == results[1][1]
+
+
 def test_two_beams_with_different_lattices_interleaved():
     """The record table travels with each launch (kernel parameters): beams with different lattices on different
     streams, interleaved, must each see their own table."""
