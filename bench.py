@@ -72,20 +72,62 @@ def load_peaks():
     return {"hbm_gbs": 6650.0, "sm_max_mhz": 1965.0}, "fallback"
 
 
+def _source_digest(name):
+    """sha256 of a kernel source under csrc/ ('file' or 'bt_internal.h#device_records' = the device-visible part of that header)."""
+    import hashlib
+    csrc = os.path.join(ROOT, "paper_2208_02382_b200", "csrc")
+    if name == "bt_internal.h#device_records":
+        with open(os.path.join(csrc, "bt_internal.h")) as f:
+            text = f.read()
+        return hashlib.sha256(text[text.index("// ---- device op records"):text.index("struct TrackLaunchInfo")].encode()).hexdigest()
+    with open(os.path.join(csrc, name), "rb") as f:
+        return hashlib.sha256(f.read()).hexdigest()
+
+
 def load_traffic():
     """dram__bytes_read.sum + dram__bytes_write.sum per launch from the ncu --set full captures summarised under
-    profiles/ (text, written by hand from `ncu -i ... --page raw --csv`): {key: (bytes, source)}."""
+    profiles/ (text, written from `ncu -i ... --page raw --csv`): {key: (bytes, source)}, plus "_provenance".
+    The table is STATIC (captured once, at the commit profiles/r02_traffic_sources.json names), not measured in this run:
+    a value is handed out only while the sources of its kernel are byte-identical to what was captured."""
     out = {}
     path = os.path.join(ROOT, "profiles", "r02_traffic.csv")
-    if os.path.exists(path):
+    side = os.path.join(ROOT, "profiles", "r02_traffic_sources.json")
+    if os.path.exists(path) and os.path.exists(side):
         with open(path) as f:
             for row in csv.DictReader(f):
                 out[row["key"]] = (float(row["dram_read_bytes"]) + float(row["dram_write_bytes"]), row["source"])
+        with open(side) as f:
+            prov = json.load(f)
+        changed = {}
+        for fam, files in prov["kernel_sources"].items():
+            try:
+                changed[fam] = [x for x in files if _source_digest(x) != prov["sha256"].get(x)]
+            except (OSError, ValueError):
+                changed[fam] = list(files)
+        out["_provenance"] = {"file": "profiles/r02_traffic.csv", "captured_at": prov["captured_at"], "changed": changed}
     return out
 
 
 def traffic_of(table, key):
-    return table[key][0] if key in table else None
+    """Value of the static table, or None when the table is missing or the kernel's sources changed since the capture."""
+    prov = table.get("_provenance")
+    if key not in table or prov is None or prov["changed"].get(key.split(":")[0], ["?"]):
+        return None
+    return table[key][0]
+
+
+def traffic_source(table, key):
+    """Goes beside every `traffic`: where the number comes from and whether it is still valid for the kernels as built."""
+    prov = table.get("_provenance")
+    if prov is None:
+        return {"file": None, "reason": "no traffic table under profiles/"}
+    src = {"file": prov["file"], "captured_at": prov["captured_at"], "kind": "static table from ncu --set full captures, not measured in this run"}
+    stale = prov["changed"].get(key.split(":")[0], ["?"])
+    if key not in table:
+        src["reason"] = "no capture for this kernel/workload"
+    elif stale:
+        src["reason"] = "stale: %s changed since the capture; traffic withheld until re-captured" % ", ".join(stale)
+    return src
 
 
 def cpu_model():
@@ -331,6 +373,7 @@ def bench_other_configs(bt, torch, flush, peaks, nominal_peak, traffic, with_cpu
     """bt_track on configs[0], [1], [2] at full size (one call = the config's nturns), each with the oracle timed beside it."""
     out = []
     hbm = float(peaks["hbm_gbs"]) * 1e9
+    measured_fp64 = None
     for idx, reps in ((0, 5), (1, 10), (2, 5)):
         cfg = W.config(idx)
         n = cfg.n
@@ -359,6 +402,13 @@ def bench_other_configs(bt, torch, flush, peaks, nominal_peak, traffic, with_cpu
                     "(SURVEY 8d); roofline time %.2f us shown for information" % (roof["roofline_time_ms"] * 1e3)}
         else:
             roof["traffic"] = traffic_of(traffic, "walk:" + cfg.name)
+            roof["traffic_source"] = traffic_source(traffic, "walk:" + cfg.name)
+            if roof["bound"] == "alu":
+                if measured_fp64 is None:
+                    measured_fp64 = bt.calib_fp64(300.0)
+                roof["peak_kind"] = "derived: 148 SMs x 64 FP64 lanes x sm_max_mhz (DESIGN.md s7)"
+                roof["peak_measured_dfma_chain"] = measured_fp64 / 1e12
+                roof["frac_of_measured_dfma_chain"] = roof["achieved"] * 1e12 / measured_fp64
         entry["roofline"] = roof
         if idx == 2:
             # beam statistics: bt_beam_moments = 1 launch + a 336-byte read-back, 48 B/particle
@@ -369,7 +419,8 @@ def bench_other_configs(bt, torch, flush, peaks, nominal_peak, traffic, with_cpu
             ta = statistics.mean(_event_ms(torch, lambda: beam.moments_device(dev_out), 5, flush)) * 1e-3
             entry["moments"] = {"ms": tm * 1e3, "roofline": {"bound": "hbm", "achieved": 48.0 * n / tm / 1e9, "peak": hbm / 1e9,
                                                               "unit": "GB/s", "frac": 48.0 * n / tm / hbm,
-                                                              "traffic": traffic_of(traffic, "moments:%d" % n)},
+                                                              "traffic": traffic_of(traffic, "moments:%d" % n),
+                                                              "traffic_source": traffic_source(traffic, "moments:%d" % n)},
                                 "device_variant": {"call": "bt_beam_moments_device (result stays on the device, no synchronisation)",
                                                    "ms": ta * 1e3, "frac": 48.0 * n / ta / hbm}}
         if idx == 1:
@@ -396,7 +447,11 @@ def bench_spacecharge(bt, torch, flush, peaks, traffic, interval, with_cpu=True)
     gather+kick+drift 96 B/particle + 24 B/node."""
     hbm = float(peaks["hbm_gbs"])
     out = {}
+    default_interval = interval
     for variant, order in (("A", 1), ("B", 1), ("A", 2)):
+        # order 2: 27-node stencils reach further, so chunks of wandered particles cost more per step and the measured optimum
+        # is a shorter window (DESIGN.md section 11: 3 against 5); an explicit --resort-interval other than 5 is used as given
+        interval = 3 if (order == 2 and default_interval == 5) else default_interval
         sc = W.spacecharge_config(variant)
         c = W.make_spacecharge_bunch(sc)
         E = W.gaussian_bunch_field(sc)
@@ -447,7 +502,7 @@ def bench_spacecharge(bt, torch, flush, peaks, traffic, interval, with_cpu=True)
             mp_ = statistics.mean(t_ps) * 1e-3
             poisson = {"ms": mp_ * 1e3, "padded_box": [2 * s for s in sc.shape],
                        "roofline": {"bound": "hbm", "achieved": ps_bytes / mp_ / 1e9, "peak": hbm, "unit": "GB/s",
-                                    "frac": ps_bytes / mp_ / 1e9 / hbm, "traffic": traffic_of(traffic, "poisson:128"),
+                                    "frac": ps_bytes / mp_ / 1e9 / hbm, "traffic": traffic_of(traffic, "poisson:128"), "traffic_source": traffic_source(traffic, "poisson:128"),
                                     "note": "bytes = single-pass lower bound of the pad/FFT/multiply/FFT/extract/gradient chain"}}
             grid.set_field(*E)
         md_all, mg = statistics.mean(t_dep) * 1e-3, statistics.mean(t_gat) * 1e-3
@@ -463,11 +518,13 @@ def bench_spacecharge(bt, torch, flush, peaks, traffic, interval, with_cpu=True)
                                 "(steps 0, %d, ... contain bt_beam_sort_by_cell)" % interval,
                         "roofline": {"bound": "hbm", "achieved": dep_bytes / md / 1e9, "peak": hbm, "unit": "GB/s",
                                      "frac": dep_bytes / md / 1e9 / hbm, "frac_incl_resorts": dep_bytes / md_all / 1e9 / hbm,
-                                     "traffic": traffic_of(traffic, "deposit:%s:%d" % (variant, order))}},
+                                     "traffic": traffic_of(traffic, "deposit:%s:%d" % (variant, order)),
+                                     "traffic_source": traffic_source(traffic, "deposit:%s:%d" % (variant, order))}},
             "gather_kick_drift": {"ms": mg * 1e3, "ms_per_step": t_gat, "unsorted_kick_only_ms": t_gat_u,
                                   "roofline": {"bound": "hbm", "achieved": gat_bytes / mg / 1e9, "peak": hbm, "unit": "GB/s",
                                                "frac": gat_bytes / mg / 1e9 / hbm,
-                                               "traffic": traffic_of(traffic, "gather:%s:%d" % (variant, order))}},
+                                               "traffic": traffic_of(traffic, "gather:%s:%d" % (variant, order)),
+                                               "traffic_source": traffic_source(traffic, "gather:%s:%d" % (variant, order))}},
             "ms_per_step_incl_sort_amortised": (md_all + mg) * 1e3,
             "ms_per_step_steady_state": (md + mg) * 1e3 + min(t_resort) / interval,
             "steady_state_note": "deposit (no sort) + gather + one re-sort of the sorted beam per %d steps; "
@@ -573,6 +630,8 @@ def run_ours(args):
     step_ms = [a.elapsed_time(b) for a, b in ev]
     ms_sum = sum(step_ms)
     launch_info = beam.last_launch()         # geometry of the timed launches (the e2e leg below launches per chunk)
+    # every 64th particle of the device-resident result of the last timed step, kept to check the e2e leg against (untimed)
+    dev_sample = [t[::64].cpu() for t in beam.tensors]
 
     # ---- end to end through the C-ABI with host buffers -----------------------------------------
     # bt_track_host = upload + walk + download with the bunch cut into chunks on three streams (copies overlap the walk)
@@ -589,6 +648,9 @@ def run_ours(args):
     barrier()
     t_e2e = time.perf_counter() - t0
     clocks = sampler.stop() if rank == 0 else None
+    # outside the timed region: the host buffers bt_track_host filled hold the same bits as the device-resident walk
+    # (same seeded input, same reference energy; the chunking cannot change a particle's arithmetic)
+    e2e_checked = all(bool((o[::64].view(torch.int64) == d.view(torch.int64)).all()) for o, d in zip(pinned_out, dev_sample))
 
     ms_sum, t_e2e, t_wall = max_over_ranks([ms_sum, t_e2e, t_wall], device="cuda")   # max over ranks
 
@@ -604,6 +666,7 @@ def run_ours(args):
         launches_per_step = launches // args.steps
         roof = walk_roofline(n, cfg.lattice, cfg.nturns, launches_per_step, statistics.mean(step_ms) * 1e-3, peaks, nominal_peak)
         roof["traffic"] = traffic_of(traffic, "walk:" + cfg.name)
+        roof["traffic_source"] = traffic_source(traffic, "walk:" + cfg.name)
         roof["traffic_unit"] = "dram bytes per launch (ncu --set full; profiles/r02_traffic.csv names the capture)"
         roof["launches_per_step"] = launches_per_step
         roof["kernel"] = "bt::track_kernel<P=%d> grid=%d block=%d, record table in kernel parameters" % (
@@ -620,6 +683,11 @@ def run_ours(args):
                                 "execute per half cell (120 400 instead of 125 400 per particle: sm__inst_executed_pipe_fp64 in "
                                 "profiles/): pipe utilisation = frac x 120400/125400")
                 roof["pipe_utilisation_executed"] = roof["frac"] * 120400.0 / 125400.0
+                # a fraction above 1 is not a share of a peak.  `frac` stays achieved/peak on the ALGORITHMIC slots (the
+                # bench contract's definition); frac_executed is the share of the FP64 pipe's issue slots actually occupied.
+                roof["frac_algorithmic"] = roof["frac"]
+                roof["frac_executed"] = roof["pipe_utilisation_executed"]
+                roof["achieved_executed"] = roof["achieved"] * 120400.0 / 125400.0
         else:
             roof["peak_kind"] = peaks_kind + " copy bandwidth"
         # CPU baseline: the oracle as it stands, bounded sample, host cores (all cores, and one thread)
@@ -639,6 +707,9 @@ def run_ours(args):
             "roofline": roof, "cpu_baseline": cpu_baseline,
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": 48 * n, "d2h_bytes_per_step": 48 * n,
                     "ms_per_step": t_e2e / args.steps * 1e3, "vs_device_time": t_e2e / args.steps * 1e3 / ms_per_step,
+                    "e2e_checked": e2e_checked,
+                    "e2e_checked_how": "host output of the last bt_track_host call == device-resident result of the last timed "
+                                       "bt_track step, bitwise, on every 64th particle (outside the timed region)",
                     "call": "bt_track_host(pinned in, pinned out, nturns, nchunks=%d): H2D / walk / D2H of the chunks overlap "
                             "on three streams; every launch carries its own coefficient table" % args.e2e_chunks},
             "gpu_launches": int(launches), "clocks": clocks,
@@ -646,6 +717,12 @@ def run_ours(args):
             "wall_s_timed_region": t_wall,
         }
         result.update(extras)
+        result["e2e_checked"] = e2e_checked
+        # Round-over-round trend: the N=1 default workload moved from configs[1] (round 1) to configs[3] (round 2 on), so the
+        # round-1 headline lives on under this key.
+        for e in extras.get("other_configs", []):
+            if e["workload"].startswith("configs[1]"):
+                result["trend_configs1_pushes_per_s"] = e["pushes_per_s"]
     beam.close()
     if world > 1:
         dist.destroy_process_group()

@@ -179,6 +179,9 @@ int bt_beam_ids(bt_beam *beam, int32_t **dev_ids_out);
  * when bt_track needs them and packed into 64-byte records; a launch of the walk carries its records as kernel
  * parameters (<= 510 records; constant bank 0), so nothing on the device is shared between beams or streams:
  * beams may be used concurrently from different host threads / streams (one thread per beam at a time).
+ * A bt_grid carries unsynchronised bookkeeping of which stream touched it last (bt_deposit_cic, bt_gather_kick -- through
+ * its const pointer too -- and bt_grid_solve_poisson update it): a grid and every beam used with it must be driven from ONE
+ * host thread at a time.  bt_debug_knob is process-wide and meant to be set while no other thread is inside the library.
  */
 int bt_lattice_set(bt_beam *beam, const bt_element *elems, int32_t n_elems);
 
@@ -342,6 +345,18 @@ int bt_moments_static(const double *const dev_q[6], int64_t n, double *dev_out, 
  */
 enum { BT_DIAG_ELEMENT = 0, BT_DIAG_SLICE = 1 };
 int bt_track_diagnostics(bt_beam *beam, int32_t nturns, int32_t granularity, double *host_moments);
+/* How many 42-double records bt_track_diagnostics(beam, nturns, granularity, ...) writes for the beam's current lattice
+ * (nturns x number of elements, resp. x the sum of their nslice): size host_moments from this. */
+int bt_track_diagnostics_records(const bt_beam *beam, int32_t nturns, int32_t granularity, int64_t *n_records);
+/* bt_track_diagnostics with the capacity of host_moments stated (in records of 42 doubles): BT_ERR_INVALID, and nothing
+ * launched, when the call would write more.  Prefer this one from any language where the buffer's size is a separate fact. */
+int bt_track_diagnostics_n(bt_beam *beam, int32_t nturns, int32_t granularity, double *host_moments, int64_t capacity_records);
+/* Frees what the beam keeps between calls for the diagnostics walk (the row buffer, up to 1 GiB, and the record buffer) and
+ * bt_beam_download's un-permute scratch; they are re-allocated on demand.  Synchronises the beam's stream. */
+int bt_beam_release_scratch(bt_beam *beam);
+/* Failure part-way: if a launch fails inside bt_track, bt_track_host or bt_track_diagnostics (BT_ERR_CUDA), the particles
+ * have been advanced through part of the lattice while the reference energy, s and turn are left as they were.  The
+ * beam's state is then undefined: upload the bunch and set the reference again. */
 
 /* ---- utilities ------------------------------------------------------------------------------ */
 int bt_sync(bt_beam *beam); /* cudaStreamSynchronize on the beam's stream */

@@ -68,6 +68,9 @@ EXPORTS = {
     "bt_beam_moments_device": (C.c_int, [_vp, _vp]),
     "bt_moments_static": (C.c_int, [C.POINTER(_vp), C.c_int64, _vp, _vp]),
     "bt_track_diagnostics": (C.c_int, [_vp, C.c_int32, C.c_int32, _dp]),
+    "bt_track_diagnostics_records": (C.c_int, [_vp, C.c_int32, C.c_int32, C.POINTER(C.c_int64)]),
+    "bt_track_diagnostics_n": (C.c_int, [_vp, C.c_int32, C.c_int32, _dp, C.c_int64]),
+    "bt_beam_release_scratch": (C.c_int, [_vp]),
     "bt_sync": (C.c_int, [_vp]),
     "bt_last_error": (C.c_char_p, []),
     "bt_version": (C.c_int, []),
@@ -282,14 +285,24 @@ class Beam:
         c = (C.c_double * 3)(*coef)
         _check(lib.bt_gather_kick(self._h, grid._h, c, zscale, half_drift_before, half_drift_after), "bt_gather_kick")
 
-    def track_diagnostics(self, nturns, n_boundaries, granularity="element"):
-        """bt_track(nturns) with the beam statistics taken inside the walk after every element ("element": n_boundaries =
-        number of elements) or every slice ("slice": n_boundaries = sum of nslice): returns
-        (mean[nturns, n_boundaries, 6], cov[nturns, n_boundaries, 6, 6])."""
+    def track_diagnostics(self, nturns, n_boundaries=None, granularity="element"):
+        """bt_track(nturns) with the beam statistics taken inside the walk after every element ("element") or every slice
+        ("slice"): returns (mean[nturns, B, 6], cov[nturns, B, 6, 6]) with B = boundaries per turn = number of elements,
+        resp. the sum of their nslice.  The output is sized from the library's own count (bt_track_diagnostics_records) and
+        passed with its capacity; n_boundaries, when given, is only checked against B."""
         gran = {"element": 0, "slice": 1}[granularity]
-        out = np.zeros((int(nturns), int(n_boundaries), 42))
-        _check(lib.bt_track_diagnostics(self._h, int(nturns), gran, out.ctypes.data_as(_dp)), "bt_track_diagnostics")
-        return out[:, :, :6].copy(), out[:, :, 6:].reshape(int(nturns), int(n_boundaries), 6, 6).copy()
+        nturns = int(nturns)
+        per_turn = C.c_int64()
+        _check(lib.bt_track_diagnostics_records(self._h, 1, gran, C.byref(per_turn)), "bt_track_diagnostics_records")
+        nb = int(per_turn.value)
+        if n_boundaries is not None and int(n_boundaries) != nb:
+            raise ValueError("track_diagnostics: the lattice has %d boundaries per turn at %s granularity, not %d" % (nb, granularity, int(n_boundaries)))
+        out = np.zeros((nturns, nb, 42))
+        _check(lib.bt_track_diagnostics_n(self._h, nturns, gran, out.ctypes.data_as(_dp), nturns * nb), "bt_track_diagnostics_n")
+        return out[:, :, :6].copy(), out[:, :, 6:].reshape(nturns, nb, 6, 6).copy()
+
+    def release_scratch(self):
+        _check(lib.bt_beam_release_scratch(self._h), "bt_beam_release_scratch")
 
     def moments(self):
         """(mean[6], cov[6, 6]) of x, px, y, py, t, pt -- computed on the device, returned as numpy arrays."""

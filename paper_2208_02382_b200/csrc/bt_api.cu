@@ -323,10 +323,12 @@ static int32_t plan_walk(Beam &b, double gamma, int32_t nturns, WalkPlan &plan) 
         for (size_t o = 0; o < len; o += K) plan.launches.push_back({lo + o, (int32_t)(len - o < K ? len - o : K), 1, spr});
     };
     if (!b.energy_changes) {
-        if (!b.table_valid) {
+        const int fuse_now = knob(KNOB_TRACK_FUSE, 1) != 0;
+        if (!b.table_valid || b.table_fuse != fuse_now) {  // the cached table was built under the knob's value at the time
             b.h_table.clear();
             build_turn_table(b.lattice, gamma, b.h_table, &b.table_slots);
             b.table_valid = true;
+            b.table_fuse = fuse_now;
         }
         plan.ops = &b.h_table;
         plan.gamma_after = gamma;
@@ -645,6 +647,39 @@ int bt_track(bt_beam *beam, int32_t nturns) {
 // Slice-step / element-step diagnostics fused into the walk (P:l.61 set_slice_step_diagnostics): O(1)
 // launches per table -- the diagnostics walk writes one 216-byte row per (warp, boundary), a combine kernel turns the
 // rows of a launch into records.  Launches are cut where the record table (510 records) or the row buffer (1 GiB) is full.
+int bt_track_diagnostics_records(const bt_beam *beam, int32_t nturns, int32_t granularity, int64_t *n_records) {
+    if (!beam || !n_records) return fail(BT_ERR_INVALID, "bt_track_diagnostics_records: NULL argument");
+    if (nturns < 0) return fail(BT_ERR_INVALID, "bt_track_diagnostics_records: nturns < 0");
+    if (granularity != BT_DIAG_ELEMENT && granularity != BT_DIAG_SLICE) return fail(BT_ERR_INVALID, "bt_track_diagnostics_records: granularity must be BT_DIAG_ELEMENT or BT_DIAG_SLICE");
+    if (beam->b.lattice.empty()) return fail(BT_ERR_STATE, "bt_track_diagnostics_records: bt_lattice_set not called");
+    long long per_turn = 0;
+    for (const bt_element &e : beam->b.lattice) per_turn += granularity == BT_DIAG_SLICE ? e.nslice : 1;
+    *n_records = per_turn * nturns;
+    return BT_OK;
+}
+
+int bt_track_diagnostics_n(bt_beam *beam, int32_t nturns, int32_t granularity, double *host_moments, int64_t capacity_records) {
+    int64_t need = 0;
+    const int rc = bt_track_diagnostics_records(beam, nturns, granularity, &need);
+    if (rc != BT_OK) return rc;
+    if (capacity_records < need)
+        return fail(BT_ERR_INVALID, "bt_track_diagnostics_n: host_moments holds " + std::to_string((long long)capacity_records) +
+                                        " records of 42 doubles, the call writes " + std::to_string((long long)need));
+    return bt_track_diagnostics(beam, nturns, granularity, host_moments);
+}
+
+int bt_beam_release_scratch(bt_beam *beam) {
+    if (!beam) return fail(BT_ERR_INVALID, "bt_beam_release_scratch: beam is NULL");
+    Beam &b = beam->b;
+    BT_CUDA_TRY(cudaStreamSynchronize(b.stream));
+    if (b.diag_rows) cudaFree(b.diag_rows);
+    if (b.diag_out) cudaFree(b.diag_out);
+    if (b.dl_tmp) cudaFree(b.dl_tmp);
+    b.diag_rows = b.diag_out = b.dl_tmp = nullptr;
+    b.diag_rows_bytes = b.diag_out_bytes = 0;
+    return BT_OK;
+}
+
 int bt_track_diagnostics(bt_beam *beam, int32_t nturns, int32_t granularity, double *host_moments) {
     if (!beam || !host_moments) return fail(BT_ERR_INVALID, "bt_track_diagnostics: NULL argument");
     if (nturns < 0) return fail(BT_ERR_INVALID, "bt_track_diagnostics: nturns < 0");

@@ -111,6 +111,7 @@ struct Beam {
     double lattice_length = 0.0;
     std::vector<DevOp> h_table;  // single-turn record table for the current lattice and gamma (static lattices)
     bool table_valid = false;    // h_table is up to date
+    int table_fuse = 1;          // value of the track_fuse knob h_table was built under
     double table_slots = 0.0;    // FP64 slots per particle per turn of that table
     TrackLaunchInfo last_launch;
     // S4 cell binning: storage order != original order once sorted; ids[j] = original index of slot j

@@ -143,7 +143,7 @@ def test_config4_in_run_reduced(variant, resort):
     run_config4(sc, resort)
 
 
-def run_config4(sc, resort_interval=0):
+def run_config4(sc, resort_interval=0, order=1):
     """oracle = 10 x [D(.005); deposit; gather+kick(.01); D(.005)]; library = bt_track(D(.005)) once, then per step
     bt_deposit_cic + bt_gather_kick(0, .01 -- .005 on the last step): deposit and gather see the same positions.
     Checked: R15 (ii) (in-run: |rho - rho_ref| <= 1e-12 max(rho_ref, q_weight)) and the total charge at the first and at the
@@ -162,13 +162,14 @@ def run_config4(sc, resort_interval=0):
     for step in range(sc.nsteps):
         O.track(ref, half, 1, g0)
         if step in check_steps:
-            rho_ref[step] = O.deposit_cic(ref[0], ref[2], ref[4], sc.shape, sc.lo, sc.d, sc.q_weight, sc.zscale)
+            rho_ref[step] = O.deposit_cic(ref[0], ref[2], ref[4], sc.shape, sc.lo, sc.d, sc.q_weight, sc.zscale, order=order)
             pos_ref[step] = [a.copy() for a in ref]
-        O.gather_kick(ref, sc.shape, sc.lo, sc.d, E, sc.kick_coef, sc.zscale)
+        O.gather_kick(ref, sc.shape, sc.lo, sc.d, E, sc.kick_coef, sc.zscale, order=order)
         O.track(ref, half, 1, g0)
     # library
     beam = bt.Beam(sc.n)
     grid = bt.Grid(sc.shape, sc.lo, sc.d)
+    grid.set_particle_shape(order)
     beam.set_ref(sc.kin_energy_MeV, sc.mass_MeV, sc.charge_qe)
     grid.set_field(*E)
     beam.upload(c)
@@ -200,12 +201,22 @@ def run_config4(sc, resort_interval=0):
     grid.close()
 
 
-@pytest.mark.parametrize("resort", [0, 10])
+@pytest.mark.parametrize("resort", [0, 5, 10])
 @pytest.mark.parametrize("variant", ["A", "B"])
 def test_config4_full_size(variant, resort):
-    """configs[4] as BASELINE states it -- 8e6 particles, 128^3 nodes, all 10 steps -- in the caller's order and with
-    bt_beam_set_resort_interval(10); criteria in run_config4."""
+    """configs[4] as BASELINE states it -- 8e6 particles, 128^3 nodes, all 10 steps -- in the caller's order, with
+    bt_beam_set_resort_interval(10), and with the interval bench.py times (5: a second library-triggered re-sort in the middle
+    of the run -- the bunch ping-pongs back into its home arrays, the ids are composed twice -- followed by five more steps);
+    criteria in run_config4."""
     run_config4(W.spacecharge_config(variant), resort)
+
+
+@pytest.mark.parametrize("variant,resort", [("A", 3), ("A", 5), ("B", 3)])
+def test_config4_full_size_order2(variant, resort):
+    """The same run with the listing's own particle shape (P:l.60 set_particle_shape(2)) at the size and re-sort cadence
+    bench.py's A_order2 leg times (8e6 particles, 128^3 nodes, 10 steps, interval 3; 5 = the order-1 cadence): the order-2-keyed
+    sort, the 27-node deposit and the regrouping tile gather against the oracle's order-2 loop, same criteria."""
+    run_config4(W.spacecharge_config(variant), resort, order=2)
 
 
 # ---- S4 cell binning ---------------------------------------------------------------------------------

@@ -197,6 +197,21 @@ def test_track_diagnostics_many_boundaries_are_cut_into_launches():
     assert ends.shape == (100,) and np.max(np.abs(ends / ends[0] - 1.0)) < 2e-2
     assert np.all(np.isfinite(cov)) and np.all(np.isfinite(mean))
     assert bt.lib.bt_track_diagnostics(beam._h, 1, 7, np.zeros(42).ctypes.data_as(bt._dp)) == bt.BT_ERR_INVALID
+    # the output is sized by the library's own count; a buffer that is too small is refused before anything runs
+    import ctypes
+    need = ctypes.c_int64()
+    assert bt.lib.bt_track_diagnostics_records(beam._h, 2, 1, ctypes.byref(need)) == bt.BT_OK and need.value == 2 * nb
+    assert bt.lib.bt_track_diagnostics_records(beam._h, 3, 0, ctypes.byref(need)) == bt.BT_OK and need.value == 3 * len(cfg.lattice)
+    before, turn = bt.launch_count(), beam.get_ref()[2]
+    small = np.zeros((nb - 1, 42))
+    assert bt.lib.bt_track_diagnostics_n(beam._h, 1, 1, small.ctypes.data_as(bt._dp), nb - 1) == bt.BT_ERR_INVALID
+    assert b"records" in bt.lib.bt_last_error() and bt.launch_count() == before and beam.get_ref()[2] == turn
+    with pytest.raises(ValueError):
+        beam.track_diagnostics(1, nb - 1, "slice")
+    # the buffers the walk keeps on the beam can be given back and come back on demand
+    beam.release_scratch()
+    m2, c2 = beam.track_diagnostics(1, granularity="element")
+    assert m2.shape == (1, len(cfg.lattice), 6) and np.all(np.isfinite(c2))
     beam.close()
 
 
