@@ -546,6 +546,114 @@ def bench_spacecharge(bt, torch, flush, peaks, traffic, interval, with_cpu=True)
 
 
 # ---------------------------------------------------------------------------------------------------
+# the closed space-charge step with the method's one collective
+# ---------------------------------------------------------------------------------------------------
+def run_closed(args):
+    """--workload spacecharge_closed, any N (weak scaling): every rank owns 8e6 particles of configs[4] A (its own seed) and a
+    private 128^3 charge grid; a step is shard.spacecharge_step = bt_deposit_cic -> all-reduce of rho over the ranks (NCCL on
+    the zero-copy view of the library's array, issued even in a one-rank group) -> bt_grid_solve_poisson (replicated) ->
+    bt_gather_kick with a drift.  Metric: particle space-charge steps per second (particles of all ranks x steps / time); every
+    phase is bracketed by CUDA events on the beam's stream.  Nothing here has run on more than one GPU yet."""
+    import socket
+    import torch
+    import torch.distributed as dist
+    import paper_2208_02382_b200 as bt
+    from paper_2208_02382_b200 import shard
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if world != args.gpus:
+        raise SystemExit("bench.py: --gpus %d needs torchrun with %d ranks" % (args.gpus, args.gpus))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the product path has no CPU fallback")
+    torch.cuda.set_device(local)
+    os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+    if "MASTER_PORT" not in os.environ:
+        with socket.socket() as sk:
+            sk.bind(("127.0.0.1", 0))
+            os.environ["MASTER_PORT"] = str(sk.getsockname()[1])
+    dist.init_process_group("nccl", rank=rank, world_size=world, device_id=torch.device("cuda", local))
+    sc = W.spacecharge_config("A")
+    sc.seed = W.rank_seed(sc.seed, rank)
+    c = W.make_spacecharge_bunch(sc)
+    n, nn = sc.n, sc.shape[0] * sc.shape[1] * sc.shape[2]
+    gz = 1.0 + sc.kin_energy_MeV / sc.mass_MeV
+    coef = (2.0e-9, 2.0e-9, -1.0e-9)               # the caller's rest-frame -> kick factors (R12); any finite values time the same
+    beam, grid = bt.Beam(n), bt.Grid(sc.shape, sc.lo, sc.d)
+    beam.set_ref(sc.kin_energy_MeV, sc.mass_MeV, sc.charge_qe)
+    beam.upload(c)
+    beam.set_resort_interval(args.resort_interval)
+    phases = ("deposit", "allreduce", "solve", "gather")
+    marks = []
+
+    def step(record):
+        ev = [torch.cuda.Event(enable_timing=True) for _ in range(5)] if record else None
+        if record:
+            ev[0].record()
+        k = [1]
+
+        def mark(_name):
+            if record:
+                ev[k[0]].record()
+                k[0] += 1
+        shard.spacecharge_step(lambda: beam.deposit_cic(grid, sc.q_weight, sc.zscale, True),
+                               lambda: shard.allreduce_rho(grid, always=True),
+                               lambda: grid.solve_poisson(gz),
+                               lambda: beam.gather_kick(grid, coef, sc.zscale, 0.0, sc.ds), mark)
+        if record:
+            marks.append(ev)
+
+    for _ in range(max(args.warmup, 3)):
+        step(False)
+    torch.cuda.synchronize()
+    dist.barrier()
+    torch.cuda.synchronize()
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+    launches0 = bt.launch_count()
+    for _ in range(args.steps):
+        step(True)
+    dist.barrier()
+    torch.cuda.synchronize()
+    launches = bt.launch_count() - launches0
+    clocks = sampler.stop() if rank == 0 else None
+    split = [sum(ev[i].elapsed_time(ev[i + 1]) for ev in marks) / args.steps for i in range(4)]
+    total = sum(ev[0].elapsed_time(ev[4]) for ev in marks) / args.steps
+    vals = shard.max_over_ranks([total] + split, device="cuda")
+    rho_sum = float(grid.rho_tensor().sum().item())
+    beam.close()
+    grid.close()
+    backend = dist.get_backend()
+    dist.destroy_process_group()
+    if rank == 0:
+        peaks, _kind = load_peaks()
+        hbm = float(peaks["hbm_gbs"])
+        bytes_step = (24.0 * n + 16.0 * nn) + (96.0 * n + 24.0 * nn)
+        print(json.dumps({
+            "metric": "particle space-charge steps/s (fp64)", "value": world * n / (vals[0] * 1e-3), "unit": "particle-steps/s",
+            "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": vals[0], "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": "spacecharge_closed: configs[4] A per rank (%d particles, %dx%dx%d nodes), deposit -> all-reduce(rho) "
+                                   "-> Poisson -> gather+kick+drift" % ((n,) + tuple(sc.shape)),
+                       "particles_per_gpu": n, "resort_interval": args.resort_interval,
+                       "l2": "particle state (768 MB per rank) larger than L2; no flush between steps",
+                       "parallelism": "particles sharded, %d rank(s), one all-reduce of rho per step" % world},
+            "ms_split_max_over_ranks": dict(zip(phases, vals[1:])),
+            "collective": {"op": "allreduce", "bytes": 8 * nn, "backend": backend, "n_ranks": world,
+                           "on": "zero-copy view of the library's rho (bt_grid_rho), torch's current stream = the beam's stream"},
+            "roofline": {"bound": "hbm", "achieved": bytes_step / ((vals[1] + vals[4]) * 1e-3) / 1e9, "peak": hbm, "unit": "GB/s",
+                         "frac": bytes_step / ((vals[1] + vals[4]) * 1e-3) / 1e9 / hbm, "traffic": None,
+                         "note": "deposit + gather only (algorithmic bytes of SURVEY 8d over their summed time); the solve and "
+                                 "the collective are reported in ms_split"},
+            "gpu_launches": int(launches), "clocks": clocks, "rho_total_over_charge_of_all_ranks": rho_sum / (sc.q_weight * n * world),
+            "note": "never run on more than one GPU so far; at N=1 the all-reduce is a one-rank NCCL collective",
+        }), flush=True)
+    return 0
+
+
+# ---------------------------------------------------------------------------------------------------
 # our arm
 # ---------------------------------------------------------------------------------------------------
 def run_ours(args):
@@ -737,7 +845,7 @@ def main():
     ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="nonlinear_ring", choices=sorted(WORKLOADS))
+    ap.add_argument("--workload", default="nonlinear_ring", choices=sorted(WORKLOADS) + ["spacecharge_closed"])
     ap.add_argument("--ref-sample", type=int, default=0,
                     help="particles per step the oracle is timed on in --impl reference (0 = sized for ~60 s in total)")
     ap.add_argument("--e2e-chunks", type=int, default=16, help="chunks of the bunch in bt_track_host (e2e leg)")
@@ -750,7 +858,12 @@ def main():
     ap.add_argument("--no-cpu", action="store_true", help="skip the oracle timings (profiling runs only)")
     args = ap.parse_args()
     if args.impl == "reference":
+        if args.workload == "spacecharge_closed":
+            print(json.dumps({"impl": "reference", "unavailable": "the reference arm times the oracle on the tracking workloads only"}))
+            return 0
         return run_reference(args)
+    if args.workload == "spacecharge_closed":
+        return run_closed(args)
     return run_ours(args)
 
 

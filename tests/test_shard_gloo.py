@@ -22,6 +22,7 @@ def _free_port():
 
 def _worker(rank, world, port, out_dir):
     sys.path.insert(0, ROOT)
+    sys.path.insert(0, os.path.join(ROOT, "tests"))
     os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), WORLD_SIZE=str(world),
                       LOCAL_RANK=str(rank), OMP_NUM_THREADS="1")
     import oracle as O
@@ -58,6 +59,44 @@ def _worker(rank, world, port, out_dir):
         assert np.array_equal(r == 0.0, rho_all == 0.0)
         nz = rho_all != 0.0
         assert np.max(np.abs(r[nz] - rho_all[nz]) / rho_all[nz]) <= 1e-12
+        # ---- the closed space-charge step, driven through shard.spacecharge_step with the oracle standing in for the kernels:
+        # two ranks, each with half the particles and a private grid == one rank with the whole bunch (R15 on rho, R14 after) ----
+        sc = W.spacecharge_config("A", n=20_001, shape=(12, 12, 12))
+        c = W.make_spacecharge_bunch(sc)
+        coef = (2.0e-9, 2.0e-9, -1.0e-9)
+        gsc = O.ref_from_kinetic(sc.kin_energy_MeV, sc.mass_MeV)[0]
+        drift = [("drift", sc.ds, 1)]
+
+        def run(coords, reduce_fn, rhos):
+            st = {}
+
+            def deposit():
+                st["rho"] = torch.from_numpy(O.deposit_cic(coords[0], coords[2], coords[4], sc.shape, sc.lo, sc.d, sc.q_weight, sc.zscale)[0].copy())
+
+            def solve():
+                rho = st["rho"].numpy()
+                rhos.append(rho.copy())
+                st["E"] = O.efield(O.poisson(rho, sc.d, gsc), sc.d, gsc)
+
+            def gather():
+                O.gather_kick(coords, sc.shape, sc.lo, sc.d, st["E"], coef, sc.zscale)
+                O.track(coords, drift, 1, gsc)
+
+            phases = []
+            for _ in range(2):
+                shard.spacecharge_step(deposit, lambda: reduce_fn(st["rho"]), solve, gather, mark=phases.append)
+            assert phases == ["deposit", "allreduce", "solve", "gather"] * 2
+            return coords
+
+        lo, hi = shard.shard_bounds(sc.n, rank, world)
+        rhos_mine, rhos_whole = [], []
+        mine = run([a[lo:hi].copy() for a in c], shard.allreduce_rho, rhos_mine)
+        whole = run([a.copy() for a in c], lambda t: t, rhos_whole)          # one rank, the whole bunch, no collective
+        for a, b in zip(rhos_mine, rhos_whole):
+            assert np.all(np.abs(a - b) <= 1e-12 * np.maximum(b, sc.q_weight))     # R15 (ii)
+        from _util import r14_error
+        assert max(r14_error(mine, [a[lo:hi] for a in whole])) <= 1e-11             # R14
+        assert np.max(np.abs(whole[1] - c[1])) > 0.0
         # ---- timing reduction: slowest rank ----
         assert shard.max_over_ranks([rank + 1.0, 5.0 - rank]) == [float(world), 5.0]
         assert W.rank_seed(1, rank) == 1 + 1000 * rank
