@@ -84,18 +84,19 @@ def _source_digest(name):
         return hashlib.sha256(f.read()).hexdigest()
 
 
+TRAFFIC_TABLES = (("r02_traffic.csv", "r02_traffic_sources.json"), ("r03_traffic.csv", "r03_traffic_sources.json"))
+
+
 def load_traffic():
-    """dram__bytes_read.sum + dram__bytes_write.sum per launch from the ncu --set full captures summarised under
-    profiles/ (text, written from `ncu -i ... --page raw --csv`): {key: (bytes, source)}, plus "_provenance".
-    The table is STATIC (captured once, at the commit profiles/r02_traffic_sources.json names), not measured in this run:
-    a value is handed out only while the sources of its kernel are byte-identical to what was captured."""
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch from the ncu captures summarised under profiles/ (text, written
+    from `ncu -i ... --page raw --csv` / `--csv --log-file`): {key: (bytes, source, provenance)}; a later table overrides an
+    earlier one key by key.  The tables are STATIC (captured once, at the commit their *_sources.json names), not measured in
+    this run: a value is handed out only while the sources of its kernel are byte-identical to what was captured."""
     out = {}
-    path = os.path.join(ROOT, "profiles", "r02_traffic.csv")
-    side = os.path.join(ROOT, "profiles", "r02_traffic_sources.json")
-    if os.path.exists(path) and os.path.exists(side):
-        with open(path) as f:
-            for row in csv.DictReader(f):
-                out[row["key"]] = (float(row["dram_read_bytes"]) + float(row["dram_write_bytes"]), row["source"])
+    for table, sidecar in TRAFFIC_TABLES:
+        path, side = os.path.join(ROOT, "profiles", table), os.path.join(ROOT, "profiles", sidecar)
+        if not (os.path.exists(path) and os.path.exists(side)):
+            continue
         with open(side) as f:
             prov = json.load(f)
         changed = {}
@@ -104,29 +105,30 @@ def load_traffic():
                 changed[fam] = [x for x in files if _source_digest(x) != prov["sha256"].get(x)]
             except (OSError, ValueError):
                 changed[fam] = list(files)
-        out["_provenance"] = {"file": "profiles/r02_traffic.csv", "captured_at": prov["captured_at"], "changed": changed}
+        with open(path) as f:
+            for row in csv.DictReader(f):
+                fam = row["key"].split(":")[0]
+                out[row["key"]] = (float(row["dram_read_bytes"]) + float(row["dram_write_bytes"]), row["source"],
+                                   {"file": "profiles/" + table, "captured_at": prov["captured_at"], "changed": changed.get(fam, ["?"])})
     return out
 
 
 def traffic_of(table, key):
-    """Value of the static table, or None when the table is missing or the kernel's sources changed since the capture."""
-    prov = table.get("_provenance")
-    if key not in table or prov is None or prov["changed"].get(key.split(":")[0], ["?"]):
+    """Value of the static table, or None when there is no capture or the kernel's sources changed since the capture."""
+    if key not in table or table[key][2]["changed"]:
         return None
     return table[key][0]
 
 
 def traffic_source(table, key):
     """Goes beside every `traffic`: where the number comes from and whether it is still valid for the kernels as built."""
-    prov = table.get("_provenance")
-    if prov is None:
-        return {"file": None, "reason": "no traffic table under profiles/"}
-    src = {"file": prov["file"], "captured_at": prov["captured_at"], "kind": "static table from ncu --set full captures, not measured in this run"}
-    stale = prov["changed"].get(key.split(":")[0], ["?"])
     if key not in table:
-        src["reason"] = "no capture for this kernel/workload"
-    elif stale:
-        src["reason"] = "stale: %s changed since the capture; traffic withheld until re-captured" % ", ".join(stale)
+        return {"file": None, "reason": "no capture for this kernel/workload under profiles/"}
+    prov = table[key][2]
+    src = {"file": prov["file"], "captured_at": prov["captured_at"], "capture": table[key][1],
+           "kind": "static table from ncu captures, not measured in this run"}
+    if prov["changed"]:
+        src["reason"] = "stale: %s changed since the capture; traffic withheld until re-captured" % ", ".join(prov["changed"])
     return src
 
 
@@ -775,7 +777,7 @@ def run_ours(args):
         roof = walk_roofline(n, cfg.lattice, cfg.nturns, launches_per_step, statistics.mean(step_ms) * 1e-3, peaks, nominal_peak)
         roof["traffic"] = traffic_of(traffic, "walk:" + cfg.name)
         roof["traffic_source"] = traffic_source(traffic, "walk:" + cfg.name)
-        roof["traffic_unit"] = "dram bytes per launch (ncu --set full; profiles/r02_traffic.csv names the capture)"
+        roof["traffic_unit"] = "dram bytes per launch (ncu --set full; traffic_source names the table and the capture)"
         roof["launches_per_step"] = launches_per_step
         roof["kernel"] = "bt::track_kernel<P=%d> grid=%d block=%d, record table in kernel parameters" % (
             launch_info["particles_per_thread"], launch_info["grid"], launch_info["block"])

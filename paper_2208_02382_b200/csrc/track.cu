@@ -539,7 +539,7 @@ __device__ __forceinline__ void diag_emit_shfl(const Ptc<P> &p, const double (&k
 // included -- and a row follows every record marked OP_MARK (the last record of an element); SLICE = true: one slice at a
 // time, a row after each.
 template <int P, bool NL, int NREC, bool SLICE>
-__global__ void __launch_bounds__(128, P == 4 ? 3 : 4) track_diag_kernel(const __grid_constant__ DiagArgs<NREC> a) {
+__global__ void __launch_bounds__(128, P == 8 ? 2 : P == 4 ? 3 : 4) track_diag_kernel(const __grid_constant__ DiagArgs<NREC> a) {
     const int tid = threadIdx.x, B = blockDim.x;
     const long long gw = (long long)blockIdx.x * (B >> 5) + (tid >> 5);
     const long long base = (long long)blockIdx.x * (P * B);
@@ -726,10 +726,14 @@ int launch_track(Beam *b, const DevOp *h_table, int32_t n_ops, int32_t nturns, d
 
 // ---- diagnostics walk: one launch over `n_ops` un-fused records, rows for `nb` boundaries, then their combination ----------
 int diag_warps(const Beam *b, int *P_out, int *block_out) {
-    int P = (b->aligned16 && b->n >= 65536) ? 4 : 1;
+    // The lane reduction and the 216-byte row are per warp and boundary, so they are amortised over the 32 P particles of a
+    // warp: P = 8 where the bunch still fills the machine (configs[1], 10^6 particles: element granularity 1.77 -> 1.69 x the
+    // plain walk, slice granularity 10.4 -> 8.7 x, rows 834 -> 417 MB; P = 2 and 1 measured 2.04 / 3.51 x and 15.2 / 27.2 x)
+    int P = !b->aligned16 ? 1 : b->n >= 524288 ? 8 : b->n >= 65536 ? 4 : 1;
     P = knob(KNOB_TRACK_PPT, P);
-    if (P != 1 && !(b->aligned16 && (P == 2 || P == 4))) P = 1;
-    const int block = 128;
+    if (P != 1 && !(b->aligned16 && (P == 2 || P == 4 || P == 8))) P = 1;
+    int block = knob(KNOB_TRACK_BLOCK, 128);
+    if (block != 64 && block != 128) block = 128;
     *P_out = P;
     *block_out = block;
     const long long per_block = (long long)P * block;
@@ -751,7 +755,8 @@ static cudaError_t launch_diag_p(const DiagArgs<NREC> &a, bool nl, bool slice, i
 template <int NREC>
 static cudaError_t launch_diag_sized(DiagArgs<NREC> &a, const DevOp *h_table, int n_ops, int P, bool nl, int grid, int block, cudaStream_t s) {
     memcpy(a.tab, h_table, (size_t)n_ops * sizeof(DevOp));
-    return P == 4 ? launch_diag_p<4, NREC>(a, nl, a.slice_gran != 0, grid, block, s)
+    return P == 8 ? launch_diag_p<8, NREC>(a, nl, a.slice_gran != 0, grid, block, s)
+         : P == 4 ? launch_diag_p<4, NREC>(a, nl, a.slice_gran != 0, grid, block, s)
          : P == 2 ? launch_diag_p<2, NREC>(a, nl, a.slice_gran != 0, grid, block, s)
                   : launch_diag_p<1, NREC>(a, nl, a.slice_gran != 0, grid, block, s);
 }

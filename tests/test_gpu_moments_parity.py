@@ -131,9 +131,14 @@ def _slice_lattice(lat):
     return out
 
 
-@pytest.mark.parametrize("idx,n,granularity", [(0, 20_000, "element"), (0, 20_000, "slice"), (3, 20_000, "element"),
-                                               (3, 70_001, "element"), (1, 70_001, "slice")])
-def test_track_diagnostics_inside_the_walk(idx, n, granularity):
+@pytest.mark.parametrize("idx,n,granularity,ppt,block", [
+    (0, 20_000, "element", -1, -1), (0, 20_000, "slice", -1, -1), (3, 20_000, "element", -1, -1), (3, 70_001, "element", -1, -1),
+    (1, 70_001, "slice", -1, -1),
+    # the geometry large bunches get by default (eight particles per thread: n >= 524 288), forced here at a size the oracle
+    # can follow boundary by boundary, with both block sizes and a ragged last block
+    (3, 70_001, "element", 8, 128), (1, 70_001, "slice", 8, 128), (3, 70_001, "element", 8, 64), (0, 20_000, "slice", 8, 64),
+    (3, 70_001, "element", 2, 128)])
+def test_track_diagnostics_inside_the_walk(idx, n, granularity, ppt, block, knobs):
     """bt_track_diagnostics (statistics taken inside the fused walk): final state bit-identical to bt_track; every record
     equals the oracle's moments of the oracle's bunch at that boundary of the walk -- after every element or after every
     slice (config 0: FODO cell with 10-slice quads; config 3: ring with kicks and an RF cavity that moves the reference
@@ -153,7 +158,13 @@ def test_track_diagnostics_inside_the_walk(idx, n, granularity):
     beam.upload(c)
     steps = _slice_lattice(lat) if granularity == "slice" else lat
     n0 = bt.launch_count()
+    knobs("track_ppt", ppt)
+    knobs("track_block", block)
     mean, cov = beam.track_diagnostics(nturns, len(steps), granularity)
+    if ppt > 0:
+        assert beam.last_launch()["particles_per_thread"] == ppt and beam.last_launch()["block"] == block
+    knobs("track_ppt", -1)
+    knobs("track_block", -1)
     launches = bt.launch_count() - n0
     assert launches <= 1 + 2 * 2, launches             # centre + (walk, combine) per record table; RF lattices: one table per turn here
     got = beam.download()
